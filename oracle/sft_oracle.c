@@ -1,0 +1,654 @@
+/*
+ * sft_oracle.c -- CPU oracle for the HipFT surface-flux-transport time step.
+ *
+ * TEST INFRASTRUCTURE ONLY.  This file is the plain, slow, obviously-correct
+ * restatement of what the hot path computes, written from the paper
+ * (arxiv 2501.06377, /root/reference/PAPER.md; cited below as PAPER.md:<line>)
+ * and the readings listed in DESIGN.md ("Readings of the paper").  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may call it.  It shares no code, header, table or constant generator with the
+ * CUDA path under paper_2501_06377_b200/csrc/, and neither imports the other.
+ *
+ * Compiled twice: -DORACLE_FP32 -> symbols *_f32 (state and arithmetic in float),
+ * otherwise *_f64 (double).  Tables are always formed in fp64 and rounded once to
+ * the state precision; phi-sums (polar caps, diagnostics) are accumulated in fp64
+ * with compensated (Kahan) summation in index order.  Build with
+ *     gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC
+ * so that no FMA contraction happens: every expression is evaluated left to
+ * right exactly as written here.  OpenMP is used only as `parallel for` over rows
+ * (each row's result is independent of the thread count).
+ *
+ * Parity pins (tests/test_oracle_*.py, all `-m "not gpu"`):
+ *   units            PAPER.md:298 printed constants, :257 rigid-rotation speed
+ *   diffusion L      Y_l^m eigenfunction decay exp(-l(l+1) nu t) (Eq. 19, :261), 2nd order;
+ *                    dA-weighted symmetry (:448); constants in the null space; flux conservation
+ *   STS              scalar stability polynomial: order conditions, |R|<=1 on the stated interval,
+ *                    time ratio sqrt(6/4) (:476); dense-matrix polynomial on 8x16 (brute force)
+ *   advection        upwind+Euler at Courant 1 = exact one-cell shift; phi-flux == textbook WENO3 (JS
+ *                    weights 1/3,2/3) for uniform speed; 3rd-order convergence with eps=h and loss of
+ *                    order with eps=1e-12 (:670, Fig. 15); App. C analytic theta solution (:697-731);
+ *                    flux conservation incl. polar caps (App. A :622-648)
+ *   assimilation     Eq. 8 (:131) closed form, Eq. 10-11 (:144-153) flux balance => net flux of dB is 0
+ *   PARITY UNPINNED against HipFT itself (no HipFT output in the container): which faces use upwind
+ *   next to the poles (reading U6), the stage-count rule (U9), eps_w = coordinate spacing (U11).
+ *   They are pinned oracle<->GPU by definition only; see DESIGN.md.
+ *
+ * Index convention: rows j = 0..nt+1, row 0 = north polar cap, row nt+1 = south
+ * polar cap, theta_j = j*dth, dth = pi/(nt+1); theta-faces j+1/2 (index j = 0..nt) at (j+1/2)*dth;
+ * columns k = 0..np-1, phi_k = k*dph, dph = 2*pi/np, periodic.  A full field is (nt+2)*np values,
+ * the two cap rows hold one value each, stored replicated.  (App. A :628.)
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifdef ORACLE_FP32
+typedef float real;
+#define SUF(n) n##_f32
+#else
+typedef double real;
+#define SUF(n) n##_f64
+#endif
+
+#define PI 3.14159265358979323846264338327950288
+
+/* unit conversions to R_sun and hours (R_sun = 6.96e10 cm, :292). */
+#define M_S_TO_RS_HR 5.172413793103448e-6
+#define KM2_S_TO_RS2_HR 7.43162901307967e-9
+
+typedef struct {
+    int nt, np, nr;
+    double dth, dph;
+    double radius_cm;
+    double *st;   /* sin(theta_j),        j = 0..nt+1 */
+    double *sth;  /* sin(theta_{j+1/2}),  j = 0..nt   */
+    double P;     /* polar prefactor, App. A :646 (exact form) */
+    double Apole; /* polar cap area 2*pi*(1-cos(dth/2)), App. A :642 */
+    double *nu;   /* [nr] diffusivity in R_sun^2/hr */
+    double *vt;   /* [nr][nt+1] v_theta at theta-faces, R_sun/hr (Eq. 4 :84) */
+    double *om;   /* [nr][nt+2] Omega = v_phi/sin(theta) at rows, rad/hr (Eq. 3 :78) */
+    real *B;      /* [nr][nt+2][np] state */
+} oracle_t;
+
+/* ------------------------------------------------------------------ tables */
+
+/* Step 0 of DESIGN.md: grid metric.  1-cos(x) is evaluated as 2 sin^2(x/2) (identical function,
+ * no cancellation); P*Apole == sin(dth/2) to round-off, which is what makes the cap update
+ * cancel the theta-face term of row 1 (flux conservation). */
+static void make_grid(oracle_t *o) {
+    int nt = o->nt;
+    o->dth = PI / (double)(nt + 1);
+    o->dph = 2.0 * PI / (double)o->np;
+    for (int j = 0; j <= nt + 1; j++) o->st[j] = sin((double)j * o->dth);
+    for (int j = 0; j <= nt; j++) o->sth[j] = sin(((double)j + 0.5) * o->dth);
+    double s4 = sin(0.25 * o->dth);
+    double one_minus_cos = 2.0 * s4 * s4;
+    o->Apole = 2.0 * PI * one_minus_cos;
+    o->P = sin(0.5 * o->dth) / (2.0 * PI * one_minus_cos);
+}
+
+/* params per realization: eta_km2_s, d0, d2, d4, m1, m3, m5 (Eq. 3, 4, 6; units m/s, km^2/s). */
+static void make_flow(oracle_t *o, int r, const double *p) {
+    int nt = o->nt;
+    o->nu[r] = p[0] * KM2_S_TO_RS2_HR;
+    double d0 = p[1], d2 = p[2], d4 = p[3], m1 = p[4], m3 = p[5], m5 = p[6];
+    for (int j = 0; j <= nt; j++) { /* Eq. 4 at the face angle */
+        double th = ((double)j + 0.5) * o->dth;
+        double c = cos(th), s = sin(th);
+        o->vt[(size_t)r * (nt + 1) + j] = -(m1 * c + m3 * c * c * c + m5 * c * c * c * c * c) * s * M_S_TO_RS_HR;
+    }
+    for (int j = 0; j <= nt + 1; j++) { /* Eq. 3 divided by sin(theta) */
+        double c = cos((double)j * o->dth);
+        o->om[(size_t)r * (nt + 2) + j] = (d0 + d2 * c * c + d4 * c * c * c * c) * M_S_TO_RS_HR;
+    }
+}
+
+void *SUF(sft_oracle_create)(int nt, int np, int nr, const double *params /*[nr][7]*/, double radius_cm) {
+    oracle_t *o = (oracle_t *)calloc(1, sizeof(oracle_t));
+    o->nt = nt; o->np = np; o->nr = nr; o->radius_cm = radius_cm;
+    o->st = (double *)calloc(nt + 2, sizeof(double));
+    o->sth = (double *)calloc(nt + 1, sizeof(double));
+    o->nu = (double *)calloc(nr, sizeof(double));
+    o->vt = (double *)calloc((size_t)nr * (nt + 1), sizeof(double));
+    o->om = (double *)calloc((size_t)nr * (nt + 2), sizeof(double));
+    o->B = (real *)calloc((size_t)nr * (nt + 2) * np, sizeof(real));
+    make_grid(o);
+    for (int r = 0; r < nr; r++) make_flow(o, r, params + 7 * r);
+    return o;
+}
+
+void SUF(sft_oracle_destroy)(void *h) {
+    oracle_t *o = (oracle_t *)h;
+    free(o->st); free(o->sth); free(o->nu); free(o->vt); free(o->om); free(o->B); free(o);
+}
+
+/* Custom per-row flow tables (needed for the App. C constant-v_theta test, :703): vt in R_sun/hr at
+ * the nt+1 theta-faces, om in rad/hr at the nt+2 rows. */
+void SUF(sft_oracle_set_flow_tables)(void *h, int r, const double *vt, const double *om) {
+    oracle_t *o = (oracle_t *)h;
+    memcpy(o->vt + (size_t)r * (o->nt + 1), vt, sizeof(double) * (o->nt + 1));
+    memcpy(o->om + (size_t)r * (o->nt + 2), om, sizeof(double) * (o->nt + 2));
+}
+
+void SUF(sft_oracle_get_tables)(void *h, int r, double *st, double *sth, double *vt, double *om, double *scal /*[5]: dth,dph,P,Apole,nu*/) {
+    oracle_t *o = (oracle_t *)h;
+    memcpy(st, o->st, sizeof(double) * (o->nt + 2));
+    memcpy(sth, o->sth, sizeof(double) * (o->nt + 1));
+    memcpy(vt, o->vt + (size_t)r * (o->nt + 1), sizeof(double) * (o->nt + 1));
+    memcpy(om, o->om + (size_t)r * (o->nt + 2), sizeof(double) * (o->nt + 2));
+    scal[0] = o->dth; scal[1] = o->dph; scal[2] = o->P; scal[3] = o->Apole; scal[4] = o->nu[r];
+}
+
+/* ------------------------------------------------------------ small helpers */
+
+static real *field(oracle_t *o, int r) { return o->B + (size_t)r * (o->nt + 2) * o->np; }
+static size_t fsize(const oracle_t *o) { return (size_t)(o->nt + 2) * o->np; }
+
+/* Kahan-compensated sum in index order, fp64 accumulator. */
+typedef struct { double s, c; } kahan_t;
+static void kadd(kahan_t *k, double x) {
+    double y = x - k->c;
+    double t = k->s + y;
+    k->c = (t - k->s) - y;
+    k->s = t;
+}
+
+static void fill_row(real *row, int np, real v) { for (int k = 0; k < np; k++) row[k] = v; }
+
+/* mean of a row over phi (dph-weighted mean on a uniform grid = arithmetic mean) */
+static double row_mean(const real *row, int np) {
+    kahan_t a = {0.0, 0.0};
+    for (int k = 0; k < np; k++) kadd(&a, (double)row[k]);
+    return a.s / (double)np;
+}
+
+/* ----------------------------------------------------------------- set/get */
+
+/* User maps are [nt][np] (rows 1..nt).  Caps := dph-weighted mean of the adjacent row
+ * (reading U18: "pole-cell averaging"). r = -1 broadcasts to all realizations. */
+void SUF(sft_oracle_set_map)(void *h, int r, const real *map) {
+    oracle_t *o = (oracle_t *)h;
+    int nt = o->nt, np = o->np;
+    for (int q = 0; q < o->nr; q++) {
+        if (r >= 0 && q != r) continue;
+        real *B = field(o, q);
+        memcpy(B + np, map, sizeof(real) * (size_t)nt * np);
+        fill_row(B, np, (real)row_mean(B + np, np));
+        fill_row(B + (size_t)(nt + 1) * np, np, (real)row_mean(B + (size_t)nt * np, np));
+    }
+}
+
+void SUF(sft_oracle_get_map)(void *h, int r, real *out) {
+    oracle_t *o = (oracle_t *)h;
+    memcpy(out, field(o, r) + o->np, sizeof(real) * (size_t)o->nt * o->np);
+}
+
+/* full (nt+2)*np field incl. replicated cap rows -- for tests */
+void SUF(sft_oracle_get_full)(void *h, int r, real *out) {
+    oracle_t *o = (oracle_t *)h;
+    memcpy(out, field(o, r), sizeof(real) * fsize(o));
+}
+void SUF(sft_oracle_set_full)(void *h, int r, const real *in) {
+    oracle_t *o = (oracle_t *)h;
+    memcpy(field(o, r), in, sizeof(real) * fsize(o));
+}
+
+/* ------------------------------------------------------ diffusion operator */
+
+/* Step 4: L(B) = discrete div(nu grad B), Eq. 27/28 (:438-460) with spatially constant nu and
+ * uniform spacing:
+ *   rows 1..nt:  c+_j (B[j+1,k]-B[j,k]) - c-_j (B[j,k]-B[j-1,k]) + cphi_j (B[j,k+1] - 2 B[j,k] + B[j,k-1])
+ *   c+-_j = nu sin(theta_{j+-1/2}) / (sin(theta_j) dth^2),  cphi_j = nu / (sin^2(theta_j) dph^2)
+ *   caps (App. A :624-648, F = nu dB/dtheta by central differences at the first half-mesh point):
+ *     north: P (nu/dth) sum_k (B[1,k]-B[0]) dph ;  south: P (nu/dth) sum_k (B[nt,k]-B[nt+1]) dph
+ * Row coefficients are formed in fp64 and rounded once to `real`. */
+static void diffusion_op(const oracle_t *o, int r, const real *B, real *out) {
+    int nt = o->nt, np = o->np;
+    double nu = o->nu[r];
+    #pragma omp parallel for schedule(static)
+    for (int j = 1; j <= nt; j++) {
+        real cp = (real)(nu * o->sth[j] / (o->st[j] * o->dth * o->dth));
+        real cm = (real)(nu * o->sth[j - 1] / (o->st[j] * o->dth * o->dth));
+        real cf = (real)(nu / (o->st[j] * o->st[j] * o->dph * o->dph));
+        const real *Bc = B + (size_t)j * np, *Bn = Bc - np, *Bs = Bc + np; /* Bn = row j-1 (towards north), Bs = row j+1 */
+        real *oc = out + (size_t)j * np;
+        for (int k = 0; k < np; k++) {
+            int kw = (k + np - 1) % np, ke = (k + 1) % np;
+            real tth = cp * (Bs[k] - Bc[k]) - cm * (Bc[k] - Bn[k]);
+            real tph = cf * (Bc[ke] - (real)2 * Bc[k] + Bc[kw]);
+            oc[k] = tth + tph;
+        }
+    }
+    double capc = o->P * (nu / o->dth) * o->dph;
+    kahan_t a = {0, 0}, b = {0, 0};
+    for (int k = 0; k < np; k++) {
+        kadd(&a, (double)(B[np + k] - B[0]));
+        kadd(&b, (double)(B[(size_t)nt * np + k] - B[(size_t)(nt + 1) * np]));
+    }
+    fill_row(out, np, (real)(capc * a.s));
+    fill_row(out + (size_t)(nt + 1) * np, np, (real)(capc * b.s));
+}
+
+void SUF(sft_oracle_diffusion_op)(void *h, int r, const real *in, real *out) {
+    diffusion_op((oracle_t *)h, r, in, out);
+}
+
+/* Step 5: Euler limit.  Gershgorin: spectral radius <= 2 max|diag|, dt_expl = 2/rho =
+ * 1 / max( max_j (c+_j + c-_j + 2 cphi_j), 2 pi P nu / dth ), with nu = max_r nu_r (reading U8). */
+static double diffusion_dt_expl(const oracle_t *o) {
+    double nu = 0.0;
+    for (int r = 0; r < o->nr; r++) if (o->nu[r] > nu) nu = o->nu[r];
+    double dmax = 2.0 * PI * o->P * nu / o->dth;
+    for (int j = 1; j <= o->nt; j++) {
+        double cp = nu * o->sth[j] / (o->st[j] * o->dth * o->dth);
+        double cm = nu * o->sth[j - 1] / (o->st[j] * o->dth * o->dth);
+        double cf = nu / (o->st[j] * o->st[j] * o->dph * o->dph);
+        double d = cp + cm + 2.0 * cf;
+        if (d > dmax) dmax = d;
+    }
+    return dmax > 0.0 ? 1.0 / dmax : INFINITY;
+}
+
+/* ------------------------------------------------------------ STS schemes */
+
+/* Step 7 coefficient families (reading U7).  scheme 2 = RKL2 (Legendre; Meyer et al. 2014 via
+ * PAPER.md:470-474), scheme 3 = RKG2(3/2) (Gegenbauer lambda = 3/2, normalised G_j(1) = 1; Skaras et
+ * al. 2021 via :472).  Arrays are indexed 0..s.  mu[j], nu[j], mut[j] (mu-tilde), gt[j] (gamma-tilde)
+ * for j >= 2; mut[1] = b_1 w_1.  b_0 = b_1 = b_2.  a_j = 1 - b_j. */
+static double sts_b(int scheme, int j) {
+    if (j < 2) j = 2;
+    double dj = (double)j;
+    if (scheme == 2) return (dj * dj + dj - 2.0) / (2.0 * dj * (dj + 1.0));
+    return 2.0 * (dj - 1.0) * (dj + 4.0) / (3.0 * dj * (dj + 3.0));
+}
+static double sts_w1(int scheme, int s) {
+    double ds = (double)s;
+    if (scheme == 2) return 4.0 / (ds * ds + ds - 2.0);
+    return 6.0 / ((ds - 1.0) * (ds + 4.0));
+}
+void SUF(sft_oracle_sts_coeffs)(int scheme, int s, double *mu, double *nu, double *mut, double *gt, double *b) {
+    double w1 = sts_w1(scheme, s);
+    for (int j = 0; j <= s; j++) { b[j] = sts_b(scheme, j); mu[j] = nu[j] = mut[j] = gt[j] = 0.0; }
+    mut[1] = b[1] * w1;
+    for (int j = 2; j <= s; j++) {
+        double dj = (double)j, A, Bc;
+        if (scheme == 2) { A = (2.0 * dj - 1.0) / dj; Bc = (dj - 1.0) / dj; }
+        else             { A = (2.0 * dj + 1.0) / (dj + 2.0); Bc = (dj - 1.0) / (dj + 2.0); }
+        mu[j] = A * b[j] / b[j - 1];
+        nu[j] = -Bc * b[j] / b[j - 2];
+        mut[j] = mu[j] * w1;
+        gt[j] = -(1.0 - b[j - 1]) * mut[j];
+    }
+}
+
+/* Step 6 (reading U9): smallest s >= 2 with dt <= dt_expl * C(s); RKL2: C = (s^2+s-2)/4;
+ * RKG2(3/2): C = (s^2+3s-4)/6.  One s for all realizations. */
+static int sts_stage_count(int scheme, double dt, double dt_expl) {
+    int s = 2;
+    for (;;) {
+        double ds = (double)s;
+        double C = (scheme == 2) ? (ds * ds + ds - 2.0) / 4.0 : (ds * ds + 3.0 * ds - 4.0) / 6.0;
+        if (dt <= dt_expl * C) return s;
+        s++;
+        if (s > 10000000) return -1;
+    }
+}
+
+int SUF(sft_oracle_sts_stage_count)(void *h, double dt, int scheme) {
+    return sts_stage_count(scheme, dt, diffusion_dt_expl((oracle_t *)h));
+}
+
+/* One STS step of size dt with s stages, in the deviation form:
+ *   delta_j = Y_j - Y_0 ;  delta_0 = 0 ;  delta_1 = mut_1 dt L(Y_0)
+ *   delta_j = mu_j delta_{j-1} + nu_j delta_{j-2} + mut_j dt L(delta_{j-1}) + mut_j b_{j-1} dt L(Y_0)
+ *   Y_s = Y_0 + delta_s
+ * which is the textbook recurrence
+ *   Y_j = mu_j Y_{j-1} + nu_j Y_{j-2} + (1-mu_j-nu_j) Y_0 + mut_j dt L(Y_{j-1}) + gt_j dt L(Y_0)
+ * rewritten using the linearity of L (caps included) and mut_j + gt_j = mut_j b_{j-1}.
+ * Per-stage scalars are formed in fp64 and rounded once to `real`. */
+static void sts_step(oracle_t *o, int r, int scheme, int s, double dt) {
+    size_t n = fsize(o);
+    real *Y = field(o, r);
+    real *LY0 = (real *)malloc(n * sizeof(real)), *d1 = (real *)malloc(n * sizeof(real));
+    real *d2 = (real *)calloc(n, sizeof(real)), *Ld = (real *)malloc(n * sizeof(real));
+    double *mu = (double *)malloc((s + 1) * sizeof(double)), *nu = (double *)malloc((s + 1) * sizeof(double));
+    double *mut = (double *)malloc((s + 1) * sizeof(double)), *gt = (double *)malloc((s + 1) * sizeof(double));
+    double *b = (double *)malloc((s + 1) * sizeof(double));
+    SUF(sft_oracle_sts_coeffs)(scheme, s, mu, nu, mut, gt, b);
+    diffusion_op(o, r, Y, LY0);
+    real a1 = (real)(mut[1] * dt);
+    for (size_t i = 0; i < n; i++) d1[i] = a1 * LY0[i];
+    for (int j = 2; j <= s; j++) {
+        diffusion_op(o, r, d1, Ld);
+        real mj = (real)mu[j], nj = (real)nu[j], aj = (real)(mut[j] * dt), gj = (real)(mut[j] * b[j - 1] * dt);
+        #pragma omp parallel for schedule(static)
+        for (size_t i = 0; i < n; i++) {
+            real dn = mj * d1[i] + nj * d2[i] + aj * Ld[i] + gj * LY0[i];
+            d2[i] = d1[i];
+            d1[i] = dn;
+        }
+    }
+    for (size_t i = 0; i < n; i++) Y[i] = Y[i] + d1[i];
+    free(LY0); free(d1); free(d2); free(Ld); free(mu); free(nu); free(mut); free(gt); free(b);
+}
+
+/* The same step in the textbook form (used only by tests to pin the deviation form). */
+static void sts_step_textbook(oracle_t *o, int r, int scheme, int s, double dt) {
+    size_t n = fsize(o);
+    real *Y0 = field(o, r);
+    real *LY0 = (real *)malloc(n * sizeof(real)), *y1 = (real *)malloc(n * sizeof(real));
+    real *y2 = (real *)malloc(n * sizeof(real)), *Ly = (real *)malloc(n * sizeof(real));
+    double *mu = (double *)malloc((s + 1) * sizeof(double)), *nu = (double *)malloc((s + 1) * sizeof(double));
+    double *mut = (double *)malloc((s + 1) * sizeof(double)), *gt = (double *)malloc((s + 1) * sizeof(double));
+    double *b = (double *)malloc((s + 1) * sizeof(double));
+    SUF(sft_oracle_sts_coeffs)(scheme, s, mu, nu, mut, gt, b);
+    diffusion_op(o, r, Y0, LY0);
+    real a1 = (real)(mut[1] * dt);
+    for (size_t i = 0; i < n; i++) { y2[i] = Y0[i]; y1[i] = Y0[i] + a1 * LY0[i]; }
+    for (int j = 2; j <= s; j++) {
+        diffusion_op(o, r, y1, Ly);
+        real mj = (real)mu[j], nj = (real)nu[j], cj = (real)(1.0 - mu[j] - nu[j]);
+        real aj = (real)(mut[j] * dt), gj = (real)(gt[j] * dt);
+        for (size_t i = 0; i < n; i++) {
+            real yn = mj * y1[i] + nj * y2[i] + cj * Y0[i] + aj * Ly[i] + gj * LY0[i];
+            y2[i] = y1[i];
+            y1[i] = yn;
+        }
+    }
+    memcpy(Y0, y1, n * sizeof(real));
+    free(LY0); free(y1); free(y2); free(Ly); free(mu); free(nu); free(mut); free(gt); free(b);
+}
+
+/* explicit Euler diffusion step (reference scheme, :474) */
+static void diffusion_euler_step(oracle_t *o, int r, double dt) {
+    size_t n = fsize(o);
+    real *Y = field(o, r), *LY = (real *)malloc(n * sizeof(real));
+    diffusion_op(o, r, Y, LY);
+    real a = (real)dt;
+    for (size_t i = 0; i < n; i++) Y[i] = Y[i] + a * LY[i];
+    free(LY);
+}
+
+/* --------------------------------------------------------------- advection */
+
+/* Upwind flux (:362-366 with alpha_uw = 1): F_{i-1/2} = v B_{i-1} if v > 0, v B_i if v < 0, 0 if v = 0. */
+static real upwind_flux(real v, real Bm, real Bp) {
+    if (v > (real)0) return v * Bm;
+    if (v < (real)0) return v * Bp;
+    return (real)0;
+}
+
+/* WENO3-CS(h) face value from three split fluxes (App. B :658-676 on a uniform grid: D^{c/cm} =
+ * D^{c/cp} = 1/2, D^{p/t} = D^{m/t} = 1/3, D^{cp/t} = D^{cm/t} = 2/3, reading U12):
+ *   p0 = 3/2 f_near - 1/2 f_far ; p1 = 1/2 f_near + 1/2 f_other
+ *   beta0 = (f_near - f_far)^2 ; beta1 = (f_other - f_near)^2
+ *   w0 = (1/3)/(eps+beta0)^2 ; w1 = (2/3)/(eps+beta1)^2 ; u = (w0 p0 + w1 p1)/(w0 + w1)
+ * For u^- (right-moving, from LM): far = LM_{i-2}, near = LM_{i-1}, other = LM_i.
+ * For u^+ (left-moving, from LP):  far = LP_{i+1}, near = LP_i,     other = LP_{i-1}. */
+static real weno3_side(real far, real near, real other, real eps) {
+    real p0 = (real)1.5 * near - (real)0.5 * far;
+    real p1 = (real)0.5 * near + (real)0.5 * other;
+    real b0 = (near - far) * (near - far);
+    real b1 = (other - near) * (other - near);
+    real w0 = (real)(1.0 / 3.0) / ((eps + b0) * (eps + b0));
+    real w1 = (real)(2.0 / 3.0) / ((eps + b1) * (eps + b1));
+    return (w0 * p0 + w1 * p1) / (w0 + w1);
+}
+
+/* Steps 1-2: advection tendency F_A(B) = div_s(B v), :354, with
+ *   theta-faces 1/2, 3/2, nt-1/2, nt+1/2 upwind (:388, reading U6), all others WENO3-CS(h) with
+ *   LLF splitting (B2 :684): LP_i = B_i (v_{i+1/2} - alpha_i)/2, LM_i = B_i (v_{i-1/2} + alpha_i)/2,
+ *   alpha_i = max|v| over faces i-5/2..i+5/2 clipped to existing faces (:689);
+ *   phi-faces of rows 1..nt: WENO with the row speed v_phi = Omega_j sin(theta_j) at every face;
+ *   eps_w = dth for theta-faces, dph for phi-faces (:670, reading U11);
+ *   caps: north +P sum_k F_theta[1/2,k] dph, south -P sum_k F_theta[nt+1/2,k] dph (App. A :646, U5).
+ * flux_mode 1 = upwind everywhere, 2 = WENO3-CS(h), 3 = WENO3 with eps_w = 1e-12 (test only, Fig. 15).
+ * Ft: (nt+1)*np theta-face fluxes, Fp: (nt+2)*np phi-face fluxes, Fp[j][k] = flux at face k-1/2. */
+static void advection_tendency(const oracle_t *o, int r, const real *B, real *out, int flux_mode, real *Ft, real *Fp) {
+    int nt = o->nt, np = o->np;
+    const double *vtd = o->vt + (size_t)r * (nt + 1);
+    const double *omd = o->om + (size_t)r * (nt + 2);
+    real eps_t = (real)o->dth, eps_p = (real)o->dph;
+    if (flux_mode == 3) { eps_t = (real)1e-12; eps_p = (real)1e-12; }
+    real *vt = (real *)malloc((nt + 1) * sizeof(real));
+    real *al = (real *)malloc((nt + 2) * sizeof(real)); /* alpha_i for theta direction at rows */
+    for (int j = 0; j <= nt; j++) vt[j] = (real)vtd[j];
+    for (int i = 0; i <= nt + 1; i++) {
+        double a = 0.0;
+        for (int q = i - 3; q <= i + 2; q++) if (q >= 0 && q <= nt && fabs(vtd[q]) > a) a = fabs(vtd[q]);
+        al[i] = (real)a;
+    }
+    /* theta-face fluxes: face f lies between rows f and f+1 (cell i = f+1, face i-1/2) */
+    #pragma omp parallel for schedule(static)
+    for (int f = 0; f <= nt; f++) {
+        int use_upwind = (flux_mode == 1) || f <= 1 || f >= nt - 1;
+        for (int k = 0; k < np; k++) {
+            real F;
+            if (use_upwind) {
+                F = upwind_flux(vt[f], B[(size_t)f * np + k], B[(size_t)(f + 1) * np + k]);
+            } else {
+                int i = f + 1;
+                real LMm2 = (real)0.5 * B[(size_t)(i - 2) * np + k] * (vt[i - 3] + al[i - 2]);
+                real LMm1 = (real)0.5 * B[(size_t)(i - 1) * np + k] * (vt[i - 2] + al[i - 1]);
+                real LM0  = (real)0.5 * B[(size_t)(i    ) * np + k] * (vt[i - 1] + al[i    ]);
+                real LPp1 = (real)0.5 * B[(size_t)(i + 1) * np + k] * (vt[i + 1] - al[i + 1]);
+                real LP0  = (real)0.5 * B[(size_t)(i    ) * np + k] * (vt[i    ] - al[i    ]);
+                real LPm1 = (real)0.5 * B[(size_t)(i - 1) * np + k] * (vt[i - 1] - al[i - 1]);
+                real um = weno3_side(LMm2, LMm1, LM0, eps_t);
+                real up = weno3_side(LPp1, LP0, LPm1, eps_t);
+                F = up + um;
+            }
+            Ft[(size_t)f * np + k] = F;
+        }
+    }
+    /* phi-face fluxes for rows 1..nt: face k-1/2 lies between columns k-1 and k */
+    #pragma omp parallel for schedule(static)
+    for (int j = 1; j <= nt; j++) {
+        real v = (real)(omd[j] * o->st[j]);
+        real a = (real)fabs(omd[j] * o->st[j]);
+        const real *Bc = B + (size_t)j * np;
+        for (int k = 0; k < np; k++) {
+            int km2 = (k + np - 2) % np, km1 = (k + np - 1) % np, kp1 = (k + 1) % np;
+            real F;
+            if (flux_mode == 1) {
+                F = upwind_flux(v, Bc[km1], Bc[k]);
+            } else {
+                real LMm2 = (real)0.5 * Bc[km2] * (v + a), LMm1 = (real)0.5 * Bc[km1] * (v + a), LM0 = (real)0.5 * Bc[k] * (v + a);
+                real LPp1 = (real)0.5 * Bc[kp1] * (v - a), LP0 = (real)0.5 * Bc[k] * (v - a), LPm1 = (real)0.5 * Bc[km1] * (v - a);
+                real um = weno3_side(LMm2, LMm1, LM0, eps_p);
+                real up = weno3_side(LPp1, LP0, LPm1, eps_p);
+                F = up + um;
+            }
+            Fp[(size_t)j * np + k] = F;
+        }
+    }
+    /* divergence, rows 1..nt (:354) */
+    #pragma omp parallel for schedule(static)
+    for (int j = 1; j <= nt; j++) {
+        real sp = (real)o->sth[j], sm = (real)o->sth[j - 1];
+        real dt_den = (real)(o->st[j] * o->dth), dp_den = (real)(o->st[j] * o->dph);
+        for (int k = 0; k < np; k++) {
+            int kp1 = (k + 1) % np;
+            real tth = (sp * Ft[(size_t)j * np + k] - sm * Ft[(size_t)(j - 1) * np + k]) / dt_den;
+            real tph = (Fp[(size_t)j * np + kp1] - Fp[(size_t)j * np + k]) / dp_den;
+            out[(size_t)j * np + k] = tth + tph;
+        }
+    }
+    kahan_t a = {0, 0}, b = {0, 0};
+    for (int k = 0; k < np; k++) { kadd(&a, (double)Ft[k]); kadd(&b, (double)Ft[(size_t)nt * np + k]); }
+    fill_row(out, np, (real)(o->P * o->dph * a.s));
+    fill_row(out + (size_t)(nt + 1) * np, np, (real)(-(o->P * o->dph * b.s)));
+    free(vt); free(al);
+}
+
+void SUF(sft_oracle_advection_tendency)(void *h, int r, const real *in, real *out, int flux_mode) {
+    oracle_t *o = (oracle_t *)h;
+    real *Ft = (real *)malloc((size_t)(o->nt + 1) * o->np * sizeof(real));
+    real *Fp = (real *)calloc(fsize(o), sizeof(real));
+    advection_tendency(o, r, in, out, flux_mode, Ft, Fp);
+    free(Ft); free(Fp);
+}
+
+/* Step 3: advection time integrators.  adv_time 1 = forward Euler (Eq. 23 :396),
+ * 3 = SSPRK(3,3) (:412-416), 4 = SSPRK(4,3) (Eq. 25 :418-424). */
+static void advection_step(oracle_t *o, int r, int flux_mode, int adv_time, double dt) {
+    size_t n = fsize(o);
+    real *f = field(o, r);
+    real *T = (real *)malloc(n * sizeof(real)), *f1 = (real *)malloc(n * sizeof(real)), *f2 = (real *)malloc(n * sizeof(real));
+    real *Ft = (real *)malloc((size_t)(o->nt + 1) * o->np * sizeof(real)), *Fp = (real *)calloc(n, sizeof(real));
+    real h = (real)dt;
+    if (adv_time == 1) {
+        advection_tendency(o, r, f, T, flux_mode, Ft, Fp);
+        for (size_t i = 0; i < n; i++) f[i] = f[i] - h * T[i];
+    } else if (adv_time == 3) {
+        advection_tendency(o, r, f, T, flux_mode, Ft, Fp);
+        for (size_t i = 0; i < n; i++) f1[i] = f[i] - h * T[i];
+        advection_tendency(o, r, f1, T, flux_mode, Ft, Fp);
+        for (size_t i = 0; i < n; i++) f2[i] = (real)0.75 * f[i] + (real)0.25 * f1[i] - (real)0.25 * h * T[i];
+        advection_tendency(o, r, f2, T, flux_mode, Ft, Fp);
+        for (size_t i = 0; i < n; i++) f[i] = (real)(1.0 / 3.0) * f[i] + (real)(2.0 / 3.0) * f2[i] - (real)(2.0 / 3.0) * h * T[i];
+    } else {
+        advection_tendency(o, r, f, T, flux_mode, Ft, Fp);
+        for (size_t i = 0; i < n; i++) f1[i] = f[i] - (real)0.5 * h * T[i];
+        advection_tendency(o, r, f1, T, flux_mode, Ft, Fp);
+        for (size_t i = 0; i < n; i++) f2[i] = f1[i] - (real)0.5 * h * T[i];
+        advection_tendency(o, r, f2, T, flux_mode, Ft, Fp);
+        for (size_t i = 0; i < n; i++) f1[i] = (real)(2.0 / 3.0) * f[i] + (real)(1.0 / 3.0) * f2[i] - (real)(1.0 / 6.0) * h * T[i];
+        advection_tendency(o, r, f1, T, flux_mode, Ft, Fp);
+        for (size_t i = 0; i < n; i++) f[i] = f1[i] - (real)0.5 * h * T[i];
+    }
+    free(T); free(f1); free(f2); free(Ft); free(Fp);
+}
+
+/* Advective limit, Eq. 26 form (:430) with the velocities taken as the maximum of the flanking
+ * staggered values (:406): min over rows 1..nt and realizations of
+ *   [ max(|v_theta,j-1/2|, |v_theta,j+1/2|)/dth + |Omega_j|/dph ]^-1      (|v_phi|/(sin(theta) dph) = |Omega|/dph)
+ * No safety factor is applied here (reading U15: the caller multiplies by its CFL number). */
+static double advection_dt_limit(const oracle_t *o) {
+    double best = INFINITY;
+    for (int r = 0; r < o->nr; r++) {
+        const double *vt = o->vt + (size_t)r * (o->nt + 1), *om = o->om + (size_t)r * (o->nt + 2);
+        for (int j = 1; j <= o->nt; j++) {
+            double a = fabs(vt[j - 1]) > fabs(vt[j]) ? fabs(vt[j - 1]) : fabs(vt[j]);
+            double rate = a / o->dth + fabs(om[j]) / o->dph;
+            if (rate > 0.0 && 1.0 / rate < best) best = 1.0 / rate;
+        }
+    }
+    return best;
+}
+
+void SUF(sft_oracle_stable_dt)(void *h, double *dt_adv, double *dt_diff) {
+    *dt_adv = advection_dt_limit((oracle_t *)h);
+    *dt_diff = diffusion_dt_expl((oracle_t *)h);
+}
+
+/* ------------------------------------------------------------------- step */
+
+/* Step 8: n_steps of B^{n+1} = D(A(B^n)) (Eq. 21 :308-313, S omitted).
+ * adv_flux 0 off / 1 upwind / 2 WENO3-CS(h) / 3 WENO3 eps=1e-12 (test only);
+ * adv_time 1 / 3 / 4; diff_time 0 off / 1 Euler / 2 RKL2 / 3 RKG2(3/2) / 12, 13 = textbook-form
+ * RKL2 / RKG2 (test only); sts_stages 0 = auto (Step 6) else forced.  Returns the stage count used. */
+int SUF(sft_oracle_step)(void *h, int n_steps, double dt, int adv_flux, int adv_time, int diff_time, int sts_stages) {
+    oracle_t *o = (oracle_t *)h;
+    int s = 0;
+    if (diff_time == 2 || diff_time == 3 || diff_time == 12 || diff_time == 13) {
+        int scheme = diff_time % 10;
+        s = sts_stages > 0 ? sts_stages : sts_stage_count(scheme, dt, diffusion_dt_expl(o));
+        if (s < 2) return -1;
+    }
+    for (int n = 0; n < n_steps; n++) {
+        for (int r = 0; r < o->nr; r++) {
+            if (adv_flux != 0) advection_step(o, r, adv_flux, adv_time, dt);
+            if (diff_time == 1) diffusion_euler_step(o, r, dt);
+            else if (diff_time == 2 || diff_time == 3) sts_step(o, r, diff_time, s, dt);
+            else if (diff_time == 12 || diff_time == 13) sts_step_textbook(o, r, diff_time % 10, s, dt);
+        }
+    }
+    return s;
+}
+
+/* ----------------------------------------------------- assimilation, Step 9 */
+
+/* Eq. 8 (:131): B <- F B_d + (1-F) B on rows 1..nt; flags bit0: flux-balanced form Eq. 10-11
+ * (:144-153): dB = F (B_d - B); Phi+ / Phi- = surface integrals of dB over dB > 0 / dB <= 0;
+ * dB > 0 is divided by sqrt|Phi+/Phi-|, dB <= 0 multiplied by it; if either is 0, no scaling.
+ * Caps (reading U18): cap obs and cap weight are the dph-weighted means of the adjacent row's obs and
+ * weight, the cap is blended with them like any cell (one value, stored replicated).
+ * obs, w: [nr or 1][nt][np] (`shared` != 0: one map for all realizations). Quadrature (reading U19):
+ * dA_j = sin(theta_j) dth dph, cap area Apole. */
+void SUF(sft_oracle_assimilate)(void *h, const real *obs, const real *w, int shared, int flags) {
+    oracle_t *o = (oracle_t *)h;
+    int nt = o->nt, np = o->np;
+    size_t mapn = (size_t)nt * np;
+    for (int r = 0; r < o->nr; r++) {
+        const real *ob = obs + (shared ? 0 : (size_t)r * mapn);
+        const real *wt = w + (shared ? 0 : (size_t)r * mapn);
+        real *B = field(o, r);
+        real obN = (real)row_mean(ob, np), obS = (real)row_mean(ob + (size_t)(nt - 1) * np, np);
+        real wN = (real)row_mean(wt, np), wS = (real)row_mean(wt + (size_t)(nt - 1) * np, np);
+        if (!(flags & 1)) {
+            for (int j = 1; j <= nt; j++)
+                for (int k = 0; k < np; k++) {
+                    real F = wt[(size_t)(j - 1) * np + k], Bd = ob[(size_t)(j - 1) * np + k];
+                    B[(size_t)j * np + k] = F * Bd + ((real)1 - F) * B[(size_t)j * np + k];
+                }
+            fill_row(B, np, wN * obN + ((real)1 - wN) * B[0]);
+            fill_row(B + (size_t)(nt + 1) * np, np, wS * obS + ((real)1 - wS) * B[(size_t)(nt + 1) * np]);
+        } else {
+            kahan_t pp = {0, 0}, pm = {0, 0};
+            real dN = wN * (obN - B[0]), dS = wS * (obS - B[(size_t)(nt + 1) * np]);
+            if (dN > (real)0) kadd(&pp, (double)dN * o->Apole); else kadd(&pm, (double)dN * o->Apole);
+            for (int j = 1; j <= nt; j++) {
+                double dA = o->st[j] * o->dth * o->dph;
+                for (int k = 0; k < np; k++) {
+                    real d = wt[(size_t)(j - 1) * np + k] * (ob[(size_t)(j - 1) * np + k] - B[(size_t)j * np + k]);
+                    if (d > (real)0) kadd(&pp, (double)d * dA); else kadd(&pm, (double)d * dA);
+                }
+            }
+            if (dS > (real)0) kadd(&pp, (double)dS * o->Apole); else kadd(&pm, (double)dS * o->Apole);
+            real sc = (real)1;
+            if (pp.s != 0.0 && pm.s != 0.0) sc = (real)sqrt(fabs(pp.s / pm.s));
+            for (int j = 1; j <= nt; j++)
+                for (int k = 0; k < np; k++) {
+                    real d = wt[(size_t)(j - 1) * np + k] * (ob[(size_t)(j - 1) * np + k] - B[(size_t)j * np + k]);
+                    d = (d > (real)0) ? d / sc : d * sc;
+                    B[(size_t)j * np + k] = B[(size_t)j * np + k] + d;
+                }
+            dN = (dN > (real)0) ? dN / sc : dN * sc;
+            dS = (dS > (real)0) ? dS / sc : dS * sc;
+            fill_row(B, np, B[0] + dN);
+            fill_row(B + (size_t)(nt + 1) * np, np, B[(size_t)(nt + 1) * np] + dS);
+        }
+    }
+}
+
+/* ------------------------------------------------------ diagnostics, Step 10 */
+
+/* :225-230: Phi+ = int_{B>0} B dOmega, Phi- = int_{B<0} B dOmega; out[r] = {signed = Phi+ + Phi-,
+ * unsigned = Phi+ - Phi-, Phi+, Phi-}, midpoint quadrature dA_j = sin(theta_j) dth dph plus the two
+ * caps with area Apole (reading U19), times radius_cm^2 (Mx if B is in Gauss; 1 = unit sphere). */
+void SUF(sft_oracle_diagnostics)(void *h, double *out /*[nr][4]*/) {
+    oracle_t *o = (oracle_t *)h;
+    int nt = o->nt, np = o->np;
+    double r2 = o->radius_cm * o->radius_cm;
+    for (int r = 0; r < o->nr; r++) {
+        const real *B = field(o, r);
+        kahan_t pp = {0, 0}, pm = {0, 0};
+        double c0 = (double)B[0];
+        if (c0 > 0) kadd(&pp, c0 * o->Apole); else if (c0 < 0) kadd(&pm, c0 * o->Apole);
+        for (int j = 1; j <= nt; j++) {
+            double dA = o->st[j] * o->dth * o->dph;
+            for (int k = 0; k < np; k++) {
+                double v = (double)B[(size_t)j * np + k];
+                if (v > 0) kadd(&pp, v * dA); else if (v < 0) kadd(&pm, v * dA);
+            }
+        }
+        double c1 = (double)B[(size_t)(nt + 1) * np];
+        if (c1 > 0) kadd(&pp, c1 * o->Apole); else if (c1 < 0) kadd(&pm, c1 * o->Apole);
+        out[4 * r + 0] = (pp.s + pm.s) * r2;
+        out[4 * r + 1] = (pp.s - pm.s) * r2;
+        out[4 * r + 2] = pp.s * r2;
+        out[4 * r + 3] = pm.s * r2;
+    }
+}
