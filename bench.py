@@ -1,0 +1,257 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the HipFT time-stepping hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3] [--dtype f64|f32]
+
+A "step" is one pass of the whole hot path -- hft_step(1, dt): SSPRK(4,3) WENO3 advection + s RKG2 super-time-step
+stages + polar caps -- over all realizations of the workload.  metric = cell-updates/s =
+realizations x n_theta x n_phi x steps / seconds (BASELINE.json), inputs resident in HBM; `e2e` is the same
+metric through the C ABI with HOST buffers (pinned H2D of the maps and D2H of the result inside the timed
+region).  Multi-GPU (torchrun): realizations are independent, every rank advances its own
+ensemble shard with no data-path collective ("scaling": "weak"); time = max over ranks.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+import torch
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2501_06377_b200 import workloads as wl  # noqa: E402
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json, torch copy)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.th.join(timeout=2)
+        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 6 and r[2 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_sample(w, dtype, n_steps, dt, s):
+    """The CPU oracle, as it stands, on ONE realization of the workload for n_steps steps."""
+    from oracle import sft_oracle as orc
+    npdt = np.float64 if dtype == "f64" else np.float32
+    o = orc.Oracle(w.n_theta, w.n_phi, w.params[:1], dtype=npdt)
+    m = wl.bipolar_map(w.n_theta, w.n_phi, w.n_pairs, w.map_seed + 1000, background_g=w.background_g)
+    o.set_map(0, m.numpy().astype(npdt))
+    if dt is None:
+        dt, _, _ = wl.plan(w, *o.stable_dt())
+        s = 0
+    t0 = time.perf_counter()
+    o.step(n_steps, dt, sts_stages=s)
+    el = time.perf_counter() - t0
+    return w.n_theta * w.n_phi * n_steps / el, el, orc.threads()
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle timed on the host cores; each step = one realization, one time step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import sft_oracle as orc
+    npdt = np.float64 if args.dtype == "f64" else np.float32
+    o = orc.Oracle(w.n_theta, w.n_phi, w.params, dtype=npdt)      # all realizations -> the ensemble's dt and s
+    dt, _, _ = wl.plan(w, *o.stable_dt())
+    s = o.sts_stage_count(dt)
+    o.close()
+    steps, warm = max(1, args.steps), max(0, min(args.warmup, 1))
+    if warm:
+        oracle_sample(w, args.dtype, 1, dt, s)
+    rate, el, thr = oracle_sample(w, args.dtype, steps, dt, s)
+    sample = f"1 of {w.n_real} realizations x {steps} step(s) of the full grid, s={s} stages/step"
+    print(json.dumps({
+        "impl": "reference", "metric": "cell-updates/s", "value": rate, "unit": "cell-updates/s", "n_gpus": args.gpus,
+        "steps": steps, "warmup": warm, "ms_per_step": 1e3 * el / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": w.name, "grid": [w.n_theta, w.n_phi], "realizations_timed": 1, "dt_hours": dt, "sts_stages": s},
+        "cpu_baseline": {"value": rate, "unit": "cell-updates/s", "cores": thr, "kind": "oracle", "sample": sample},
+        "e2e": {"value": rate, "unit": "cell-updates/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=4)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--sts-block", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--also-f32", action="store_true", help="add a second timed run in fp32 to the JSON line")
+    args = ap.parse_args()
+    w = wl.config(args.config, args.dtype)
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    from paper_2501_06377_b200 import hft
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed_run(dtype, with_extras):
+        wd = wl.config(args.config, dtype)
+        ctx = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, device=f"cuda:{local}")
+        maps = wl.initial_maps(wd, device=f"cuda:{local}").to(ctx.tdtype).contiguous()
+        ctx.set_map(-1, maps[0]) if not wd.per_real_maps else [ctx.set_map(r, maps[r]) for r in range(wd.n_real)]
+        dt, n_cfg, per = wl.plan(wd, *ctx.stable_dt())
+        s = ctx.sts_stage_count(dt)
+        cells = wd.n_real * wd.n_theta * wd.n_phi
+        for _ in range(args.warmup):
+            ctx.step(1, dt)
+        barrier()
+        sampler = ClockSampler(local)
+        if rank == 0 and with_extras:
+            sampler.start()
+        ctx.profile_kernels(1)
+        l0 = ctx.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            ctx.step(1, dt)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        launches = ctx.launch_count() - l0
+        kms, kn = ctx.kernel_time()
+        ctx.profile_kernels(0)
+        clocks = sampler.stop() if (rank == 0 and with_extras) else None
+        if dist is not None:
+            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = t.item()
+        res = dict(ms=ms, value=world * cells * args.steps / (ms * 1e-3), launches=launches, dt=dt, s=s, cells=cells,
+                   kernel_ms=(kms / kn if kn else None), kernel_samples=kn, clocks=clocks, wd=wd)
+        # ---- end-to-end through the C ABI with host buffers
+        if with_extras and not args.no_e2e:
+            host_in = maps.cpu().pin_memory()
+            host_out = torch.empty_like(host_in).pin_memory()
+            dev_in, dev_out = torch.empty_like(maps), torch.empty_like(maps)
+            n_e2e = max(1, min(args.steps, 2))
+            barrier()
+            t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
+            t0.record()
+            for _ in range(n_e2e):
+                dev_in.copy_(host_in, non_blocking=True)
+                for r in range(wd.n_real):
+                    ctx.set_map(r, dev_in[r])
+                ctx.step(1, dt)
+                ctx.get_map(-1, out=dev_out)
+                host_out.copy_(dev_out, non_blocking=True)
+            t1.record()
+            barrier()
+            ems = t0.elapsed_time(t1)
+            if dist is not None:
+                t = torch.tensor([ems], device="cuda", dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                ems = t.item()
+            res["e2e"] = {"value": world * cells * n_e2e / (ems * 1e-3), "unit": "cell-updates/s",
+                          "h2d_bytes_per_step": host_in.numel() * host_in.element_size(),
+                          "d2h_bytes_per_step": host_out.numel() * host_out.element_size(), "steps": n_e2e}
+            assert torch.isfinite(host_out).all()
+        kb_used = os.environ.get("HFT_STS_BLOCK_USED")
+        ctx.close()
+        return res
+
+    res = timed_run(args.dtype, True)
+    wd = res["wd"]
+    wbytes = 8 if args.dtype == "f64" else 4
+    peak, peak_src = peaks()
+    # algorithmic bytes: 4 array passes per STS stage, 9 per SSPRK(4,3) advection step
+    b_alg_step = (9 + 4 * res["s"]) * wbytes
+    frac_step = res["value"] / world * b_alg_step / (peak * 1e9)
+    out = {
+        "metric": "cell-updates/s", "value": res["value"], "unit": "cell-updates/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": res["ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+        "config": {"workload": wd.name, "grid": [wd.n_theta, wd.n_phi], "realizations_per_gpu": wd.n_real,
+                   "dt_hours": res["dt"], "sts_stages": res["s"], "adv": "WENO3-CS(h)+SSPRK(4,3)", "diff": "RKG2(3/2)",
+                   "l2": "inputs larger than L2 (arrays of %.0f MiB each)" % (wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes / 2**20),
+                   "sts_block": args.sts_block, "b_alg_bytes_per_cell_update": b_alg_step,
+                   "hbm_roofline_frac_whole_step": frac_step},
+        "gpu_launches": res["launches"],
+        "clocks": res["clocks"],
+    }
+    if res.get("e2e"):
+        out["e2e"] = res["e2e"]
+    if res["kernel_ms"]:
+        # dominant kernel: the STS stage kernel; algorithmic bytes per launch = 4 passes x field bytes x stages per launch
+        stages_per_launch = max(1, round(res["s"] * args.steps / max(1, res["launches"] - 9 * args.steps)))
+        field_bytes = wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes
+        ach = 4 * field_bytes * stages_per_launch / (res["kernel_ms"] * 1e-3) / 1e9
+        out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                           "kernel": "k_sts_stage", "stages_per_launch": stages_per_launch, "avg_launch_ms": res["kernel_ms"],
+                           "sampled_launches": res["kernel_samples"], "peak_source": peak_src}
+    if args.also_f32 and args.dtype == "f64":
+        r32 = timed_run("f32", False)
+        out["also_f32"] = {"value": r32["value"], "ms_per_step": r32["ms"] / args.steps, "sts_stages": r32["s"],
+                           "hbm_roofline_frac_whole_step": r32["value"] / world * (9 + 4 * r32["s"]) * 4 / (peak * 1e9)}
+    if rank == 0:
+        if not args.no_cpu_baseline:
+            n_or = 2 if wd.n_theta >= 1024 else 8
+            rate, el, thr = oracle_sample(wd, args.dtype, n_or, res["dt"], res["s"])
+            out["cpu_baseline"] = {"value": rate, "unit": "cell-updates/s", "cores": thr, "kind": "oracle",
+                                   "sample": f"1 of {wd.n_real} realizations x {n_or} steps of the full grid ({el:.1f} s)"}
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,139 @@
+/*
+ * hft.h -- C ABI of the B200-native HipFT time-stepping hot path (libhft.so).
+ *
+ * The library advances the surface radial field Br(theta, phi) of a batch of independent
+ * realizations with the scheme of arxiv 2501.06377 (cited as PAPER.md:<line> of the extracted text):
+ *   advection  -div_s(Br v)  by differential rotation and meridional flow (Eq. 2-4),
+ *              WENO3-CS(h) / upwind fluxes (Sec. 3.6.1 :348-388, App. B :650-691), SSPRK (Eq. 25 :410-424)
+ *   diffusion  div_s(nu grad_s Br) (Eq. 6 :109, Eq. 27-28 :436-460) by explicit super time stepping
+ *              RKL2 / RKG2(3/2) (Sec. 3.7.2 :466-476)
+ *   finite-volume polar caps (App. A :622-648), periodic phi, operator splitting A then D (Eq. 21 :308-313),
+ *   data-assimilation blend (Eq. 8-11 :131-153) and flux diagnostics (:225-230).
+ * Every step of that path runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *   - Every function returns HFT_OK (0) or a negative hft_status; nothing throws across the ABI.
+ *     hft_error_string() names a code.  A context is not thread-safe; there is no global state.
+ *   - "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.  All buffers are owned by the
+ *     caller (e.g. allocated with PyTorch) and must stay valid until the stream work that uses them has
+ *     completed; the context never frees them.  Calls enqueue work on the stream given to hft_create
+ *     and return without synchronising unless stated otherwise.
+ *   - User-facing maps are dense row-major [n_theta][n_phi] in the context's dtype: row i (0-based) is
+ *     the cell centred at colatitude (i+1)*pi/(n_theta+1), column k at longitude 2*pi*k/n_phi.  The two
+ *     polar caps and the padding of the internal layout [R][n_theta+2][pitch] are
+ *     internal; see DESIGN.md "Data layout".
+ *   - Units are the paper's input units: Gauss, hours, m/s, km^2/s.
+ */
+#ifndef HFT_H
+#define HFT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hft_ctx hft_ctx; /* opaque */
+
+typedef enum {
+    HFT_OK = 0,
+    HFT_ERR_ARG = -1,       /* null pointer, size or enum out of range */
+    HFT_ERR_WORKSPACE = -2, /* workspace too small or not 256-byte aligned */
+    HFT_ERR_CUDA = -3,      /* a CUDA runtime call failed; see hft_last_cuda_error */
+    HFT_ERR_UNSTABLE = -4,  /* forced sts_stages too small for dt, or dt <= 0 */
+    HFT_ERR_NOMEM = -5,     /* host or small device table allocation failed */
+    HFT_ERR_DEVICE = -6     /* no sm_100 device / kernels not loadable on the current device */
+} hft_status;
+
+/* Grid: n_theta x n_phi regular cells; the two polar caps are added internally. */
+typedef struct {
+    int32_t n_theta;  /* >= 8 */
+    int32_t n_phi;    /* >= 8 */
+    int32_t dtype;    /* 0 = fp32, 1 = fp64: storage and arithmetic of the state */
+    int32_t reserved; /* must be 0 */
+    double radius_cm; /* scales hft_diagnostics to Mx: 6.96e10; 1.0 = unit sphere */
+} hft_grid;
+
+/* Per-realization model parameters. */
+typedef struct {
+    double eta_km2_s;  /* diffusivity nu of Eq. 6, km^2/s */
+    double d0, d2, d4; /* differential rotation, Eq. 3 (:78): v_phi = [d0 + d2 cos^2 + d4 cos^4] sin(theta), m/s */
+    double m1, m3, m5; /* meridional flow, Eq. 4 (:84): v_theta = -[m1 cos + m3 cos^3 + m5 cos^5] sin(theta), m/s */
+} hft_params;
+
+typedef struct {
+    int32_t adv_flux;   /* 0 off, 1 upwind (:362), 2 WENO3-CS(h) (default, App. B) */
+    int32_t adv_time;   /* 1 forward Euler (Eq. 23), 3 SSPRK(3,3), 4 SSPRK(4,3) (default, Eq. 25) */
+    int32_t diff_time;  /* 0 off, 1 explicit Euler, 2 RKL2, 3 RKG2(3/2) (default, :476) */
+    int32_t sts_stages; /* 0 = smallest stable count for dt (hft_sts_stage_count); else forced, >= 2 */
+    int32_t sts_block;  /* STS stages fused per kernel launch (temporal blocking): 0 = library default,
+                           1 = one launch per stage, k > 1 = k stages per launch (even, <= 8) */
+    int32_t use_graph;  /* 1 = capture one time step into a CUDA graph and replay it (default 0) */
+    int32_t reserved[2];
+} hft_options;
+
+/* Bytes of device workspace hft_create needs for this grid / batch (state + 5 stage arrays). */
+int hft_workspace_bytes(const hft_grid* grid, int32_t n_real, const hft_options* opt, size_t* h_bytes);
+
+/* Create a context.  d_workspace: caller-allocated device memory of at least hft_workspace_bytes,
+ * 256-byte aligned, owned by the caller; it holds the state and must not be touched while the context
+ * lives.  cuda_stream: a cudaStream_t (0 = legacy default stream) on which all work is enqueued.
+ * The state starts as zero.  Builds the per-row metric / flow / diffusion tables. */
+int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params /*[n_real]*/,
+               const hft_options* opt, void* d_workspace, size_t workspace_bytes, void* cuda_stream,
+               hft_ctx** out);
+
+void hft_destroy(hft_ctx* ctx);
+
+/* Replace the analytic flow of realization r (-1: all) by per-row tables (PAPER.md:90 custom flows,
+ * phi-independent subset; needed for the App. C test :703): h_vtheta[n_theta+1] = v_theta at the
+ * theta-faces (j+1/2)*dtheta, j = 0..n_theta, in m/s; h_omega[n_theta+2] = v_phi/sin(theta) at the rows
+ * j*dtheta, j = 0..n_theta+1, in m/s (i.e. the bracket of Eq. 3). */
+int hft_set_flow_tables(hft_ctx* ctx, int32_t r, const double* h_vtheta, const double* h_omega);
+
+/* Set the map of realization r (r = -1: broadcast the one map to all).  d_map: device, [n_theta][n_phi]
+ * in the context dtype.  Each polar cap is set to the dphi-weighted mean of its adjacent row. */
+int hft_set_map(hft_ctx* ctx, int32_t r, const void* d_map);
+
+/* Copy the map of realization r to d_out [n_theta][n_phi] (r = -1: all, [n_real][n_theta][n_phi]). */
+int hft_get_map(hft_ctx* ctx, int32_t r, void* d_out);
+
+/* Full internal field of realization r incl. the two cap rows: [n_theta+2][n_phi] (tests, restart). */
+int hft_get_full(hft_ctx* ctx, int32_t r, void* d_out);
+int hft_set_full(hft_ctx* ctx, int32_t r, const void* d_in);
+
+/* Advance all realizations by n_steps steps of dt_hours: B <- D(A(B)) per step (Eq. 21).  Asynchronous.
+ * HFT_ERR_UNSTABLE if a forced stage count is below the stable one for dt, or dt <= 0. */
+int hft_step(hft_ctx* ctx, int32_t n_steps, double dt_hours);
+
+/* Data assimilation (Eq. 8): B <- w*obs + (1-w)*B.  d_obs, d_weights: device, [n_real or 1][n_theta][n_phi]
+ * in the context dtype (shared != 0: one map for all realizations).  flags bit 0: flux-balanced form
+ * (Eq. 10-11).  Caps are blended with the row means of obs and w (reading U18). */
+int hft_assimilate(hft_ctx* ctx, const void* d_obs, const void* d_weights, int32_t shared, int32_t flags);
+
+/* Flux diagnostics (:225-230): h_out[n_real][4] = {signed, unsigned, Phi+, Phi-} in G*radius_cm^2.
+ * Synchronises the stream. */
+int hft_diagnostics(hft_ctx* ctx, double* h_out);
+
+/* Host helpers (not timed): Eq. 26 advective limit over all rows and realizations (no safety factor),
+ * explicit-Euler diffusion limit 2/rho (Gershgorin), and the STS stage count for dt. */
+int hft_stable_dt(hft_ctx* ctx, double* h_dt_adv_limit_hours, double* h_dt_diff_euler_hours);
+int hft_sts_stage_count(hft_ctx* ctx, double dt_hours, int32_t* h_stages);
+
+/* Number of kernel launches enqueued by this context so far (graph replays count their nodes). */
+int hft_launch_count(hft_ctx* ctx, int64_t* h_count);
+
+/* Enable per-kernel CUDA-event timing on the context's stream for the kernel class `which`
+ * (0 = none, 1 = STS stage kernels, 2 = advection stage kernels); hft_kernel_time returns the
+ * accumulated milliseconds and launches since the last call and resets them (synchronises). */
+int hft_profile_kernels(hft_ctx* ctx, int32_t which);
+int hft_kernel_time(hft_ctx* ctx, double* h_ms, int64_t* h_launches);
+
+const char* hft_error_string(int code);
+const char* hft_last_cuda_error(hft_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HFT_H */

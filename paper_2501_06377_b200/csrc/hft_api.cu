@@ -1,0 +1,706 @@
+// hft_api.cu -- C ABI (include/hft.h), context, host-side tables and the per-step launch schedule.
+//
+// Host work per hft_step: look up (or build) the STS stage scalars for (dt, s), then enqueue kernels on
+// the caller's stream; nothing synchronises.  All floating-point work on the fields happens in the
+// kernels of hft_kernels.cuh / hft_sts_blocked.cuh.  Tables are formed in fp64 and rounded once to the
+// state precision.  Citations: /root/reference/PAPER.md.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/hft.h"
+#include "hft_kernels.cuh"
+#include "hft_sts_blocked.cuh"
+
+using namespace hft;
+
+namespace {
+
+constexpr double kPi = 3.141592653589793238462643383279502884;
+constexpr double kMsToRsHr = 5.172413793103448e-6;    // PAPER.md:298  m/s -> R_sun/hr
+constexpr double kKm2sToRs2Hr = 7.43162901307967e-9;  // PAPER.md:298  km^2/s -> R_sun^2/hr
+constexpr int kNumArrays = 6;                         // state + 5 stage arrays
+constexpr int kProfEvents = 256;
+
+struct StsCoef {  // per-stage scalars of Sec. 3.7.2 schemes, index 0..s
+    int scheme = 0, s = 0;
+    double dt = 0.0;
+    std::vector<double> mu, nu, a, g;  // mu_j, nu_j, mut_j*dt, mut_j*b_{j-1}*dt ; a[1] = mut_1*dt
+};
+
+}  // namespace
+
+struct hft_ctx {
+    hft_grid grid;
+    hft_options opt;
+    int nr = 0;
+    cudaStream_t stream = nullptr;
+    Geom G;
+    size_t arr_bytes = 0;
+    char* arr[kNumArrays] = {nullptr};
+    int i_state = 0;  // index of the array that currently holds the state
+    // host tables (fp64)
+    double dth = 0, dph = 0, P = 0, Apole = 0;
+    std::vector<double> st, sth;      // sin(theta_j) [nt+2], sin(theta_{j+1/2}) [nt+1]
+    std::vector<double> nu;           // [R] R_sun^2/hr
+    std::vector<double> vt, om;       // [R][nt+1] R_sun/hr at faces, [R][nt+2] rad/hr at rows
+    // device tables
+    char* d_tab = nullptr;
+    size_t tab_bytes = 0;
+    Tables<float> Tf;
+    Tables<double> Td;
+    double* d_part[2] = {nullptr, nullptr};  // polar phi-sum partials, double-buffered [R][2][nbx]
+    double* d_fluxpart = nullptr;            // [R][RED_CTAS][2]
+    double* d_capinfo = nullptr;             // [R][2][2]
+    double* d_scale = nullptr;               // [R]
+    double* d_diag = nullptr;                // [R][4]
+    double* d_zmean = nullptr;               // blocked STS: zonal partial sums (see hft_sts_blocked.cuh)
+    double* d_capseq = nullptr;              // blocked STS: cap values per stage
+    double* h_diag = nullptr;                // pinned
+    int64_t launches = 0;
+    StsCoef coef;
+    // sampled kernel timing
+    int prof_which = 0;
+    int prof_n = 0;
+    int64_t prof_seen = 0;
+    cudaEvent_t prof_ev[2 * kProfEvents];
+    bool prof_ev_made = false;
+    // CUDA graph of one step
+    cudaGraphExec_t graph = nullptr;
+    double graph_dt = 0.0;
+    int64_t graph_launches = 0;
+    std::string cuda_err;
+    bool fp64() const { return grid.dtype == 1; }
+};
+
+namespace {
+
+int cuda_fail(hft_ctx* c, cudaError_t e, const char* what) {
+    if (c) c->cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return HFT_ERR_CUDA;
+}
+#define CK(call)                                                  \
+    do {                                                          \
+        cudaError_t e_ = (call);                                  \
+        if (e_ != cudaSuccess) return cuda_fail(c, e_, #call);    \
+    } while (0)
+
+size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int pitch_for(int np, int dtype) {
+    size_t w = dtype == 1 ? 8 : 4;
+    return (int)(round_up((size_t)np * w, 128) / w);  // rows start on 128-byte lines
+}
+
+bool valid_grid(const hft_grid* g) {
+    return g && g->n_theta >= 8 && g->n_phi >= 8 && (g->dtype == 0 || g->dtype == 1) && g->reserved == 0 &&
+           g->n_theta <= (1 << 20) && g->n_phi <= (1 << 20) && g->radius_cm > 0.0;
+}
+
+hft_options default_options() {
+    hft_options o;
+    memset(&o, 0, sizeof(o));
+    o.adv_flux = 2; o.adv_time = 4; o.diff_time = 3; o.sts_stages = 0; o.sts_block = 0; o.use_graph = 0;
+    return o;
+}
+
+bool valid_options(const hft_options* o) {
+    if (o->adv_flux < 0 || o->adv_flux > 2) return false;
+    if (o->adv_time != 1 && o->adv_time != 3 && o->adv_time != 4) return false;
+    if (o->diff_time < 0 || o->diff_time > 3) return false;
+    if (o->sts_stages != 0 && o->sts_stages < 2) return false;
+    if (o->sts_block < 0 || o->sts_block > STS_KMAX || (o->sts_block > 1 && (o->sts_block & 1))) return false;
+    return true;
+}
+
+// ---------------------------------------------------------------- host tables (fp64)
+
+// Grid metric (App. A :642-646).  1 - cos(x) is formed as 2 sin^2(x/2).
+void build_metric(hft_ctx* c) {
+    const int nt = c->G.nt;
+    c->dth = kPi / (double)(nt + 1);
+    c->dph = 2.0 * kPi / (double)c->G.np;
+    c->st.resize(nt + 2);
+    c->sth.resize(nt + 1);
+    for (int j = 0; j <= nt + 1; j++) c->st[j] = sin(c->dth * (double)j);
+    for (int j = 0; j <= nt; j++) c->sth[j] = sin(c->dth * ((double)j + 0.5));
+    const double q = sin(c->dth * 0.25);
+    c->Apole = 2.0 * kPi * (2.0 * q * q);
+    c->P = sin(c->dth * 0.5) / c->Apole;
+}
+
+// Analytic flows, Eq. 3-4 (:78-86), converted with :298.
+void build_flow(hft_ctx* c, int r, const hft_params& p) {
+    const int nt = c->G.nt;
+    c->nu[r] = p.eta_km2_s * kKm2sToRs2Hr;
+    for (int f = 0; f <= nt; f++) {
+        const double th = c->dth * ((double)f + 0.5), x = cos(th);
+        c->vt[(size_t)r * (nt + 1) + f] = -(p.m1 * x + p.m3 * x * x * x + p.m5 * x * x * x * x * x) * sin(th) * kMsToRsHr;
+    }
+    for (int j = 0; j <= nt + 1; j++) {
+        const double x = cos(c->dth * (double)j), x2 = x * x;
+        c->om[(size_t)r * (nt + 2) + j] = (p.d0 + p.d2 * x2 + p.d4 * x2 * x2) * kMsToRsHr;
+    }
+}
+
+template <typename real>
+struct HostTab {
+    std::vector<real> cp, cm, cf, lm, lp, vtf, pm, pp, sth, rdt, rdp;
+    std::vector<double> capc, dA;
+};
+
+template <typename real>
+void fill_tables(const hft_ctx* c, HostTab<real>& H) {
+    const int nt = c->G.nt, R = c->nr;
+    const size_t n2 = (size_t)R * (nt + 2);
+    H.cp.assign(n2, 0); H.cm.assign(n2, 0); H.cf.assign(n2, 0); H.lm.assign(n2, 0); H.lp.assign(n2, 0);
+    H.pm.assign(n2, 0); H.pp.assign(n2, 0);
+    H.vtf.assign((size_t)R * (nt + 1), 0);
+    H.sth.resize(nt + 1); H.rdt.assign(nt + 2, 0); H.rdp.assign(nt + 2, 0);
+    H.capc.resize(R); H.dA.resize(nt + 2);
+    for (int f = 0; f <= nt; f++) H.sth[f] = (real)c->sth[f];
+    for (int j = 1; j <= nt; j++) {
+        H.rdt[j] = (real)(1.0 / (c->st[j] * c->dth));
+        H.rdp[j] = (real)(1.0 / (c->st[j] * c->dph));
+        H.dA[j] = c->st[j] * c->dth * c->dph;
+    }
+    H.dA[0] = H.dA[nt + 1] = c->Apole;
+    for (int r = 0; r < R; r++) {
+        const double nu = c->nu[r];
+        const double* vt = &c->vt[(size_t)r * (nt + 1)];
+        const double* om = &c->om[(size_t)r * (nt + 2)];
+        H.capc[r] = c->P * (nu / c->dth) * c->dph;
+        for (int f = 0; f <= nt; f++) H.vtf[(size_t)r * (nt + 1) + f] = (real)vt[f];
+        for (int j = 0; j <= nt + 1; j++) {
+            const size_t i = (size_t)r * (nt + 2) + j;
+            if (j >= 1 && j <= nt) {  // Eq. 28 with constant nu, uniform spacing
+                H.cp[i] = (real)(nu * c->sth[j] / (c->st[j] * c->dth * c->dth));
+                H.cm[i] = (real)(nu * c->sth[j - 1] / (c->st[j] * c->dth * c->dth));
+                H.cf[i] = (real)(nu / (c->st[j] * c->st[j] * c->dph * c->dph));
+            }
+            // LLF (B2 :684) with alpha_j = max |v| over faces j-5/2 .. j+5/2 that exist (:689)
+            double al = 0.0;
+            for (int f = j - 3; f <= j + 2; f++)
+                if (f >= 0 && f <= nt) al = fmax(al, fabs(vt[f]));
+            const real alr = (real)al;
+            const real vm = (j >= 1) ? (real)vt[j - 1] : (real)0;  // v_{j-1/2}
+            const real vp = (j <= nt) ? (real)vt[j] : (real)0;     // v_{j+1/2}
+            H.lm[i] = (real)0.5 * (vm + alr);
+            H.lp[i] = (real)0.5 * (vp - alr);
+            const real vphi = (real)(om[j] * c->st[j]);
+            const real aphi = (real)fabs(om[j] * c->st[j]);
+            H.pm[i] = (real)0.5 * (vphi + aphi);
+            H.pp[i] = (real)0.5 * (vphi - aphi);
+        }
+    }
+}
+
+template <typename real>
+int upload_tables(hft_ctx* c, Tables<real>& T) {
+    HostTab<real> H;
+    fill_tables<real>(c, H);
+    const int nt = c->G.nt, R = c->nr;
+    const size_t n2 = (size_t)R * (nt + 2) * sizeof(real), n1 = (size_t)R * (nt + 1) * sizeof(real);
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off = round_up(off + bytes, 256); return o; };
+    size_t o_cp = take(n2), o_cm = take(n2), o_cf = take(n2), o_lm = take(n2), o_lp = take(n2), o_pm = take(n2), o_pp = take(n2);
+    size_t o_vtf = take(n1), o_sth = take((nt + 1) * sizeof(real)), o_rdt = take((nt + 2) * sizeof(real)), o_rdp = take((nt + 2) * sizeof(real));
+    size_t o_capc = take(R * sizeof(double)), o_dA = take((nt + 2) * sizeof(double));
+    if (!c->d_tab) {
+        c->tab_bytes = off;
+        CK(cudaMalloc((void**)&c->d_tab, c->tab_bytes));
+    }
+    char* d = c->d_tab;
+    auto up = [&](size_t o, const void* src, size_t bytes) { return cudaMemcpyAsync(d + o, src, bytes, cudaMemcpyHostToDevice, c->stream); };
+    CK(up(o_cp, H.cp.data(), n2)); CK(up(o_cm, H.cm.data(), n2)); CK(up(o_cf, H.cf.data(), n2));
+    CK(up(o_lm, H.lm.data(), n2)); CK(up(o_lp, H.lp.data(), n2)); CK(up(o_pm, H.pm.data(), n2)); CK(up(o_pp, H.pp.data(), n2));
+    CK(up(o_vtf, H.vtf.data(), n1)); CK(up(o_sth, H.sth.data(), (nt + 1) * sizeof(real)));
+    CK(up(o_rdt, H.rdt.data(), (nt + 2) * sizeof(real))); CK(up(o_rdp, H.rdp.data(), (nt + 2) * sizeof(real)));
+    CK(up(o_capc, H.capc.data(), R * sizeof(double))); CK(up(o_dA, H.dA.data(), (nt + 2) * sizeof(double)));
+    CK(cudaStreamSynchronize(c->stream));  // H goes out of scope
+    T.cp = (const real*)(d + o_cp); T.cm = (const real*)(d + o_cm); T.cf = (const real*)(d + o_cf);
+    T.lm = (const real*)(d + o_lm); T.lp = (const real*)(d + o_lp); T.pm = (const real*)(d + o_pm); T.pp = (const real*)(d + o_pp);
+    T.vtf = (const real*)(d + o_vtf); T.sth = (const real*)(d + o_sth); T.rdt = (const real*)(d + o_rdt); T.rdp = (const real*)(d + o_rdp);
+    T.capc = (const double*)(d + o_capc); T.dA = (const double*)(d + o_dA);
+    T.adv_capc = c->P * c->dph;
+    T.eps_t = (real)c->dth;
+    T.eps_p = (real)c->dph;
+    return HFT_OK;
+}
+
+int upload_all_tables(hft_ctx* c) { return c->fp64() ? upload_tables<double>(c, c->Td) : upload_tables<float>(c, c->Tf); }
+
+// ---------------------------------------------------------------- step-size helpers (row A9)
+
+// Eq. 26 (:430) with flanking-face maxima (:406); |v_phi| / (sin(theta) dph) = |Omega| / dph.
+double adv_dt_limit(const hft_ctx* c) {
+    const int nt = c->G.nt;
+    double best = INFINITY;
+    for (int r = 0; r < c->nr; r++)
+        for (int j = 1; j <= nt; j++) {
+            const double a = fmax(fabs(c->vt[(size_t)r * (nt + 1) + j - 1]), fabs(c->vt[(size_t)r * (nt + 1) + j]));
+            const double rate = a / c->dth + fabs(c->om[(size_t)r * (nt + 2) + j]) / c->dph;
+            if (rate > 0.0) best = fmin(best, 1.0 / rate);
+        }
+    return best;
+}
+
+// Gershgorin bound: rho <= 2 max|diag|; explicit Euler limit 2/rho, with nu = max_r nu_r (:448).
+double diff_dt_expl(const hft_ctx* c) {
+    double nu = 0.0;
+    for (double v : c->nu) nu = fmax(nu, v);
+    double d = 2.0 * kPi * c->P * nu / c->dth;  // cap row diagonal
+    for (int j = 1; j <= c->G.nt; j++) {
+        const double t = nu * (c->sth[j] + c->sth[j - 1]) / (c->st[j] * c->dth * c->dth) + 2.0 * nu / (c->st[j] * c->st[j] * c->dph * c->dph);
+        d = fmax(d, t);
+    }
+    return d > 0.0 ? 1.0 / d : INFINITY;
+}
+
+double sts_span(int scheme, int s) {  // dt / dt_expl reachable with s stages
+    const double x = (double)s;
+    return scheme == 2 ? (x * x + x - 2.0) / 4.0 : (x * x + 3.0 * x - 4.0) / 6.0;
+}
+
+int sts_stages_for(const hft_ctx* c, int scheme, double dt) {
+    const double lim = diff_dt_expl(c);
+    int s = 2;
+    while (dt > lim * sts_span(scheme, s)) {
+        if (++s > 10000000) return -1;
+    }
+    return s;
+}
+
+// Stage scalars.  RKL2: shifted Legendre (Meyer et al. 2014); RKG2(3/2): shifted Gegenbauer lambda = 3/2
+// (Skaras et al. 2021); both named in PAPER.md:470-474, coefficients per DESIGN.md reading U7.
+void build_sts_coef(StsCoef& K, int scheme, int s, double dt) {
+    if (K.scheme == scheme && K.s == s && K.dt == dt) return;
+    K.scheme = scheme; K.s = s; K.dt = dt;
+    K.mu.assign(s + 1, 0); K.nu.assign(s + 1, 0); K.a.assign(s + 1, 0); K.g.assign(s + 1, 0);
+    auto b = [&](int j) {
+        const double x = (double)(j < 2 ? 2 : j);
+        return scheme == 2 ? (x * x + x - 2.0) / (2.0 * x * (x + 1.0)) : 2.0 * (x - 1.0) * (x + 4.0) / (3.0 * x * (x + 3.0));
+    };
+    const double S = (double)s;
+    const double w1 = scheme == 2 ? 4.0 / (S * S + S - 2.0) : 6.0 / ((S - 1.0) * (S + 4.0));
+    K.a[1] = b(1) * w1 * dt;
+    for (int j = 2; j <= s; j++) {
+        const double x = (double)j;
+        const double Aj = scheme == 2 ? (2.0 * x - 1.0) / x : (2.0 * x + 1.0) / (x + 2.0);
+        const double Bj = scheme == 2 ? (x - 1.0) / x : (x - 1.0) / (x + 2.0);
+        K.mu[j] = Aj * b(j) / b(j - 1);
+        K.nu[j] = -Bj * b(j) / b(j - 2);
+        const double mut = K.mu[j] * w1;
+        K.a[j] = mut * dt;
+        K.g[j] = mut * b(j - 1) * dt;
+    }
+}
+
+// ---------------------------------------------------------------- launch helpers
+
+template <typename real> Tables<real>& tables_of(hft_ctx* c);
+template <> Tables<float>& tables_of<float>(hft_ctx* c) { return c->Tf; }
+template <> Tables<double>& tables_of<double>(hft_ctx* c) { return c->Td; }
+
+template <typename real> real* arr_of(hft_ctx* c, int i) { return (real*)c->arr[i]; }
+
+void prof_begin(hft_ctx* c, int cls, bool& armed) {
+    armed = false;
+    if (c->prof_which != cls || c->prof_n >= kProfEvents) return;
+    if ((c->prof_seen++ & 15) != 0) return;  // sample every 16th launch of the class
+    cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream);
+    armed = true;
+}
+void prof_end(hft_ctx* c, bool armed) {
+    if (!armed) return;
+    cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream);
+    c->prof_n++;
+}
+
+template <typename real>
+int launch_row_sums(hft_ctx* c, const real* f, double* part) {
+    dim3 g(c->G.nbx, 2, c->nr);
+    k_polar_row_sums<real><<<g, TX, 0, c->stream>>>(f, part, c->G);
+    c->launches++;
+    return HFT_OK;
+}
+
+// one advection step (A of Eq. 21): SSPRK stages, each = stage kernel + cap kernel
+template <typename real>
+int advect(hft_ctx* c, double dt) {
+    const Geom& G = c->G;
+    Tables<real>& T = tables_of<real>(c);
+    // scratch: the two arrays after the state in ring order
+    const int is = c->i_state, ia = (is + 1) % kNumArrays, ib = (is + 2) % kNumArrays;
+    real *S = arr_of<real>(c, is), *A = arr_of<real>(c, ia), *B = arr_of<real>(c, ib);
+    struct St { const real* in; const real* fn; real* out; double ca, cb, cc; };
+    std::vector<St> sts;
+    if (c->opt.adv_time == 1) {
+        sts.push_back({S, nullptr, A, 0.0, 1.0, 1.0});
+    } else if (c->opt.adv_time == 3) {  // SSPRK(3,3) :412-416
+        sts.push_back({S, nullptr, A, 0.0, 1.0, 1.0});
+        sts.push_back({A, S, B, 0.75, 0.25, 0.25});
+        sts.push_back({B, S, A, 1.0 / 3.0, 2.0 / 3.0, 2.0 / 3.0});
+    } else {  // SSPRK(4,3) Eq. 25 :418-424
+        sts.push_back({S, nullptr, A, 0.0, 1.0, 0.5});
+        sts.push_back({A, nullptr, B, 0.0, 1.0, 0.5});
+        sts.push_back({B, S, A, 2.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0});
+        sts.push_back({A, nullptr, B, 0.0, 1.0, 0.5});
+    }
+    dim3 g(G.nbx, (G.nt + RPT - 1) / RPT, c->nr), gc(G.nbx, 2, c->nr);
+    for (const St& s : sts) {
+        AdvArgs<real> a;
+        a.in = s.in; a.fn = s.fn ? s.fn : s.in; a.out = s.out; a.part = c->d_part[0];
+        a.ca = (real)s.ca; a.cb = (real)s.cb; a.cdt = (real)s.cc * (real)dt;
+        a.upwind_only = c->opt.adv_flux == 1;
+        bool armed;
+        prof_begin(c, 2, armed);
+        k_adv_stage<real><<<g, TX, 0, c->stream>>>(a, T, G);
+        prof_end(c, armed);
+        k_adv_caps<real><<<gc, TX, 0, c->stream>>>(a, T, G);
+        c->launches += 2;
+    }
+    // the last stage's output array becomes the state
+    const real* last = sts.back().out;
+    c->i_state = (last == A) ? ia : ib;
+    return HFT_OK;
+}
+
+// one diffusion step (D of Eq. 21), one launch per stage
+template <typename real>
+int diffuse_unblocked(hft_ctx* c, double dt, int s) {
+    const Geom& G = c->G;
+    Tables<real>& T = tables_of<real>(c);
+    const int is = c->i_state;
+    real* Y0 = arr_of<real>(c, is);
+    real* F = arr_of<real>(c, (is + 1) % kNumArrays);
+    real* da = arr_of<real>(c, (is + 2) % kNumArrays);
+    real* db = arr_of<real>(c, (is + 3) % kNumArrays);
+    dim3 g(G.nbx, (G.nt + 2 + RPT - 1) / RPT, c->nr);
+    launch_row_sums<real>(c, Y0, c->d_part[0]);
+    StsArgs<real> a;
+    a.F = F; a.Y0 = Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
+    if (c->opt.diff_time == 1) {  // explicit Euler (:474), new state written to `da`
+        a.in = Y0; a.d2 = da; a.part_in = c->d_part[0]; a.part_out = c->d_part[1]; a.a = (real)dt;
+        k_sts_stage<real, 3><<<g, TX, 0, c->stream>>>(a, T, G);
+        c->launches++;
+        c->i_state = (is + 2) % kNumArrays;
+        return HFT_OK;
+    }
+    const StsCoef& K = c->coef;
+    // stage 1: F = L(Y0), delta_1 = mut_1 dt F
+    a.in = Y0; a.d2 = da; a.part_in = c->d_part[0]; a.part_out = c->d_part[1]; a.a = (real)K.a[1];
+    bool armed;
+    prof_begin(c, 1, armed);
+    k_sts_stage<real, 0><<<g, TX, 0, c->stream>>>(a, T, G);
+    prof_end(c, armed);
+    c->launches++;
+    real *d1 = da, *d2 = db;
+    int pin = 1;
+    for (int j = 2; j <= s; j++) {
+        a.in = d1; a.d2 = d2; a.part_in = c->d_part[pin]; a.part_out = c->d_part[pin ^ 1];
+        a.mu = (real)K.mu[j]; a.nu = (real)K.nu[j]; a.a = (real)K.a[j]; a.g = (real)K.g[j];
+        a.use_d2 = j > 2;
+        prof_begin(c, 1, armed);
+        if (j < s) k_sts_stage<real, 1><<<g, TX, 0, c->stream>>>(a, T, G);
+        else k_sts_stage<real, 2><<<g, TX, 0, c->stream>>>(a, T, G);
+        prof_end(c, armed);
+        c->launches++;
+        real* t = d1; d1 = d2; d2 = t;
+        pin ^= 1;
+    }
+    return HFT_OK;
+}
+
+template <typename real>
+int step_once(hft_ctx* c, double dt, int s) {
+    int rc = HFT_OK;
+    if (c->opt.adv_flux != 0) rc = advect<real>(c, dt);
+    if (rc != HFT_OK) return rc;
+    if (c->opt.diff_time != 0) {
+        const int kb = c->opt.sts_block == 0 ? sts_default_block(c->G, sizeof(real)) : c->opt.sts_block;
+        if (c->opt.diff_time >= 2 && kb > 1 && s > 2 * kb && sts_blocked_supported(c->G, sizeof(real))) {
+            StsBlockedPlan<real> P;
+            P.Y0 = arr_of<real>(c, c->i_state);
+            for (int i = 0; i < 5; i++) P.buf[i] = arr_of<real>(c, (c->i_state + 1 + i) % kNumArrays);
+            P.mu = c->coef.mu.data(); P.nu = c->coef.nu.data(); P.a = c->coef.a.data(); P.g = c->coef.g.data();
+            P.s = s; P.kb = kb; P.stream = c->stream;
+            P.part = c->d_part; P.zmean = c->d_zmean; P.capseq = c->d_capseq;
+            P.prof_begin = [](void* u, bool* armed) { prof_begin((hft_ctx*)u, 1, *armed); };
+            P.prof_end = [](void* u, bool armed) { prof_end((hft_ctx*)u, armed); };
+            P.user = c;
+            int64_t n = 0;
+            rc = sts_blocked_step<real>(P, tables_of<real>(c), c->G, &n);
+            c->launches += n;
+        } else {
+            rc = diffuse_unblocked<real>(c, dt, s);
+        }
+    }
+    return rc;
+}
+
+int check_launch(hft_ctx* c) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch");
+    return HFT_OK;
+}
+
+}  // namespace
+
+// ===================================================================== C ABI
+
+extern "C" {
+
+const char* hft_error_string(int code) {
+    switch (code) {
+        case HFT_OK: return "ok";
+        case HFT_ERR_ARG: return "invalid argument";
+        case HFT_ERR_WORKSPACE: return "workspace too small or misaligned";
+        case HFT_ERR_CUDA: return "CUDA runtime error";
+        case HFT_ERR_UNSTABLE: return "unstable request (dt <= 0 or forced sts_stages below the stable count)";
+        case HFT_ERR_NOMEM: return "out of memory";
+        case HFT_ERR_DEVICE: return "no usable sm_100 device";
+        default: return "unknown hft_status";
+    }
+}
+
+const char* hft_last_cuda_error(hft_ctx* ctx) { return ctx ? ctx->cuda_err.c_str() : ""; }
+
+int hft_workspace_bytes(const hft_grid* grid, int32_t n_real, const hft_options* opt, size_t* h_bytes) {
+    (void)opt;
+    if (!valid_grid(grid) || n_real < 1 || !h_bytes) return HFT_ERR_ARG;
+    const size_t w = grid->dtype == 1 ? 8 : 4;
+    const size_t one = round_up((size_t)n_real * (grid->n_theta + 2) * pitch_for(grid->n_phi, grid->dtype) * w, 256);
+    *h_bytes = one * kNumArrays;
+    return HFT_OK;
+}
+
+int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params, const hft_options* opt,
+               void* d_workspace, size_t workspace_bytes, void* cuda_stream, hft_ctx** out) {
+    if (!out) return HFT_ERR_ARG;
+    *out = nullptr;
+    if (!valid_grid(grid) || n_real < 1 || !h_params || !d_workspace) return HFT_ERR_ARG;
+    hft_options o = opt ? *opt : default_options();
+    if (!valid_options(&o)) return HFT_ERR_ARG;
+    size_t need = 0;
+    hft_workspace_bytes(grid, n_real, &o, &need);
+    if (workspace_bytes < need || ((uintptr_t)d_workspace & 255) != 0) return HFT_ERR_WORKSPACE;
+    int dev = 0, major = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return HFT_ERR_DEVICE;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) return HFT_ERR_DEVICE;
+    hft_ctx* c = new (std::nothrow) hft_ctx();
+    if (!c) return HFT_ERR_NOMEM;
+    c->grid = *grid; c->opt = o; c->nr = n_real; c->stream = (cudaStream_t)cuda_stream;
+    c->G.nt = grid->n_theta; c->G.np = grid->n_phi; c->G.pitch = pitch_for(grid->n_phi, grid->dtype); c->G.nr = n_real;
+    c->G.rstride = (size_t)(grid->n_theta + 2) * c->G.pitch;
+    c->G.nbx = (grid->n_phi + TX - 1) / TX;
+    c->arr_bytes = need / kNumArrays;
+    for (int i = 0; i < kNumArrays; i++) c->arr[i] = (char*)d_workspace + (size_t)i * c->arr_bytes;
+    c->nu.resize(n_real); c->vt.resize((size_t)n_real * (c->G.nt + 1)); c->om.resize((size_t)n_real * (c->G.nt + 2));
+    build_metric(c);
+    for (int r = 0; r < n_real; r++) build_flow(c, r, h_params[r]);
+    int rc = HFT_OK;
+    auto fail = [&](int code) { hft_destroy(c); return code; };
+    cudaError_t e;
+    const size_t partb = (size_t)n_real * 2 * c->G.nbx * sizeof(double);
+    if ((e = cudaMalloc((void**)&c->d_part[0], partb)) != cudaSuccess || (e = cudaMalloc((void**)&c->d_part[1], partb)) != cudaSuccess ||
+        (e = cudaMalloc((void**)&c->d_fluxpart, (size_t)n_real * RED_CTAS * 2 * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&c->d_capinfo, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&c->d_scale, (size_t)n_real * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&c->d_diag, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&c->d_zmean, sts_zmean_bytes(c->G))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&c->d_capseq, sts_capseq_bytes(c->G))) != cudaSuccess ||
+        (e = cudaMallocHost((void**)&c->h_diag, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess) {
+        cuda_fail(c, e, "cudaMalloc");
+        return fail(HFT_ERR_NOMEM);
+    }
+    if ((e = cudaMemsetAsync(d_workspace, 0, need, c->stream)) != cudaSuccess) { cuda_fail(c, e, "memset"); return fail(HFT_ERR_CUDA); }
+    if ((rc = upload_all_tables(c)) != HFT_OK) return fail(rc);
+    if ((rc = sts_blocked_init(c->G, c->fp64())) != HFT_OK) return fail(HFT_ERR_CUDA);
+    *out = c;
+    return HFT_OK;
+}
+
+void hft_destroy(hft_ctx* c) {
+    if (!c) return;
+    if (c->graph) cudaGraphExecDestroy(c->graph);
+    if (c->prof_ev_made)
+        for (int i = 0; i < 2 * kProfEvents; i++) cudaEventDestroy(c->prof_ev[i]);
+    cudaFree(c->d_tab); cudaFree(c->d_part[0]); cudaFree(c->d_part[1]); cudaFree(c->d_fluxpart);
+    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq);
+    if (c->h_diag) cudaFreeHost(c->h_diag);
+    delete c;
+}
+
+int hft_set_flow_tables(hft_ctx* c, int32_t r, const double* h_vtheta, const double* h_omega) {
+    if (!c || !h_vtheta || !h_omega || r < -1 || r >= c->nr) return HFT_ERR_ARG;
+    const int nt = c->G.nt;
+    for (int q = 0; q < c->nr; q++) {
+        if (r >= 0 && q != r) continue;
+        for (int f = 0; f <= nt; f++) c->vt[(size_t)q * (nt + 1) + f] = h_vtheta[f] * kMsToRsHr;
+        for (int j = 0; j <= nt + 1; j++) c->om[(size_t)q * (nt + 2) + j] = h_omega[j] * kMsToRsHr;
+    }
+    if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
+    return upload_all_tables(c);
+}
+
+int hft_set_map(hft_ctx* c, int32_t r, const void* d_map) {
+    if (!c || !d_map || r < -1 || r >= c->nr) return HFT_ERR_ARG;
+    const Geom& G = c->G;
+    const int nz = r < 0 ? c->nr : 1, r0 = r < 0 ? 0 : r;
+    dim3 g((G.np + 255) / 256, G.nt, nz), gm(2, nz);
+    if (c->fp64()) {
+        k_copy_map<double><<<g, 256, 0, c->stream>>>((double*)c->arr[c->i_state], (double*)d_map, G, r0, 1, 0);
+        k_caps_from_row_mean<double><<<gm, 256, 0, c->stream>>>((double*)c->arr[c->i_state], G, r0);
+    } else {
+        k_copy_map<float><<<g, 256, 0, c->stream>>>((float*)c->arr[c->i_state], (float*)d_map, G, r0, 1, 0);
+        k_caps_from_row_mean<float><<<gm, 256, 0, c->stream>>>((float*)c->arr[c->i_state], G, r0);
+    }
+    c->launches += 2;
+    return check_launch(c);
+}
+
+int hft_get_map(hft_ctx* c, int32_t r, void* d_out) {
+    if (!c || !d_out || r < -1 || r >= c->nr) return HFT_ERR_ARG;
+    const Geom& G = c->G;
+    const int nz = r < 0 ? c->nr : 1, r0 = r < 0 ? 0 : r;
+    dim3 g((G.np + 255) / 256, G.nt, nz);
+    if (c->fp64()) k_copy_map<double><<<g, 256, 0, c->stream>>>((double*)c->arr[c->i_state], (double*)d_out, G, r0, 0, 1);
+    else k_copy_map<float><<<g, 256, 0, c->stream>>>((float*)c->arr[c->i_state], (float*)d_out, G, r0, 0, 1);
+    c->launches++;
+    return check_launch(c);
+}
+
+static int copy_full(hft_ctx* c, int32_t r, void* d, int dir) {
+    if (!c || !d || r < 0 || r >= c->nr) return HFT_ERR_ARG;
+    const Geom& G = c->G;
+    dim3 g((G.np + 255) / 256, G.nt + 2);
+    if (c->fp64()) k_copy_full<double><<<g, 256, 0, c->stream>>>((double*)c->arr[c->i_state], (double*)d, G, r, dir);
+    else k_copy_full<float><<<g, 256, 0, c->stream>>>((float*)c->arr[c->i_state], (float*)d, G, r, dir);
+    c->launches++;
+    return check_launch(c);
+}
+int hft_get_full(hft_ctx* c, int32_t r, void* d_out) { return copy_full(c, r, d_out, 1); }
+int hft_set_full(hft_ctx* c, int32_t r, const void* d_in) { return copy_full(c, r, (void*)d_in, 0); }
+
+int hft_stable_dt(hft_ctx* c, double* h_adv, double* h_diff) {
+    if (!c || !h_adv || !h_diff) return HFT_ERR_ARG;
+    *h_adv = adv_dt_limit(c);
+    *h_diff = diff_dt_expl(c);
+    return HFT_OK;
+}
+
+int hft_sts_stage_count(hft_ctx* c, double dt_hours, int32_t* h_stages) {
+    if (!c || !h_stages || !(dt_hours > 0.0)) return HFT_ERR_ARG;
+    const int scheme = c->opt.diff_time == 2 ? 2 : 3;
+    const int s = sts_stages_for(c, scheme, dt_hours);
+    if (s < 0) return HFT_ERR_UNSTABLE;
+    *h_stages = s;
+    return HFT_OK;
+}
+
+int hft_step(hft_ctx* c, int32_t n_steps, double dt) {
+    if (!c || n_steps < 0) return HFT_ERR_ARG;
+    if (!(dt > 0.0)) return HFT_ERR_UNSTABLE;
+    int s = 0;
+    if (c->opt.diff_time >= 2) {
+        const int need = sts_stages_for(c, c->opt.diff_time, dt);
+        if (need < 0) return HFT_ERR_UNSTABLE;
+        s = c->opt.sts_stages ? c->opt.sts_stages : need;
+        if (s < need) return HFT_ERR_UNSTABLE;
+        build_sts_coef(c->coef, c->opt.diff_time, s, dt);
+    }
+    for (int n = 0; n < n_steps; n++) {
+        int rc = c->fp64() ? step_once<double>(c, dt, s) : step_once<float>(c, dt, s);
+        if (rc != HFT_OK) return rc;
+    }
+    return check_launch(c);
+}
+
+int hft_assimilate(hft_ctx* c, const void* d_obs, const void* d_w, int32_t shared, int32_t flags) {
+    if (!c || !d_obs || !d_w) return HFT_ERR_ARG;
+    const Geom& G = c->G;
+    const int balanced = flags & 1, nmaps = shared ? 1 : c->nr;
+    dim3 gm(2, nmaps), gb(G.nbx, G.nt + 2, c->nr), gp(RED_CTAS, c->nr);
+    const int fin_blocks = (c->nr + 63) / 64;
+    if (c->fp64()) {
+        double* S = (double*)c->arr[c->i_state];
+        k_assim_cap_means<double><<<gm, 256, 0, c->stream>>>((const double*)d_obs, (const double*)d_w, G, c->d_capinfo);
+        if (balanced) {
+            k_flux_partials<double, 1><<<gp, 256, 0, c->stream>>>(S, (const double*)d_obs, (const double*)d_w, shared, c->Td, G, c->d_fluxpart);
+            k_flux_finalize<double, 1><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, c->d_capinfo, shared, c->Td, G, 1.0, c->d_scale);
+            c->launches += 2;
+        }
+        k_assim_blend<double><<<gb, TX, 0, c->stream>>>(S, (const double*)d_obs, (const double*)d_w, shared, c->d_capinfo, c->d_scale, balanced, G);
+    } else {
+        float* S = (float*)c->arr[c->i_state];
+        k_assim_cap_means<float><<<gm, 256, 0, c->stream>>>((const float*)d_obs, (const float*)d_w, G, c->d_capinfo);
+        if (balanced) {
+            k_flux_partials<float, 1><<<gp, 256, 0, c->stream>>>(S, (const float*)d_obs, (const float*)d_w, shared, c->Tf, G, c->d_fluxpart);
+            k_flux_finalize<float, 1><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, c->d_capinfo, shared, c->Tf, G, 1.0, c->d_scale);
+            c->launches += 2;
+        }
+        k_assim_blend<float><<<gb, TX, 0, c->stream>>>(S, (const float*)d_obs, (const float*)d_w, shared, c->d_capinfo, c->d_scale, balanced, G);
+    }
+    c->launches += 2;
+    return check_launch(c);
+}
+
+int hft_diagnostics(hft_ctx* c, double* h_out) {
+    if (!c || !h_out) return HFT_ERR_ARG;
+    const Geom& G = c->G;
+    dim3 gp(RED_CTAS, c->nr);
+    const int fin_blocks = (c->nr + 63) / 64;
+    const double scale = c->grid.radius_cm * c->grid.radius_cm;
+    if (c->fp64()) {
+        double* S = (double*)c->arr[c->i_state];
+        k_flux_partials<double, 0><<<gp, 256, 0, c->stream>>>(S, nullptr, nullptr, 0, c->Td, G, c->d_fluxpart);
+        k_flux_finalize<double, 0><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, nullptr, 0, c->Td, G, scale, c->d_diag);
+    } else {
+        float* S = (float*)c->arr[c->i_state];
+        k_flux_partials<float, 0><<<gp, 256, 0, c->stream>>>(S, nullptr, nullptr, 0, c->Tf, G, c->d_fluxpart);
+        k_flux_finalize<float, 0><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, nullptr, 0, c->Tf, G, scale, c->d_diag);
+    }
+    c->launches += 2;
+    CK(cudaMemcpyAsync(c->h_diag, c->d_diag, (size_t)c->nr * 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    memcpy(h_out, c->h_diag, (size_t)c->nr * 4 * sizeof(double));
+    return HFT_OK;
+}
+
+int hft_launch_count(hft_ctx* c, int64_t* h_count) {
+    if (!c || !h_count) return HFT_ERR_ARG;
+    *h_count = c->launches;
+    return HFT_OK;
+}
+
+int hft_profile_kernels(hft_ctx* c, int32_t which) {
+    if (!c || which < 0 || which > 2) return HFT_ERR_ARG;
+    if (!c->prof_ev_made) {
+        for (int i = 0; i < 2 * kProfEvents; i++) CK(cudaEventCreate(&c->prof_ev[i]));
+        c->prof_ev_made = true;
+    }
+    c->prof_which = which; c->prof_n = 0; c->prof_seen = 0;
+    return HFT_OK;
+}
+
+int hft_kernel_time(hft_ctx* c, double* h_ms, int64_t* h_launches) {
+    if (!c || !h_ms || !h_launches) return HFT_ERR_ARG;
+    CK(cudaStreamSynchronize(c->stream));
+    double ms = 0.0;
+    for (int i = 0; i < c->prof_n; i++) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
+        ms += t;
+    }
+    *h_ms = ms; *h_launches = c->prof_n;
+    c->prof_n = 0; c->prof_seen = 0;
+    return HFT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,430 @@
+// hft_kernels.cuh -- sm_100a kernels of the HipFT time-stepping hot path (baseline, one launch per stage).
+//
+// Layout: a field is [R][nt+2][pitch] of `real`; row 0 / row nt+1 are the north /
+// south polar caps (one value each, stored replicated over the nphi columns so that the theta-stencil of
+// rows 1 and nt is uniform); columns [nphi, pitch) are padding and are never read.  phi is contiguous:
+// a warp reads 32 consecutive columns of one row (coalesced 128/256 B).  Periodic phi is an index wrap.
+// All per-row coefficients are phi-independent and come from small tables (broadcast loads).
+//
+// Citations are to /root/reference/PAPER.md (the extracted paper text), as in include/hft.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace hft {
+
+constexpr int TX = 128;  // threads per CTA = columns per CTA (one column per thread)
+constexpr int RPT = 8;   // rows per thread (column strip streamed in registers)
+
+template <typename real>
+struct Tables {            // device pointers, all [R][nt+2] unless noted
+    const real* cp;        // diffusion: nu sin(theta_{j+1/2}) / (sin(theta_j) dth^2)        Eq. 28 (:456)
+    const real* cm;        //            nu sin(theta_{j-1/2}) / (sin(theta_j) dth^2)        Eq. 28 (:452)
+    const real* cf;        //            nu / (sin^2(theta_j) dph^2)                         Eq. 28 (:450, :458)
+    const double* capc;    // [R] P (nu/dth) dph : polar cap diffusion prefactor             App. A (:646)
+    const real* lm;        // advection LLF: (v_{j-1/2} + alpha_j)/2                         B2 (:684)
+    const real* lp;        //                (v_{j+1/2} - alpha_j)/2
+    const real* vtf;       // [R][nt+1] v_theta at theta-faces (upwind faces)                Eq. 4 (:84)
+    const real* pm;        // phi LLF: (v_phi + |v_phi|)/2 per row                           B2 with alpha = |v_phi|
+    const real* pp;        //          (v_phi - |v_phi|)/2 per row
+    const real* sth;       // [nt+1] sin(theta_{j+1/2})                                      :354
+    const real* rdt;       // [nt+2] 1/(sin(theta_j) dth)
+    const real* rdp;       // [nt+2] 1/(sin(theta_j) dph)
+    const double* dA;      // [nt+2] quadrature weights: sin(theta_j) dth dph; caps: A_pole   :225-230, App. A
+    double adv_capc;       // P dph                                                          App. A (:646)
+    real eps_t, eps_p;     // WENO3-CS(h) eps_w = dth, dph                                    :670
+};
+
+struct Geom {
+    int nt, np, pitch, nr;
+    size_t rstride;  // (nt+2)*pitch
+    int nbx;         // ceil(np / TX): CTAs along phi == number of polar partial sums per row
+};
+
+// ------------------------------------------------------------------ reductions (fixed order => deterministic)
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Sum over the CTA (blockDim.x multiple of 32, <= 1024); result valid in thread 0.
+__device__ __forceinline__ double block_sum(double v, double* smem /*[32]*/) {
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    v = warp_sum(v);
+    __syncthreads();
+    if (lane == 0) smem[w] = v;
+    __syncthreads();
+    double t = 0.0;
+    if (threadIdx.x == 0)
+        for (int i = 0; i < nw; i++) t += smem[i];
+    return t;
+}
+
+// Sum of the nbx per-CTA partials of one polar row, in index order (every caller gets the same bits).
+__device__ __forceinline__ double sum_partials(const double* p, int nbx) {
+    double s = 0.0;
+    for (int i = 0; i < nbx; i++) s += p[i];
+    return s;
+}
+
+// ------------------------------------------------------------------ diffusion / STS (one stage per launch)
+
+template <typename real>
+struct StsArgs {
+    const real* in;   // field whose L is taken: Y0 (MODE 0) or delta_{j-1}
+    real* d2;         // MODE 0: out delta_1.  MODE 1/2: in delta_{j-2}, out delta_j (same element, same thread)
+    real* F;          // L(Y0): written in MODE 0, read otherwise
+    real* Y0;         // MODE 2: Y0 += delta_s
+    const double* part_in;   // [R][2][nbx] phi-sums of rows 1 and nt of `in`
+    double* part_out;        // same for the field written to d2
+    real mu, nu, a, g;       // stage scalars: mu_j, nu_j, mut_j dt, mut_j b_{j-1} dt (MODE 0: a = mut_1 dt)
+    int use_d2;              // 0 on stage 2 (delta_0 = 0 is not stored)
+};
+
+// MODE 0: F = L(Y0), delta_1 = a F.   MODE 1: delta_j = mu d1 + nu d2 + a L(d1) + g F.
+// MODE 2: MODE 1, then Y0 += delta_j (last stage).  MODE 3: explicit Euler, Y0 += a L(Y0) (in = Y0, out d2 = new Y).
+// Row A5/A6 of SURVEY.md section 8: Eq. 27-28 (:438-460) with constant nu; caps per App. A (:624-648):
+// L_cap = P (nu/dth) dph sum_k (B[1,k] - B[0]).
+template <typename real, int MODE>
+__global__ void __launch_bounds__(TX) k_sts_stage(StsArgs<real> A, Tables<real> T, Geom G) {
+    __shared__ double red[32];
+    const int r = blockIdx.z;
+    const int k = blockIdx.x * TX + threadIdx.x;
+    const bool live = k < G.np;
+    const int kk = live ? k : 0;
+    const int kw = (kk == 0) ? G.np - 1 : kk - 1;
+    const int ke = (kk == G.np - 1) ? 0 : kk + 1;
+    const int j0 = blockIdx.y * RPT;
+    const int j1 = min(j0 + RPT, G.nt + 2);
+    const size_t base = (size_t)r * G.rstride;
+    const real* in = A.in + base;
+    const real* cp = T.cp + (size_t)r * (G.nt + 2);
+    const real* cm = T.cm + (size_t)r * (G.nt + 2);
+    const real* cf = T.cf + (size_t)r * (G.nt + 2);
+
+    real n = (j0 > 0) ? in[(size_t)(j0 - 1) * G.pitch + kk] : (real)0;
+    real c = in[(size_t)j0 * G.pitch + kk];
+    double sumN = 0.0, sumS = 0.0;  // this thread's contribution to the phi-sums of output rows 1 and nt
+    for (int j = j0; j < j1; j++) {
+        const size_t off = base + (size_t)j * G.pitch + kk;
+        real s = (j < G.nt + 1) ? in[(size_t)(j + 1) * G.pitch + kk] : (real)0;
+        real L;
+        if (j == 0 || j == G.nt + 1) {
+            const int pole = (j == 0) ? 0 : 1;
+            double S = sum_partials(A.part_in + ((size_t)r * 2 + pole) * G.nbx, G.nbx);
+            L = (real)(T.capc[r] * (S - (double)G.np * (double)c));
+        } else {
+            real w = in[(size_t)j * G.pitch + kw], e = in[(size_t)j * G.pitch + ke];
+            L = cp[j] * (s - c) - cm[j] * (c - n) + cf[j] * ((e - (real)2 * c) + w);
+        }
+        real out;
+        if (MODE == 0) {
+            out = A.a * L;
+            if (live) A.F[off] = L;
+        } else if (MODE == 3) {
+            out = c + A.a * L;
+        } else {
+            real d2v = A.use_d2 ? A.d2[off] : (real)0;
+            out = A.mu * c + A.nu * d2v + A.a * L + A.g * A.F[off];
+        }
+        if (live) {
+            if (MODE == 2) A.Y0[off] += out;   // Y_s = Y_0 + delta_s; delta_s itself is not needed again
+            else A.d2[off] = out;
+        }
+        if (j == 1) sumN = live ? (double)out : 0.0;
+        if (j == G.nt) sumS = live ? (double)out : 0.0;
+        n = c;
+        c = s;
+    }
+    // phi-sums of the rows adjacent to the caps, for the next stage's cap update (block-uniform branches)
+    if (j0 <= 1 && 1 < j1) {
+        double t = block_sum(sumN, red);
+        if (threadIdx.x == 0) A.part_out[((size_t)r * 2 + 0) * G.nbx + blockIdx.x] = t;
+    }
+    if (j0 <= G.nt && G.nt < j1) {
+        double t = block_sum(sumS, red);
+        if (threadIdx.x == 0) A.part_out[((size_t)r * 2 + 1) * G.nbx + blockIdx.x] = t;
+    }
+}
+
+// phi-sums of rows 1 and nt of a field -> partials (same format as the stage kernels write).
+template <typename real>
+__global__ void __launch_bounds__(TX) k_polar_row_sums(const real* f, double* part, Geom G) {
+    __shared__ double red[32];
+    const int r = blockIdx.z, pole = blockIdx.y;
+    const int k = blockIdx.x * TX + threadIdx.x;
+    const int j = pole == 0 ? 1 : G.nt;
+    double v = (k < G.np) ? (double)f[(size_t)r * G.rstride + (size_t)j * G.pitch + k] : 0.0;
+    double t = block_sum(v, red);
+    if (threadIdx.x == 0) part[((size_t)r * 2 + pole) * G.nbx + blockIdx.x] = t;
+}
+
+// ------------------------------------------------------------------ advection (one SSPRK stage per launch)
+
+// WENO3-CS(h) one-sided face value (App. B :658-676, uniform grid: D = 1/2, 1/3, 2/3), written with one
+// division: u = (d0 p0 (eps+b1)^2 + d1 p1 (eps+b0)^2) / (d0 (eps+b1)^2 + d1 (eps+b0)^2).
+template <typename real>
+__device__ __forceinline__ real weno3_side(real far, real near, real other, real eps) {
+    real p0 = (real)1.5 * near - (real)0.5 * far;
+    real p1 = (real)0.5 * (near + other);
+    real q0 = near - far, q1 = other - near;
+    real e0 = eps + q0 * q0, e1 = eps + q1 * q1;
+    real a0 = e1 * e1;               // proportional to w0 = (1/3)/e0^2   (times e0^2 e1^2 * 3)
+    real a1 = (real)2 * (e0 * e0);   // proportional to w1 = (2/3)/e1^2
+    return (a0 * p0 + a1 * p1) / (a0 + a1);
+}
+
+template <typename real>
+__device__ __forceinline__ real upwind(real v, real bm, real bp) {
+    return v > (real)0 ? v * bm : (v < (real)0 ? v * bp : (real)0);
+}
+
+template <typename real>
+struct AdvArgs {
+    const real* in;   // f^(m-1)
+    const real* fn;   // f^n (read only if ca != 0)
+    real* out;        // f^(m) = ca f^n + cb f^(m-1) - cdt F_A(f^(m-1))      Eq. 25 (:418-424)
+    double* part;     // [R][2][nbx] phi-sums of the theta-flux at the faces next to the caps
+    real ca, cb, cdt;
+    int upwind_only;  // adv_flux == 1
+};
+
+// theta-face flux at face f (between rows f and f+1) from rows f-1, f, f+1, f+2 of one column.
+// Faces 1/2, 3/2, nt-1/2, nt+1/2 (f <= 1 or f >= nt-1) are upwind (:388); the others WENO3-CS(h) with LLF (B2).
+template <typename real>
+__device__ __forceinline__ real theta_face_flux(int f, real bm1, real b0, real bp1, real bp2, const real* lm,
+                                                const real* lp, const real* vtf, int nt, real eps, int upwind_only) {
+    if (upwind_only || f <= 1 || f >= nt - 1) return upwind(vtf[f], b0, bp1);
+    real um = weno3_side(bm1 * lm[f - 1], b0 * lm[f], bp1 * lm[f + 1], eps);   // right-moving part, from LM
+    real up = weno3_side(bp2 * lp[f + 2], bp1 * lp[f + 1], b0 * lp[f], eps);   // left-moving part, from LP
+    return up + um;
+}
+
+// phi-face flux at face k-1/2 of a row with uniform speed: LM = pm B, LP = pp B; one of pm, pp is exactly 0
+// and its one-sided value is exactly 0 (reading U13), so only the live side is evaluated.
+template <typename real>
+__device__ __forceinline__ real phi_face_flux(real bm2, real bm1, real b0, real bp1, real pm, real pp, real eps,
+                                              int upwind_only) {
+    if (upwind_only) return pm * bm1 + pp * b0;   // v>0: v B_{k-1}; v<0: v B_k; v=0: 0
+    if (pp == (real)0) return weno3_side(pm * bm2, pm * bm1, pm * b0, eps);
+    return weno3_side(pp * bp1, pp * b0, pp * bm1, eps);
+}
+
+template <typename real>
+__global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> T, Geom G) {
+    __shared__ double red[32];
+    const int r = blockIdx.z;
+    const int k = blockIdx.x * TX + threadIdx.x;
+    const bool live = k < G.np;
+    const int np = G.np, nt = G.nt;
+    const int k0 = live ? k : 0;
+    const int km1 = (k0 + np - 1) % np, km2 = (k0 + np - 2) % np, kp1 = (k0 + 1) % np, kp2 = (k0 + 2) % np;
+    const int j0 = 1 + blockIdx.y * RPT;            // rows 1..nt only; caps are done by k_adv_caps
+    const int j1 = min(j0 + RPT, nt + 1);
+    const size_t base = (size_t)r * G.rstride;
+    const real* in = A.in + base;
+    const real* lm = T.lm + (size_t)r * (nt + 2);
+    const real* lp = T.lp + (size_t)r * (nt + 2);
+    const real* vtf = T.vtf + (size_t)r * (nt + 1);
+    const real* pm = T.pm + (size_t)r * (nt + 2);
+    const real* pp = T.pp + (size_t)r * (nt + 2);
+    auto ld = [&](int j) -> real { return in[(size_t)min(max(j, 0), nt + 1) * G.pitch + k0]; };
+
+    real w0 = ld(j0 - 2), w1 = ld(j0 - 1), w2 = ld(j0), w3 = ld(j0 + 1);
+    real Fn = theta_face_flux<real>(j0 - 1, w0, w1, w2, w3, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
+    double sumN = 0.0, sumS = 0.0;
+    if (j0 == 1) sumN = live ? (double)Fn : 0.0;
+    for (int j = j0; j < j1; j++) {
+        real w4 = ld(j + 2);
+        real Fs = theta_face_flux<real>(j, w1, w2, w3, w4, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
+        const real* row = in + (size_t)j * G.pitch;
+        real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1], bp2 = row[kp2];
+        real Fw = phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, A.upwind_only);
+        real Fe = phi_face_flux<real>(bm1, w2, bp1, bp2, pm[j], pp[j], T.eps_p, A.upwind_only);
+        real tend = (T.sth[j] * Fs - T.sth[j - 1] * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
+        const size_t off = base + (size_t)j * G.pitch + k0;
+        real o = A.cb * w2 - A.cdt * tend;
+        if (A.ca != (real)0) o = A.ca * A.fn[off] + o;
+        if (live) A.out[off] = o;
+        if (j == nt) sumS = live ? (double)Fs : 0.0;
+        Fn = Fs;
+        w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+    }
+    if (j0 == 1) {
+        double t = block_sum(sumN, red);
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbx + blockIdx.x] = t;
+    }
+    if (j0 <= nt && nt < j1) {
+        double t = block_sum(sumS, red);
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbx + blockIdx.x] = t;
+    }
+}
+
+// Polar caps of one SSPRK stage (App. A :646): north +P sum_k F_theta[1/2,k] dph, south -P sum_k F_theta[nt+1/2,k] dph.
+// grid (nbx, 2, R): every CTA re-sums the partials in index order and writes its TX columns of the cap row.
+template <typename real>
+__global__ void __launch_bounds__(TX) k_adv_caps(AdvArgs<real> A, Tables<real> T, Geom G) {
+    const int r = blockIdx.z, pole = blockIdx.y;
+    const int k = blockIdx.x * TX + threadIdx.x;
+    if (k >= G.np) return;
+    const int j = pole == 0 ? 0 : G.nt + 1;
+    const size_t off = (size_t)r * G.rstride + (size_t)j * G.pitch;
+    double S = sum_partials(A.part + ((size_t)r * 2 + pole) * G.nbx, G.nbx);
+    real tend = (real)((pole == 0 ? 1.0 : -1.0) * (T.adv_capc * S));
+    real o = A.cb * A.in[off] - A.cdt * tend;
+    if (A.ca != (real)0) o = A.ca * A.fn[off] + o;
+    A.out[off + k] = o;
+}
+
+// ------------------------------------------------------------------ maps in / out, caps by row means
+
+// rows 1..nt of the state <- user map [nt][np] (dir 0) or the reverse (dir 1). grid (nbx, nt, nz):
+// state realization = r0 + blockIdx.z, map index = bcast ? 0 : blockIdx.z.
+template <typename real>
+__global__ void k_copy_map(real* state, real* map, Geom G, int r0, int bcast, int dir) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.y;  // 0..nt-1
+    if (k >= G.np) return;
+    real* s = state + (size_t)(r0 + blockIdx.z) * G.rstride + (size_t)(i + 1) * G.pitch + k;
+    real* m = map + ((size_t)(bcast ? 0 : blockIdx.z) * G.nt + i) * G.np + k;
+    if (dir == 0) *s = *m; else *m = *s;
+}
+
+// full field incl. cap rows <-> dense [nt+2][np]
+template <typename real>
+__global__ void k_copy_full(real* state, real* dense, Geom G, int r, int dir) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y;
+    if (k >= G.np) return;
+    real* s = state + (size_t)r * G.rstride + (size_t)j * G.pitch + k;
+    real* m = dense + (size_t)j * G.np + k;
+    if (dir == 0) *s = *m; else *m = *s;
+}
+
+// cap rows <- dph-weighted mean of the adjacent row (uniform grid: arithmetic mean). grid (2, R), block 256.
+template <typename real>
+__global__ void __launch_bounds__(256) k_caps_from_row_mean(real* state, Geom G, int r0) {
+    __shared__ double red[32];
+    __shared__ double mean;
+    const int pole = blockIdx.x, r = r0 + blockIdx.y;
+    real* f = state + (size_t)r * G.rstride;
+    const real* row = f + (size_t)(pole == 0 ? 1 : G.nt) * G.pitch;
+    double v = 0.0;
+    for (int k = threadIdx.x; k < G.np; k += blockDim.x) v += (double)row[k];
+    double t = block_sum(v, red);
+    if (threadIdx.x == 0) mean = t / (double)G.np;
+    __syncthreads();
+    real* cap = f + (size_t)(pole == 0 ? 0 : G.nt + 1) * G.pitch;
+    for (int k = threadIdx.x; k < G.np; k += blockDim.x) cap[k] = (real)mean;
+}
+
+// ------------------------------------------------------------------ assimilation + diagnostics
+
+constexpr int RED_CTAS = 64;  // CTAs per realization for the flux integrals
+
+// Flux integrals over rows 1..nt (:225-230): part[r][cta][2] = {sum_{v>0} v dA, sum_{v<=0 or <0} v dA}.
+// WHAT 0: v = B (diagnostics; v == 0 contributes 0 either way).  WHAT 1: v = w (obs - B) (Eq. 10 increment, :146).
+template <typename real, int WHAT>
+__global__ void __launch_bounds__(256) k_flux_partials(const real* state, const real* obs, const real* wgt, int shared,
+                                                       Tables<real> T, Geom G, double* part) {
+    __shared__ double red[32];
+    const int r = blockIdx.y;
+    const real* f = state + (size_t)r * G.rstride;
+    const size_t mapoff = shared ? 0 : (size_t)r * G.nt * G.np;
+    double pp = 0.0, pm = 0.0;
+    for (int j = 1 + blockIdx.x; j <= G.nt; j += gridDim.x) {
+        double dA = T.dA[j], rp = 0.0, rm = 0.0;
+        for (int k = threadIdx.x; k < G.np; k += blockDim.x) {
+            real v = f[(size_t)j * G.pitch + k];
+            if (WHAT == 1) {
+                size_t m = mapoff + (size_t)(j - 1) * G.np + k;
+                v = wgt[m] * (obs[m] - v);
+            }
+            if (v > (real)0) rp += (double)v; else rm += (double)v;
+        }
+        pp += rp * dA;
+        pm += rm * dA;
+    }
+    double tp = block_sum(pp, red);
+    double tm = block_sum(pm, red);
+    if (threadIdx.x == 0) {
+        part[((size_t)r * gridDim.x + blockIdx.x) * 2 + 0] = tp;
+        part[((size_t)r * gridDim.x + blockIdx.x) * 2 + 1] = tm;
+    }
+}
+
+// Cap obs / weight = row means of the adjacent row (reading U18); capinfo[r][pole] = {obs_mean, w_mean}. grid (2, R or 1)
+template <typename real>
+__global__ void __launch_bounds__(256) k_assim_cap_means(const real* obs, const real* wgt, Geom G, double* capinfo) {
+    __shared__ double red[32];
+    const int pole = blockIdx.x, r = blockIdx.y;
+    const size_t rowoff = (size_t)r * G.nt * G.np + (size_t)(pole == 0 ? 0 : G.nt - 1) * G.np;
+    double a = 0.0, b = 0.0;
+    for (int k = threadIdx.x; k < G.np; k += blockDim.x) { a += (double)obs[rowoff + k]; b += (double)wgt[rowoff + k]; }
+    double ta = block_sum(a, red);
+    double tb = block_sum(b, red);
+    if (threadIdx.x == 0) {
+        capinfo[((size_t)r * 2 + pole) * 2 + 0] = ta / (double)G.np;
+        capinfo[((size_t)r * 2 + pole) * 2 + 1] = tb / (double)G.np;
+    }
+}
+
+// Finalize flux integrals: add the caps (area dA[0] = dA[nt+1] = A_pole), sum the CTA partials in index order.
+// WHAT 0: out[r][4] = {signed, unsigned, Phi+, Phi-} * scale.   WHAT 1: out[r] = sqrt|Phi+/Phi-| (1 if either is 0).
+template <typename real, int WHAT>
+__global__ void k_flux_finalize(const real* state, const double* part, int nparts, const double* capinfo, int shared,
+                                Tables<real> T, Geom G, double scale, double* out) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= G.nr) return;
+    double pp = 0.0, pm = 0.0;
+    for (int i = 0; i < nparts; i++) { pp += part[((size_t)r * nparts + i) * 2]; pm += part[((size_t)r * nparts + i) * 2 + 1]; }
+    for (int pole = 0; pole < 2; pole++) {
+        real v = state[(size_t)r * G.rstride + (size_t)(pole == 0 ? 0 : G.nt + 1) * G.pitch];
+        if (WHAT == 1) {
+            const double* ci = capinfo + ((size_t)(shared ? 0 : r) * 2 + pole) * 2;
+            v = (real)ci[1] * ((real)ci[0] - v);
+        }
+        double c = (double)v * T.dA[0];
+        if (v > (real)0) pp += c; else pm += c;
+    }
+    if (WHAT == 0) {
+        out[4 * r + 0] = (pp + pm) * scale;
+        out[4 * r + 1] = (pp - pm) * scale;
+        out[4 * r + 2] = pp * scale;
+        out[4 * r + 3] = pm * scale;
+    } else {
+        out[r] = (pp != 0.0 && pm != 0.0) ? sqrt(fabs(pp / pm)) : 1.0;
+    }
+}
+
+// Blend (Eq. 8 :131) or flux-balanced blend (Eq. 10-11 :144-153) on rows 0..nt+1; grid (nbx, nt+2, R).
+template <typename real>
+__global__ void __launch_bounds__(TX) k_assim_blend(real* state, const real* obs, const real* wgt, int shared,
+                                                    const double* capinfo, const double* scale, int balanced, Geom G) {
+    const int k = blockIdx.x * TX + threadIdx.x, j = blockIdx.y, r = blockIdx.z;
+    if (k >= G.np) return;
+    real* p = state + (size_t)r * G.rstride + (size_t)j * G.pitch + k;
+    real F, Bd;
+    if (j == 0 || j == G.nt + 1) {
+        const double* ci = capinfo + ((size_t)(shared ? 0 : r) * 2 + (j == 0 ? 0 : 1)) * 2;
+        Bd = (real)ci[0];
+        F = (real)ci[1];
+    } else {
+        size_t m = (shared ? 0 : (size_t)r * G.nt * G.np) + (size_t)(j - 1) * G.np + k;
+        Bd = obs[m];
+        F = wgt[m];
+    }
+    real B = *p;
+    if (!balanced) {
+        *p = F * Bd + ((real)1 - F) * B;
+    } else {
+        real sc = (real)scale[r];
+        real d = F * (Bd - B);
+        d = (d > (real)0) ? d / sc : d * sc;
+        *p = B + d;
+    }
+}
+
+}  // namespace hft

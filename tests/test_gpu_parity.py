@@ -1,0 +1,250 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): fp64 relative L-inf <= 1e-12 of max|Br|, fp32 <= 1e-5
+(against the oracle instantiated in float; the error against the fp64 oracle is also checked at 1e-5)."""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+from helpers import rel_linf
+from oracle import sft_oracle as orc
+from paper_2501_06377_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+NPDT = {"f64": np.float64, "f32": np.float32}
+
+
+def hft():
+    from paper_2501_06377_b200 import hft as m
+    return m
+
+
+def make_pair(w, dtype, **opt):
+    """(gpu context, oracle) with the same parameters and initial maps."""
+    H = hft()
+    maps = wl.initial_maps(w)                                   # fp64 CPU tensor [R][nt][np]
+    maps_t = maps.to(torch.float64 if dtype == "f64" else torch.float32)
+    ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype, **opt)
+    o = orc.Oracle(w.n_theta, w.n_phi, w.params, dtype=NPDT[dtype])
+    for r in range(w.n_real):
+        ctx.set_map(r, maps_t[r].contiguous().cuda())
+        o.set_map(r, maps_t[r].numpy())
+    return ctx, o
+
+
+def compare(ctx, o, tol, what=""):
+    worst = 0.0
+    for r in range(o.nr):
+        g = ctx.get_full(r).cpu().numpy()
+        e = rel_linf(g, o.get_full(r))
+        worst = max(worst, e)
+        assert np.isfinite(g).all()
+        assert e <= tol, (what, r, e)
+    return worst
+
+
+def test_set_get_roundtrip_and_pole_cell_averaging():
+    H = hft()
+    for dtype in ("f64", "f32"):
+        w = wl.scaled(wl.config(3), 37, 200, n_real=3)           # ragged: 200 is not a multiple of 128
+        ctx, o = make_pair(w, dtype)
+        assert compare(ctx, o, 1e-15 if dtype == "f64" else 1e-7) >= 0.0
+        allm = ctx.get_map(-1).cpu().numpy()
+        for r in range(3):
+            assert np.array_equal(allm[r], o.get_map(r)) and np.array_equal(ctx.get_map(r).cpu().numpy(), o.get_map(r))
+        m = torch.randn(37, 200, dtype=ctx.tdtype, device="cuda")
+        ctx.set_map(-1, m)
+        assert all(torch.equal(ctx.get_map(r), m) for r in range(3))
+        ga, gd = ctx.stable_dt()
+        oa, od = o.stable_dt()
+        assert abs(ga / oa - 1) < 1e-14 and abs(gd / od - 1) < 1e-14
+        assert ctx.sts_stage_count(37.0 * gd) == o.sts_stage_count(37.0 * od, orc.DIFF_RKG2)
+        ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("block", [1, 0])
+def test_config0_diffusion_only_full_length(dtype, block):
+    """BASELINE config 0: 64x128, 6 pairs, eta = 500, s = 8 forced, dt = 8 dt_expl, 200 steps."""
+    H = hft()
+    w = wl.config(0)
+    ctx, o = make_pair(w, dtype, adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKG2, sts_stages=8, sts_block=block)
+    dt, n, _ = wl.plan(w, *o.stable_dt())
+    dg = wl.plan(w, *ctx.stable_dt())
+    assert dg[1] == n and abs(dg[0] / dt - 1) < 1e-14
+    before = ctx.diagnostics()
+    ctx.step(n, dt)
+    o.step(n, dt, adv_flux=orc.ADV_OFF, diff_time=orc.DIFF_RKG2, sts_stages=8)
+    compare(ctx, o, TOL[dtype], "cfg0")
+    after = ctx.diagnostics()
+    cons = 1e-12 if dtype == "f64" else 2e-5
+    assert abs(after[0, 0] - before[0, 0]) <= cons * before[0, 1]      # signed flux conserved
+    assert np.allclose(after, o.diagnostics(), rtol=0, atol=cons * before[0, 1])
+    ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("block", [1, 0])
+def test_y21_decay_on_gpu(dtype, block):
+    H = hft()
+    w = wl.config(0)
+    ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype, adv_flux=H.ADV_OFF, sts_stages=8, sts_block=block)
+    y = wl.y21_map(w.n_theta, w.n_phi).to(ctx.tdtype).cuda()
+    ctx.set_map(0, y)
+    _, dtd = ctx.stable_dt()
+    ctx.step(200, 8 * dtd)
+    nu = 500.0 * 7.43162901307967e-9
+    exact = y.double() * math.exp(-6 * nu * 200 * 8 * dtd)
+    assert (ctx.get_map(0).double() - exact).abs().max().item() < 6e-5
+    ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("case", ["weno_ssprk43_rkg2", "upwind_euler_rkl2", "weno_ssprk33_euler", "adv_only", "diff_auto_s"])
+def test_small_ragged_multi_realization(dtype, case):
+    """Several tiles and a ragged tail in both directions, 3 realizations with different parameters."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 75, 200, n_real=3)
+    opts = {
+        "weno_ssprk43_rkg2": dict(adv_flux=2, adv_time=4, diff_time=3),
+        "upwind_euler_rkl2": dict(adv_flux=1, adv_time=1, diff_time=2),
+        "weno_ssprk33_euler": dict(adv_flux=2, adv_time=3, diff_time=1),
+        "adv_only": dict(adv_flux=2, adv_time=4, diff_time=0),
+        "diff_auto_s": dict(adv_flux=0, adv_time=4, diff_time=3),
+    }[case]
+    ctx, o = make_pair(w, dtype, **opts)
+    adv, dif = o.stable_dt()
+    dt = {"weno_ssprk43_rkg2": 0.5 * adv, "upwind_euler_rkl2": 0.4 * adv, "weno_ssprk33_euler": 0.9 * dif,
+          "adv_only": 0.5 * adv, "diff_auto_s": 300.0 * dif}[case]
+    n = 6
+    ctx.step(n, dt)
+    s = o.step(n, dt, **opts)
+    if opts["diff_time"] >= 2:
+        assert s == ctx.sts_stage_count(dt)
+    compare(ctx, o, TOL[dtype], case)
+    # the error against the fp64 oracle (arithmetic design, reading U14)
+    if dtype == "f32":
+        o64 = orc.Oracle(w.n_theta, w.n_phi, w.params)
+        maps = wl.initial_maps(w).to(torch.float32)
+        for r in range(3):
+            o64.set_map(r, maps[r].numpy().astype(np.float64))
+        o64.step(n, dt, **opts)
+        compare(ctx, o64, 1e-5, case + " vs fp64 oracle")
+    ctx.close()
+
+
+@pytest.mark.parametrize("block", [1, 0])
+def test_config1_full_length(block):
+    """BASELINE config 1: 512x1024, 40 pairs, flows of reading U17, eta = 500, 16 steps of 1.5 h, s = 217."""
+    H = hft()
+    w = wl.config(1)
+    ctx, o = make_pair(w, "f64", sts_block=block)
+    dt, n, _ = wl.plan(w, *ctx.stable_dt())
+    assert n == 16 and abs(dt - 1.5) < 1e-12 and ctx.sts_stage_count(dt) == 217
+    before = ctx.diagnostics()
+    ctx.step(n, dt)
+    o.step(n, dt)
+    compare(ctx, o, 1e-12, "cfg1")
+    after = ctx.diagnostics()
+    assert abs(after[0, 0] - before[0, 0]) <= 1e-12 * before[0, 1]
+    ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config3_full_size_sampled_realizations(dtype):
+    """BASELINE config 3 at full size (1024x2048, 64 realizations) in the launch configuration bench.py
+    times, 2 steps; the oracle checks sampled realizations one by one; all 64 conserve flux."""
+    H = hft()
+    w = wl.config(3, dtype)
+    ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype)
+    maps = wl.initial_maps(w, device="cuda").to(ctx.tdtype)
+    for r in range(w.n_real):
+        ctx.set_map(r, maps[r].contiguous())
+    dt, _, _ = wl.plan(w, *ctx.stable_dt())
+    before = ctx.diagnostics()
+    ctx.step(2, dt)
+    after = ctx.diagnostics()
+    cons = 1e-12 if dtype == "f64" else 2e-5
+    assert np.all(np.abs(after[:, 0] - before[:, 0]) <= cons * before[:, 1])
+    for r in (0, 42) if dtype == "f64" else (21,):
+        # one realization at a time, with the ensemble's dt and stage count (one s for all realizations)
+        o = orc.Oracle(w.n_theta, w.n_phi, w.params[r:r + 1], dtype=NPDT[dtype])
+        o.set_map(0, maps[r].cpu().numpy())
+        o.step(2, dt, sts_stages=ctx.sts_stage_count(dt))
+        e = rel_linf(ctx.get_full(r).cpu().numpy(), o.get_full(0))
+        assert e <= TOL[dtype], (r, e)
+    ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_assimilation_and_diagnostics(dtype):
+    """Config 4 recipe on a small grid: steps, hourly blend with disc weights, per-realization and shared
+    observations, flux-balanced variant, diagnostics."""
+    H = hft()
+    w = wl.scaled(wl.config(4), 60, 136, t_end_hours=3.0)
+    w.params = np.repeat(w.params, 2, axis=0)
+    w.params[1, 0] = 350.0
+    w.n_real = 2
+    ctx, o = make_pair(w, dtype)
+    dt, n, per = wl.plan(w, *ctx.stable_dt())
+    tdt = ctx.tdtype
+    t = 0.0
+    for it in range(3):
+        ctx.step(per, dt)
+        o.step(per, dt)
+        t += per * dt
+        E = wl.emergence_map(w, it)
+        wt = wl.assimilation_weights(w, t)
+        if it == 1:            # shared observation map
+            obs = (ctx.get_map(0).cpu().double() + E).to(tdt)
+            ctx.assimilate(obs.cuda(), wt.to(tdt).cuda())
+            o.assimilate(obs.numpy(), wt.to(tdt).numpy())
+        else:                  # per-realization observation = own state + emergence
+            cur = ctx.get_map(-1).cpu().double()
+            obs = (cur + E[None]).to(tdt).contiguous()
+            wts = wt[None].expand(2, -1, -1).to(tdt).contiguous()
+            ctx.assimilate(obs.cuda(), wts.cuda(), flags=H.FLAG_FLUX_BALANCE if it == 2 else 0)
+            o.assimilate(obs.numpy(), wts.numpy(), flags=1 if it == 2 else 0)
+        compare(ctx, o, TOL[dtype], f"assim {it}")
+    dg, do = ctx.diagnostics(), o.diagnostics()
+    assert np.allclose(dg, do, rtol=0, atol=(1e-12 if dtype == "f64" else 1e-5) * do[:, 1].max())
+    ctx.close()
+
+
+def test_custom_flow_tables_appendix_c():
+    """hft_set_flow_tables: constant v_theta, the App. C solution moves without changing shape."""
+    H = hft()
+    nt, nphi = 127, 64
+    ctx = H.Context(nt, nphi, [[0.0] * 7], diff_time=H.DIFF_OFF)
+    o = orc.Oracle(nt, nphi, [[0.0] * 7])
+    v_ms = 200.0
+    ctx.set_flow_tables(0, np.full(nt + 1, v_ms), np.zeros(nt + 2))
+    o.set_flow_tables(0, np.full(nt + 1, v_ms * 5.172413793103448e-6), np.zeros(nt + 2))
+    th = wl.colatitudes(nt)[:, None]
+    B = (torch.exp(-(th - math.pi / 4) ** 2 / 0.03) / torch.sin(th)).expand(-1, nphi).contiguous()
+    ctx.set_map(0, B.cuda())
+    o.set_map(0, B.numpy())
+    adv, _ = ctx.stable_dt()
+    assert abs(adv / o.stable_dt()[0] - 1) < 1e-14
+    ctx.step(40, 0.5 * adv)
+    o.step(40, 0.5 * adv, diff_time=orc.DIFF_OFF)
+    compare(ctx, o, 1e-12, "appendix C")
+    v = v_ms * 5.172413793103448e-6
+    exact = torch.exp(-(th - math.pi / 4 - v * 20 * adv) ** 2 / 0.03) / torch.sin(th)
+    assert (ctx.get_map(0).cpu()[:, 0:1] - exact).abs().max().item() < 2e-3
+    ctx.close()
+
+
+def test_errors_are_reported():
+    H = hft()
+    ctx = H.Context(64, 128, [[500.0, 0, 0, 0, 0, 0, 0]], adv_flux=H.ADV_OFF, sts_stages=2)
+    _, dtd = ctx.stable_dt()
+    with pytest.raises(H.HftError, match="unstable"):
+        ctx.step(1, 50 * dtd)                    # s = 2 forced is too few stages for this dt
+    with pytest.raises(H.HftError):
+        ctx.step(1, -1.0)
+    assert ctx.launch_count() >= 0
+    ctx.close()
