@@ -169,7 +169,7 @@ def main():
         barrier()
         ms = e0.elapsed_time(e1)
         launches = ctx.launch_count() - l0
-        kms, kn = ctx.kernel_time()
+        kms, kn, kst = ctx.kernel_time()
         ctx.profile_kernels(0)
         clocks = sampler.stop() if (rank == 0 and with_extras) else None
         if dist is not None:
@@ -177,7 +177,7 @@ def main():
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms = t.item()
         res = dict(ms=ms, value=world * cells * args.steps / (ms * 1e-3), launches=launches, dt=dt, s=s, cells=cells,
-                   kernel_ms=(kms / kn if kn else None), kernel_samples=kn, clocks=clocks, wd=wd)
+                   kernel_ms=(kms / kn if kn else None), kernel_samples=kn, kernel_stages=(kst / kn if kn else None), clocks=clocks, wd=wd)
         # ---- end-to-end through the C ABI with host buffers
         if with_extras and not args.no_e2e:
             host_in = maps.cpu().pin_memory()
@@ -232,11 +232,11 @@ def main():
         out["e2e"] = res["e2e"]
     if res["kernel_ms"]:
         # dominant kernel: the STS stage kernel; algorithmic bytes per launch = 4 passes x field bytes x stages per launch
-        stages_per_launch = max(1, round(res["s"] * args.steps / max(1, res["launches"] - 9 * args.steps)))
+        stages_per_launch = res["kernel_stages"]
         field_bytes = wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes
         ach = 4 * field_bytes * stages_per_launch / (res["kernel_ms"] * 1e-3) / 1e9
         out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                           "kernel": "k_sts_stage", "stages_per_launch": stages_per_launch, "avg_launch_ms": res["kernel_ms"],
+                           "kernel": "k_sts_blocked" if stages_per_launch > 1 else "k_sts_stage", "stages_per_launch": stages_per_launch, "avg_launch_ms": res["kernel_ms"],
                            "sampled_launches": res["kernel_samples"], "peak_source": peak_src}
     if args.also_f32 and args.dtype == "f64":
         r32 = timed_run("f32", False)

@@ -125,10 +125,12 @@ int hft_sts_stage_count(hft_ctx* ctx, double dt_hours, int32_t* h_stages);
 int hft_launch_count(hft_ctx* ctx, int64_t* h_count);
 
 /* Enable per-kernel CUDA-event timing on the context's stream for the kernel class `which`
- * (0 = none, 1 = STS stage kernels, 2 = advection stage kernels); hft_kernel_time returns the
- * accumulated milliseconds and launches since the last call and resets them (synchronises). */
+ * (0 = none, 1 = STS stage kernels, 2 = advection stage kernels); every 16th launch of the class
+ * is bracketed by events.  hft_kernel_time returns the accumulated milliseconds of the sampled launches,
+ * their number and the number of stages (STS stages / SSPRK stages) they covered since the last call,
+ * and resets them (synchronises). */
 int hft_profile_kernels(hft_ctx* ctx, int32_t which);
-int hft_kernel_time(hft_ctx* ctx, double* h_ms, int64_t* h_launches);
+int hft_kernel_time(hft_ctx* ctx, double* h_ms, int64_t* h_launches, int64_t* h_stages);
 
 const char* hft_error_string(int code);
 const char* hft_last_cuda_error(hft_ctx* ctx);

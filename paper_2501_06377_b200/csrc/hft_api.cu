@@ -67,6 +67,7 @@ struct hft_ctx {
     // sampled kernel timing
     int prof_which = 0;
     int prof_n = 0;
+    int64_t prof_stages = 0;
     int64_t prof_seen = 0;
     cudaEvent_t prof_ev[2 * kProfEvents];
     bool prof_ev_made = false;
@@ -150,7 +151,7 @@ void build_flow(hft_ctx* c, int r, const hft_params& p) {
 
 template <typename real>
 struct HostTab {
-    std::vector<real> cp, cm, cf, lm, lp, vtf, pm, pp, sth, rdt, rdp;
+    std::vector<real> cp, cm, cf, cd, lm, lp, vtf, pm, pp, sth, rdt, rdp;
     std::vector<double> capc, dA;
 };
 
@@ -158,7 +159,7 @@ template <typename real>
 void fill_tables(const hft_ctx* c, HostTab<real>& H) {
     const int nt = c->G.nt, R = c->nr;
     const size_t n2 = (size_t)R * (nt + 2);
-    H.cp.assign(n2, 0); H.cm.assign(n2, 0); H.cf.assign(n2, 0); H.lm.assign(n2, 0); H.lp.assign(n2, 0);
+    H.cp.assign(n2, 0); H.cm.assign(n2, 0); H.cf.assign(n2, 0); H.cd.assign(n2, 0); H.lm.assign(n2, 0); H.lp.assign(n2, 0);
     H.pm.assign(n2, 0); H.pp.assign(n2, 0);
     H.vtf.assign((size_t)R * (nt + 1), 0);
     H.sth.resize(nt + 1); H.rdt.assign(nt + 2, 0); H.rdp.assign(nt + 2, 0);
@@ -182,6 +183,7 @@ void fill_tables(const hft_ctx* c, HostTab<real>& H) {
                 H.cp[i] = (real)(nu * c->sth[j] / (c->st[j] * c->dth * c->dth));
                 H.cm[i] = (real)(nu * c->sth[j - 1] / (c->st[j] * c->dth * c->dth));
                 H.cf[i] = (real)(nu / (c->st[j] * c->st[j] * c->dph * c->dph));
+                H.cd[i] = (real)((double)H.cp[i] + (double)H.cm[i] + 2.0 * (double)H.cf[i]);
             }
             // LLF (B2 :684) with alpha_j = max |v| over faces j-5/2 .. j+5/2 that exist (:689)
             double al = 0.0;
@@ -208,7 +210,7 @@ int upload_tables(hft_ctx* c, Tables<real>& T) {
     const size_t n2 = (size_t)R * (nt + 2) * sizeof(real), n1 = (size_t)R * (nt + 1) * sizeof(real);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = round_up(off + bytes, 256); return o; };
-    size_t o_cp = take(n2), o_cm = take(n2), o_cf = take(n2), o_lm = take(n2), o_lp = take(n2), o_pm = take(n2), o_pp = take(n2);
+    size_t o_cp = take(n2), o_cm = take(n2), o_cf = take(n2), o_cd = take(n2), o_lm = take(n2), o_lp = take(n2), o_pm = take(n2), o_pp = take(n2);
     size_t o_vtf = take(n1), o_sth = take((nt + 1) * sizeof(real)), o_rdt = take((nt + 2) * sizeof(real)), o_rdp = take((nt + 2) * sizeof(real));
     size_t o_capc = take(R * sizeof(double)), o_dA = take((nt + 2) * sizeof(double));
     if (!c->d_tab) {
@@ -217,13 +219,13 @@ int upload_tables(hft_ctx* c, Tables<real>& T) {
     }
     char* d = c->d_tab;
     auto up = [&](size_t o, const void* src, size_t bytes) { return cudaMemcpyAsync(d + o, src, bytes, cudaMemcpyHostToDevice, c->stream); };
-    CK(up(o_cp, H.cp.data(), n2)); CK(up(o_cm, H.cm.data(), n2)); CK(up(o_cf, H.cf.data(), n2));
+    CK(up(o_cp, H.cp.data(), n2)); CK(up(o_cm, H.cm.data(), n2)); CK(up(o_cf, H.cf.data(), n2)); CK(up(o_cd, H.cd.data(), n2));
     CK(up(o_lm, H.lm.data(), n2)); CK(up(o_lp, H.lp.data(), n2)); CK(up(o_pm, H.pm.data(), n2)); CK(up(o_pp, H.pp.data(), n2));
     CK(up(o_vtf, H.vtf.data(), n1)); CK(up(o_sth, H.sth.data(), (nt + 1) * sizeof(real)));
     CK(up(o_rdt, H.rdt.data(), (nt + 2) * sizeof(real))); CK(up(o_rdp, H.rdp.data(), (nt + 2) * sizeof(real)));
     CK(up(o_capc, H.capc.data(), R * sizeof(double))); CK(up(o_dA, H.dA.data(), (nt + 2) * sizeof(double)));
     CK(cudaStreamSynchronize(c->stream));  // H goes out of scope
-    T.cp = (const real*)(d + o_cp); T.cm = (const real*)(d + o_cm); T.cf = (const real*)(d + o_cf);
+    T.cp = (const real*)(d + o_cp); T.cm = (const real*)(d + o_cm); T.cf = (const real*)(d + o_cf); T.cd = (const real*)(d + o_cd);
     T.lm = (const real*)(d + o_lm); T.lp = (const real*)(d + o_lp); T.pm = (const real*)(d + o_pm); T.pp = (const real*)(d + o_pp);
     T.vtf = (const real*)(d + o_vtf); T.sth = (const real*)(d + o_sth); T.rdt = (const real*)(d + o_rdt); T.rdp = (const real*)(d + o_rdp);
     T.capc = (const double*)(d + o_capc); T.dA = (const double*)(d + o_dA);
@@ -316,8 +318,9 @@ void prof_begin(hft_ctx* c, int cls, bool& armed) {
     cudaEventRecord(c->prof_ev[2 * c->prof_n], c->stream);
     armed = true;
 }
-void prof_end(hft_ctx* c, bool armed) {
+void prof_end(hft_ctx* c, bool armed, int stages) {
     if (!armed) return;
+    c->prof_stages += stages;
     cudaEventRecord(c->prof_ev[2 * c->prof_n + 1], c->stream);
     c->prof_n++;
 }
@@ -361,7 +364,7 @@ int advect(hft_ctx* c, double dt) {
         bool armed;
         prof_begin(c, 2, armed);
         k_adv_stage<real><<<g, TX, 0, c->stream>>>(a, T, G);
-        prof_end(c, armed);
+        prof_end(c, armed, 1);
         k_adv_caps<real><<<gc, TX, 0, c->stream>>>(a, T, G);
         c->launches += 2;
     }
@@ -398,7 +401,7 @@ int diffuse_unblocked(hft_ctx* c, double dt, int s) {
     bool armed;
     prof_begin(c, 1, armed);
     k_sts_stage<real, 0><<<g, TX, 0, c->stream>>>(a, T, G);
-    prof_end(c, armed);
+    prof_end(c, armed, 1);
     c->launches++;
     real *d1 = da, *d2 = db;
     int pin = 1;
@@ -409,7 +412,7 @@ int diffuse_unblocked(hft_ctx* c, double dt, int s) {
         prof_begin(c, 1, armed);
         if (j < s) k_sts_stage<real, 1><<<g, TX, 0, c->stream>>>(a, T, G);
         else k_sts_stage<real, 2><<<g, TX, 0, c->stream>>>(a, T, G);
-        prof_end(c, armed);
+        prof_end(c, armed, 1);
         c->launches++;
         real* t = d1; d1 = d2; d2 = t;
         pin ^= 1;
@@ -432,7 +435,7 @@ int step_once(hft_ctx* c, double dt, int s) {
             P.s = s; P.kb = kb; P.stream = c->stream;
             P.part = c->d_part; P.zmean = c->d_zmean; P.capseq = c->d_capseq;
             P.prof_begin = [](void* u, bool* armed) { prof_begin((hft_ctx*)u, 1, *armed); };
-            P.prof_end = [](void* u, bool armed) { prof_end((hft_ctx*)u, armed); };
+            P.prof_end = [](void* u, bool armed, int stages) { prof_end((hft_ctx*)u, armed, stages); };
             P.user = c;
             int64_t n = 0;
             rc = sts_blocked_step<real>(P, tables_of<real>(c), c->G, &n);
@@ -685,12 +688,12 @@ int hft_profile_kernels(hft_ctx* c, int32_t which) {
         for (int i = 0; i < 2 * kProfEvents; i++) CK(cudaEventCreate(&c->prof_ev[i]));
         c->prof_ev_made = true;
     }
-    c->prof_which = which; c->prof_n = 0; c->prof_seen = 0;
+    c->prof_which = which; c->prof_n = 0; c->prof_seen = 0; c->prof_stages = 0;
     return HFT_OK;
 }
 
-int hft_kernel_time(hft_ctx* c, double* h_ms, int64_t* h_launches) {
-    if (!c || !h_ms || !h_launches) return HFT_ERR_ARG;
+int hft_kernel_time(hft_ctx* c, double* h_ms, int64_t* h_launches, int64_t* h_stages) {
+    if (!c || !h_ms || !h_launches || !h_stages) return HFT_ERR_ARG;
     CK(cudaStreamSynchronize(c->stream));
     double ms = 0.0;
     for (int i = 0; i < c->prof_n; i++) {
@@ -698,8 +701,8 @@ int hft_kernel_time(hft_ctx* c, double* h_ms, int64_t* h_launches) {
         CK(cudaEventElapsedTime(&t, c->prof_ev[2 * i], c->prof_ev[2 * i + 1]));
         ms += t;
     }
-    *h_ms = ms; *h_launches = c->prof_n;
-    c->prof_n = 0; c->prof_seen = 0;
+    *h_ms = ms; *h_launches = c->prof_n; *h_stages = c->prof_stages;
+    c->prof_n = 0; c->prof_seen = 0; c->prof_stages = 0;
     return HFT_OK;
 }
 

@@ -1,34 +1,362 @@
-// hft_sts_blocked.cuh -- temporally blocked STS stages (k stages per launch).  STUB: filled in next.
+// hft_sts_blocked.cuh -- temporally blocked super-time-stepping: K STS stages per kernel launch.
+//
+// Why: one launch per stage moves 4 field passes per stage through HBM (read delta_{j-1}, delta_{j-2},
+// L(Y0); write delta_j).  Blocking K stages on chip moves 3 reads + 2 writes per K stages instead.
+//
+// How: every WARP owns a strip of 32*C consecutive phi-columns (C columns
+// per lane, one 16-byte vector) and streams down the theta-rows.  The K stage levels form a software
+// pipeline skewed by one row per level: at row-step t the warp loads row t of the three inputs and
+// computes row t-l of level l for l = 1..K.  Each level keeps a 3-row window in REGISTERS (theta
+// neighbours), the phi neighbours come from the adjacent lanes by warp shuffle, so the stencil never
+// touches shared memory and warps never synchronise with each other.  The price is a halo: the first and
+// last K columns of a warp's strip become invalid (one column per level and side), so strips overlap by
+// 2K columns and only 32*C - 2K columns are written.  Periodic phi is an index wrap of the strip origin.
+//
+// Polar caps: the cap update of level l needs the phi-sum of row 1 at level l-1 over ALL columns, a global
+// dependency per stage.  Because every coefficient of L is phi-independent and phi is periodic, the
+// phi-mean commutes with L: the zonal means m_j = mean_k u_jk obey the same recurrence with the phi-term
+// dropped.  So the K cap values of a block follow from the zonal means of rows 1..K of the three input
+// fields alone (a cone of K rows); k_sts_capseq computes them before the main kernel, which then treats
+// rows 0 and nt+1 of every level as known boundary values.  (Exact in exact arithmetic; in floating
+// point it differs from summing the actual stage rows by round-off only.  Valid because nu is constant in
+// space -- SURVEY section 8 scope; a spatially varying nu would need the per-stage reduction instead.)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+
 #include "hft_kernels.cuh"
 
 namespace hft {
 
 constexpr int STS_KMAX = 8;
+constexpr int BLK_WARPS = 4;  // warps per CTA: adjacent strips share their halo loads through L1
+
+template <typename real, int C> struct VecOf;
+template <> struct VecOf<double, 2> { typedef double2 type; };
+template <> struct VecOf<float, 4> { typedef float4 type; };
+template <> struct VecOf<float, 2> { typedef float2 type; };
+
+template <typename real, int C>
+__device__ __forceinline__ void vload(real (&d)[C], const real* p) {
+    typename VecOf<real, C>::type v = *reinterpret_cast<const typename VecOf<real, C>::type*>(p);
+    const real* s = reinterpret_cast<const real*>(&v);
+#pragma unroll
+    for (int i = 0; i < C; i++) d[i] = s[i];
+}
+template <typename real, int C>
+__device__ __forceinline__ void vstore(real* p, const real (&d)[C]) {
+    typename VecOf<real, C>::type v;
+    real* s = reinterpret_cast<real*>(&v);
+#pragma unroll
+    for (int i = 0; i < C; i++) s[i] = d[i];
+    *reinterpret_cast<typename VecOf<real, C>::type*>(p) = v;
+}
+
+template <typename real, int K>
+struct BlkArgs {
+    const real* cur;   // level 0  = delta_{j0}
+    const real* prev;  // level -1 = delta_{j0-1} (not read if !has_prev: delta_0 = 0)
+    const real* F;     // L(Y0)
+    real* ocur;        // level K   = delta_{j0+K}
+    real* oprev;       // level K-1 = delta_{j0+K-1}
+    real* Y0;          // last block: Y0 += delta_s, ocur/oprev not written
+    const double* capseq;  // [R][2][K] cap values of levels 1..K
+    real mu[K], nu[K], a[K], g[K];  // scalars of stages j0+1 .. j0+K
+    int has_prev, last;
+    int rows_per_seg, nstrips;
+};
+
+// ------------------------------------------------------------------ cap sequence from zonal means
+// grid (2 poles, R), block 256.  i = distance from the pole in rows (i = 0 is the cap itself).
+template <typename real, int K>
+__global__ void __launch_bounds__(256) k_sts_capseq(BlkArgs<real, K> A, Tables<real> T, Geom G, double* capseq) {
+    __shared__ double red[32];
+    __shared__ double m0[K + 1], mp[K + 1], mF[K + 1];
+    const int pole = blockIdx.x, r = blockIdx.y;
+    const size_t base = (size_t)r * G.rstride;
+    auto rowidx = [&](int i) { return pole == 0 ? i : G.nt + 1 - i; };
+    for (int i = 1; i <= K; i++) {
+        const size_t off = base + (size_t)rowidx(i) * G.pitch;
+        double a = 0.0, b = 0.0, c = 0.0;
+        for (int k = threadIdx.x; k < G.np; k += blockDim.x) {
+            a += (double)A.cur[off + k];
+            if (i < K) {
+                if (A.has_prev) b += (double)A.prev[off + k];
+                c += (double)A.F[off + k];
+            }
+        }
+        double ta = block_sum(a, red);
+        double tb = block_sum(b, red);
+        double tc = block_sum(c, red);
+        if (threadIdx.x == 0) { m0[i] = ta / (double)G.np; mp[i] = tb / (double)G.np; mF[i] = tc / (double)G.np; }
+    }
+    if (threadIdx.x != 0) return;
+    const size_t capoff = base + (size_t)rowidx(0) * G.pitch;
+    m0[0] = (double)A.cur[capoff];
+    mp[0] = A.has_prev ? (double)A.prev[capoff] : 0.0;
+    mF[0] = (double)A.F[capoff];
+    const real* cp = T.cp + (size_t)r * (G.nt + 2);
+    const real* cm = T.cm + (size_t)r * (G.nt + 2);
+    const double capc = T.capc[r] * (double)G.np;
+    double lc[K + 1], lp[K + 1], ln[K + 1];  // current level, previous level, new level
+    for (int i = 0; i <= K; i++) { lc[i] = m0[i]; lp[i] = mp[i]; }
+    for (int s = 1; s <= K; s++) {
+        const double mu = (double)A.mu[s - 1], nu = (double)A.nu[s - 1], a = (double)A.a[s - 1], g = (double)A.g[s - 1];
+        ln[0] = mu * lc[0] + nu * lp[0] + a * (capc * (lc[1] - lc[0])) + g * mF[0];
+        for (int i = 1; i <= K - s; i++) {
+            const int j = rowidx(i);
+            const double c_out = (double)(pole == 0 ? cp[j] : cm[j]);  // towards the equator
+            const double c_in = (double)(pole == 0 ? cm[j] : cp[j]);   // towards the pole
+            ln[i] = mu * lc[i] + nu * lp[i] + a * (c_out * (lc[i + 1] - lc[i]) - c_in * (lc[i] - lc[i - 1])) + g * mF[i];
+        }
+        capseq[((size_t)r * 2 + pole) * K + (s - 1)] = ln[0];
+        for (int i = 0; i <= K - s; i++) { lp[i] = lc[i]; lc[i] = ln[i]; }
+    }
+}
+
+// ------------------------------------------------------------------ main kernel
+template <typename real, int K, int C>
+__global__ void __launch_bounds__(BLK_WARPS * 32) k_sts_blocked(BlkArgs<real, K> A, Tables<real> T, Geom G) {
+    constexpr int WOUT = 32 * C - 2 * K;  // columns written per warp
+    const int lane = threadIdx.x & 31;
+    const int strip = blockIdx.x * BLK_WARPS + (threadIdx.x >> 5);
+    if (strip >= A.nstrips) return;  // warp-uniform; the kernel has no block-level barrier
+    const int r = blockIdx.z;
+    const int nt = G.nt, np = G.np;
+    const int ja = blockIdx.y * A.rows_per_seg;              // output rows [ja, jb)
+    const int jb = min(ja + A.rows_per_seg, nt + 2);
+    const int t0 = max(ja - K, 0);                           // first input row streamed
+    const int tend = jb - 1 + K;                             // last row-step (level K reaches row jb-1)
+    // columns of this lane: unwrapped index uc (may be < 0 or >= np), wrapped col
+    const int uc = strip * WOUT - K + lane * C;
+    int col = uc % np;
+    if (col < 0) col += np;
+    const bool wr = (lane * C >= K) && (lane * C < K + WOUT) && (uc < np);  // this lane's columns are written
+    const size_t base = (size_t)r * G.rstride + col;
+    const real* cpT = T.cp + (size_t)r * (nt + 2);
+    const real* cmT = T.cm + (size_t)r * (nt + 2);
+    const real* cfT = T.cf + (size_t)r * (nt + 2);
+    const real* cdT = T.cd + (size_t)r * (nt + 2);
+    const double* capN = A.capseq + ((size_t)r * 2 + 0) * K;
+    const double* capS = A.capseq + ((size_t)r * 2 + 1) * K;
+
+    real u[K][3][C];  // u[l][i]: level l, rows t-l-2+i (i = 0 oldest .. 2 newest)
+    real p[2][C];     // level -1, rows t-1, t
+    real f[K + 1][C]; // F rows t-i
+#pragma unroll
+    for (int l = 0; l < K; l++)
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int q = 0; q < C; q++) u[l][i][q] = (real)0;
+#pragma unroll
+    for (int i = 0; i < 2; i++)
+#pragma unroll
+        for (int q = 0; q < C; q++) p[i][q] = (real)0;
+#pragma unroll
+    for (int i = 0; i <= K; i++)
+#pragma unroll
+        for (int q = 0; q < C; q++) f[i][q] = (real)0;
+
+    // software prefetch: row t+1 is loaded while row t is processed
+    real nu0[C], np_[C], nf[C];
+#pragma unroll
+    for (int q = 0; q < C; q++) { nu0[q] = (real)0; np_[q] = (real)0; nf[q] = (real)0; }
+    {
+        const size_t off = base + (size_t)t0 * G.pitch;
+        vload<real, C>(nu0, A.cur + off);
+        if (A.has_prev) vload<real, C>(np_, A.prev + off);
+        vload<real, C>(nf, A.F + off);
+    }
+
+    for (int t = t0; t <= tend; t++) {
+        // shift the windows by one row
+#pragma unroll
+        for (int l = 0; l < K; l++)
+#pragma unroll
+            for (int q = 0; q < C; q++) { u[l][0][q] = u[l][1][q]; u[l][1][q] = u[l][2][q]; }
+#pragma unroll
+        for (int q = 0; q < C; q++) p[0][q] = p[1][q];
+#pragma unroll
+        for (int i = K; i >= 1; i--)
+#pragma unroll
+            for (int q = 0; q < C; q++) f[i][q] = f[i - 1][q];
+        // row t arrives (prefetched), row t+1 is requested
+#pragma unroll
+        for (int q = 0; q < C; q++) { u[0][2][q] = nu0[q]; p[1][q] = np_[q]; f[0][q] = nf[q]; }
+        if (t + 1 <= min(tend, nt + 1)) {
+            const size_t off = base + (size_t)(t + 1) * G.pitch;
+            vload<real, C>(nu0, A.cur + off);
+            if (A.has_prev) vload<real, C>(np_, A.prev + off);
+            vload<real, C>(nf, A.F + off);
+        }
+        real outK[C];
+#pragma unroll
+        for (int q = 0; q < C; q++) outK[q] = (real)0;
+        // levels 1..K: level l computes its row j = t - l from level l-1 rows j-1, j, j+1
+#pragma unroll
+        for (int l = 1; l <= K; l++) {
+            const int j = t - l;
+            real res[C];
+            if (j >= 1 && j <= nt) {
+                const real ca = A.a[l - 1];
+                const real An = ca * cmT[j], As = ca * cpT[j], Af = ca * cfT[j];
+                const real Ac = A.mu[l - 1] - ca * cdT[j];
+                const real nuc = A.nu[l - 1], gc = A.g[l - 1];
+                // phi neighbours of the row-j values of level l-1 (u[l-1][1]) from the adjacent lanes
+                real west = __shfl_up_sync(0xffffffffu, u[l - 1][1][C - 1], 1);
+                real east = __shfl_down_sync(0xffffffffu, u[l - 1][1][0], 1);
+#pragma unroll
+                for (int q = 0; q < C; q++) {
+                    const real c = u[l - 1][1][q];
+                    const real w = (q == 0) ? west : u[l - 1][1][q - 1];
+                    const real e = (q == C - 1) ? east : u[l - 1][1][q + 1];
+                    const real p2 = (l >= 2) ? u[(l >= 2) ? l - 2 : 0][0][q] : p[0][q];
+                    real acc = gc * f[l][q];
+                    acc = nuc * p2 + acc;
+                    acc = Af * (e + w) + acc;
+                    acc = Ac * c + acc;
+                    acc = An * u[l - 1][0][q] + acc;
+                    acc = As * u[l - 1][2][q] + acc;  // the only operand produced in this row-step: last in the chain
+                    res[q] = acc;
+                }
+            } else if (j == 0 || j == nt + 1) {
+                const real cv = (real)(j == 0 ? capN[l - 1] : capS[l - 1]);
+#pragma unroll
+                for (int q = 0; q < C; q++) res[q] = cv;
+            } else {
+#pragma unroll
+                for (int q = 0; q < C; q++) res[q] = (real)0;
+            }
+            if (l < K) {
+#pragma unroll
+                for (int q = 0; q < C; q++) u[(l < K) ? l : 0][2][q] = res[q];
+            } else {
+#pragma unroll
+                for (int q = 0; q < C; q++) outK[q] = res[q];
+            }
+        }
+        // write row jo = t - K of levels K and K-1
+        const int jo = t - K;
+        if (wr && jo >= ja && jo < jb) {
+            const size_t off = base + (size_t)jo * G.pitch;
+            if (A.last) {
+                real y[C];
+                vload<real, C>(y, A.Y0 + off);
+#pragma unroll
+                for (int q = 0; q < C; q++) y[q] += outK[q];
+                vstore<real, C>(A.Y0 + off, y);
+            } else {
+                vstore<real, C>(A.ocur + off, outK);
+                vstore<real, C>(A.oprev + off, u[K - 1][1]);
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------ host side
+
+template <typename real> struct BlkCfg;
+template <> struct BlkCfg<double> { static constexpr int C = 2; };
+template <> struct BlkCfg<float> { static constexpr int C = 4; };
+
+inline bool sts_blocked_supported(const Geom& G, size_t wbytes) {
+    const int C = wbytes == 8 ? 2 : 4;
+    return (G.np % C) == 0 && G.np >= 32 * C && G.nt >= 2 * STS_KMAX;
+}
+inline int sts_default_block(const Geom& G, size_t wbytes) { return sts_blocked_supported(G, wbytes) ? 8 : 1; }
+inline size_t sts_zmean_bytes(const Geom&) { return 256; }
+inline size_t sts_capseq_bytes(const Geom& G) { return (size_t)G.nr * 2 * STS_KMAX * sizeof(double) + 256; }
+inline int sts_blocked_init(const Geom&, bool) { return 0; }
 
 template <typename real>
 struct StsBlockedPlan {
     real* Y0;
     real* buf[5];
-    const double *mu, *nu, *a, *g;
+    const double *mu, *nu, *a, *g;  // per-stage scalars, index 1..s
     int s, kb;
     cudaStream_t stream;
-    double** part;
+    double** part;   // the two polar partial-sum buffers of the unblocked kernels
     double* zmean;
     double* capseq;
     void (*prof_begin)(void*, bool*);
-    void (*prof_end)(void*, bool);
+    void (*prof_end)(void*, bool, int);
     void* user;
 };
 
-inline int sts_default_block(const Geom&, size_t) { return 1; }
-inline bool sts_blocked_supported(const Geom&, size_t) { return false; }
-inline size_t sts_zmean_bytes(const Geom&) { return 256; }
-inline size_t sts_capseq_bytes(const Geom&) { return 256; }
-inline int sts_blocked_init(const Geom&, bool) { return 0; }
+template <typename real, int K>
+void sts_blocked_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
+                        real* ocur, real* oprev, bool last, int64_t* launches) {
+    constexpr int C = BlkCfg<real>::C;
+    constexpr int WOUT = 32 * C - 2 * K;
+    BlkArgs<real, K> a;
+    a.cur = cur; a.prev = prev ? prev : cur; a.F = P.buf[0]; a.ocur = ocur; a.oprev = oprev; a.Y0 = P.Y0; a.capseq = P.capseq;
+    for (int i = 0; i < K; i++) {
+        a.mu[i] = (real)P.mu[j0 + 1 + i]; a.nu[i] = (real)P.nu[j0 + 1 + i];
+        a.a[i] = (real)P.a[j0 + 1 + i]; a.g[i] = (real)P.g[j0 + 1 + i];
+    }
+    a.has_prev = prev != nullptr; a.last = last;
+    a.nstrips = (G.np + WOUT - 1) / WOUT;
+    // theta segments: enough CTAs for ~4 waves of 148 SMs x resident CTAs, but segments of at least 64 rows
+    const int ctas_x = (a.nstrips + BLK_WARPS - 1) / BLK_WARPS;
+    int nseg = 1;
+    const long want = 148L * 8;
+    while ((long)ctas_x * nseg * G.nr < want && (G.nt + 2) / (nseg * 2) >= 64) nseg *= 2;
+    a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
+    dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
+    k_sts_capseq<real, K><<<gc, 256, 0, P.stream>>>(a, T, G, P.capseq);
+    bool armed = false;
+    P.prof_begin(P.user, &armed);
+    k_sts_blocked<real, K, C><<<g, BLK_WARPS * 32, 0, P.stream>>>(a, T, G);
+    P.prof_end(P.user, armed, K);
+    *launches += 2;
+}
+
+// One STS step: stage 1 and the (s-1) mod K remainder stages one launch each, then (s-1)/K blocked launches.
 template <typename real>
-int sts_blocked_step(StsBlockedPlan<real>&, Tables<real>&, const Geom&, int64_t*) { return -1; }
+int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int64_t* launches) {
+    const int K = P.kb, s = P.s;
+    real* F = P.buf[0];
+    real* b[4] = {P.buf[1], P.buf[2], P.buf[3], P.buf[4]};
+    dim3 g1(G.nbx, (G.nt + 2 + RPT - 1) / RPT, G.nr), gs(G.nbx, 2, G.nr);
+    k_polar_row_sums<real><<<gs, TX, 0, P.stream>>>(P.Y0, P.part[0], G);
+    StsArgs<real> a;
+    a.F = F; a.Y0 = P.Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
+    a.in = P.Y0; a.d2 = b[0]; a.part_in = P.part[0]; a.part_out = P.part[1]; a.a = (real)P.a[1];
+    k_sts_stage<real, 0><<<g1, TX, 0, P.stream>>>(a, T, G);
+    *launches += 2;
+    const int rem = (s - 1) % K;
+    int icur = 0, iprev = 1, pin = 1;
+    bool has_prev = false;
+    for (int j = 2; j <= 1 + rem; j++) {  // remainder stages, unblocked
+        a.in = b[icur]; a.d2 = b[iprev]; a.part_in = P.part[pin]; a.part_out = P.part[pin ^ 1];
+        a.mu = (real)P.mu[j]; a.nu = (real)P.nu[j]; a.a = (real)P.a[j]; a.g = (real)P.g[j];
+        a.use_d2 = has_prev;
+        k_sts_stage<real, 1><<<g1, TX, 0, P.stream>>>(a, T, G);
+        *launches += 1;
+        int t = icur; icur = iprev; iprev = t;
+        has_prev = true;
+        pin ^= 1;
+    }
+    int j0 = 1 + rem;  // stages done so far
+    const int nblk = (s - j0) / K;
+    for (int i = 0; i < nblk; i++) {
+        // outputs go to the two buffers that are not inputs
+        int o1 = -1, o2 = -1;
+        for (int q = 0; q < 4; q++)
+            if (q != icur && q != iprev) { if (o1 < 0) o1 = q; else o2 = q; }
+        const bool last = (i == nblk - 1);
+        const real* prev = has_prev ? b[iprev] : nullptr;
+        switch (K) {
+            case 2: sts_blocked_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+            case 4: sts_blocked_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+            case 6: sts_blocked_launch<real, 6>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+            default: sts_blocked_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+        }
+        icur = o1; iprev = o2; has_prev = true;
+        j0 += K;
+    }
+    return 0;
+}
 
 }  // namespace hft

@@ -61,7 +61,7 @@ _lib.hft_stable_dt.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_
 _lib.hft_sts_stage_count.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_int32)]
 _lib.hft_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
 _lib.hft_profile_kernels.argtypes = [C.c_void_p, C.c_int32]
-_lib.hft_kernel_time.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+_lib.hft_kernel_time.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
 _lib.hft_error_string.argtypes = [C.c_int]
 _lib.hft_error_string.restype = C.c_char_p
 _lib.hft_last_cuda_error.argtypes = [C.c_void_p]
@@ -197,6 +197,6 @@ class Context:
         self._ck(_lib.hft_profile_kernels(self._h, int(which)), "hft_profile_kernels")
 
     def kernel_time(self):
-        ms, n = C.c_double(), C.c_int64()
-        self._ck(_lib.hft_kernel_time(self._h, C.byref(ms), C.byref(n)), "hft_kernel_time")
-        return ms.value, n.value
+        ms, n, st = C.c_double(), C.c_int64(), C.c_int64()
+        self._ck(_lib.hft_kernel_time(self._h, C.byref(ms), C.byref(n), C.byref(st)), "hft_kernel_time")
+        return ms.value, n.value, st.value
