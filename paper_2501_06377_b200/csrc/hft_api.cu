@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -16,6 +17,7 @@
 #include "../../include/hft.h"
 #include "hft_kernels.cuh"
 #include "hft_sts_blocked.cuh"
+#include "hft_sts_pipe.cuh"
 
 using namespace hft;
 
@@ -63,6 +65,7 @@ struct hft_ctx {
     double* d_capseq = nullptr;              // blocked STS: cap values per stage
     double* h_diag = nullptr;                // pinned
     int64_t launches = 0;
+    int sts_pipe = 1;  // 1: k_sts_pipe, 0: first-generation k_sts_blocked (env HFT_STS_PIPE=0, for A/B timing)
     StsCoef coef;
     // sampled kernel timing
     int prof_which = 0;
@@ -151,7 +154,7 @@ void build_flow(hft_ctx* c, int r, const hft_params& p) {
 
 template <typename real>
 struct HostTab {
-    std::vector<real> cp, cm, cf, cd, lm, lp, vtf, pm, pp, sth, rdt, rdp;
+    std::vector<real> cp, cm, cf, cd, c4, lm, lp, vtf, pm, pp, sth, rdt, rdp;
     std::vector<double> capc, dA;
 };
 
@@ -160,7 +163,7 @@ void fill_tables(const hft_ctx* c, HostTab<real>& H) {
     const int nt = c->G.nt, R = c->nr;
     const size_t n2 = (size_t)R * (nt + 2);
     H.cp.assign(n2, 0); H.cm.assign(n2, 0); H.cf.assign(n2, 0); H.cd.assign(n2, 0); H.lm.assign(n2, 0); H.lp.assign(n2, 0);
-    H.pm.assign(n2, 0); H.pp.assign(n2, 0);
+    H.pm.assign(n2, 0); H.pp.assign(n2, 0); H.c4.assign(4 * n2, 0);
     H.vtf.assign((size_t)R * (nt + 1), 0);
     H.sth.resize(nt + 1); H.rdt.assign(nt + 2, 0); H.rdp.assign(nt + 2, 0);
     H.capc.resize(R); H.dA.resize(nt + 2);
@@ -184,6 +187,7 @@ void fill_tables(const hft_ctx* c, HostTab<real>& H) {
                 H.cm[i] = (real)(nu * c->sth[j - 1] / (c->st[j] * c->dth * c->dth));
                 H.cf[i] = (real)(nu / (c->st[j] * c->st[j] * c->dph * c->dph));
                 H.cd[i] = (real)((double)H.cp[i] + (double)H.cm[i] + 2.0 * (double)H.cf[i]);
+                H.c4[4 * i + 0] = H.cm[i]; H.c4[4 * i + 1] = H.cp[i]; H.c4[4 * i + 2] = H.cf[i]; H.c4[4 * i + 3] = H.cd[i];
             }
             // LLF (B2 :684) with alpha_j = max |v| over faces j-5/2 .. j+5/2 that exist (:689)
             double al = 0.0;
@@ -210,7 +214,7 @@ int upload_tables(hft_ctx* c, Tables<real>& T) {
     const size_t n2 = (size_t)R * (nt + 2) * sizeof(real), n1 = (size_t)R * (nt + 1) * sizeof(real);
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off = round_up(off + bytes, 256); return o; };
-    size_t o_cp = take(n2), o_cm = take(n2), o_cf = take(n2), o_cd = take(n2), o_lm = take(n2), o_lp = take(n2), o_pm = take(n2), o_pp = take(n2);
+    size_t o_cp = take(n2), o_cm = take(n2), o_cf = take(n2), o_cd = take(n2), o_c4 = take(4 * n2), o_lm = take(n2), o_lp = take(n2), o_pm = take(n2), o_pp = take(n2);
     size_t o_vtf = take(n1), o_sth = take((nt + 1) * sizeof(real)), o_rdt = take((nt + 2) * sizeof(real)), o_rdp = take((nt + 2) * sizeof(real));
     size_t o_capc = take(R * sizeof(double)), o_dA = take((nt + 2) * sizeof(double));
     if (!c->d_tab) {
@@ -219,13 +223,13 @@ int upload_tables(hft_ctx* c, Tables<real>& T) {
     }
     char* d = c->d_tab;
     auto up = [&](size_t o, const void* src, size_t bytes) { return cudaMemcpyAsync(d + o, src, bytes, cudaMemcpyHostToDevice, c->stream); };
-    CK(up(o_cp, H.cp.data(), n2)); CK(up(o_cm, H.cm.data(), n2)); CK(up(o_cf, H.cf.data(), n2)); CK(up(o_cd, H.cd.data(), n2));
+    CK(up(o_cp, H.cp.data(), n2)); CK(up(o_cm, H.cm.data(), n2)); CK(up(o_cf, H.cf.data(), n2)); CK(up(o_cd, H.cd.data(), n2)); CK(up(o_c4, H.c4.data(), 4 * n2));
     CK(up(o_lm, H.lm.data(), n2)); CK(up(o_lp, H.lp.data(), n2)); CK(up(o_pm, H.pm.data(), n2)); CK(up(o_pp, H.pp.data(), n2));
     CK(up(o_vtf, H.vtf.data(), n1)); CK(up(o_sth, H.sth.data(), (nt + 1) * sizeof(real)));
     CK(up(o_rdt, H.rdt.data(), (nt + 2) * sizeof(real))); CK(up(o_rdp, H.rdp.data(), (nt + 2) * sizeof(real)));
     CK(up(o_capc, H.capc.data(), R * sizeof(double))); CK(up(o_dA, H.dA.data(), (nt + 2) * sizeof(double)));
     CK(cudaStreamSynchronize(c->stream));  // H goes out of scope
-    T.cp = (const real*)(d + o_cp); T.cm = (const real*)(d + o_cm); T.cf = (const real*)(d + o_cf); T.cd = (const real*)(d + o_cd);
+    T.cp = (const real*)(d + o_cp); T.cm = (const real*)(d + o_cm); T.cf = (const real*)(d + o_cf); T.cd = (const real*)(d + o_cd); T.c4 = (const real*)(d + o_c4);
     T.lm = (const real*)(d + o_lm); T.lp = (const real*)(d + o_lp); T.pm = (const real*)(d + o_pm); T.pp = (const real*)(d + o_pp);
     T.vtf = (const real*)(d + o_vtf); T.sth = (const real*)(d + o_sth); T.rdt = (const real*)(d + o_rdt); T.rdp = (const real*)(d + o_rdp);
     T.capc = (const double*)(d + o_capc); T.dA = (const double*)(d + o_dA);
@@ -438,7 +442,7 @@ int step_once(hft_ctx* c, double dt, int s) {
             P.prof_end = [](void* u, bool armed, int stages) { prof_end((hft_ctx*)u, armed, stages); };
             P.user = c;
             int64_t n = 0;
-            rc = sts_blocked_step<real>(P, tables_of<real>(c), c->G, &n);
+            rc = sts_blocked_step<real>(P, tables_of<real>(c), c->G, c->sts_pipe, &n) == 0 ? HFT_OK : HFT_ERR_CUDA;
             c->launches += n;
         } else {
             rc = diffuse_unblocked<real>(c, dt, s);
@@ -499,6 +503,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     hft_ctx* c = new (std::nothrow) hft_ctx();
     if (!c) return HFT_ERR_NOMEM;
     c->grid = *grid; c->opt = o; c->nr = n_real; c->stream = (cudaStream_t)cuda_stream;
+    if (const char* e = getenv("HFT_STS_PIPE")) c->sts_pipe = atoi(e) != 0;
     c->G.nt = grid->n_theta; c->G.np = grid->n_phi; c->G.pitch = pitch_for(grid->n_phi, grid->dtype); c->G.nr = n_real;
     c->G.rstride = (size_t)(grid->n_theta + 2) * c->G.pitch;
     c->G.nbx = (grid->n_phi + TX - 1) / TX;

@@ -22,6 +22,7 @@ struct Tables {            // device pointers, all [R][nt+2] unless noted
     const real* cm;        //            nu sin(theta_{j-1/2}) / (sin(theta_j) dth^2)        Eq. 28 (:452)
     const real* cf;        //            nu / (sin^2(theta_j) dph^2)                         Eq. 28 (:450, :458)
     const real* cd;        //            cp + cm + 2 cf  (minus the diagonal a_{j,k} of Eq. 28, :454)
+    const real* c4;        // [R][nt+2][4] = (cm, cp, cf, cd) interleaved, zero on the cap rows (k_sts_pipe)
     const double* capc;    // [R] P (nu/dth) dph : polar cap diffusion prefactor             App. A (:646)
     const real* lm;        // advection LLF: (v_{j-1/2} + alpha_j)/2                         B2 (:684)
     const real* lp;        //                (v_{j+1/2} - alpha_j)/2

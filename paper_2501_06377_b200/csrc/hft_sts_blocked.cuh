@@ -117,7 +117,8 @@ __global__ void __launch_bounds__(256) k_sts_capseq(BlkArgs<real, K> A, Tables<r
 // ------------------------------------------------------------------ main kernel
 template <typename real, int K, int C>
 __global__ void __launch_bounds__(BLK_WARPS * 32) k_sts_blocked(BlkArgs<real, K> A, Tables<real> T, Geom G) {
-    constexpr int WOUT = 32 * C - 2 * K;  // columns written per warp
+    constexpr int HALO = (K + C - 1) / C * C;  // invalid columns per side, in whole 16-byte vectors
+    constexpr int WOUT = 32 * C - 2 * HALO;    // columns written per warp
     const int lane = threadIdx.x & 31;
     const int strip = blockIdx.x * BLK_WARPS + (threadIdx.x >> 5);
     if (strip >= A.nstrips) return;  // warp-uniform; the kernel has no block-level barrier
@@ -128,10 +129,10 @@ __global__ void __launch_bounds__(BLK_WARPS * 32) k_sts_blocked(BlkArgs<real, K>
     const int t0 = max(ja - K, 0);                           // first input row streamed
     const int tend = jb - 1 + K;                             // last row-step (level K reaches row jb-1)
     // columns of this lane: unwrapped index uc (may be < 0 or >= np), wrapped col
-    const int uc = strip * WOUT - K + lane * C;
+    const int uc = strip * WOUT - HALO + lane * C;
     int col = uc % np;
     if (col < 0) col += np;
-    const bool wr = (lane * C >= K) && (lane * C < K + WOUT) && (uc < np);  // this lane's columns are written
+    const bool wr = (lane * C >= HALO) && (lane * C < HALO + WOUT) && (uc < np);  // this lane's columns are written
     const size_t base = (size_t)r * G.rstride + col;
     const real* cpT = T.cp + (size_t)r * (nt + 2);
     const real* cmT = T.cm + (size_t)r * (nt + 2);
@@ -288,7 +289,7 @@ template <typename real, int K>
 void sts_blocked_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
                         real* ocur, real* oprev, bool last, int64_t* launches) {
     constexpr int C = BlkCfg<real>::C;
-    constexpr int WOUT = 32 * C - 2 * K;
+    constexpr int WOUT = 32 * C - 2 * ((K + C - 1) / C * C);
     BlkArgs<real, K> a;
     a.cur = cur; a.prev = prev ? prev : cur; a.F = P.buf[0]; a.ocur = ocur; a.oprev = oprev; a.Y0 = P.Y0; a.capseq = P.capseq;
     for (int i = 0; i < K; i++) {
@@ -310,53 +311,6 @@ void sts_blocked_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Ge
     k_sts_blocked<real, K, C><<<g, BLK_WARPS * 32, 0, P.stream>>>(a, T, G);
     P.prof_end(P.user, armed, K);
     *launches += 2;
-}
-
-// One STS step: stage 1 and the (s-1) mod K remainder stages one launch each, then (s-1)/K blocked launches.
-template <typename real>
-int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int64_t* launches) {
-    const int K = P.kb, s = P.s;
-    real* F = P.buf[0];
-    real* b[4] = {P.buf[1], P.buf[2], P.buf[3], P.buf[4]};
-    dim3 g1(G.nbx, (G.nt + 2 + RPT - 1) / RPT, G.nr), gs(G.nbx, 2, G.nr);
-    k_polar_row_sums<real><<<gs, TX, 0, P.stream>>>(P.Y0, P.part[0], G);
-    StsArgs<real> a;
-    a.F = F; a.Y0 = P.Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
-    a.in = P.Y0; a.d2 = b[0]; a.part_in = P.part[0]; a.part_out = P.part[1]; a.a = (real)P.a[1];
-    k_sts_stage<real, 0><<<g1, TX, 0, P.stream>>>(a, T, G);
-    *launches += 2;
-    const int rem = (s - 1) % K;
-    int icur = 0, iprev = 1, pin = 1;
-    bool has_prev = false;
-    for (int j = 2; j <= 1 + rem; j++) {  // remainder stages, unblocked
-        a.in = b[icur]; a.d2 = b[iprev]; a.part_in = P.part[pin]; a.part_out = P.part[pin ^ 1];
-        a.mu = (real)P.mu[j]; a.nu = (real)P.nu[j]; a.a = (real)P.a[j]; a.g = (real)P.g[j];
-        a.use_d2 = has_prev;
-        k_sts_stage<real, 1><<<g1, TX, 0, P.stream>>>(a, T, G);
-        *launches += 1;
-        int t = icur; icur = iprev; iprev = t;
-        has_prev = true;
-        pin ^= 1;
-    }
-    int j0 = 1 + rem;  // stages done so far
-    const int nblk = (s - j0) / K;
-    for (int i = 0; i < nblk; i++) {
-        // outputs go to the two buffers that are not inputs
-        int o1 = -1, o2 = -1;
-        for (int q = 0; q < 4; q++)
-            if (q != icur && q != iprev) { if (o1 < 0) o1 = q; else o2 = q; }
-        const bool last = (i == nblk - 1);
-        const real* prev = has_prev ? b[iprev] : nullptr;
-        switch (K) {
-            case 2: sts_blocked_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-            case 4: sts_blocked_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-            case 6: sts_blocked_launch<real, 6>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-            default: sts_blocked_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-        }
-        icur = o1; iprev = o2; has_prev = true;
-        j0 += K;
-    }
-    return 0;
 }
 
 }  // namespace hft

@@ -1,0 +1,342 @@
+// hft_sts_pipe.cuh -- temporally blocked super-time-stepping, second generation: K STS stages per launch with
+// (i) register windows that ROTATE by unrolling instead of moving, (ii) an asynchronous shared-memory ring
+// (cp.async, several rows per warp in flight) for the three input streams, (iii) the per-(stage,row)
+// coefficient products formed once per warp row-step by the 32 lanes together instead of by every lane.
+//
+// Same decomposition as k_sts_blocked (hft_sts_blocked.cuh): a WARP owns a strip of
+// 32*C phi-columns (one 16-byte vector per lane) and streams down the theta-rows; level l (= stage j0+l) lags
+// level l-1 by one row; phi-neighbours come from the adjacent lanes by shuffle; warps never synchronise with
+// each other.  What changed is the instruction stream (profiles/r01_cfg3_f64_first_pass.md: 523 warp
+// instructions per row-step of which 112 were the stencil's DFMAs):
+//
+//  * Row-step t keeps, for every level, rows t-l, t-l-1, t-l-2 in registers.  Row rho of level l lives in slot
+//    rho mod 3, F row rho in slot rho mod (K+1).  The row loop is unrolled U = lcm(3, K+1) times, so every slot
+//    index is a compile-time constant and no register is ever copied.
+//  * Inputs (delta_{j0}, delta_{j0-1}, L(Y0)) arrive through a per-warp ring of D = K+1 rows in shared memory
+//    filled by cp.async 16 B per lane, D-2 rows ahead: each lane copies and later reads only ITS OWN 16 bytes,
+//    so no barrier of any kind is needed for the data, and ~10 KB per warp are in flight instead of one row.
+//  * The products a_l*cm_j, a_l*cp_j, a_l*cf_j, mu_l - a_l*cd_j of level l at row j = t-l are warp-uniform.
+//    Lane (l-1)*4+q forms product q of level l with ONE fma per row-step and publishes it in shared memory;
+//    every lane then reads the 4 products of a level with one or two broadcast LDS.128.
+//  * Two code paths per warp: the steady-state path (all K levels on interior rows) has no branch on the row
+//    index; the generic path (first / last rows of the sphere) overrides the polar-cap rows with the values of
+//    k_sts_capseq.
+//
+// Arithmetic per cell and level (Eq. 27-28 with constant nu; recurrence DESIGN.md U20):
+//   delta_l[j,k] = g_l F + nu_l delta_{l-2} + Af (e + w) + Ac c + An n + As s      (7 flops as 1 add + 6 fma)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "hft_sts_blocked.cuh"
+
+namespace hft {
+
+__host__ __device__ constexpr int pmod(int a, int m) { return ((a % m) + m) % m; }
+
+template <typename real, int K>
+struct PipeCfg {
+    static constexpr int C = 16 / (int)sizeof(real);          // columns per lane
+    static constexpr int NF = K + 1;                          // F rows alive in registers
+    static constexpr int U = (NF % 3 == 0) ? NF : 3 * NF;     // row-steps per unrolled macro-iteration
+    static constexpr int D = NF;                              // ring depth in rows (divides U)
+    static constexpr int DP = D - 2;                          // prefetch distance in rows
+    static constexpr int ROW = 32 * C;                        // reals per ring row (512 B)
+    static constexpr int NCS = 3;                             // coefficient ring slots (divides U)
+    static constexpr int WARP_REALS = 3 * D * ROW + NCS * K * 4;
+    static constexpr int WARP_BYTES = WARP_REALS * (int)sizeof(real);
+    static constexpr int HALO = (K + C - 1) / C * C;          // invalid columns per strip side, whole 16-byte vectors
+    static constexpr int WOUT = 32 * C - 2 * HALO;            // columns written per warp
+    static_assert(DP >= 1, "K >= 2");
+    static_assert(K * 4 <= 32, "one lane per (level, coefficient)");
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ double fma_r(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ float fma_r(float a, float b, float c) { return fmaf(a, b, c); }
+
+template <typename real, int K>
+struct PipeWarp {
+    using P = PipeCfg<real, K>;
+    static constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, NF = P::NF, ROW = P::ROW, NCS = P::NCS;
+
+    // registers
+    real u[K][3][C];   // level l (0..K-1), row rho in slot rho mod 3 (relative to the macro-iteration origin)
+    real f[NF][C];     // F row rho in slot rho mod NF
+    // per-warp constants
+    const BlkArgs<real, K>& A;
+    const real *gcur, *gprev, *gF;   // this lane's column of row 0 of the three inputs
+    real *gocur, *goprev, *gY0;
+    real *s_cur, *s_prev, *s_F, *s_coef;   // shared: this lane's 16 bytes of ring slot 0; coefficient ring
+    const real* c4;                  // raw row coefficients [nt+2][4] of this realization, offset by this lane's q
+    const double *capN, *capS;
+    real sa, sadd;                   // this lane's product: fma(sa, raw, sadd)
+    int cl;                          // this lane's level - 1
+    int nt, pitch, ja, jb, lane;
+    bool wr;
+
+    __device__ __forceinline__ PipeWarp(const BlkArgs<real, K>& A_) : A(A_) {}
+
+    __device__ __forceinline__ void prefetch(int row, int slot) {
+        if (row <= nt + 1) {
+            const size_t o = (size_t)row * pitch;
+            cp_async16(smem_u32(s_cur + slot * ROW), gcur + o);
+            cp_async16(smem_u32(s_prev + slot * ROW), gprev + o);
+            cp_async16(smem_u32(s_F + slot * ROW), gF + o);
+        }
+        cp_async_commit();
+    }
+
+    // products used by row-step t: level cl+1 works on row t-(cl+1)
+    __device__ __forceinline__ void gen_coef(int t, int slot) {
+        const int j = min(max(t - (cl + 1), 0), nt + 1);
+        const real raw = c4[j * 4];
+        if (cl < K) s_coef[slot * (K * 4) + lane] = fma_r(sa, raw, sadd);
+    }
+
+    template <int PH, bool GEN>
+    __device__ __forceinline__ void rowstep(int t) {
+        cp_async_wait<DP - 1>();   // this lane's copies of row t have landed
+        __syncwarp();              // the products written during the previous row-step are visible
+        constexpr int sl = PH % D;
+        vload<real, C>(u[0][PH % 3], s_cur + sl * ROW);
+        vload<real, C>(f[PH % NF], s_F + sl * ROW);
+        real pl1[C];               // delta_{j0-1} row t-1: the "two levels back" operand of level 1
+        vload<real, C>(pl1, s_prev + pmod(PH - 1, D) * ROW);
+        prefetch(t + DP, (PH + DP) % D);   // overwrites the slot of row t-2, last read one row-step ago
+        const real raw_next = c4[min(max(t + 1 - (cl + 1), 0), nt + 1) * 4];
+        const real* cfs = s_coef + (PH % NCS) * (K * 4);
+        real outK[C];
+#pragma unroll
+        for (int l = 1; l <= K; l++) {
+            // level l-1: newest row t-l+1 (s), centre t-l (c), oldest t-l-1 (n)
+            const int sN = pmod(PH - (l - 1), 3), sC = pmod(PH - l, 3), sO = pmod(PH - l - 1, 3);
+            real cf4[4];
+            vload<real, C>(*reinterpret_cast<real(*)[C]>(&cf4[0]), cfs + (l - 1) * 4);
+            if constexpr (C < 4) vload<real, C>(*reinterpret_cast<real(*)[C]>(&cf4[4 - C]), cfs + (l - 1) * 4 + (4 - C));
+            const real An = cf4[0], As = cf4[1], Af = cf4[2], Ac = cf4[3];
+            const real nuc = A.nu[l - 1], gc = A.g[l - 1];
+            const real west = __shfl_up_sync(0xffffffffu, u[l - 1][sC][C - 1], 1);
+            const real east = __shfl_down_sync(0xffffffffu, u[l - 1][sC][0], 1);
+            real res[C];
+#pragma unroll
+            for (int q = 0; q < C; q++) {
+                const real c = u[l - 1][sC][q];
+                const real w = (q == 0) ? west : u[l - 1][sC][q > 0 ? q - 1 : 0];
+                const real e = (q == C - 1) ? east : u[l - 1][sC][q < C - 1 ? q + 1 : 0];
+                const real p2 = (l == 1) ? pl1[q] : u[l >= 2 ? l - 2 : 0][sC][q];   // level l-2 row t-l is ITS oldest: slot (PH-(l-2)-2) mod 3 = sC
+                real acc = gc * f[pmod(PH - l, NF)][q];
+                acc = fma_r(nuc, p2, acc);
+                acc = fma_r(Af, e + w, acc);
+                acc = fma_r(Ac, c, acc);
+                acc = fma_r(An, u[l - 1][sO][q], acc);
+                acc = fma_r(As, u[l - 1][sN][q], acc);   // the only operand produced in this row-step
+                res[q] = acc;
+            }
+            if (GEN) {
+                const int j = t - l;
+                if (j == 0 || j == nt + 1) {
+                    const real cv = (real)(j == 0 ? capN[l - 1] : capS[l - 1]);
+#pragma unroll
+                    for (int q = 0; q < C; q++) res[q] = cv;
+                }
+            }
+            if (l < K) {
+#pragma unroll
+                for (int q = 0; q < C; q++) u[l < K ? l : 0][sC][q] = res[q];   // level l newest = row t-l: slot (PH-l) mod 3 = sC
+            } else {
+#pragma unroll
+                for (int q = 0; q < C; q++) outK[q] = res[q];
+            }
+        }
+        // products for the next row-step (slot last read two row-steps ago)
+        if (cl < K) s_coef[((PH + 1) % NCS) * (K * 4) + lane] = fma_r(sa, raw_next, sadd);
+        // row jo = t-K of levels K and K-1 (level K-1 row t-K is its centre: slot (PH-(K-1)-1) mod 3)
+        const int jo = t - K;
+        if (wr && jo >= ja && jo < jb) {
+            const size_t o = (size_t)jo * pitch;
+            if (A.last) {
+                real y[C];
+                vload<real, C>(y, gY0 + o);
+#pragma unroll
+                for (int q = 0; q < C; q++) y[q] += outK[q];
+                vstore<real, C>(gY0 + o, y);
+            } else {
+                vstore<real, C>(gocur + o, outK);
+                vstore<real, C>(goprev + o, u[K - 1][pmod(PH - K, 3)]);
+            }
+        }
+    }
+
+    template <int PH, bool GEN>
+    __device__ __forceinline__ void macro(int tb) {
+        rowstep<PH, GEN>(tb + PH);
+        if constexpr (PH + 1 < U) macro<PH + 1, GEN>(tb);
+    }
+};
+
+template <typename real, int K>
+__global__ void __launch_bounds__(BLK_WARPS * 32, 2) k_sts_pipe(const __grid_constant__ BlkArgs<real, K> A, Tables<real> T, Geom G) {
+    using P = PipeCfg<real, K>;
+    constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, ROW = P::ROW;
+    extern __shared__ __align__(128) unsigned char pipe_smem[];
+    const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+    const int strip = blockIdx.x * BLK_WARPS + wrp;
+    if (strip >= A.nstrips) return;   // warp-uniform; the kernel has no block-level barrier
+    const int r = blockIdx.z, nt = G.nt, np = G.np;
+    PipeWarp<real, K> W(A);
+    W.nt = nt; W.pitch = G.pitch; W.lane = lane;
+    W.ja = blockIdx.y * A.rows_per_seg;
+    W.jb = min(W.ja + A.rows_per_seg, nt + 2);
+    const int t0 = max(W.ja - K, 0), tend = W.jb - 1 + K;
+    const int uc = strip * P::WOUT - P::HALO + lane * C;   // unwrapped first column of this lane
+    int col = uc % np;
+    if (col < 0) col += np;
+    W.wr = (lane * C >= P::HALO) && (lane * C < P::HALO + P::WOUT) && (uc < np);
+    const size_t base = (size_t)r * G.rstride + col;
+    W.gcur = A.cur + base; W.gprev = A.prev + base; W.gF = A.F + base;
+    W.gocur = A.ocur + base; W.goprev = A.oprev + base; W.gY0 = A.Y0 + base;
+    real* ws = reinterpret_cast<real*>(pipe_smem) + (size_t)wrp * P::WARP_REALS;
+    W.s_cur = ws + lane * C; W.s_prev = W.s_cur + D * ROW; W.s_F = W.s_prev + D * ROW;
+    W.s_coef = ws + 3 * D * ROW;
+    W.capN = A.capseq + ((size_t)r * 2 + 0) * K;
+    W.capS = A.capseq + ((size_t)r * 2 + 1) * K;
+    W.cl = lane >> 2;
+    const int cq = lane & 3;
+    W.c4 = T.c4 + (size_t)r * (nt + 2) * 4 + cq;
+    W.sa = (real)0; W.sadd = (real)0;
+    if (W.cl < K) {
+        const real a = A.a[W.cl];
+        W.sa = cq < 3 ? a : -a;
+        W.sadd = cq < 3 ? (real)0 : A.mu[W.cl];
+    }
+#pragma unroll
+    for (int l = 0; l < K; l++)
+#pragma unroll
+        for (int i = 0; i < 3; i++)
+#pragma unroll
+            for (int q = 0; q < C; q++) W.u[l][i][q] = (real)0;
+#pragma unroll
+    for (int i = 0; i < P::NF; i++)
+#pragma unroll
+        for (int q = 0; q < C; q++) W.f[i][q] = (real)0;
+    // clear this warp's shared memory (the ring slot of "row t0-1" is read before it is ever written)
+    for (int i = lane; i < P::WARP_REALS; i += 32) ws[i] = (real)0;
+    __syncwarp();
+    for (int i = 0; i < DP; i++) W.prefetch(t0 + i, i);
+    W.gen_coef(t0, 0);
+    for (int tb = t0; tb <= tend; tb += U) {
+        // steady state: every level of every row-step of this macro-iteration works on an interior row
+        if (tb >= K + 1 && tb + U - 2 <= nt) W.template macro<0, false>(tb);
+        else W.template macro<0, true>(tb);
+    }
+    cp_async_wait<0>();
+}
+
+// ------------------------------------------------------------------ host side
+
+template <typename real, int K>
+int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
+                    real* ocur, real* oprev, bool last, int64_t* launches) {
+    using PC = PipeCfg<real, K>;
+    static bool attr_done = false;
+    const int smem = BLK_WARPS * PC::WARP_BYTES;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_sts_pipe<real, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        if (e != cudaSuccess) return -1;
+        attr_done = true;
+    }
+    BlkArgs<real, K> a;
+    a.cur = cur; a.prev = prev; a.F = P.buf[0]; a.ocur = ocur; a.oprev = oprev; a.Y0 = P.Y0; a.capseq = P.capseq;
+    for (int i = 0; i < K; i++) {
+        a.mu[i] = (real)P.mu[j0 + 1 + i]; a.nu[i] = (real)P.nu[j0 + 1 + i];
+        a.a[i] = (real)P.a[j0 + 1 + i]; a.g[i] = (real)P.g[j0 + 1 + i];
+    }
+    a.has_prev = 1; a.last = last;
+    a.nstrips = (G.np + PC::WOUT - 1) / PC::WOUT;
+    const int ctas_x = (a.nstrips + BLK_WARPS - 1) / BLK_WARPS;
+    int nseg = 1;
+    const long want = 148L * 4;   // 2 CTAs per SM resident; >= 2 waves
+    while ((long)ctas_x * nseg * G.nr < want && (G.nt + 2) / (nseg * 2) >= 64) nseg *= 2;
+    a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
+    dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
+    k_sts_capseq<real, K><<<gc, 256, 0, P.stream>>>(a, T, G, P.capseq);
+    bool armed = false;
+    P.prof_begin(P.user, &armed);
+    k_sts_pipe<real, K><<<g, BLK_WARPS * 32, smem, P.stream>>>(a, T, G);
+    P.prof_end(P.user, armed, K);
+    *launches += 2;
+    return 0;
+}
+
+// One STS step: stage 1 and the (s-1) mod K remainder stages one launch each, then (s-1)/K blocked launches.
+// pipe != 0: k_sts_pipe (default); pipe == 0: the first-generation k_sts_blocked (kept for comparison).
+template <typename real>
+int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int pipe, int64_t* launches) {
+    const int K = P.kb, s = P.s;
+    real* F = P.buf[0];
+    real* b[4] = {P.buf[1], P.buf[2], P.buf[3], P.buf[4]};
+    dim3 g1(G.nbx, (G.nt + 2 + RPT - 1) / RPT, G.nr), gs(G.nbx, 2, G.nr);
+    k_polar_row_sums<real><<<gs, TX, 0, P.stream>>>(P.Y0, P.part[0], G);
+    StsArgs<real> a;
+    a.F = F; a.Y0 = P.Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
+    a.in = P.Y0; a.d2 = b[0]; a.part_in = P.part[0]; a.part_out = P.part[1]; a.a = (real)P.a[1];
+    k_sts_stage<real, 0><<<g1, TX, 0, P.stream>>>(a, T, G);
+    *launches += 2;
+    const int rem = (s - 1) % K;
+    int icur = 0, iprev = 1, pin = 1;
+    bool has_prev = false;
+    for (int j = 2; j <= 1 + rem; j++) {  // remainder stages, unblocked
+        a.in = b[icur]; a.d2 = b[iprev]; a.part_in = P.part[pin]; a.part_out = P.part[pin ^ 1];
+        a.mu = (real)P.mu[j]; a.nu = (real)P.nu[j]; a.a = (real)P.a[j]; a.g = (real)P.g[j];
+        a.use_d2 = has_prev;
+        k_sts_stage<real, 1><<<g1, TX, 0, P.stream>>>(a, T, G);
+        *launches += 1;
+        int t = icur; icur = iprev; iprev = t;
+        has_prev = true;
+        pin ^= 1;
+    }
+    int j0 = 1 + rem;  // stages done so far
+    const int nblk = (s - j0) / K;
+    for (int i = 0; i < nblk; i++) {
+        // outputs go to the two buffers that are not inputs
+        int o1 = -1, o2 = -1;
+        for (int q = 0; q < 4; q++)
+            if (q != icur && q != iprev) { if (o1 < 0) o1 = q; else o2 = q; }
+        const bool last = (i == nblk - 1);
+        if (pipe && !has_prev) {  // delta_0 = 0 is not stored: the pipe kernel reads it, so write it once
+            if (cudaMemsetAsync(b[iprev], 0, (size_t)G.nr * G.rstride * sizeof(real), P.stream) != cudaSuccess) return -1;
+            has_prev = true;
+        }
+        const real* prev = has_prev ? b[iprev] : nullptr;
+        int rc = 0;
+        if (pipe) {
+            switch (K) {
+                case 2: rc = sts_pipe_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+                case 4: rc = sts_pipe_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+                case 6: rc = sts_pipe_launch<real, 6>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+                default: rc = sts_pipe_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+            }
+        } else {
+            switch (K) {
+                case 2: sts_blocked_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+                case 4: sts_blocked_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+                case 6: sts_blocked_launch<real, 6>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+                default: sts_blocked_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+            }
+        }
+        if (rc != 0) return rc;
+        icur = o1; iprev = o2; has_prev = true;
+        j0 += K;
+    }
+    return 0;
+}
+
+}  // namespace hft

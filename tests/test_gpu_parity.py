@@ -136,6 +136,26 @@ def test_small_ragged_multi_realization(dtype, case):
     ctx.close()
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("block", [2, 4, 6, 8])
+@pytest.mark.parametrize("s_forced", [0, 41])
+def test_sts_block_sizes_ragged(dtype, block, s_forced):
+    """Every temporal-blocking depth K of the STS kernel (hft_options.sts_block) on a grid with ragged strips, a
+    phi seam inside a strip and theta segments: s = 42 -> (s-1) mod K remainder stages un-blocked; s_forced = 41
+    -> (s-1) mod 8 = 0, the block that starts from delta_0 = 0."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 150, 328, n_real=2)
+    ctx, o = make_pair(w, dtype, adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKG2, sts_block=block, sts_stages=s_forced)
+    _, dif = o.stable_dt()
+    dt = 250.0 * dif
+    s = ctx.sts_stage_count(dt)
+    assert s <= 41
+    ctx.step(3, dt)
+    o.step(3, dt, adv_flux=orc.ADV_OFF, diff_time=orc.DIFF_RKG2, sts_stages=s_forced)
+    compare(ctx, o, TOL[dtype], f"K={block}")
+    ctx.close()
+
+
 @pytest.mark.parametrize("block", [1, 0])
 def test_config1_full_length(block):
     """BASELINE config 1: 512x1024, 40 pairs, flows of reading U17, eta = 500, 16 steps of 1.5 h, s = 217."""
