@@ -34,6 +34,15 @@ namespace hft {
 
 __host__ __device__ constexpr int pmod(int a, int m) { return ((a % m) + m) % m; }
 
+#ifndef HFT_PIPE_WARPS
+#define HFT_PIPE_WARPS 4
+#endif
+#ifndef HFT_PIPE_MINB
+#define HFT_PIPE_MINB 2
+#endif
+constexpr int PIPE_WARPS = HFT_PIPE_WARPS;   // warps (= strips) per CTA; warps never synchronise with each other
+constexpr int PIPE_MINB = HFT_PIPE_MINB;     // resident CTAs per SM the register budget is set for
+
 template <typename real, int K>
 struct PipeCfg {
     static constexpr int C = 16 / (int)sizeof(real);          // columns per lane
@@ -78,6 +87,7 @@ struct PipeWarp {
     const real* c4;                  // raw row coefficients [nt+2][4] of this realization, offset by this lane's q
     const double *capN, *capS;
     real sa, sadd;                   // this lane's product: fma(sa, raw, sadd)
+    real rawq[3];                    // raw coefficient of row-steps t+1..t+3, slot = (row-step - t0) mod 3
     int cl;                          // this lane's level - 1
     int nt, pitch, ja, jb, lane;
     bool wr;
@@ -94,11 +104,12 @@ struct PipeWarp {
         cp_async_commit();
     }
 
-    // products used by row-step t: level cl+1 works on row t-(cl+1)
+    // raw row coefficient behind this lane's product of row-step t: level cl+1 works on row t-(cl+1)
+    __device__ __forceinline__ real raw_of(int t) const { return c4[min(max(t - (cl + 1), 0), nt + 1) * 4]; }
+
+    // products used by row-step t
     __device__ __forceinline__ void gen_coef(int t, int slot) {
-        const int j = min(max(t - (cl + 1), 0), nt + 1);
-        const real raw = c4[j * 4];
-        if (cl < K) s_coef[slot * (K * 4) + lane] = fma_r(sa, raw, sadd);
+        if (cl < K) s_coef[slot * (K * 4) + lane] = fma_r(sa, raw_of(t), sadd);
     }
 
     template <int PH, bool GEN>
@@ -111,7 +122,10 @@ struct PipeWarp {
         real pl1[C];               // delta_{j0-1} row t-1: the "two levels back" operand of level 1
         vload<real, C>(pl1, s_prev + pmod(PH - 1, D) * ROW);
         prefetch(t + DP, (PH + DP) % D);   // overwrites the slot of row t-2, last read one row-step ago
-        const real raw_next = c4[min(max(t + 1 - (cl + 1), 0), nt + 1) * 4];
+        // the raw coefficient of row-step t+1 was requested three row-steps ago (an L2 hit takes about as long
+        // as one row-step: profiles/r01_pipe_f64.md); request the one of row-step t+4 into the freed slot
+        const real raw_next = rawq[(PH + 1) % 3];
+        rawq[(PH + 1) % 3] = raw_of(t + 4);
         const real* cfs = s_coef + (PH % NCS) * (K * 4);
         real outK[C];
 #pragma unroll
@@ -183,12 +197,12 @@ struct PipeWarp {
 };
 
 template <typename real, int K>
-__global__ void __launch_bounds__(BLK_WARPS * 32, 2) k_sts_pipe(const __grid_constant__ BlkArgs<real, K> A, Tables<real> T, Geom G) {
+__global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const __grid_constant__ BlkArgs<real, K> A, Tables<real> T, Geom G) {
     using P = PipeCfg<real, K>;
     constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, ROW = P::ROW;
     extern __shared__ __align__(128) unsigned char pipe_smem[];
     const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-    const int strip = blockIdx.x * BLK_WARPS + wrp;
+    const int strip = blockIdx.x * PIPE_WARPS + wrp;
     if (strip >= A.nstrips) return;   // warp-uniform; the kernel has no block-level barrier
     const int r = blockIdx.z, nt = G.nt, np = G.np;
     PipeWarp<real, K> W(A);
@@ -232,6 +246,7 @@ __global__ void __launch_bounds__(BLK_WARPS * 32, 2) k_sts_pipe(const __grid_con
     __syncwarp();
     for (int i = 0; i < DP; i++) W.prefetch(t0 + i, i);
     W.gen_coef(t0, 0);
+    W.rawq[1] = W.raw_of(t0 + 1); W.rawq[2] = W.raw_of(t0 + 2); W.rawq[0] = W.raw_of(t0 + 3);
     for (int tb = t0; tb <= tend; tb += U) {
         // steady state: every level of every row-step of this macro-iteration works on an interior row
         if (tb >= K + 1 && tb + U - 2 <= nt) W.template macro<0, false>(tb);
@@ -246,12 +261,16 @@ template <typename real, int K>
 int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
                     real* ocur, real* oprev, bool last, int64_t* launches) {
     using PC = PipeCfg<real, K>;
-    static bool attr_done = false;
-    const int smem = BLK_WARPS * PC::WARP_BYTES;
-    if (!attr_done) {
+    static int slots = 0;   // CTAs resident on the whole device
+    const int smem = PIPE_WARPS * PC::WARP_BYTES;
+    if (!slots) {
         cudaError_t e = cudaFuncSetAttribute(k_sts_pipe<real, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return -1;
-        attr_done = true;
+        int dev = 0, sms = 0, per_sm = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sts_pipe<real, K>, PIPE_WARPS * 32, smem) != cudaSuccess || per_sm < 1)
+            return -1;
+        slots = sms * per_sm;
     }
     BlkArgs<real, K> a;
     a.cur = cur; a.prev = prev; a.F = P.buf[0]; a.ocur = ocur; a.oprev = oprev; a.Y0 = P.Y0; a.capseq = P.capseq;
@@ -261,16 +280,22 @@ int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& 
     }
     a.has_prev = 1; a.last = last;
     a.nstrips = (G.np + PC::WOUT - 1) / PC::WOUT;
-    const int ctas_x = (a.nstrips + BLK_WARPS - 1) / BLK_WARPS;
+    const int ctas_x = (a.nstrips + PIPE_WARPS - 1) / PIPE_WARPS;
+    // theta segments: every segment re-streams K rows above and below its own (the cone of K stages), and the grid
+    // runs in waves of `slots` CTAs; take the count that minimises waves x row-steps per segment
     int nseg = 1;
-    const long want = 148L * 4;   // 2 CTAs per SM resident; >= 2 waves
-    while ((long)ctas_x * nseg * G.nr < want && (G.nt + 2) / (nseg * 2) >= 64) nseg *= 2;
+    long best = -1;
+    for (int n = 1; n <= 32 && (G.nt + 2) / n >= 4 * K; n++) {
+        const long rows = (G.nt + 2 + n - 1) / n + 2 * K;
+        const long waves = ((long)ctas_x * n * G.nr + slots - 1) / slots;
+        if (best < 0 || waves * rows < best) { best = waves * rows; nseg = n; }
+    }
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
     dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
     k_sts_capseq<real, K><<<gc, 256, 0, P.stream>>>(a, T, G, P.capseq);
     bool armed = false;
     P.prof_begin(P.user, &armed);
-    k_sts_pipe<real, K><<<g, BLK_WARPS * 32, smem, P.stream>>>(a, T, G);
+    k_sts_pipe<real, K><<<g, PIPE_WARPS * 32, smem, P.stream>>>(a, T, G);
     P.prof_end(P.user, armed, K);
     *launches += 2;
     return 0;
@@ -319,16 +344,20 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
         int rc = 0;
         if (pipe) {
             switch (K) {
+#ifndef HFT_FAST_BUILD   // experiment builds instantiate K = 8 only
                 case 2: rc = sts_pipe_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
                 case 4: rc = sts_pipe_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
                 case 6: rc = sts_pipe_launch<real, 6>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+#endif
                 default: rc = sts_pipe_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
             }
         } else {
             switch (K) {
+#ifndef HFT_FAST_BUILD
                 case 2: sts_blocked_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
                 case 4: sts_blocked_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
                 case 6: sts_blocked_launch<real, 6>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
+#endif
                 default: sts_blocked_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
             }
         }
