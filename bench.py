@@ -25,6 +25,7 @@ import torch
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
+from paper_2501_06377_b200 import ensemble as ens  # noqa: E402
 from paper_2501_06377_b200 import workloads as wl  # noqa: E402
 
 
@@ -146,12 +147,18 @@ def main():
         torch.cuda.synchronize()
 
     def timed_run(dtype, with_extras):
-        wd = wl.config(args.config, dtype)
+        # rank k owns realizations [k R, (k+1) R) of the weak-scaled ensemble; one clock for the whole ensemble
+        wd = ens.shard(args.config, dtype, rank, world)
         ctx = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, device=f"cuda:{local}")
-        maps = wl.initial_maps(wd, device=f"cuda:{local}").to(ctx.tdtype).contiguous()
+        maps = ens.shard_maps(wd, device=f"cuda:{local}").to(ctx.tdtype).contiguous()
         ctx.set_map(-1, maps[0]) if not wd.per_real_maps else [ctx.set_map(r, maps[r]) for r in range(wd.n_real)]
-        dt, n_cfg, per = wl.plan(wd, *ctx.stable_dt())
-        s = ctx.sts_stage_count(dt)
+        dt, n_cfg, per = wl.plan(wd, *ens.global_limits(*ctx.stable_dt()))
+        s = int(ens.max_over_ranks(float(ctx.sts_stage_count(dt))))
+        if s != ctx.sts_stage_count(dt):          # another rank's realizations need more stages: force the same s
+            ctx.close()
+            ctx = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, sts_stages=s,
+                              device=f"cuda:{local}")
+            ctx.set_map(-1, maps[0]) if not wd.per_real_maps else [ctx.set_map(r, maps[r]) for r in range(wd.n_real)]
         cells = wd.n_real * wd.n_theta * wd.n_phi
         for _ in range(args.warmup):
             ctx.step(1, dt)
@@ -172,10 +179,7 @@ def main():
         kms, kn, kst = ctx.kernel_time()
         ctx.profile_kernels(0)
         clocks = sampler.stop() if (rank == 0 and with_extras) else None
-        if dist is not None:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = t.item()
+        ms = ens.max_over_ranks(ms)
         res = dict(ms=ms, value=world * cells * args.steps / (ms * 1e-3), launches=launches, dt=dt, s=s, cells=cells,
                    kernel_ms=(kms / kn if kn else None), kernel_samples=kn, kernel_stages=(kst / kn if kn else None), clocks=clocks, wd=wd)
         # ---- end-to-end through the C ABI with host buffers
@@ -197,10 +201,7 @@ def main():
             t1.record()
             barrier()
             ems = t0.elapsed_time(t1)
-            if dist is not None:
-                t = torch.tensor([ems], device="cuda", dtype=torch.float64)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                ems = t.item()
+            ems = ens.max_over_ranks(ems)
             res["e2e"] = {"value": world * cells * n_e2e / (ems * 1e-3), "unit": "cell-updates/s",
                           "h2d_bytes_per_step": host_in.numel() * host_in.element_size(),
                           "d2h_bytes_per_step": host_out.numel() * host_out.element_size(), "steps": n_e2e}

@@ -55,31 +55,45 @@ def flow_params(eta, v0, a_deg=14.71, b_deg=-2.40, c_deg=-1.79):
     return [eta, d0, d2, d4, K_MERID * v0, -K_MERID * v0, 0.0]
 
 
-def config(idx: int, dtype: str = "f64") -> Workload:
+def ensemble_params(idx: int, n_real: int) -> np.ndarray:
+    """[n_real][7] parameters of the first n_real realizations of configuration idx's ensemble.  Realization r
+    has the same parameters whatever n_real is (draws are consumed row by row), so an ensemble can be extended
+    over more GPUs without changing the realizations already there (ensemble.shard)."""
     if idx == 0:
-        return Workload("cfg0_64x128_r1_diffusion", 64, 128, 1, "f64", np.array([[500.0, 0, 0, 0, 0, 0, 0]]),
-                        t_end_hours=0.0, advect=False, sts_stages=8, dt_in_dt_expl=8.0, n_steps_fixed=200,
-                        n_pairs=6, map_seed=0)
-    if idx == 1:
-        return Workload("cfg1_512x1024_r1", 512, 1024, 1, "f64", np.array([flow_params(500.0, 15.0)]),
-                        t_end_hours=24.0, n_pairs=40, map_seed=1)
-    if idx == 2:
-        p = np.array([flow_params(250.0 + 50.0 * r, 10.0 + (10.0 / 7.0) * r) for r in range(8)])
-        return Workload("cfg2_1024x2048_r8", 1024, 2048, 8, "f64", p, t_end_hours=24.0, n_pairs=120,
-                        map_seed=2, background_g=2.0)
-    if idx == 3:
+        return np.tile(np.array([[500.0, 0, 0, 0, 0, 0, 0]]), (n_real, 1))
+    if idx in (1, 4):
+        return np.tile(np.array([flow_params(500.0, 15.0)]), (n_real, 1))
+    if idx == 2:      # reading U16: eta = 250 + 50 r, v0 = 10 + (10/7) r, r = 0..7 (repeats beyond 8)
+        return np.array([flow_params(250.0 + 50.0 * (r % 8), 10.0 + (10.0 / 7.0) * (r % 8)) for r in range(n_real)])
+    if idx == 3:      # reading U16: eta, v0, (A - 13.2), B, C each x (1 + 0.2 u), u ~ U(-1, 1), seed 3
         rng = np.random.default_rng(3)
-        u = rng.uniform(-1.0, 1.0, size=(64, 5))
+        u = rng.uniform(-1.0, 1.0, size=(n_real, 5))
         p = []
-        for r in range(64):
+        for r in range(n_real):
             f = 1.0 + 0.2 * u[r]
             eta, v0 = 500.0 * f[0], 15.0 * f[1]
             a = CARRINGTON_DEG_PER_DAY + (14.71 - CARRINGTON_DEG_PER_DAY) * f[2]
             p.append(flow_params(eta, v0, a, -2.40 * f[3], -1.79 * f[4]))
-        return Workload("cfg3_1024x2048_r64_" + dtype, 1024, 2048, 64, dtype, np.array(p), t_end_hours=48.0,
-                        n_pairs=120, map_seed=3, per_real_maps=True)
+        return np.array(p)
+    raise ValueError(idx)
+
+
+def config(idx: int, dtype: str = "f64") -> Workload:
+    if idx == 0:
+        return Workload("cfg0_64x128_r1_diffusion", 64, 128, 1, "f64", ensemble_params(0, 1),
+                        t_end_hours=0.0, advect=False, sts_stages=8, dt_in_dt_expl=8.0, n_steps_fixed=200,
+                        n_pairs=6, map_seed=0)
+    if idx == 1:
+        return Workload("cfg1_512x1024_r1", 512, 1024, 1, "f64", ensemble_params(1, 1),
+                        t_end_hours=24.0, n_pairs=40, map_seed=1)
+    if idx == 2:
+        return Workload("cfg2_1024x2048_r8", 1024, 2048, 8, "f64", ensemble_params(2, 8), t_end_hours=24.0,
+                        n_pairs=120, map_seed=2, background_g=2.0)
+    if idx == 3:
+        return Workload("cfg3_1024x2048_r64_" + dtype, 1024, 2048, 64, dtype, ensemble_params(3, 64),
+                        t_end_hours=48.0, n_pairs=120, map_seed=3, per_real_maps=True)
     if idx == 4:
-        return Workload("cfg4_2048x4096_r1_assim", 2048, 4096, 1, "f64", np.array([flow_params(500.0, 15.0)]),
+        return Workload("cfg4_2048x4096_r1_assim", 2048, 4096, 1, "f64", ensemble_params(4, 1),
                         t_end_hours=24.0, n_pairs=120, map_seed=4, assim_every_hours=1.0)
     raise ValueError(idx)
 
