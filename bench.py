@@ -237,7 +237,7 @@ def main():
         field_bytes = wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes
         ach = 4 * field_bytes * stages_per_launch / (res["kernel_ms"] * 1e-3) / 1e9
         out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                           "kernel": "k_sts_blocked" if stages_per_launch > 1 else "k_sts_stage", "stages_per_launch": stages_per_launch, "avg_launch_ms": res["kernel_ms"],
+                           "kernel": "k_sts_pipe" if stages_per_launch > 1 else "k_sts_stage", "stages_per_launch": stages_per_launch, "avg_launch_ms": res["kernel_ms"],
                            "sampled_launches": res["kernel_samples"], "peak_source": peak_src}
     if args.also_f32 and args.dtype == "f64":
         r32 = timed_run("f32", False)
