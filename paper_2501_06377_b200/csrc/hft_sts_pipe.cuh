@@ -52,7 +52,7 @@ struct PipeCfg {
     static constexpr int DP = D - 2;                          // prefetch distance in rows
     static constexpr int ROW = 32 * C;                        // reals per ring row (512 B)
     static constexpr int NCS = 3;                             // coefficient ring slots (divides U)
-    static constexpr int WARP_REALS = 3 * D * ROW + NCS * K * 4;
+    static constexpr int WARP_REALS = 3 * D * ROW + NCS * K * 4 + D * 32;   // data rings, product ring, raw-coefficient ring
     static constexpr int WARP_BYTES = WARP_REALS * (int)sizeof(real);
     static constexpr int HALO = (K + C - 1) / C * C;          // invalid columns per strip side, whole 16-byte vectors
     static constexpr int WOUT = 32 * C - 2 * HALO;            // columns written per warp
@@ -63,6 +63,12 @@ struct PipeCfg {
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_small(uint32_t dst, const double* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_small(uint32_t dst, const float* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;\n" ::"r"(dst), "l"(src) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N>
@@ -84,10 +90,10 @@ struct PipeWarp {
     const real *gcur, *gprev, *gF;   // this lane's column of row 0 of the three inputs
     real *gocur, *goprev, *gY0;
     real *s_cur, *s_prev, *s_F, *s_coef;   // shared: this lane's 16 bytes of ring slot 0; coefficient ring
+    real* s_raw;                     // shared: this lane's raw coefficient of ring slot 0 (one real per lane and slot)
     const real* c4;                  // raw row coefficients [nt+2][4] of this realization, offset by this lane's q
     const double *capN, *capS;
     real sa, sadd;                   // this lane's product: fma(sa, raw, sadd)
-    real rawq[3];                    // raw coefficient of row-steps t+1..t+3, slot = (row-step - t0) mod 3
     int cl;                          // this lane's level - 1
     int nt, pitch, ja, jb, lane;
     bool wr;
@@ -101,6 +107,10 @@ struct PipeWarp {
             cp_async16(smem_u32(s_prev + slot * ROW), gprev + o);
             cp_async16(smem_u32(s_F + slot * ROW), gF + o);
         }
+        // the raw row coefficient behind this lane's product of row-step row+1 rides in the same group, so it has
+        // landed when the data of `row` has (an LDG issued three row-steps ahead still stalled 17 % of the warp
+        // samples: profiles/r01_pipe_cfg3_gen2.md)
+        if (cl < K) cp_async_small(smem_u32(s_raw + slot * 32), c4 + min(max(row - cl, 0), nt + 1) * 4);
         cp_async_commit();
     }
 
@@ -122,10 +132,7 @@ struct PipeWarp {
         real pl1[C];               // delta_{j0-1} row t-1: the "two levels back" operand of level 1
         vload<real, C>(pl1, s_prev + pmod(PH - 1, D) * ROW);
         prefetch(t + DP, (PH + DP) % D);   // overwrites the slot of row t-2, last read one row-step ago
-        // the raw coefficient of row-step t+1 was requested three row-steps ago (an L2 hit takes about as long
-        // as one row-step: profiles/r01_pipe_f64.md); request the one of row-step t+4 into the freed slot
-        const real raw_next = rawq[(PH + 1) % 3];
-        rawq[(PH + 1) % 3] = raw_of(t + 4);
+        const real raw_next = s_raw[sl * 32];   // this lane's own copy, arrived with the group of row t
         const real* cfs = s_coef + (PH % NCS) * (K * 4);
         real outK[C];
 #pragma unroll
@@ -220,6 +227,7 @@ __global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const _
     real* ws = reinterpret_cast<real*>(pipe_smem) + (size_t)wrp * P::WARP_REALS;
     W.s_cur = ws + lane * C; W.s_prev = W.s_cur + D * ROW; W.s_F = W.s_prev + D * ROW;
     W.s_coef = ws + 3 * D * ROW;
+    W.s_raw = W.s_coef + P::NCS * K * 4 + lane;
     W.capN = A.capseq + ((size_t)r * 2 + 0) * K;
     W.capS = A.capseq + ((size_t)r * 2 + 1) * K;
     W.cl = lane >> 2;
@@ -246,7 +254,6 @@ __global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const _
     __syncwarp();
     for (int i = 0; i < DP; i++) W.prefetch(t0 + i, i);
     W.gen_coef(t0, 0);
-    W.rawq[1] = W.raw_of(t0 + 1); W.rawq[2] = W.raw_of(t0 + 2); W.rawq[0] = W.raw_of(t0 + 3);
     for (int tb = t0; tb <= tend; tb += U) {
         // steady state: every level of every row-step of this macro-iteration works on an interior row
         if (tb >= K + 1 && tb + U - 2 <= nt) W.template macro<0, false>(tb);
