@@ -29,6 +29,13 @@ from paper_2501_06377_b200 import ensemble as ens  # noqa: E402
 from paper_2501_06377_b200 import workloads as wl  # noqa: E402
 
 
+# per-launch DRAM bytes of k_sts_pipe<K = 8> from the committed ncu --set full captures (profiles/)
+NCU_TRAFFIC_BYTES = {(3, "f64"): 3.326450e9 + 2.118438e9, (3, "f32"): 1.966273e9 + 1.046607e9}
+# FMA-class lane-operations per second measured on this pool's B200 with a register-only loop
+# (profiles/r01_pipe_cfg3_gen2.md): 64 DFMA / 128 FFMA lanes per clock per SM
+ALU_PEAK_FMA_PER_S = {"f64": 1.70e13, "f32": 3.53e13}
+
+
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -235,17 +242,34 @@ def main():
         # dominant kernel: the STS stage kernel; algorithmic bytes per launch = 4 passes x field bytes x stages per launch
         stages_per_launch = res["kernel_stages"]
         field_bytes = wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes
-        ach = 4 * field_bytes * stages_per_launch / (res["kernel_ms"] * 1e-3) / 1e9
+        sec = res["kernel_ms"] * 1e-3
+        ach = 4 * field_bytes * stages_per_launch / sec / 1e9
+        blocked = stages_per_launch > 1
         out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                           "kernel": "k_sts_pipe" if stages_per_launch > 1 else "k_sts_stage", "stages_per_launch": stages_per_launch, "avg_launch_ms": res["kernel_ms"],
-                           "sampled_launches": res["kernel_samples"], "peak_source": peak_src}
+                           "kernel": "k_sts_pipe" if blocked else "k_sts_stage", "stages_per_launch": stages_per_launch,
+                           "avg_launch_ms": res["kernel_ms"], "sampled_launches": res["kernel_samples"], "peak_source": peak_src}
+        if blocked:
+            # a K-stage block moves 5 array passes (3 in, 2 out) however large K is; the
+            # distance of THIS kernel from the DRAM roof is that traffic / time, and from the ALU roof its
+            # fp64 / fp32 FMA-class lane-operations / time against the FMA peak measured on this pool
+            traffic = NCU_TRAFFIC_BYTES.get((args.config, args.dtype)) if stages_per_launch == 8 else None
+            out["roofline"]["traffic"] = traffic
+            out["roofline"]["traffic_source"] = "ncu --set full dram__bytes_read+write.sum per launch (profiles/r01_pipe_cfg3_gen2.md)" if traffic else None
+            out["roofline"]["frac_of_blocked_traffic"] = 5 * field_bytes / sec / 1e9 / peak
+            cols = 16 // wbytes * 32                           # columns per warp strip
+            halo = 8                                           # K = 8 invalid columns per side
+            redundancy = cols / (cols - 2 * halo)
+            lane_ops = 7 * stages_per_launch * wd.n_real * (wd.n_theta + 2) * wd.n_phi * redundancy
+            alu_peak = ALU_PEAK_FMA_PER_S[args.dtype]
+            out["roofline"]["alu_frac"] = lane_ops / sec / alu_peak
+            out["roofline"]["alu_peak_fma_per_s"] = alu_peak
     if args.also_f32 and args.dtype == "f64":
         r32 = timed_run("f32", False)
         out["also_f32"] = {"value": r32["value"], "ms_per_step": r32["ms"] / args.steps, "sts_stages": r32["s"],
                            "hbm_roofline_frac_whole_step": r32["value"] / world * (9 + 4 * r32["s"]) * 4 / (peak * 1e9)}
     if rank == 0:
         if not args.no_cpu_baseline:
-            n_or = 2 if wd.n_theta >= 1024 else 8
+            n_or = 24 if wd.n_theta >= 1024 else 200        # ~10-30 s of oracle work on the box's host cores
             rate, el, thr = oracle_sample(wd, args.dtype, n_or, res["dt"], res["s"])
             out["cpu_baseline"] = {"value": rate, "unit": "cell-updates/s", "cores": thr, "kind": "oracle",
                                    "sample": f"1 of {wd.n_real} realizations x {n_or} steps of the full grid ({el:.1f} s)"}

@@ -199,6 +199,55 @@ def test_config3_full_size_sampled_realizations(dtype):
     ctx.close()
 
 
+def test_config2_full_size_sampled_realizations():
+    """BASELINE config 2 at full size (1024x2048, 8 realizations with eta = 250..600, v0 = 10..20, shared map),
+    2 of its 31 steps; the oracle checks realizations 0 and 7 (smallest and largest diffusivity) one by one."""
+    H = hft()
+    w = wl.config(2)
+    ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype="f64")
+    maps = wl.initial_maps(w, device="cuda")
+    ctx.set_map(-1, maps[0].contiguous())
+    dt, n, _ = wl.plan(w, *ctx.stable_dt())
+    s = ctx.sts_stage_count(dt)
+    assert n == 31 and 600 < s < 760, (n, s)
+    before = ctx.diagnostics()
+    ctx.step(2, dt)
+    after = ctx.diagnostics()
+    assert np.all(np.abs(after[:, 0] - before[:, 0]) <= 1e-12 * before[:, 1])
+    for r in (0, 7):
+        o = orc.Oracle(w.n_theta, w.n_phi, w.params[r:r + 1])
+        o.set_map(0, maps[r].cpu().numpy())
+        o.step(2, dt, sts_stages=s)
+        e = rel_linf(ctx.get_full(r).cpu().numpy(), o.get_full(0))
+        assert e <= 1e-12, (r, e)
+    ctx.close()
+
+
+def test_config4_full_size_first_assimilation_hour():
+    """BASELINE config 4 at full size (2048x4096, fp64): the first simulated hour (its steps at CFL 0.5, s ~ 1640
+    stages each) followed by the hourly assimilation of the synthetic observation with the disc weights; element by
+    element against the oracle, then diagnostics."""
+    H = hft()
+    w = wl.config(4)
+    ctx, o = make_pair(w, "f64")
+    dt, n, per = wl.plan(w, *ctx.stable_dt())
+    assert n == 24 * per and abs(per * dt - 1.0) < 1e-12
+    s = ctx.sts_stage_count(dt)
+    assert s == o.sts_stage_count(dt) and s > 1000, s
+    ctx.step(per, dt)
+    o.step(per, dt)
+    compare(ctx, o, 1e-12, "cfg4 hour 1")
+    E = wl.emergence_map(w, 0)
+    wt = wl.assimilation_weights(w, per * dt)
+    obs = (ctx.get_map(0).cpu() + E).contiguous()
+    ctx.assimilate(obs.cuda(), wt.cuda())
+    o.assimilate(obs.numpy(), wt.numpy())
+    compare(ctx, o, 1e-12, "cfg4 assimilation 1")
+    dg, do = ctx.diagnostics(), o.diagnostics()
+    assert np.allclose(dg, do, rtol=0, atol=1e-12 * do[:, 1].max())
+    ctx.close()
+
+
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_assimilation_and_diagnostics(dtype):
     """Config 4 recipe on a small grid: steps, hourly blend with disc weights, per-realization and shared
