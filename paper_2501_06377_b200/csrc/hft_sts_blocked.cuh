@@ -67,29 +67,41 @@ struct BlkArgs {
 };
 
 // ------------------------------------------------------------------ cap sequence from zonal means
-// grid (2 poles, R), block 256.  i = distance from the pole in rows (i = 0 is the cap itself).
+// grid (2 poles, R), block 32 * STS_KMAX.  i = distance from the pole in rows (i = 0 is the cap itself).  Warp i-1
+// sums row i of the three inputs (16-byte loads, lane-strided partial sums, shuffle tree: a fixed order, so the
+// result is deterministic); thread 0 then runs the K-stage recurrence on the K+1 zonal means.
 template <typename real, int K>
-__global__ void __launch_bounds__(256) k_sts_capseq(BlkArgs<real, K> A, Tables<real> T, Geom G, double* capseq) {
-    __shared__ double red[32];
+__global__ void __launch_bounds__(32 * STS_KMAX) k_sts_capseq(BlkArgs<real, K> A, Tables<real> T, Geom G, double* capseq) {
+    constexpr int C = 16 / (int)sizeof(real);
     __shared__ double m0[K + 1], mp[K + 1], mF[K + 1];
     const int pole = blockIdx.x, r = blockIdx.y;
+    const int lane = threadIdx.x & 31, i = (threadIdx.x >> 5) + 1;
     const size_t base = (size_t)r * G.rstride;
-    auto rowidx = [&](int i) { return pole == 0 ? i : G.nt + 1 - i; };
-    for (int i = 1; i <= K; i++) {
+    auto rowidx = [&](int d) { return pole == 0 ? d : G.nt + 1 - d; };
+    if (i <= K) {
         const size_t off = base + (size_t)rowidx(i) * G.pitch;
+        const bool lower = i < K;   // prev and F are needed on rows 1..K-1 only
         double a = 0.0, b = 0.0, c = 0.0;
-        for (int k = threadIdx.x; k < G.np; k += blockDim.x) {
-            a += (double)A.cur[off + k];
-            if (i < K) {
-                if (A.has_prev) b += (double)A.prev[off + k];
-                c += (double)A.F[off + k];
+        for (int k = lane * C; k < G.np; k += 32 * C) {
+            real v[C];
+            vload<real, C>(v, A.cur + off + k);
+#pragma unroll
+            for (int q = 0; q < C; q++) a += (double)v[q];
+            if (lower) {
+                if (A.has_prev) {
+                    vload<real, C>(v, A.prev + off + k);
+#pragma unroll
+                    for (int q = 0; q < C; q++) b += (double)v[q];
+                }
+                vload<real, C>(v, A.F + off + k);
+#pragma unroll
+                for (int q = 0; q < C; q++) c += (double)v[q];
             }
         }
-        double ta = block_sum(a, red);
-        double tb = block_sum(b, red);
-        double tc = block_sum(c, red);
-        if (threadIdx.x == 0) { m0[i] = ta / (double)G.np; mp[i] = tb / (double)G.np; mF[i] = tc / (double)G.np; }
+        a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
+        if (lane == 0) { m0[i] = a / (double)G.np; mp[i] = b / (double)G.np; mF[i] = c / (double)G.np; }
     }
+    __syncthreads();
     if (threadIdx.x != 0) return;
     const size_t capoff = base + (size_t)rowidx(0) * G.pitch;
     m0[0] = (double)A.cur[capoff];
@@ -99,18 +111,18 @@ __global__ void __launch_bounds__(256) k_sts_capseq(BlkArgs<real, K> A, Tables<r
     const real* cm = T.cm + (size_t)r * (G.nt + 2);
     const double capc = T.capc[r] * (double)G.np;
     double lc[K + 1], lp[K + 1], ln[K + 1];  // current level, previous level, new level
-    for (int i = 0; i <= K; i++) { lc[i] = m0[i]; lp[i] = mp[i]; }
+    for (int d = 0; d <= K; d++) { lc[d] = m0[d]; lp[d] = mp[d]; }
     for (int s = 1; s <= K; s++) {
         const double mu = (double)A.mu[s - 1], nu = (double)A.nu[s - 1], a = (double)A.a[s - 1], g = (double)A.g[s - 1];
         ln[0] = mu * lc[0] + nu * lp[0] + a * (capc * (lc[1] - lc[0])) + g * mF[0];
-        for (int i = 1; i <= K - s; i++) {
-            const int j = rowidx(i);
+        for (int d = 1; d <= K - s; d++) {
+            const int j = rowidx(d);
             const double c_out = (double)(pole == 0 ? cp[j] : cm[j]);  // towards the equator
             const double c_in = (double)(pole == 0 ? cm[j] : cp[j]);   // towards the pole
-            ln[i] = mu * lc[i] + nu * lp[i] + a * (c_out * (lc[i + 1] - lc[i]) - c_in * (lc[i] - lc[i - 1])) + g * mF[i];
+            ln[d] = mu * lc[d] + nu * lp[d] + a * (c_out * (lc[d + 1] - lc[d]) - c_in * (lc[d] - lc[d - 1])) + g * mF[d];
         }
         capseq[((size_t)r * 2 + pole) * K + (s - 1)] = ln[0];
-        for (int i = 0; i <= K - s; i++) { lp[i] = lc[i]; lc[i] = ln[i]; }
+        for (int d = 0; d <= K - s; d++) { lp[d] = lc[d]; lc[d] = ln[d]; }
     }
 }
 
@@ -305,7 +317,7 @@ void sts_blocked_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Ge
     while ((long)ctas_x * nseg * G.nr < want && (G.nt + 2) / (nseg * 2) >= 64) nseg *= 2;
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
     dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
-    k_sts_capseq<real, K><<<gc, 256, 0, P.stream>>>(a, T, G, P.capseq);
+    k_sts_capseq<real, K><<<gc, 32 * STS_KMAX, 0, P.stream>>>(a, T, G, P.capseq);
     bool armed = false;
     P.prof_begin(P.user, &armed);
     k_sts_blocked<real, K, C><<<g, BLK_WARPS * 32, 0, P.stream>>>(a, T, G);

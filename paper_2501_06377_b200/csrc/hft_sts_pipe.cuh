@@ -299,7 +299,7 @@ int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& 
     }
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
     dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
-    k_sts_capseq<real, K><<<gc, 256, 0, P.stream>>>(a, T, G, P.capseq);
+    k_sts_capseq<real, K><<<gc, 32 * STS_KMAX, 0, P.stream>>>(a, T, G, P.capseq);
     bool armed = false;
     P.prof_begin(P.user, &armed);
     k_sts_pipe<real, K><<<g, PIPE_WARPS * 32, smem, P.stream>>>(a, T, G);
