@@ -253,7 +253,7 @@ def main():
             # a K-stage block moves 5 array passes (3 in, 2 out) however large K is; the
             # distance of THIS kernel from the DRAM roof is that traffic / time, and from the ALU roof its
             # fp64 / fp32 FMA-class lane-operations / time against the FMA peak measured on this pool
-            traffic = NCU_TRAFFIC_BYTES.get((args.config, args.dtype)) if stages_per_launch == 8 else None
+            traffic = NCU_TRAFFIC_BYTES.get((args.config, args.dtype)) if stages_per_launch > 7 else None
             out["roofline"]["traffic"] = traffic
             out["roofline"]["traffic_source"] = "ncu --set full dram__bytes_read+write.sum per launch (profiles/r01_pipe_cfg3_gen2.md)" if traffic else None
             out["roofline"]["frac_of_blocked_traffic"] = 5 * field_bytes / sec / 1e9 / peak

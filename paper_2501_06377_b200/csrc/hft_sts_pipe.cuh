@@ -308,7 +308,8 @@ int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& 
     return 0;
 }
 
-// One STS step: stage 1 and the (s-1) mod K remainder stages one launch each, then (s-1)/K blocked launches.
+// One STS step: stage 1, the (s-1) mod K remainder stages (pipe: one un-blocked stage if odd, then one shorter block;
+// first generation: one launch each), then (s-1)/K blocked launches of K stages.
 // pipe != 0: k_sts_pipe (default); pipe == 0: the first-generation k_sts_blocked (kept for comparison).
 template <typename real>
 int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int pipe, int64_t* launches) {
@@ -323,9 +324,14 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
     k_sts_stage<real, 0><<<g1, TX, 0, P.stream>>>(a, T, G);
     *launches += 2;
     const int rem = (s - 1) % K;
+    // the remainder: one un-blocked stage if it is odd, then (pipe only) ONE shorter block of rem - (rem & 1) stages
+    int rem_single = rem;
+#ifndef HFT_FAST_BUILD
+    if (pipe) rem_single = rem & 1;
+#endif
     int icur = 0, iprev = 1, pin = 1;
     bool has_prev = false;
-    for (int j = 2; j <= 1 + rem; j++) {  // remainder stages, unblocked
+    for (int j = 2; j <= 1 + rem_single; j++) {  // remainder stages, unblocked
         a.in = b[icur]; a.d2 = b[iprev]; a.part_in = P.part[pin]; a.part_out = P.part[pin ^ 1];
         a.mu = (real)P.mu[j]; a.nu = (real)P.nu[j]; a.a = (real)P.a[j]; a.g = (real)P.g[j];
         a.use_d2 = has_prev;
@@ -335,14 +341,14 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
         has_prev = true;
         pin ^= 1;
     }
-    int j0 = 1 + rem;  // stages done so far
-    const int nblk = (s - j0) / K;
-    for (int i = 0; i < nblk; i++) {
+    int j0 = 1 + rem_single;  // stages done so far
+    while (j0 < s) {
+        const int kb = (rem - rem_single > 0 && j0 == 1 + rem_single) ? rem - rem_single : K;   // stages in this block
         // outputs go to the two buffers that are not inputs
         int o1 = -1, o2 = -1;
         for (int q = 0; q < 4; q++)
             if (q != icur && q != iprev) { if (o1 < 0) o1 = q; else o2 = q; }
-        const bool last = (i == nblk - 1);
+        const bool last = (j0 + kb == s);
         if (pipe && !has_prev) {  // delta_0 = 0 is not stored: the pipe kernel reads it, so write it once
             if (cudaMemsetAsync(b[iprev], 0, (size_t)G.nr * G.rstride * sizeof(real), P.stream) != cudaSuccess) return -1;
             has_prev = true;
@@ -350,7 +356,7 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
         const real* prev = has_prev ? b[iprev] : nullptr;
         int rc = 0;
         if (pipe) {
-            switch (K) {
+            switch (kb) {
 #ifndef HFT_FAST_BUILD   // experiment builds instantiate K = 8 only
                 case 2: rc = sts_pipe_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
                 case 4: rc = sts_pipe_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
@@ -359,7 +365,7 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
                 default: rc = sts_pipe_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
             }
         } else {
-            switch (K) {
+            switch (kb) {
 #ifndef HFT_FAST_BUILD
                 case 2: sts_blocked_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
                 case 4: sts_blocked_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
@@ -370,7 +376,7 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
         }
         if (rc != 0) return rc;
         icur = o1; iprev = o2; has_prev = true;
-        j0 += K;
+        j0 += kb;
     }
     return 0;
 }
