@@ -549,7 +549,7 @@ void SUF(sft_oracle_stable_dt)(void *h, double *dt_adv, double *dt_diff) {
  * adv_flux 0 off / 1 upwind / 2 WENO3-CS(h) / 3 WENO3 eps=1e-12 (test only);
  * adv_time 1 / 3 / 4; diff_time 0 off / 1 Euler / 2 RKL2 / 3 RKG2(3/2) / 12, 13 = textbook-form
  * RKL2 / RKG2 (test only); sts_stages 0 = auto (Step 6) else forced.  Returns the stage count used. */
-int SUF(sft_oracle_step)(void *h, int n_steps, double dt, int adv_flux, int adv_time, int diff_time, int sts_stages) {
+int SUF(sft_oracle_step_ex)(void *h, int n_steps, double dt, int adv_flux, int adv_time, int diff_time, int sts_stages, int split) {
     oracle_t *o = (oracle_t *)h;
     int s = 0;
     if (diff_time == 2 || diff_time == 3 || diff_time == 12 || diff_time == 13) {
@@ -559,13 +559,20 @@ int SUF(sft_oracle_step)(void *h, int n_steps, double dt, int adv_flux, int adv_
     }
     for (int n = 0; n < n_steps; n++) {
         for (int r = 0; r < o->nr; r++) {
-            if (adv_flux != 0) advection_step(o, r, adv_flux, adv_time, dt);
+            /* split 0: Eq. 21 (:308-313) A(dt) then D(dt).  split 1: Strang, Eq. 22 (:317-326) with S omitted:
+             * A(dt/2), D(dt), A(dt/2). */
+            if (adv_flux != 0) advection_step(o, r, adv_flux, adv_time, split ? 0.5 * dt : dt);
             if (diff_time == 1) diffusion_euler_step(o, r, dt);
             else if (diff_time == 2 || diff_time == 3) sts_step(o, r, diff_time, s, dt);
             else if (diff_time == 12 || diff_time == 13) sts_step_textbook(o, r, diff_time % 10, s, dt);
+            if (split && adv_flux != 0) advection_step(o, r, adv_flux, adv_time, 0.5 * dt);
         }
     }
     return s;
+}
+
+int SUF(sft_oracle_step)(void *h, int n_steps, double dt, int adv_flux, int adv_time, int diff_time, int sts_stages) {
+    return SUF(sft_oracle_step_ex)(h, n_steps, dt, adv_flux, adv_time, diff_time, sts_stages, 0);
 }
 
 /* ----------------------------------------------------- assimilation, Step 9 */
@@ -650,5 +657,57 @@ void SUF(sft_oracle_diagnostics)(void *h, double *out /*[nr][4]*/) {
         out[4 * r + 1] = (pp.s - pm.s) * r2;
         out[4 * r + 2] = pp.s * r2;
         out[4 * r + 3] = pm.s * r2;
+    }
+}
+
+/* Remaining run-history quantities (:230-242): out[r][13] =
+ *   0..3  Phi+ and Phi- limited to the north polar region, then to the south polar region: the cells whose centre has
+ *         |latitude| >= lat_cut_deg, i.e. theta_j <= thc or theta_j >= pi - thc with thc = (90 - lat_cut_deg) pi/180,
+ *         caps included (x radius_cm^2);
+ *   4, 5  area of the two regions (x radius_cm^2);
+ *   6..8  min, max and min |B_r| over the whole map (caps included);
+ *   9     H = sqrt(h1^2 + h2^2) (Eq. 16), 10  D (Eq. 17), 11 h1 (Eq. 16a), 12 h2 (Eq. 16b), with
+ *         dOmega = sin(theta) dtheta dphi on the unit sphere and the quadrature weights of reading U19;
+ *         a cap sits at sin(theta) = 0, cos(theta) = +-1: it contributes to D only. */
+void SUF(sft_oracle_diagnostics_ext)(void *h, double lat_cut_deg, double *out /*[nr][13]*/) {
+    oracle_t *o = (oracle_t *)h;
+    int nt = o->nt, np = o->np;
+    double r2 = o->radius_cm * o->radius_cm;
+    double thc = (90.0 - lat_cut_deg) * PI / 180.0;
+    for (int r = 0; r < o->nr; r++) {
+        const real *B = field(o, r);
+        kahan_t f[4] = {{0, 0}, {0, 0}, {0, 0}, {0, 0}}, area[2] = {{0, 0}, {0, 0}}, h1 = {0, 0}, h2 = {0, 0}, d = {0, 0};
+        double bmin = (double)B[0], bmax = (double)B[0], amin = fabs((double)B[0]);
+        for (int j = 0; j <= nt + 1; j++) {
+            int cap = (j == 0 || j == nt + 1);
+            double th = (double)j * o->dth;
+            double dA = cap ? o->Apole : o->st[j] * o->dth * o->dph;
+            int region = (th <= thc) ? 0 : (th >= PI - thc ? 1 : -1);
+            int ncol = cap ? 1 : np;   /* a cap is one cell (stored replicated) */
+            for (int k = 0; k < ncol; k++) {
+                double v = (double)B[(size_t)j * np + k];
+                if (v < bmin) bmin = v;
+                if (v > bmax) bmax = v;
+                if (fabs(v) < amin) amin = fabs(v);
+                if (region >= 0) {
+                    if (v > 0) kadd(&f[2 * region], v * dA); else if (v < 0) kadd(&f[2 * region + 1], v * dA);
+                    kadd(&area[region], dA);
+                }
+                if (cap) {
+                    kadd(&d, v * (j == 0 ? 1.0 : -1.0) * dA);
+                } else {
+                    double ph = (double)k * o->dph;
+                    kadd(&h1, v * o->st[j] * cos(ph) * dA);
+                    kadd(&h2, v * o->st[j] * sin(ph) * dA);
+                    kadd(&d, v * cos(th) * dA);
+                }
+            }
+        }
+        double *q = out + 13 * r, c = 3.0 / (4.0 * PI);
+        for (int i = 0; i < 4; i++) q[i] = f[i].s * r2;
+        q[4] = area[0].s * r2; q[5] = area[1].s * r2;
+        q[6] = bmin; q[7] = bmax; q[8] = amin;
+        q[11] = c * h1.s; q[12] = c * h2.s; q[10] = c * d.s;
+        q[9] = sqrt(q[11] * q[11] + q[12] * q[12]);
     }
 }

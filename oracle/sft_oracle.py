@@ -160,11 +160,12 @@ class Oracle:
         f.argtypes = [C.c_void_p, C.c_double, C.c_int]
         return f(self.h, float(dt), scheme)
 
-    def step(self, n_steps, dt, adv_flux=ADV_WENO3, adv_time=TIME_SSPRK43, diff_time=DIFF_RKG2, sts_stages=0):
-        f = self._f("sft_oracle_step")
+    def step(self, n_steps, dt, adv_flux=ADV_WENO3, adv_time=TIME_SSPRK43, diff_time=DIFF_RKG2, sts_stages=0, strang=False):
+        """Eq. 21 (A then D) per step; strang=True: Eq. 22 with S omitted, A(dt/2) D(dt) A(dt/2)."""
+        f = self._f("sft_oracle_step_ex")
         f.restype = C.c_int
-        f.argtypes = [C.c_void_p, C.c_int, C.c_double] + [C.c_int] * 4
-        s = f(self.h, n_steps, float(dt), adv_flux, adv_time, diff_time, sts_stages)
+        f.argtypes = [C.c_void_p, C.c_int, C.c_double] + [C.c_int] * 5
+        s = f(self.h, n_steps, float(dt), adv_flux, adv_time, diff_time, sts_stages, int(bool(strang)))
         if s < 0:
             raise ValueError("oracle step: invalid STS stage count")
         return s
@@ -187,6 +188,15 @@ class Oracle:
         f.restype = None
         f.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
         f(self.h, _dp(out))
+        return out
+
+    def diagnostics_ext(self, lat_cut_deg=60.0):
+        """[nr][13]: polar Phi+-, polar areas, min / max / min|B|, H, D, h1, h2 (see sft_oracle.c)."""
+        out = np.zeros((self.nr, 13))
+        f = self._f("sft_oracle_diagnostics_ext")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
+        f(self.h, float(lat_cut_deg), _dp(out))
         return out
 
 

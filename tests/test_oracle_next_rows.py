@@ -1,0 +1,122 @@
+"""Pins for the SURVEY.md 8(f)-3 rows of the oracle: Strang splitting (Eq. 22) and the remaining
+run-history diagnostics (polar fluxes and areas, min / max / min|Br|, dipoles Eq. 16-17, :230-242).  CPU only."""
+import math
+
+import numpy as np
+
+from helpers import cell_areas, grid, rel_linf
+from oracle.sft_oracle import ADV_OFF, DIFF_OFF, DIFF_RKG2, Oracle
+from paper_2501_06377_b200 import workloads as wl
+
+
+def _params():
+    return wl.config(1).params
+
+
+def test_diag_ext_brute_force_numpy_on_tiny_grid():
+    """All 13 quantities re-derived with plain numpy sums from their definitions on an 8 x 16 grid."""
+    nt, nphi, lat = 8, 16, 35.0
+    rng = np.random.default_rng(5)
+    o = Oracle(nt, nphi, [[0.0] * 7], radius_cm=3.0)
+    o.set_map(0, rng.normal(size=(nt, nphi)))
+    B = o.get_full(0)
+    th, ph, dth, dph = grid(nt, nphi)
+    dA = cell_areas(nt, nphi)                      # caps: A_pole / nphi per replicated column
+    thc = math.radians(90.0 - lat)
+    north, south = (th <= thc) * np.ones_like(ph, bool), (th >= math.pi - thc) * np.ones_like(ph, bool)
+    assert north[:3].all() and not north[3:].any()          # rows 0..2 (theta = 0, 20, 40 deg <= 55 deg)
+    exp = np.zeros(13)
+    for i, (m, sgn) in enumerate(((north, 1), (north, -1), (south, 1), (south, -1))):
+        sel = m & ((B > 0) if sgn > 0 else (B < 0))
+        exp[i] = (B * dA)[sel].sum() * 9.0
+    exp[4], exp[5] = dA[north].sum() * 9.0, dA[south].sum() * 9.0
+    exp[6], exp[7], exp[8] = B.min(), B.max(), np.abs(B).min()
+    c = 3.0 / (4.0 * math.pi)
+    exp[11] = c * (B * np.sin(th) * np.cos(ph) * dA).sum()
+    exp[12] = c * (B * np.sin(th) * np.sin(ph) * dA).sum()
+    exp[10] = c * (B * np.cos(th) * dA).sum()
+    exp[9] = math.hypot(exp[11], exp[12])
+    got = o.diagnostics_ext(lat)[0]
+    assert np.allclose(got, exp, rtol=1e-13, atol=1e-14), (got, exp)
+    # the polar pieces add up to no more than the whole-sphere fluxes
+    whole = o.diagnostics()[0]
+    assert got[0] + got[2] <= whole[2] + 1e-12 and got[1] + got[3] >= whole[3] - 1e-12
+
+
+def test_dipoles_closed_forms_second_order():
+    """B = cos(theta) is a pure axial dipole: D = 1, H = 0 (Eq. 17).  B = sin(theta) cos(phi - phi0) is a pure
+    equatorial dipole: h1 = cos(phi0), h2 = sin(phi0), H = 1, D = 0 (Eq. 16).  Midpoint rule: O(h^2)."""
+    errD, errH = [], []
+    for nt in (31, 63):
+        nphi = 2 * (nt + 1)
+        o = Oracle(nt, nphi, [[0.0] * 7] * 2)
+        th, ph, _, _ = grid(nt, nphi)
+        o.set_full(0, np.cos(th) * np.ones_like(ph))
+        o.set_full(1, np.sin(th) * np.cos(ph - 0.3))
+        d = o.diagnostics_ext(60.0)
+        assert abs(d[0, 9]) < 1e-14 and abs(d[1, 10]) < 1e-14
+        assert abs(d[1, 11] / d[1, 9] - math.cos(0.3)) < 1e-12 and abs(d[1, 12] / d[1, 9] - math.sin(0.3)) < 1e-12
+        errD.append(abs(d[0, 10] - 1.0))
+        errH.append(abs(d[1, 9] - 1.0))
+        # polar region of cos(theta): only Phi+ in the north, only Phi- in the south, mirror images
+        assert d[0, 1] == 0.0 and d[0, 2] == 0.0 and abs(d[0, 0] + d[0, 3]) < 1e-14 and abs(d[0, 4] - d[0, 5]) < 1e-14
+        # closed forms with theta_e = the southern edge of the last row inside the region
+        jn = int(math.floor(math.radians(30.0) / (math.pi / (nt + 1)) + 1e-12))
+        the = (jn + 0.5) * math.pi / (nt + 1)
+        assert abs(d[0, 4] / (2 * math.pi * (1 - math.cos(the))) - 1) < 2e-3
+        assert abs(d[0, 0] / (math.pi * math.sin(the) ** 2) - 1) < 2e-3
+    assert 3.5 < errD[0] / errD[1] < 4.5 and errD[0] < 2e-3
+    assert errH[0] < 2e-3
+
+
+def _run(o, B, n, dt, **kw):
+    o.set_map(0, B)
+    o.step(n, dt, **kw)
+    return o.get_full(0)
+
+
+def test_strang_reduces_to_its_parts_exactly():
+    """Eq. 22 with one operator off: no diffusion -> two half advection steps per step; no advection -> Eq. 21."""
+    nt, nphi = 24, 48
+    B = wl.bipolar_map(nt, nphi, 4, 11).numpy()
+    o = Oracle(nt, nphi, _params())
+    adv, dexp = o.stable_dt()
+    dt = 0.8 * adv
+    a = _run(o, B, 3, dt, diff_time=DIFF_OFF, strang=True)
+    b = _run(o, B, 6, 0.5 * dt, diff_time=DIFF_OFF, strang=False)
+    assert np.array_equal(a, b)
+    a = _run(o, B, 3, dt, adv_flux=ADV_OFF, diff_time=DIFF_RKG2, strang=True)
+    b = _run(o, B, 3, dt, adv_flux=ADV_OFF, diff_time=DIFF_RKG2, strang=False)
+    assert np.array_equal(a, b)
+    # and the full Strang step is A(dt/2) D(dt) A(dt/2) composed by hand from the same parts
+    o.set_map(0, B)
+    s = o.sts_stage_count(dt)
+    o.step(1, 0.5 * dt, diff_time=DIFF_OFF)
+    o.step(1, dt, adv_flux=ADV_OFF, sts_stages=s)
+    o.step(1, 0.5 * dt, diff_time=DIFF_OFF)
+    byhand = o.get_full(0)
+    assert np.array_equal(_run(o, B, 1, dt, strang=True), byhand)
+    assert not np.array_equal(_run(o, B, 1, dt, strang=False), byhand)
+
+
+def test_strang_is_second_order_lie_first_order():
+    """Splitting error of Eq. 21 is O(dt), of Eq. 22 O(dt^2) (:315-326): against a fine-step reference the error of the
+    Lie sequence halves and that of the Strang sequence quarters when dt halves.  Differential rotation (theta-dependent
+    angular speed) does not commute with diffusion, so the splitting error is there to be seen; a smooth low-order map
+    keeps the spatial and per-operator temporal errors (3rd / 2nd order) below it."""
+    nt, nphi = 32, 64
+    p = np.array(_params(), dtype=float)
+    p[0, 0] = 4.0e5                       # strong diffusion so that both operators act on the time scale of the test
+    th, ph, _, _ = grid(nt, nphi)
+    B = (np.sin(th) ** 2 * np.cos(2 * ph) + 0.5 * np.sin(th) * np.cos(th) * np.sin(ph))[1:-1]
+    o = Oracle(nt, nphi, p)
+    adv, _ = o.stable_dt()
+    T = 0.9 * adv
+    ref = _run(o, B, 64, T / 64, strang=True)
+    e = {}
+    for strang in (False, True):
+        e[strang] = [rel_linf(_run(o, B, n, T / n, strang=strang), ref) for n in (2, 4, 8)]
+    lie, st = e[False], e[True]
+    assert 1.6 < lie[0] / lie[1] < 2.4 and 1.6 < lie[1] / lie[2] < 2.4, lie
+    assert 3.2 < st[0] / st[1] < 4.8, st
+    assert st[1] < 0.5 * lie[1] and st[2] < 0.25 * lie[2]
