@@ -69,8 +69,11 @@ typedef struct {
     int32_t sts_stages; /* 0 = smallest stable count for dt (hft_sts_stage_count); else forced, >= 2 */
     int32_t sts_block;  /* STS stages fused per kernel launch (temporal blocking): 0 = library default,
                            1 = one launch per stage, k > 1 = k stages per launch (even, <= 8) */
-    int32_t use_graph;  /* 1 = capture one time step into a CUDA graph and replay it (default 0) */
-    int32_t reserved[2];
+    int32_t use_graph;  /* accepted and ignored: launches go back to back on one stream and the measured step has
+                           no launch gaps (profiles/), so graph replay was not built */
+    int32_t strang;     /* 0 = Eq. 21 (:308-313): A(dt) then D(dt) per step (default);
+                           1 = Strang splitting, Eq. 22 (:317-326) with S omitted: A(dt/2), D(dt), A(dt/2) */
+    int32_t reserved;   /* must be 0 */
 } hft_options;
 
 /* Bytes of device workspace hft_create needs for this grid / batch (state + 5 stage arrays). */
@@ -115,6 +118,16 @@ int hft_assimilate(hft_ctx* ctx, const void* d_obs, const void* d_weights, int32
 /* Flux diagnostics (:225-230): h_out[n_real][4] = {signed, unsigned, Phi+, Phi-} in G*radius_cm^2.
  * Synchronises the stream. */
 int hft_diagnostics(hft_ctx* ctx, double* h_out);
+
+/* Remaining run-history diagnostics.  h_out[n_real][13]:
+ *   0..3  Phi+ and Phi- over the north polar region, then over the south polar region: the cells whose centre has
+ *         |latitude| >= polar_lat_deg (0..90), polar caps included, in G*radius_cm^2;
+ *   4, 5  area of the two regions, radius_cm^2;
+ *   6..8  min, max and min |Br| over the whole map (caps included);
+ *   9     equatorial dipole strength H = sqrt(h1^2 + h2^2) (Eq. 16), 10 axial dipole D (Eq. 17), 11 h1, 12 h2 (Eq. 16a, b),
+ *         with dOmega on the unit sphere and the quadrature weights of hft_diagnostics (reading U19).
+ * Synchronises the stream. */
+int hft_diagnostics_ext(hft_ctx* ctx, double polar_lat_deg, double* h_out);
 
 /* Host helpers (not timed): Eq. 26 advective limit over all rows and realizations (no safety factor),
  * explicit-Euler diffusion limit 2/rho (Gershgorin), and the STS stage count for dt. */

@@ -64,6 +64,7 @@ struct hft_ctx {
     double* d_zmean = nullptr;               // blocked STS: zonal partial sums (see hft_sts_blocked.cuh)
     double* d_capseq = nullptr;              // blocked STS: cap values per stage
     double* h_diag = nullptr;                // pinned
+    double *d_extpart = nullptr, *d_ext = nullptr, *h_ext = nullptr;   // hft_diagnostics_ext, allocated on first use
     int64_t launches = 0;
     int sts_pipe = 1;  // 1: k_sts_pipe, 0: first-generation k_sts_blocked (env HFT_STS_PIPE=0, for A/B timing)
     StsCoef coef;
@@ -118,6 +119,7 @@ bool valid_options(const hft_options* o) {
     if (o->adv_time != 1 && o->adv_time != 3 && o->adv_time != 4) return false;
     if (o->diff_time < 0 || o->diff_time > 3) return false;
     if (o->sts_stages != 0 && o->sts_stages < 2) return false;
+    if (o->strang != 0 && o->strang != 1) return false;
     if (o->sts_block < 0 || o->sts_block > STS_KMAX || (o->sts_block > 1 && (o->sts_block & 1))) return false;
     return true;
 }
@@ -427,7 +429,9 @@ int diffuse_unblocked(hft_ctx* c, double dt, int s) {
 template <typename real>
 int step_once(hft_ctx* c, double dt, int s) {
     int rc = HFT_OK;
-    if (c->opt.adv_flux != 0) rc = advect<real>(c, dt);
+    // Eq. 21 (:308-313): A(dt) then D(dt).  Strang, Eq. 22 (:317-326) with S omitted: A(dt/2), D(dt), A(dt/2).
+    const bool strang = c->opt.strang != 0;
+    if (c->opt.adv_flux != 0) rc = advect<real>(c, strang ? 0.5 * dt : dt);
     if (rc != HFT_OK) return rc;
     if (c->opt.diff_time != 0) {
         const int kb = c->opt.sts_block == 0 ? sts_default_block(c->G, sizeof(real)) : c->opt.sts_block;
@@ -448,6 +452,7 @@ int step_once(hft_ctx* c, double dt, int s) {
             rc = diffuse_unblocked<real>(c, dt, s);
         }
     }
+    if (rc == HFT_OK && strang && c->opt.adv_flux != 0) rc = advect<real>(c, 0.5 * dt);
     return rc;
 }
 
@@ -542,6 +547,8 @@ void hft_destroy(hft_ctx* c) {
     cudaFree(c->d_tab); cudaFree(c->d_part[0]); cudaFree(c->d_part[1]); cudaFree(c->d_fluxpart);
     cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq);
     if (c->h_diag) cudaFreeHost(c->h_diag);
+    cudaFree(c->d_extpart); cudaFree(c->d_ext);
+    if (c->h_ext) cudaFreeHost(c->h_ext);
     delete c;
 }
 
@@ -678,6 +685,38 @@ int hft_diagnostics(hft_ctx* c, double* h_out) {
     CK(cudaMemcpyAsync(c->h_diag, c->d_diag, (size_t)c->nr * 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     memcpy(h_out, c->h_diag, (size_t)c->nr * 4 * sizeof(double));
+    return HFT_OK;
+}
+
+int hft_diagnostics_ext(hft_ctx* c, double polar_lat_deg, double* h_out) {
+    if (!c || !h_out || !(polar_lat_deg >= 0.0 && polar_lat_deg <= 90.0)) return HFT_ERR_ARG;
+    const Geom& G = c->G;
+    if (!c->d_extpart) {
+        cudaError_t e;
+        if ((e = cudaMalloc((void**)&c->d_extpart, (size_t)c->nr * RED_CTAS * EXT_NPART * sizeof(double))) != cudaSuccess ||
+            (e = cudaMalloc((void**)&c->d_ext, (size_t)c->nr * EXT_NOUT * sizeof(double))) != cudaSuccess ||
+            (e = cudaMallocHost((void**)&c->h_ext, (size_t)c->nr * EXT_NOUT * sizeof(double))) != cudaSuccess) {
+            cuda_fail(c, e, "cudaMalloc");
+            return HFT_ERR_NOMEM;
+        }
+    }
+    dim3 gp(RED_CTAS, c->nr);
+    const int fin_blocks = (c->nr + 63) / 64;
+    const double scale = c->grid.radius_cm * c->grid.radius_cm;
+    const double thc = (90.0 - polar_lat_deg) * kPi / 180.0;
+    if (c->fp64()) {
+        double* S = (double*)c->arr[c->i_state];
+        k_diag_ext_partials<double><<<gp, 256, 0, c->stream>>>(S, c->Td, G, c->dth, c->dph, thc, c->d_extpart);
+        k_diag_ext_finalize<double><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_extpart, RED_CTAS, c->Td, G, c->dth, thc, scale, c->d_ext);
+    } else {
+        float* S = (float*)c->arr[c->i_state];
+        k_diag_ext_partials<float><<<gp, 256, 0, c->stream>>>(S, c->Tf, G, c->dth, c->dph, thc, c->d_extpart);
+        k_diag_ext_finalize<float><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_extpart, RED_CTAS, c->Tf, G, c->dth, thc, scale, c->d_ext);
+    }
+    c->launches += 2;
+    CK(cudaMemcpyAsync(c->h_ext, c->d_ext, (size_t)c->nr * EXT_NOUT * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    memcpy(h_out, c->h_ext, (size_t)c->nr * EXT_NOUT * sizeof(double));
     return HFT_OK;
 }
 

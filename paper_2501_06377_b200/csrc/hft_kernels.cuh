@@ -429,4 +429,100 @@ __global__ void __launch_bounds__(TX) k_assim_blend(real* state, const real* obs
     }
 }
 
+// ------------------------------------------------------------------ remaining run-history diagnostics (:230-242)
+
+constexpr int EXT_NPART = 10;  // per-CTA partials: Phi+N, Phi-N, Phi+S, Phi-S, h1, h2, d, min, max, min|B|
+constexpr int EXT_NOUT = 13;   // see include/hft.h hft_diagnostics_ext
+
+__device__ __forceinline__ double block_min(double v, double* smem /*[32]*/) {
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    __syncthreads();
+    if (lane == 0) smem[w] = v;
+    __syncthreads();
+    double t = smem[0];
+    for (int i = 1; i < nw; i++) t = fmin(t, smem[i]);
+    return t;
+}
+
+// Rows 1..nt: polar-region fluxes (cells with theta_j <= thc or >= pi - thc), the dipole integrands of Eq. 16-17 and
+// min / max / min|B|.  part[r][cta][EXT_NPART]; grid (RED_CTAS, R), block 256.  Row sums in fp64, weights per row.
+template <typename real>
+__global__ void __launch_bounds__(256) k_diag_ext_partials(const real* state, Tables<real> T, Geom G, double dth, double dph,
+                                                           double thc, double* part) {
+    __shared__ double red[32];
+    const int r = blockIdx.y;
+    const real* f = state + (size_t)r * G.rstride;
+    double acc[7] = {0, 0, 0, 0, 0, 0, 0};
+    double vmin = 1.0e300, vmax = -1.0e300, amin = 1.0e300;
+    for (int j = 1 + blockIdx.x; j <= G.nt; j += gridDim.x) {
+        const double th = (double)j * dth, dA = T.dA[j];
+        const int region = th <= thc ? 0 : (th >= 3.14159265358979323846264338327950288 - thc ? 1 : -1);
+        double rp = 0.0, rm = 0.0, rc = 0.0, rs = 0.0;
+        for (int k = threadIdx.x; k < G.np; k += blockDim.x) {
+            const double v = (double)f[(size_t)j * G.pitch + k];
+            double sn, cs;
+            sincos((double)k * dph, &sn, &cs);
+            if (v > 0.0) rp += v; else rm += v;
+            rc += v * cs;
+            rs += v * sn;
+            vmin = fmin(vmin, v); vmax = fmax(vmax, v); amin = fmin(amin, fabs(v));
+        }
+        if (region >= 0) { acc[2 * region] += rp * dA; acc[2 * region + 1] += rm * dA; }
+        const double st = sin(th), ct = cos(th);
+        acc[4] += rc * st * dA;
+        acc[5] += rs * st * dA;
+        acc[6] += (rp + rm) * ct * dA;
+    }
+    double* out = part + ((size_t)r * gridDim.x + blockIdx.x) * EXT_NPART;
+    for (int i = 0; i < 7; i++) {
+        const double t = block_sum(acc[i], red);
+        if (threadIdx.x == 0) out[i] = t;
+    }
+    const double tmin = block_min(vmin, red), tmax = -block_min(-vmax, red), tamin = block_min(amin, red);
+    if (threadIdx.x == 0) { out[7] = tmin; out[8] = tmax; out[9] = tamin; }
+}
+
+// One thread per realization: partials in index order, then the two caps (one cell each: sin(theta) = 0, so they
+// enter D, the polar fluxes / areas and the extrema only) and the region areas.
+template <typename real>
+__global__ void k_diag_ext_finalize(const real* state, const double* part, int nparts, Tables<real> T, Geom G, double dth,
+                                    double thc, double scale, double* out) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= G.nr) return;
+    const double PI_ = 3.14159265358979323846264338327950288;
+    double acc[7] = {0, 0, 0, 0, 0, 0, 0};
+    double vmin = 1.0e300, vmax = -1.0e300, amin = 1.0e300;
+    for (int i = 0; i < nparts; i++) {
+        const double* p = part + ((size_t)r * nparts + i) * EXT_NPART;
+        for (int q = 0; q < 7; q++) acc[q] += p[q];
+        vmin = fmin(vmin, p[7]); vmax = fmax(vmax, p[8]); amin = fmin(amin, p[9]);
+    }
+    double area[2] = {0.0, 0.0};
+    for (int j = 1; j <= G.nt; j++) {
+        const double th = (double)j * dth;
+        if (th <= thc) area[0] += T.dA[j] * (double)G.np;
+        else if (th >= PI_ - thc) area[1] += T.dA[j] * (double)G.np;
+    }
+    for (int pole = 0; pole < 2; pole++) {
+        const double v = (double)state[(size_t)r * G.rstride + (size_t)(pole == 0 ? 0 : G.nt + 1) * G.pitch];
+        const double th = pole == 0 ? 0.0 : (double)(G.nt + 1) * dth, dA = T.dA[0];
+        const int region = th <= thc ? 0 : (th >= PI_ - thc ? 1 : -1);
+        if (region >= 0) {
+            if (v > 0.0) acc[2 * region] += v * dA; else if (v < 0.0) acc[2 * region + 1] += v * dA;
+            area[region] += dA;
+        }
+        acc[6] += v * (pole == 0 ? 1.0 : -1.0) * dA;
+        vmin = fmin(vmin, v); vmax = fmax(vmax, v); amin = fmin(amin, fabs(v));
+    }
+    double* q = out + (size_t)r * EXT_NOUT;
+    const double c = 3.0 / (4.0 * PI_);
+    for (int i = 0; i < 4; i++) q[i] = acc[i] * scale;
+    q[4] = area[0] * scale; q[5] = area[1] * scale;
+    q[6] = vmin; q[7] = vmax; q[8] = amin;
+    q[11] = c * acc[4]; q[12] = c * acc[5]; q[10] = c * acc[6];
+    q[9] = sqrt(q[11] * q[11] + q[12] * q[12]);
+}
+
 }  // namespace hft

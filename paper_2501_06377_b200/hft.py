@@ -19,7 +19,7 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 
 EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_flow_tables", "hft_set_map", "hft_get_map",
-           "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_diagnostics", "hft_stable_dt",
+           "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_diagnostics", "hft_diagnostics_ext", "hft_stable_dt",
            "hft_sts_stage_count", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
            "hft_last_cuda_error"]
 
@@ -41,7 +41,7 @@ class hft_params(C.Structure):
 
 class hft_options(C.Structure):
     _fields_ = [("adv_flux", C.c_int32), ("adv_time", C.c_int32), ("diff_time", C.c_int32), ("sts_stages", C.c_int32),
-                ("sts_block", C.c_int32), ("use_graph", C.c_int32), ("reserved", C.c_int32 * 2)]
+                ("sts_block", C.c_int32), ("use_graph", C.c_int32), ("strang", C.c_int32), ("reserved", C.c_int32)]
 
 
 _lib.hft_workspace_bytes.argtypes = [C.POINTER(hft_grid), C.c_int32, C.POINTER(hft_options), C.POINTER(C.c_size_t)]
@@ -57,6 +57,7 @@ _lib.hft_set_full.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
 _lib.hft_step.argtypes = [C.c_void_p, C.c_int32, C.c_double]
 _lib.hft_assimilate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32]
 _lib.hft_diagnostics.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+_lib.hft_diagnostics_ext.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
 _lib.hft_stable_dt.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.hft_sts_stage_count.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_int32)]
 _lib.hft_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
@@ -89,7 +90,7 @@ class Context:
     """hft_create ... hft_destroy.  Maps are torch CUDA tensors [n_theta][n_phi] of the context dtype."""
 
     def __init__(self, n_theta, n_phi, params, dtype="f64", radius_cm=1.0, adv_flux=ADV_WENO3, adv_time=TIME_SSPRK43,
-                 diff_time=DIFF_RKG2, sts_stages=0, sts_block=0, use_graph=0, device="cuda:0", stream=None):
+                 diff_time=DIFF_RKG2, sts_stages=0, sts_block=0, use_graph=0, strang=0, device="cuda:0", stream=None):
         if not torch.cuda.is_available():
             raise HftError("no CUDA device: the hot path has no CPU fallback")
         self.device = torch.device(device)
@@ -104,7 +105,7 @@ class Context:
             nbytes = workspace_bytes(n_theta, n_phi, self.n_real, dtype)
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             grid = hft_grid(self.n_theta, self.n_phi, 1 if dtype == "f64" else 0, 0, float(radius_cm))
-            opt = hft_options(adv_flux, adv_time, diff_time, sts_stages, sts_block, use_graph)
+            opt = hft_options(adv_flux, adv_time, diff_time, sts_stages, sts_block, use_graph, int(strang), 0)
             pa = (hft_params * self.n_real)(*[hft_params(*row) for row in p])
             rc = _lib.hft_create(C.byref(grid), self.n_real, pa, C.byref(opt), C.c_void_p(self.workspace.data_ptr()),
                                  nbytes, C.c_void_p(self.stream.cuda_stream), C.byref(self._h))
@@ -176,6 +177,12 @@ class Context:
     def diagnostics(self):
         out = np.zeros((self.n_real, 4))
         self._ck(_lib.hft_diagnostics(self._h, out.ctypes.data_as(C.POINTER(C.c_double))), "hft_diagnostics")
+        return out
+
+    def diagnostics_ext(self, polar_lat_deg=60.0):
+        out = np.zeros((self.n_real, 13))
+        self._ck(_lib.hft_diagnostics_ext(self._h, float(polar_lat_deg), out.ctypes.data_as(C.POINTER(C.c_double))),
+                 "hft_diagnostics_ext")
         return out
 
     def stable_dt(self):

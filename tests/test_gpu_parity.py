@@ -317,3 +317,56 @@ def test_errors_are_reported():
         ctx.step(1, -1.0)
     assert ctx.launch_count() >= 0
     ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_strang_splitting(dtype):
+    """Eq. 22 with S omitted, A(dt/2) D(dt) A(dt/2), at the doubled step it allows (:326)."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 70, 264, n_real=3)
+    ctx, o = make_pair(w, dtype, strang=1)
+    adv, _ = ctx.stable_dt()
+    dt = 0.9 * adv                                   # each half advection step runs at CFL 0.45 of the Eq. 26 limit
+    ctx.step(3, dt)
+    o.step(3, dt, strang=True)
+    compare(ctx, o, TOL[dtype], "strang")
+    ctx.close()
+    # and it differs from the un-split sequence by the O(dt) splitting error, far above the tolerance
+    if dtype == "f64":
+        ctx2, _ = make_pair(w, dtype, strang=0)
+        ctx2.step(3, dt)
+        assert rel_linf(ctx2.get_full(0).cpu().numpy(), o.get_full(0)) > 1e4 * TOL[dtype]
+        ctx2.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_run_history_diagnostics(dtype):
+    """polar fluxes / areas, min / max / min|Br| and the dipoles of Eq. 16-17 (:230-242) after
+    a few steps, on a ragged grid with several realizations and a physical radius."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 45, 200, n_real=3)
+    maps = wl.initial_maps(w).to(torch.float64 if dtype == "f64" else torch.float32)
+    ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype, radius_cm=6.96e10)
+    o = orc.Oracle(w.n_theta, w.n_phi, w.params, dtype=NPDT[dtype], radius_cm=6.96e10)
+    for r in range(w.n_real):
+        ctx.set_map(r, maps[r].contiguous().cuda())
+        o.set_map(r, maps[r].numpy())
+    dt, _, _ = wl.plan(w, *ctx.stable_dt())
+    ctx.step(2, dt)
+    o.step(2, dt)
+    for lat in (60.0, 33.3, 90.0, 0.0):
+        g, e = ctx.diagnostics_ext(lat), o.diagnostics_ext(lat)
+        tol = 1e-12 if dtype == "f64" else 2e-5
+        flux_scale = o.diagnostics()[:, 1].max()
+        assert np.allclose(g[:, 0:4], e[:, 0:4], rtol=0, atol=tol * flux_scale), lat
+        assert np.allclose(g[:, 4:6], e[:, 4:6], rtol=1e-13, atol=0), lat            # areas: geometry only
+        bmax = np.abs(e[:, 6:8]).max()
+        assert np.allclose(g[:, 6:9], e[:, 6:9], rtol=0, atol=tol * bmax), lat
+        assert np.allclose(g[:, 9:13], e[:, 9:13], rtol=0, atol=tol * bmax), lat
+    assert np.all(g[:, 4] > 0) and abs(g[0, 4] + g[0, 5] - cell_sum(w) * 6.96e10 ** 2) < 1e-9 * g[0, 4]   # lat 0: both hemispheres
+    ctx.close()
+
+
+def cell_sum(w):
+    from helpers import cell_areas
+    return cell_areas(w.n_theta, w.n_phi).sum()
