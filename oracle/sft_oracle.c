@@ -69,6 +69,8 @@ typedef struct {
     double *vt;   /* [nr][nt+1] v_theta at theta-faces, R_sun/hr (Eq. 4 :84) */
     double *om;   /* [nr][nt+2] Omega = v_phi/sin(theta) at rows, rad/hr (Eq. 3 :78) */
     real *B;      /* [nr][nt+2][np] state */
+    const real *att_src; /* Strang step with attenuation: the field at the start of the step (else NULL) */
+    double *B0;   /* [nr] flow-attenuation saturation field of Eq. 5 (:100) in Gauss; <= 0: attenuation off */
 } oracle_t;
 
 /* ------------------------------------------------------------------ tables */
@@ -113,6 +115,7 @@ void *SUF(sft_oracle_create)(int nt, int np, int nr, const double *params /*[nr]
     o->vt = (double *)calloc((size_t)nr * (nt + 1), sizeof(double));
     o->om = (double *)calloc((size_t)nr * (nt + 2), sizeof(double));
     o->B = (real *)calloc((size_t)nr * (nt + 2) * np, sizeof(real));
+    o->B0 = (double *)calloc(nr, sizeof(double));
     make_grid(o);
     for (int r = 0; r < nr; r++) make_flow(o, r, params + 7 * r);
     return o;
@@ -120,7 +123,13 @@ void *SUF(sft_oracle_create)(int nt, int np, int nr, const double *params /*[nr]
 
 void SUF(sft_oracle_destroy)(void *h) {
     oracle_t *o = (oracle_t *)h;
-    free(o->st); free(o->sth); free(o->nu); free(o->vt); free(o->om); free(o->B); free(o);
+    free(o->st); free(o->sth); free(o->nu); free(o->vt); free(o->om); free(o->B); free(o->B0); free(o);
+}
+
+/* Flow attenuation (Sec. 2.1.3, Eq. 5 :100): B0 in Gauss for realization r (r < 0: all); B0 <= 0 switches it off. */
+void SUF(sft_oracle_set_attenuation)(void *h, int r, double B0) {
+    oracle_t *o = (oracle_t *)h;
+    for (int q = 0; q < o->nr; q++) if (r < 0 || q == r) o->B0[q] = B0;
 }
 
 /* Custom per-row flow tables (needed for the App. C constant-v_theta test, :703): vt in R_sun/hr at
@@ -482,6 +491,137 @@ static void advection_tendency(const oracle_t *o, int r, const real *B, real *ou
     free(vt); free(al);
 }
 
+/* Flow attenuation, Eq. 5 (:100-103): v -> v [1 - tanh(|B_r| / B0)].  The velocities live on the faces (:284-288), B_r at
+ * the cell centres; readings (U22, U23; the paper is silent on both):
+ *   - |B_r| at a face is the magnitude of the mean of the two cells the face separates (for theta-faces 1/2 and
+ *     nt+1/2 one of them is the polar cap);
+ *   - the attenuated velocities are formed ONCE per time step from the field at the start of the step and kept fixed
+ *     through the SSPRK stages (and through both half steps of a Strang step).
+ * VT: (nt+1)*np theta-face speeds, VT[f][k] at face f+1/2 (between rows f, f+1) of column k;
+ * VP: (nt+2)*np phi-face speeds, VP[j][k] at face k-1/2 (between columns k-1 and k) of row j (rows 1..nt). */
+static void attenuated_velocities(const oracle_t *o, int r, const real *B, real *VT, real *VP) {
+    int nt = o->nt, np = o->np;
+    const double *vtd = o->vt + (size_t)r * (nt + 1);
+    const double *omd = o->om + (size_t)r * (nt + 2);
+    real B0 = (real)o->B0[r];
+    #pragma omp parallel for schedule(static)
+    for (int f = 0; f <= nt; f++) {
+        real v = (real)vtd[f];
+        for (int k = 0; k < np; k++) {
+            real bf = (real)0.5 * (B[(size_t)f * np + k] + B[(size_t)(f + 1) * np + k]);
+            VT[(size_t)f * np + k] = v * ((real)1 - (real)tanh((double)((real)fabs((double)bf) / B0)));
+        }
+    }
+    #pragma omp parallel for schedule(static)
+    for (int j = 1; j <= nt; j++) {
+        real v = (real)(omd[j] * o->st[j]);
+        for (int k = 0; k < np; k++) {
+            int km1 = (k + np - 1) % np;
+            real bf = (real)0.5 * (B[(size_t)j * np + km1] + B[(size_t)j * np + k]);
+            VP[(size_t)j * np + k] = v * ((real)1 - (real)tanh((double)((real)fabs((double)bf) / B0)));
+        }
+    }
+}
+
+/* Steps 1-2 with face speeds that vary along both directions (flow attenuation): the same rules as
+ * advection_tendency -- upwind at theta-faces 1/2, 3/2, nt-1/2, nt+1/2, WENO3-CS(h) with LLF elsewhere -- with
+ * alpha_i = max |v| over the six faces i-5/2..i+5/2 ALONG THE SWEEP DIRECTION (:689), clipped to existing faces in
+ * theta and periodic in phi; now both LP and LM are live in phi. */
+static void advection_tendency_general(const oracle_t *o, const real *B, real *out, int flux_mode, const real *VT, const real *VP,
+                                       real *Ft, real *Fp) {
+    int nt = o->nt, np = o->np;
+    real eps_t = (real)o->dth, eps_p = (real)o->dph;
+    if (flux_mode == 3) { eps_t = (real)1e-12; eps_p = (real)1e-12; }
+    #pragma omp parallel for schedule(static)
+    for (int f = 0; f <= nt; f++) {
+        int use_upwind = (flux_mode == 1) || f <= 1 || f >= nt - 1;
+        for (int k = 0; k < np; k++) {
+            real F;
+            if (use_upwind) {
+                F = upwind_flux(VT[(size_t)f * np + k], B[(size_t)f * np + k], B[(size_t)(f + 1) * np + k]);
+            } else {
+                int i = f + 1;
+                real al[4];   /* alpha of cells i-2, i-1, i, i+1 */
+                for (int c = 0; c < 4; c++) {
+                    int ci = i - 2 + c;
+                    real a = (real)0;
+                    for (int q = ci - 3; q <= ci + 2; q++)
+                        if (q >= 0 && q <= nt) { real t = (real)fabs((double)VT[(size_t)q * np + k]); if (t > a) a = t; }
+                    al[c] = a;
+                }
+                #define VTF(q) VT[(size_t)(q) * np + k]
+                real LMm2 = (real)0.5 * B[(size_t)(i - 2) * np + k] * (VTF(i - 3) + al[0]);
+                real LMm1 = (real)0.5 * B[(size_t)(i - 1) * np + k] * (VTF(i - 2) + al[1]);
+                real LM0  = (real)0.5 * B[(size_t)(i    ) * np + k] * (VTF(i - 1) + al[2]);
+                real LPp1 = (real)0.5 * B[(size_t)(i + 1) * np + k] * (VTF(i + 1) - al[3]);
+                real LP0  = (real)0.5 * B[(size_t)(i    ) * np + k] * (VTF(i    ) - al[2]);
+                real LPm1 = (real)0.5 * B[(size_t)(i - 1) * np + k] * (VTF(i - 1) - al[1]);
+                #undef VTF
+                F = weno3_side(LPp1, LP0, LPm1, eps_t) + weno3_side(LMm2, LMm1, LM0, eps_t);
+            }
+            Ft[(size_t)f * np + k] = F;
+        }
+    }
+    #pragma omp parallel for schedule(static)
+    for (int j = 1; j <= nt; j++) {
+        const real *Bc = B + (size_t)j * np, *V = VP + (size_t)j * np;
+        for (int k = 0; k < np; k++) {
+            #define W(q) (((q) % np + np) % np)
+            real F;
+            if (flux_mode == 1) {
+                F = upwind_flux(V[k], Bc[W(k - 1)], Bc[k]);
+            } else {
+                real al[4];   /* alpha of cells k-2, k-1, k, k+1: faces c-5/2..c+5/2 = face indices c-2..c+3 */
+                for (int c = 0; c < 4; c++) {
+                    int ci = k - 2 + c;
+                    real a = (real)0;
+                    for (int q = ci - 2; q <= ci + 3; q++) { real t = (real)fabs((double)V[W(q)]); if (t > a) a = t; }
+                    al[c] = a;
+                }
+                real LMm2 = (real)0.5 * Bc[W(k - 2)] * (V[W(k - 2)] + al[0]);
+                real LMm1 = (real)0.5 * Bc[W(k - 1)] * (V[W(k - 1)] + al[1]);
+                real LM0  = (real)0.5 * Bc[k]        * (V[k]        + al[2]);
+                real LPp1 = (real)0.5 * Bc[W(k + 1)] * (V[W(k + 2)] - al[3]);
+                real LP0  = (real)0.5 * Bc[k]        * (V[W(k + 1)] - al[2]);
+                real LPm1 = (real)0.5 * Bc[W(k - 1)] * (V[k]        - al[1]);
+                F = weno3_side(LPp1, LP0, LPm1, eps_p) + weno3_side(LMm2, LMm1, LM0, eps_p);
+            }
+            #undef W
+            Fp[(size_t)j * np + k] = F;
+        }
+    }
+    #pragma omp parallel for schedule(static)
+    for (int j = 1; j <= nt; j++) {
+        real sp = (real)o->sth[j], sm = (real)o->sth[j - 1];
+        real dt_den = (real)(o->st[j] * o->dth), dp_den = (real)(o->st[j] * o->dph);
+        for (int k = 0; k < np; k++) {
+            int kp1 = (k + 1) % np;
+            real tth = (sp * Ft[(size_t)j * np + k] - sm * Ft[(size_t)(j - 1) * np + k]) / dt_den;
+            real tph = (Fp[(size_t)j * np + kp1] - Fp[(size_t)j * np + k]) / dp_den;
+            out[(size_t)j * np + k] = tth + tph;
+        }
+    }
+    kahan_t a = {0, 0}, b = {0, 0};
+    for (int k = 0; k < np; k++) { kadd(&a, (double)Ft[k]); kadd(&b, (double)Ft[(size_t)nt * np + k]); }
+    fill_row(out, np, (real)(o->P * o->dph * a.s));
+    fill_row(out + (size_t)(nt + 1) * np, np, (real)(-(o->P * o->dph * b.s)));
+}
+
+/* test hook: the general rule with the un-attenuated table speeds copied to every face must reproduce
+ * advection_tendency bit for bit (factor 1 - tanh(0) = 1) */
+void SUF(sft_oracle_advection_tendency_general)(void *h, int r, const real *in, real *out, int flux_mode, double B0) {
+    oracle_t *o = (oracle_t *)h;
+    int nt = o->nt, np = o->np;
+    real *Ft = (real *)malloc((size_t)(nt + 1) * np * sizeof(real)), *Fp = (real *)calloc(fsize(o), sizeof(real));
+    real *VT = (real *)malloc((size_t)(nt + 1) * np * sizeof(real)), *VP = (real *)calloc(fsize(o), sizeof(real));
+    double keep = o->B0[r];
+    o->B0[r] = B0;
+    attenuated_velocities(o, r, in, VT, VP);
+    o->B0[r] = keep;
+    advection_tendency_general(o, in, out, flux_mode, VT, VP, Ft, Fp);
+    free(Ft); free(Fp); free(VT); free(VP);
+}
+
 void SUF(sft_oracle_advection_tendency)(void *h, int r, const real *in, real *out, int flux_mode) {
     oracle_t *o = (oracle_t *)h;
     real *Ft = (real *)malloc((size_t)(o->nt + 1) * o->np * sizeof(real));
@@ -492,33 +632,45 @@ void SUF(sft_oracle_advection_tendency)(void *h, int r, const real *in, real *ou
 
 /* Step 3: advection time integrators.  adv_time 1 = forward Euler (Eq. 23 :396),
  * 3 = SSPRK(3,3) (:412-416), 4 = SSPRK(4,3) (Eq. 25 :418-424). */
+/* F_A with the table speeds, or with the attenuated face speeds VT, VP when flow attenuation is on */
+static void tendency(const oracle_t *o, int r, const real *in, real *out, int flux_mode, const real *VT, const real *VP, real *Ft, real *Fp) {
+    if (VT) advection_tendency_general(o, in, out, flux_mode, VT, VP, Ft, Fp);
+    else advection_tendency(o, r, in, out, flux_mode, Ft, Fp);
+}
+
 static void advection_step(oracle_t *o, int r, int flux_mode, int adv_time, double dt) {
     size_t n = fsize(o);
     real *f = field(o, r);
     real *T = (real *)malloc(n * sizeof(real)), *f1 = (real *)malloc(n * sizeof(real)), *f2 = (real *)malloc(n * sizeof(real));
     real *Ft = (real *)malloc((size_t)(o->nt + 1) * o->np * sizeof(real)), *Fp = (real *)calloc(n, sizeof(real));
     real h = (real)dt;
+    real *VT = NULL, *VP = NULL;
+    if (o->B0[r] > 0.0) {   /* Eq. 5: speeds from the field at the start of the step (reading U23) */
+        VT = (real *)malloc((size_t)(o->nt + 1) * o->np * sizeof(real));
+        VP = (real *)calloc(n, sizeof(real));
+        attenuated_velocities(o, r, o->att_src ? o->att_src : f, VT, VP);
+    }
     if (adv_time == 1) {
-        advection_tendency(o, r, f, T, flux_mode, Ft, Fp);
+        tendency(o, r, f, T, flux_mode, VT, VP, Ft, Fp);
         for (size_t i = 0; i < n; i++) f[i] = f[i] - h * T[i];
     } else if (adv_time == 3) {
-        advection_tendency(o, r, f, T, flux_mode, Ft, Fp);
+        tendency(o, r, f, T, flux_mode, VT, VP, Ft, Fp);
         for (size_t i = 0; i < n; i++) f1[i] = f[i] - h * T[i];
-        advection_tendency(o, r, f1, T, flux_mode, Ft, Fp);
+        tendency(o, r, f1, T, flux_mode, VT, VP, Ft, Fp);
         for (size_t i = 0; i < n; i++) f2[i] = (real)0.75 * f[i] + (real)0.25 * f1[i] - (real)0.25 * h * T[i];
-        advection_tendency(o, r, f2, T, flux_mode, Ft, Fp);
+        tendency(o, r, f2, T, flux_mode, VT, VP, Ft, Fp);
         for (size_t i = 0; i < n; i++) f[i] = (real)(1.0 / 3.0) * f[i] + (real)(2.0 / 3.0) * f2[i] - (real)(2.0 / 3.0) * h * T[i];
     } else {
-        advection_tendency(o, r, f, T, flux_mode, Ft, Fp);
+        tendency(o, r, f, T, flux_mode, VT, VP, Ft, Fp);
         for (size_t i = 0; i < n; i++) f1[i] = f[i] - (real)0.5 * h * T[i];
-        advection_tendency(o, r, f1, T, flux_mode, Ft, Fp);
+        tendency(o, r, f1, T, flux_mode, VT, VP, Ft, Fp);
         for (size_t i = 0; i < n; i++) f2[i] = f1[i] - (real)0.5 * h * T[i];
-        advection_tendency(o, r, f2, T, flux_mode, Ft, Fp);
+        tendency(o, r, f2, T, flux_mode, VT, VP, Ft, Fp);
         for (size_t i = 0; i < n; i++) f1[i] = (real)(2.0 / 3.0) * f[i] + (real)(1.0 / 3.0) * f2[i] - (real)(1.0 / 6.0) * h * T[i];
-        advection_tendency(o, r, f1, T, flux_mode, Ft, Fp);
+        tendency(o, r, f1, T, flux_mode, VT, VP, Ft, Fp);
         for (size_t i = 0; i < n; i++) f[i] = f1[i] - (real)0.5 * h * T[i];
     }
-    free(T); free(f1); free(f2); free(Ft); free(Fp);
+    free(T); free(f1); free(f2); free(Ft); free(Fp); free(VT); free(VP);
 }
 
 /* Advective limit, Eq. 26 form (:430) with the velocities taken as the maximum of the flanking
@@ -561,11 +713,19 @@ int SUF(sft_oracle_step_ex)(void *h, int n_steps, double dt, int adv_flux, int a
         for (int r = 0; r < o->nr; r++) {
             /* split 0: Eq. 21 (:308-313) A(dt) then D(dt).  split 1: Strang, Eq. 22 (:317-326) with S omitted:
              * A(dt/2), D(dt), A(dt/2). */
+            real *start = NULL;
+            if (split && adv_flux != 0 && o->B0[r] > 0.0) {   /* reading U23: one set of attenuated speeds per step */
+                start = (real *)malloc(fsize(o) * sizeof(real));
+                memcpy(start, field(o, r), fsize(o) * sizeof(real));
+                o->att_src = start;
+            }
             if (adv_flux != 0) advection_step(o, r, adv_flux, adv_time, split ? 0.5 * dt : dt);
             if (diff_time == 1) diffusion_euler_step(o, r, dt);
             else if (diff_time == 2 || diff_time == 3) sts_step(o, r, diff_time, s, dt);
             else if (diff_time == 12 || diff_time == 13) sts_step_textbook(o, r, diff_time % 10, s, dt);
             if (split && adv_flux != 0) advection_step(o, r, adv_flux, adv_time, 0.5 * dt);
+            o->att_src = NULL;
+            free(start);
         }
     }
     return s;

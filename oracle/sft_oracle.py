@@ -85,6 +85,23 @@ class Oracle:
         f(self.h, r, _dp(vt), _dp(om))
 
     # -- state ------------------------------------------------------------------------------
+    def set_attenuation(self, r, b0_gauss):
+        """Flow attenuation Eq. 5 (:100): saturation field B0 in Gauss for realization r (-1: all); <= 0 off."""
+        f = self._f("sft_oracle_set_attenuation")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        f(self.h, int(r), float(b0_gauss))
+
+    def advection_tendency_general(self, r, a, flux_mode=ADV_WENO3, b0_gauss=float("inf")):
+        """F_A through the variable-face-speed rule with speeds attenuated by B0 (inf: factor exactly 1)."""
+        a = np.ascontiguousarray(a, dtype=self.dtype)
+        out = np.zeros_like(a)
+        f = self._f("sft_oracle_advection_tendency_general")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_double]
+        f(self.h, int(r), self._rp(a), self._rp(out), flux_mode, float(b0_gauss))
+        return out
+
     def set_map(self, r, m):
         m = np.ascontiguousarray(m, dtype=self.dtype)
         assert m.shape == (self.nt, self.np_)

@@ -120,3 +120,94 @@ def test_strang_is_second_order_lie_first_order():
     assert 1.6 < lie[0] / lie[1] < 2.4 and 1.6 < lie[1] / lie[2] < 2.4, lie
     assert 3.2 < st[0] / st[1] < 4.8, st
     assert st[1] < 0.5 * lie[1] and st[2] < 0.25 * lie[2]
+
+
+# ---------------------------------------------------------------- flow attenuation, Eq. 5, 8(f)-1
+
+def test_attenuation_general_rule_reduces_to_table_rule_bitwise():
+    """With B0 = inf the factor 1 - tanh(0) is exactly 1: the variable-face-speed rule (alpha = max over six faces along
+    the sweep, both LLF parts live in phi) must then give the table-speed rule bit for bit, in both precisions and
+    for both flux types."""
+    nt, nphi = 21, 40
+    B = wl.bipolar_map(nt, nphi, 5, 3, sigma_deg=12.0).numpy()
+    for dtype in (np.float64, np.float32):
+        o = Oracle(nt, nphi, _params(), dtype=dtype)
+        o.set_map(0, B)
+        f = o.get_full(0)
+        for mode in (1, 2):
+            a = o.advection_tendency(0, f, flux_mode=mode)
+            b = o.advection_tendency_general(0, f, flux_mode=mode, b0_gauss=float("inf"))
+            assert np.array_equal(a, b), (dtype, mode)
+
+
+def test_attenuation_uniform_field_scales_the_flow():
+    """Eq. 5 on a uniform field c: every face speed is multiplied by g = 1 - tanh(|c| / B0), so the tendency equals
+    that of the un-attenuated scheme with all flow parameters multiplied by g."""
+    nt, nphi, c, B0 = 20, 36, 300.0, 500.0
+    g = 1.0 - math.tanh(c / B0)
+    p = np.array(_params(), dtype=float)
+    q = p.copy()
+    q[0, 1:] *= g
+    o, os_ = Oracle(nt, nphi, p), Oracle(nt, nphi, q)
+    f = np.full((nt + 2, nphi), -c)             # the sign must not matter
+    a = o.advection_tendency_general(0, f, b0_gauss=B0)
+    b = os_.advection_tendency(0, f)
+    assert np.abs(b).max() > 0 and rel_linf(a, b) < 1e-13
+    # and a different B0 gives a different answer (a dropped B0 or a wrong argument of tanh fails here)
+    assert rel_linf(o.advection_tendency_general(0, f, b0_gauss=2 * B0), b) > 0.1
+
+
+def test_attenuation_saturates_and_conserves():
+    nt, nphi = 24, 48
+    o = Oracle(nt, nphi, _params())
+    adv, _ = o.stable_dt()
+    # |B| >> B0 everywhere: tanh = 1 to the last bit, v = 0, nothing moves
+    rng = np.random.default_rng(2)
+    strong = 5.0e4 * (1.0 + 0.1 * rng.random((nt, nphi)))
+    o.set_attenuation(0, 1.0)
+    o.set_map(0, strong)
+    before = o.get_full(0)
+    o.step(2, 0.5 * adv, adv_time=1, diff_time=DIFF_OFF)          # forward Euler: f - dt * 0 is f to the last bit
+    assert np.array_equal(o.get_full(0), before)
+    o.step(2, 0.5 * adv, diff_time=DIFF_OFF)                      # SSPRK(4,3): 2/3 f + 1/3 f rounds
+    assert rel_linf(o.get_full(0), before) < 1e-15
+    # ordinary case: the flux form still conserves the signed flux to round-off (caps included)
+    o.set_attenuation(0, 500.0)
+    o.set_map(0, wl.bipolar_map(nt, nphi, 6, 8, amp=(200.0, 1500.0), sigma_deg=10.0).numpy())
+    d0 = o.diagnostics()[0]
+    o.step(5, 0.5 * adv, diff_time=DIFF_OFF)
+    d1 = o.diagnostics()[0]
+    assert abs(d1[0] - d0[0]) < 1e-13 * d0[1]
+    # switching it off again restores the table path
+    o.set_attenuation(0, 0.0)
+    o2 = Oracle(nt, nphi, _params())
+    m = wl.bipolar_map(nt, nphi, 3, 9).numpy()
+    o.set_map(0, m); o2.set_map(0, m)
+    o.step(1, 0.5 * adv); o2.step(1, 0.5 * adv)
+    assert np.array_equal(o.get_full(0), o2.get_full(0))
+
+
+def test_attenuation_slows_strong_field_only():
+    """Physical content of Eq. 5 (:98): active regions (|Br| of the order of B0 and above) are carried by a weaker flow
+    than the quiet Sun.  Rigid rotation, one Gaussian spot on the equator: a 2000 G spot drifts much less than the
+    same spot un-attenuated; a 1 G spot is unaffected to a part in a thousand."""
+    nt, nphi = 31, 128
+    p = [[0.0, 1500.0, 0, 0, 0, 0, 0]]                     # v_phi = 1500 m/s sin(theta): rigid rotation
+    th, ph, _, _ = grid(nt, nphi)
+    spot = np.exp(-((th - math.pi / 2) ** 2 + (ph - math.pi) ** 2) / (2 * 0.25 ** 2))[1:-1]
+
+    def drift(amp, b0):
+        o = Oracle(nt, nphi, p)
+        if b0:
+            o.set_attenuation(0, b0)
+        adv, _ = o.stable_dt()
+        o.set_map(0, amp * spot)
+        o.step(40, 0.5 * adv, diff_time=DIFF_OFF)
+        f = o.get_map(0)
+        w = np.abs(f).sum(axis=0)
+        return float((w * ph[0]).sum() / w.sum() - math.pi)
+
+    free = drift(1.0, 0.0)
+    assert free > 0.3
+    assert abs(drift(1.0, 500.0) / free - 1.0) < 2e-3
+    assert drift(2000.0, 500.0) < 0.5 * free
