@@ -73,10 +73,12 @@ typedef struct {
                            no launch gaps (profiles/), so graph replay was not built */
     int32_t strang;     /* 0 = Eq. 21 (:308-313): A(dt) then D(dt) per step (default);
                            1 = Strang splitting, Eq. 22 (:317-326) with S omitted: A(dt/2), D(dt), A(dt/2) */
-    int32_t reserved;   /* must be 0 */
+    int32_t flow_attenuation; /* 1 = reserve workspace for flow attenuation (Eq. 5, :100) and allow hft_set_attenuation;
+                                 6 more field arrays.  0 (default) = off */
 } hft_options;
 
-/* Bytes of device workspace hft_create needs for this grid / batch (state + 5 stage arrays). */
+/* Bytes of device workspace hft_create needs for this grid / batch (state + 5 stage arrays, + 6 with
+ * opt->flow_attenuation).  opt may be NULL (defaults). */
 int hft_workspace_bytes(const hft_grid* grid, int32_t n_real, const hft_options* opt, size_t* h_bytes);
 
 /* Create a context.  d_workspace: caller-allocated device memory of at least hft_workspace_bytes,
@@ -94,6 +96,14 @@ void hft_destroy(hft_ctx* ctx);
  * theta-faces (j+1/2)*dtheta, j = 0..n_theta, in m/s; h_omega[n_theta+2] = v_phi/sin(theta) at the rows
  * j*dtheta, j = 0..n_theta+1, in m/s (i.e. the bracket of Eq. 3). */
 int hft_set_flow_tables(hft_ctx* ctx, int32_t r, const double* h_vtheta, const double* h_omega);
+
+/* Flow attenuation (Sec. 2.1.3, Eq. 5 :100-103): v -> v [1 - tanh(|Br| / B0)] with the saturation field b0_gauss of
+ * realization r (-1: all; the paper's default is 500 G); b0_gauss <= 0 switches it off for that realization.  Needs
+ * hft_options.flow_attenuation = 1 at hft_create, else HFT_ERR_ARG.  |Br| at a face is the magnitude of the mean of the
+ * two cells the face separates; the speeds are formed once per time step from the field at its start and held through
+ * the SSPRK stages (readings U22, U23).  hft_stable_dt keeps returning the un-attenuated limit, which the
+ * attenuated flow (|v| can only shrink) also satisfies.  Synchronises the stream. */
+int hft_set_attenuation(hft_ctx* ctx, int32_t r, double b0_gauss);
 
 /* Set the map of realization r (r = -1: broadcast the one map to all).  d_map: device, [n_theta][n_phi]
  * in the context dtype.  Each polar cap is set to the dphi-weighted mean of its adjacent row. */

@@ -27,6 +27,7 @@ constexpr double kPi = 3.141592653589793238462643383279502884;
 constexpr double kMsToRsHr = 5.172413793103448e-6;    // PAPER.md:298  m/s -> R_sun/hr
 constexpr double kKm2sToRs2Hr = 7.43162901307967e-9;  // PAPER.md:298  km^2/s -> R_sun^2/hr
 constexpr int kNumArrays = 6;                         // state + 5 stage arrays
+constexpr int kNumAttArrays = 6;                      // flow attenuation: VT, VP, LMt, LPt, LMp, LPp (hft_options.flow_attenuation)
 constexpr int kProfEvents = 256;
 
 struct StsCoef {  // per-stage scalars of Sec. 3.7.2 schemes, index 0..s
@@ -46,6 +47,11 @@ struct hft_ctx {
     size_t arr_bytes = 0;
     char* arr[kNumArrays] = {nullptr};
     int i_state = 0;  // index of the array that currently holds the state
+    // flow attenuation (Eq. 5): field-shaped speed arrays behind the ring, B0 per realization, "speeds are current" flag
+    char* att[kNumAttArrays] = {nullptr};
+    std::vector<double> B0;
+    void* d_B0 = nullptr;
+    bool att_any = false, att_ready = false;
     // host tables (fp64)
     double dth = 0, dph = 0, P = 0, Apole = 0;
     std::vector<double> st, sth;      // sin(theta_j) [nt+2], sin(theta_{j+1/2}) [nt+1]
@@ -120,6 +126,7 @@ bool valid_options(const hft_options* o) {
     if (o->diff_time < 0 || o->diff_time > 3) return false;
     if (o->sts_stages != 0 && o->sts_stages < 2) return false;
     if (o->strang != 0 && o->strang != 1) return false;
+    if (o->flow_attenuation != 0 && o->flow_attenuation != 1) return false;
     if (o->sts_block < 0 || o->sts_block > STS_KMAX || (o->sts_block > 1 && (o->sts_block & 1))) return false;
     return true;
 }
@@ -362,14 +369,27 @@ int advect(hft_ctx* c, double dt) {
         sts.push_back({A, nullptr, B, 0.0, 1.0, 0.5});
     }
     dim3 g(G.nbx, (G.nt + RPT - 1) / RPT, c->nr), gc(G.nbx, 2, c->nr);
+    real* att[kNumAttArrays] = {nullptr};
+    if (c->att_any) {
+        for (int i = 0; i < kNumAttArrays; i++) att[i] = (real*)c->att[i];
+        if (!c->att_ready) {   // once per time step, from the field at its start (reading U23)
+            dim3 ga(G.nbx, G.nt + 2, c->nr);
+            k_att_faces<real><<<ga, TX, 0, c->stream>>>(S, (const real*)c->d_B0, T, G, att[0], att[1]);
+            k_att_halfspeeds<real><<<ga, TX, 0, c->stream>>>(att[0], att[1], G, att[2], att[3], att[4], att[5]);
+            c->launches += 2;
+            c->att_ready = true;
+        }
+    }
     for (const St& s : sts) {
         AdvArgs<real> a;
         a.in = s.in; a.fn = s.fn ? s.fn : s.in; a.out = s.out; a.part = c->d_part[0];
         a.ca = (real)s.ca; a.cb = (real)s.cb; a.cdt = (real)s.cc * (real)dt;
         a.upwind_only = c->opt.adv_flux == 1;
+        a.VT = att[0]; a.VP = att[1]; a.LMt = att[2]; a.LPt = att[3]; a.LMp = att[4]; a.LPp = att[5];
         bool armed;
         prof_begin(c, 2, armed);
-        k_adv_stage<real><<<g, TX, 0, c->stream>>>(a, T, G);
+        if (c->att_any) k_adv_stage<real, true><<<g, TX, 0, c->stream>>>(a, T, G);
+        else k_adv_stage<real, false><<<g, TX, 0, c->stream>>>(a, T, G);
         prof_end(c, armed, 1);
         k_adv_caps<real><<<gc, TX, 0, c->stream>>>(a, T, G);
         c->launches += 2;
@@ -429,6 +449,7 @@ int diffuse_unblocked(hft_ctx* c, double dt, int s) {
 template <typename real>
 int step_once(hft_ctx* c, double dt, int s) {
     int rc = HFT_OK;
+    c->att_ready = false;
     // Eq. 21 (:308-313): A(dt) then D(dt).  Strang, Eq. 22 (:317-326) with S omitted: A(dt/2), D(dt), A(dt/2).
     const bool strang = c->opt.strang != 0;
     if (c->opt.adv_flux != 0) rc = advect<real>(c, strang ? 0.5 * dt : dt);
@@ -484,11 +505,11 @@ const char* hft_error_string(int code) {
 const char* hft_last_cuda_error(hft_ctx* ctx) { return ctx ? ctx->cuda_err.c_str() : ""; }
 
 int hft_workspace_bytes(const hft_grid* grid, int32_t n_real, const hft_options* opt, size_t* h_bytes) {
-    (void)opt;
     if (!valid_grid(grid) || n_real < 1 || !h_bytes) return HFT_ERR_ARG;
+    if (opt && !valid_options(opt)) return HFT_ERR_ARG;
     const size_t w = grid->dtype == 1 ? 8 : 4;
     const size_t one = round_up((size_t)n_real * (grid->n_theta + 2) * pitch_for(grid->n_phi, grid->dtype) * w, 256);
-    *h_bytes = one * kNumArrays;
+    *h_bytes = one * (kNumArrays + ((opt && opt->flow_attenuation) ? kNumAttArrays : 0));
     return HFT_OK;
 }
 
@@ -512,8 +533,11 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     c->G.nt = grid->n_theta; c->G.np = grid->n_phi; c->G.pitch = pitch_for(grid->n_phi, grid->dtype); c->G.nr = n_real;
     c->G.rstride = (size_t)(grid->n_theta + 2) * c->G.pitch;
     c->G.nbx = (grid->n_phi + TX - 1) / TX;
-    c->arr_bytes = need / kNumArrays;
+    c->arr_bytes = need / (kNumArrays + (o.flow_attenuation ? kNumAttArrays : 0));
     for (int i = 0; i < kNumArrays; i++) c->arr[i] = (char*)d_workspace + (size_t)i * c->arr_bytes;
+    if (o.flow_attenuation)
+        for (int i = 0; i < kNumAttArrays; i++) c->att[i] = (char*)d_workspace + (size_t)(kNumArrays + i) * c->arr_bytes;
+    c->B0.assign(n_real, 0.0);
     c->nu.resize(n_real); c->vt.resize((size_t)n_real * (c->G.nt + 1)); c->om.resize((size_t)n_real * (c->G.nt + 2));
     build_metric(c);
     for (int r = 0; r < n_real; r++) build_flow(c, r, h_params[r]);
@@ -528,6 +552,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
         (e = cudaMalloc((void**)&c->d_diag, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_zmean, sts_zmean_bytes(c->G))) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_capseq, sts_capseq_bytes(c->G))) != cudaSuccess ||
+        (e = cudaMalloc(&c->d_B0, (size_t)n_real * sizeof(double))) != cudaSuccess ||
         (e = cudaMallocHost((void**)&c->h_diag, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess) {
         cuda_fail(c, e, "cudaMalloc");
         return fail(HFT_ERR_NOMEM);
@@ -545,7 +570,7 @@ void hft_destroy(hft_ctx* c) {
     if (c->prof_ev_made)
         for (int i = 0; i < 2 * kProfEvents; i++) cudaEventDestroy(c->prof_ev[i]);
     cudaFree(c->d_tab); cudaFree(c->d_part[0]); cudaFree(c->d_part[1]); cudaFree(c->d_fluxpart);
-    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq);
+    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq); cudaFree(c->d_B0);
     if (c->h_diag) cudaFreeHost(c->h_diag);
     cudaFree(c->d_extpart); cudaFree(c->d_ext);
     if (c->h_ext) cudaFreeHost(c->h_ext);
@@ -562,6 +587,22 @@ int hft_set_flow_tables(hft_ctx* c, int32_t r, const double* h_vtheta, const dou
     }
     if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
     return upload_all_tables(c);
+}
+
+int hft_set_attenuation(hft_ctx* c, int32_t r, double b0_gauss) {
+    if (!c || r < -1 || r >= c->nr || !c->opt.flow_attenuation || b0_gauss != b0_gauss) return HFT_ERR_ARG;
+    for (int q = 0; q < c->nr; q++)
+        if (r < 0 || q == r) c->B0[q] = b0_gauss > 0.0 ? b0_gauss : 0.0;
+    c->att_any = false;
+    for (double b : c->B0) c->att_any = c->att_any || b > 0.0;
+    CK(cudaStreamSynchronize(c->stream));   // the previous table may still be read by enqueued work
+    if (c->fp64()) {
+        CK(cudaMemcpy(c->d_B0, c->B0.data(), (size_t)c->nr * sizeof(double), cudaMemcpyHostToDevice));
+    } else {
+        std::vector<float> f(c->B0.begin(), c->B0.end());
+        CK(cudaMemcpy(c->d_B0, f.data(), (size_t)c->nr * sizeof(float), cudaMemcpyHostToDevice));
+    }
+    return HFT_OK;
 }
 
 int hft_set_map(hft_ctx* c, int32_t r, const void* d_map) {

@@ -191,6 +191,11 @@ struct AdvArgs {
     double* part;     // [R][2][nbx] phi-sums of the theta-flux at the faces next to the caps
     real ca, cb, cdt;
     int upwind_only;  // adv_flux == 1
+    // flow attenuation (Eq. 5 :100), k_adv_stage<real, true> only: field-shaped arrays [R][nt+2][pitch]
+    const real* VT;   // attenuated v_theta at face j+1/2 (row j = 0..nt)
+    const real* VP;   // attenuated v_phi at face k-1/2 (rows 1..nt)
+    const real *LMt, *LPt;   // theta LLF half-speeds of cell (j,k): (v_{j-1/2} + alpha)/2, (v_{j+1/2} - alpha)/2
+    const real *LMp, *LPp;   // phi   LLF half-speeds of cell (j,k): (v_{k-1/2} + alpha)/2, (v_{k+1/2} - alpha)/2
 };
 
 // theta-face flux at face f (between rows f and f+1) from rows f-1, f, f+1, f+2 of one column.
@@ -214,7 +219,7 @@ __device__ __forceinline__ real phi_face_flux(real bm2, real bm1, real b0, real 
     return weno3_side(pp * bp1, pp * b0, pp * bm1, eps);
 }
 
-template <typename real>
+template <typename real, bool ATT>
 __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> T, Geom G) {
     __shared__ double red[32];
     const int r = blockIdx.z;
@@ -235,16 +240,36 @@ __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> 
     auto ld = [&](int j) -> real { return in[(size_t)min(max(j, 0), nt + 1) * G.pitch + k0]; };
 
     real w0 = ld(j0 - 2), w1 = ld(j0 - 1), w2 = ld(j0), w3 = ld(j0 + 1);
-    real Fn = theta_face_flux<real>(j0 - 1, w0, w1, w2, w3, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
+    // ATT: per-cell speeds of this column / this row instead of the per-row tables
+    auto att_theta = [&](int f, real bm1, real b0, real bp1, real bp2) -> real {
+        auto at = [&](const real* p, int j) -> real { return p[base + (size_t)j * G.pitch + k0]; };
+        if (A.upwind_only || f <= 1 || f >= nt - 1) return upwind(at(A.VT, f), b0, bp1);
+        real um = weno3_side(bm1 * at(A.LMt, f - 1), b0 * at(A.LMt, f), bp1 * at(A.LMt, f + 1), T.eps_t);
+        real up = weno3_side(bp2 * at(A.LPt, f + 2), bp1 * at(A.LPt, f + 1), b0 * at(A.LPt, f), T.eps_t);
+        return up + um;
+    };
+    // face between columns kc-1 and kc of row j; (bm2, bm1, b0, bp1) = columns kc-2 .. kc+1
+    auto att_phi = [&](int j, int kc2, int kc1, int kc, int kcp, real bm2, real bm1, real b0, real bp1) -> real {
+        const size_t ro = base + (size_t)j * G.pitch;
+        if (A.upwind_only) return upwind(A.VP[ro + kc], bm1, b0);
+        real um = weno3_side(bm2 * A.LMp[ro + kc2], bm1 * A.LMp[ro + kc1], b0 * A.LMp[ro + kc], T.eps_p);
+        real up = weno3_side(bp1 * A.LPp[ro + kcp], b0 * A.LPp[ro + kc], bm1 * A.LPp[ro + kc1], T.eps_p);
+        return up + um;
+    };
+    real Fn = ATT ? att_theta(j0 - 1, w0, w1, w2, w3)
+                  : theta_face_flux<real>(j0 - 1, w0, w1, w2, w3, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
     double sumN = 0.0, sumS = 0.0;
     if (j0 == 1) sumN = live ? (double)Fn : 0.0;
     for (int j = j0; j < j1; j++) {
         real w4 = ld(j + 2);
-        real Fs = theta_face_flux<real>(j, w1, w2, w3, w4, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
+        real Fs = ATT ? att_theta(j, w1, w2, w3, w4)
+                      : theta_face_flux<real>(j, w1, w2, w3, w4, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
         const real* row = in + (size_t)j * G.pitch;
         real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1], bp2 = row[kp2];
-        real Fw = phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, A.upwind_only);
-        real Fe = phi_face_flux<real>(bm1, w2, bp1, bp2, pm[j], pp[j], T.eps_p, A.upwind_only);
+        real Fw = ATT ? att_phi(j, km2, km1, k0, kp1, bm2, bm1, w2, bp1)
+                      : phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, A.upwind_only);
+        real Fe = ATT ? att_phi(j, km1, k0, kp1, kp2, bm1, w2, bp1, bp2)
+                      : phi_face_flux<real>(bm1, w2, bp1, bp2, pm[j], pp[j], T.eps_p, A.upwind_only);
         real tend = (T.sth[j] * Fs - T.sth[j - 1] * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
         const size_t off = base + (size_t)j * G.pitch + k0;
         real o = A.cb * w2 - A.cdt * tend;
@@ -278,6 +303,57 @@ __global__ void __launch_bounds__(TX) k_adv_caps(AdvArgs<real> A, Tables<real> T
     real o = A.cb * A.in[off] - A.cdt * tend;
     if (A.ca != (real)0) o = A.ca * A.fn[off] + o;
     A.out[off + k] = o;
+}
+
+// ------------------------------------------------------------------ flow attenuation, Eq. 5 (:100-103)
+
+__device__ __forceinline__ double tanh_r(double x) { return tanh(x); }
+__device__ __forceinline__ float tanh_r(float x) { return tanhf(x); }
+
+// Face speeds v [1 - tanh(|B| / B0)] with |B| at a face = |mean of the two cells it separates| (U22), from the
+// field at the start of the step (U23).  grid (nbx, nt+2, R): thread (j, k) writes VT[j][k] (face j+1/2, j <= nt) and
+// VP[j][k] (face k-1/2, rows 1..nt).  B0[r] <= 0: no attenuation for that realization (factor exactly 1).
+template <typename real>
+__global__ void __launch_bounds__(TX) k_att_faces(const real* state, const real* B0, Tables<real> T, Geom G, real* VT, real* VP) {
+    const int k = blockIdx.x * TX + threadIdx.x, j = blockIdx.y, r = blockIdx.z;
+    if (k >= G.np) return;
+    const int nt = G.nt, km1 = (k + G.np - 1) % G.np;
+    const size_t ro = (size_t)r * G.rstride + (size_t)j * G.pitch;
+    const real b0 = B0[r], b = state[ro + k];
+    const bool on = b0 > (real)0;
+    if (j <= nt) {
+        const real bf = (real)0.5 * (b + state[ro + G.pitch + k]);
+        const real g = on ? (real)1 - tanh_r(fabs(bf) / b0) : (real)1;
+        VT[ro + k] = T.vtf[(size_t)r * (nt + 1) + j] * g;
+    }
+    if (j >= 1 && j <= nt) {
+        const real bf = (real)0.5 * (state[ro + km1] + b);
+        const real g = on ? (real)1 - tanh_r(fabs(bf) / b0) : (real)1;
+        const size_t i = (size_t)r * (nt + 2) + j;
+        VP[ro + k] = (T.pm[i] + T.pp[i]) * g;   // one of pm, pp is 0: the sum is the row speed v_phi exactly
+    }
+}
+
+// LLF half-speeds of every cell (B2 :684) with alpha = max |v| over the six faces c-5/2 .. c+5/2 along the sweep
+// (:689): clipped to existing faces in theta, periodic in phi.  grid (nbx, nt+2, R).
+template <typename real>
+__global__ void __launch_bounds__(TX) k_att_halfspeeds(const real* VT, const real* VP, Geom G, real* LMt, real* LPt, real* LMp,
+                                                       real* LPp) {
+    const int k = blockIdx.x * TX + threadIdx.x, j = blockIdx.y, r = blockIdx.z;
+    if (k >= G.np) return;
+    const int nt = G.nt, np = G.np;
+    const size_t fo = (size_t)r * G.rstride, ro = fo + (size_t)j * G.pitch;
+    real a = (real)0;
+    for (int q = j - 3; q <= j + 2; q++)
+        if (q >= 0 && q <= nt) a = fmax(a, fabs(VT[fo + (size_t)q * G.pitch + k]));
+    LMt[ro + k] = (real)0.5 * ((j >= 1 ? VT[ro - G.pitch + k] : (real)0) + a);
+    LPt[ro + k] = (real)0.5 * ((j <= nt ? VT[ro + k] : (real)0) - a);
+    if (j >= 1 && j <= nt) {
+        real ap = (real)0;
+        for (int q = k - 2; q <= k + 3; q++) ap = fmax(ap, fabs(VP[ro + (q + np) % np]));
+        LMp[ro + k] = (real)0.5 * (VP[ro + k] + ap);
+        LPp[ro + k] = (real)0.5 * (VP[ro + (k + 1) % np] - ap);
+    }
 }
 
 // ------------------------------------------------------------------ maps in / out, caps by row means

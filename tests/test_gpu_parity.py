@@ -370,3 +370,43 @@ def test_run_history_diagnostics(dtype):
 def cell_sum(w):
     from helpers import cell_areas
     return cell_areas(w.n_theta, w.n_phi).sum()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("case", ["weno", "upwind", "strang"])
+def test_flow_attenuation(dtype, case):
+    """flow attenuation Eq. 5 (:100), per-realization B0 (one realization off), strong active regions
+    (|Br| up to ~3 B0) on a ragged grid; WENO3 + SSPRK(4,3) + STS, upwind + Euler, and inside a Strang step."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 52, 200, n_real=3)
+    maps = torch.stack([wl.bipolar_map(w.n_theta, w.n_phi, 8, 50 + r, amp=(100.0, 1500.0), sigma_deg=8.0) for r in range(3)])
+    maps_t = maps.to(torch.float64 if dtype == "f64" else torch.float32)
+    opt = dict(adv_flux=H.ADV_UPWIND, adv_time=H.TIME_EULER) if case == "upwind" else {}
+    ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype, flow_attenuation=1, strang=int(case == "strang"), **opt)
+    o = orc.Oracle(w.n_theta, w.n_phi, w.params, dtype=NPDT[dtype])
+    for r, b0 in enumerate((500.0, 0.0, 120.0)):
+        ctx.set_attenuation(r, b0)
+        o.set_attenuation(r, b0)
+        ctx.set_map(r, maps_t[r].contiguous().cuda())
+        o.set_map(r, maps_t[r].numpy())
+    adv, _ = ctx.stable_dt()
+    dt = (0.9 if case == "strang" else 0.5) * adv
+    before = ctx.diagnostics()
+    ctx.step(3, dt)
+    if case == "upwind":
+        o.step(3, dt, adv_flux=orc.ADV_UPWIND, adv_time=orc.TIME_EULER)
+    else:
+        o.step(3, dt, strang=(case == "strang"))
+    compare(ctx, o, TOL[dtype], "attenuation " + case)
+    after = ctx.diagnostics()
+    assert np.all(np.abs(after[:, 0] - before[:, 0]) <= (1e-12 if dtype == "f64" else 2e-5) * before[:, 1])
+    # the attenuated realizations really moved differently from an un-attenuated run
+    if dtype == "f64" and case == "weno":
+        ctx0 = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype)
+        ctx0.set_map(0, maps_t[0].contiguous().cuda())
+        ctx0.step(3, dt)
+        assert rel_linf(ctx0.get_full(0).cpu().numpy(), o.get_full(0)) > 1e-6
+        ctx0.close()
+    with pytest.raises(H.HftError):
+        H.Context(16, 32, [[0.0] * 7]).set_attenuation(0, 500.0)           # workspace was not reserved for it
+    ctx.close()
