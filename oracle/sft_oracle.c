@@ -29,8 +29,14 @@
  *                    order with eps=1e-12 (:670, Fig. 15); App. C analytic theta solution (:697-731);
  *                    flux conservation incl. polar caps (App. A :622-648)
  *   assimilation     Eq. 8 (:131) closed form, Eq. 10-11 (:144-153) flux balance => net flux of dB is 0
+ *   splitting        Strang (Eq. 22) reduces exactly to its parts; error order 1 (Eq. 21) vs 2 (Eq. 22)
+ *   diagnostics      Eq. 16-17 dipoles of cos(theta), sin(theta)cos(phi - phi0): D = 1, H = 1 (2nd order); brute force
+ *                    of all 13 run-history numbers on 8x16
+ *   attenuation      Eq. 5: with B0 = inf the variable-speed rule equals the table rule bit for bit; uniform field =>
+ *                    flow scaled by 1 - tanh(|c|/B0); |B| >> B0 => nothing moves; flux conserved; strong spot drifts less
  *   PARITY UNPINNED against HipFT itself (no HipFT output in the container): which faces use upwind
- *   next to the poles (reading U6), the stage-count rule (U9), eps_w = coordinate spacing (U11).
+ *   next to the poles (reading U6), the stage-count rule (U9), eps_w = coordinate spacing (U11), where |Br| is taken
+ *   for a face speed and when the attenuated speeds are formed (U22, U23).
  *   They are pinned oracle<->GPU by definition only; see DESIGN.md.
  *
  * Index convention: rows j = 0..nt+1, row 0 = north polar cap, row nt+1 = south
