@@ -76,6 +76,13 @@ typedef struct {
     double *om;   /* [nr][nt+2] Omega = v_phi/sin(theta) at rows, rad/hr (Eq. 3 :78) */
     real *B;      /* [nr][nt+2][np] state */
     const real *att_src; /* Strang step with attenuation: the field at the start of the step (else NULL) */
+    /* random flux emergence (Sec. 2.4): 0 = off, 1 = Eq. 13 (per cell), 2 = Eq. 14 (per unit area) */
+    int rfe_model;
+    double rfe_flux_per_hr, rfe_tau, rfe_t1;   /* Phi/hr in G radius_cm^2 / hr; lifetime tau in hr (inf allowed); time of map 1 */
+    uint64_t rfe_seed;
+    uint32_t rfe_next;                        /* index of the next source map to generate */
+    real *S1, *S2;                            /* [nr][nt+2][np] the two current source maps, G/hr */
+    double time;                              /* simulated hours since create / the last set_rfe */
     double *B0;   /* [nr] flow-attenuation saturation field of Eq. 5 (:100) in Gauss; <= 0: attenuation off */
 } oracle_t;
 
@@ -129,7 +136,7 @@ void *SUF(sft_oracle_create)(int nt, int np, int nr, const double *params /*[nr]
 
 void SUF(sft_oracle_destroy)(void *h) {
     oracle_t *o = (oracle_t *)h;
-    free(o->st); free(o->sth); free(o->nu); free(o->vt); free(o->om); free(o->B); free(o->B0); free(o);
+    free(o->st); free(o->sth); free(o->nu); free(o->vt); free(o->om); free(o->B); free(o->B0); free(o->S1); free(o->S2); free(o);
 }
 
 /* Flow attenuation (Sec. 2.1.3, Eq. 5 :100): B0 in Gauss for realization r (r < 0: all); B0 <= 0 switches it off. */
@@ -701,6 +708,111 @@ void SUF(sft_oracle_stable_dt)(void *h, double *dt_adv, double *dt_diff) {
     *dt_diff = diffusion_dt_expl((oracle_t *)h);
 }
 
+
+/* ------------------------------------------------ random flux emergence, Sec. 2.4 (:155-209) */
+
+/* Counter-based generator Philox4x32-10 (Salmon et al. 2011, "Parallel random numbers: as easy as 1, 2, 3"): ten
+ * rounds of  (c0,c1,c2,c3) <- (hi(M1 c2) ^ c1 ^ k0, lo(M1 c2), hi(M0 c0) ^ c3 ^ k1, lo(M0 c0)),  keys bumped by the
+ * Weyl constants after every round.  The CUDA path implements the same published algorithm on its own (ground rule:
+ * each side implements the same counter-based generator); pinned by the published known-answer vectors. */
+static void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u, W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; round++) {
+        uint64_t p0 = (uint64_t)M0 * c0, p1 = (uint64_t)M1 * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += W0; k1 += W1;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+void SUF(sft_oracle_philox)(const uint32_t *ctr, const uint32_t *key, uint32_t *out) { philox4x32_10(ctr, key, out); }
+
+/* Standard normal Y_i of cell i = (j-1) np + k of source map m of realization r (reading U27): Philox counter
+ * (i, m, r, 0), key = the two halves of the seed; u1 = (x0 + 1/2) 2^-32, u2 = (x1 + 1/2) 2^-32 in (0,1);
+ * Box-Muller Y = sqrt(-2 ln u1) cos(2 pi u2), always in fp64. */
+static double rfe_normal(uint64_t seed, uint32_t cell, uint32_t map, uint32_t r) {
+    uint32_t ctr[4] = {cell, map, r, 0u}, key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)}, x[4];
+    philox4x32_10(ctr, key, x);
+    double u1 = ((double)x[0] + 0.5) * (1.0 / 4294967296.0), u2 = ((double)x[1] + 0.5) * (1.0 / 4294967296.0);
+    return sqrt(-2.0 * log(u1)) * cos(2.0 * PI * u2);
+}
+
+/* One flux-balanced source map (G/hr) for realization r: Eq. 13 (model 1) or Eq. 14 (model 2) on rows 1..nt, polar
+ * caps 0 (reading U28), then balanced "in the same manner as Eq. 11" (:207): with Phi+- = sum of S dA over S > 0 /
+ * S < 0, positive values are divided and the others multiplied by sqrt|Phi+/Phi-| (no scaling if either is 0). */
+static void rfe_make_map(const oracle_t *o, int r, uint32_t map, real *S) {
+    int nt = o->nt, np = o->np;
+    double r2 = o->radius_cm * o->radius_cm, ncells = (double)nt * (double)np;
+    memset(S, 0, fsize(o) * sizeof(real));
+    for (int j = 1; j <= nt; j++) {
+        double dA = o->st[j] * o->dth * o->dph * r2;
+        double amp = o->rfe_model == 1 ? o->rfe_flux_per_hr / (dA * ncells) * sqrt(PI / 2.0)
+                                       : o->rfe_flux_per_hr / (4.0 * PI * r2) * sqrt(PI / 2.0);
+        for (int k = 0; k < np; k++)
+            S[(size_t)j * np + k] = (real)(amp * rfe_normal(o->rfe_seed, (uint32_t)((j - 1) * np + k), map, (uint32_t)r));
+    }
+    kahan_t pp = {0, 0}, pm = {0, 0};
+    for (int j = 1; j <= nt; j++) {
+        double dA = o->st[j] * o->dth * o->dph;
+        for (int k = 0; k < np; k++) {
+            double v = (double)S[(size_t)j * np + k];
+            if (v > 0) kadd(&pp, v * dA); else kadd(&pm, v * dA);
+        }
+    }
+    if (pp.s != 0.0 && pm.s != 0.0) {
+        real sc = (real)sqrt(fabs(pp.s / pm.s));
+        for (int j = 1; j <= nt; j++)
+            for (int k = 0; k < np; k++) {
+                real v = S[(size_t)j * np + k];
+                S[(size_t)j * np + k] = v > (real)0 ? v / sc : v * sc;
+            }
+    }
+}
+
+/* model 0 switches the source off.  flux_per_hr in G radius_cm^2 per hour (Mx/hr for radius_cm = 6.96e10); tau = the
+ * lifetime tau_RFE in hours (INFINITY: the first map stays for ever).  Resets the clock to 0 and draws maps 0 and 1. */
+void SUF(sft_oracle_set_rfe)(void *h, int model, double flux_per_hr, double tau, uint64_t seed) {
+    oracle_t *o = (oracle_t *)h;
+    o->rfe_model = model; o->rfe_flux_per_hr = flux_per_hr; o->rfe_tau = tau; o->rfe_seed = seed;
+    o->time = 0.0; o->rfe_t1 = 0.0; o->rfe_next = 2;
+    if (!model) return;
+    if (!o->S1) { o->S1 = (real *)calloc((size_t)o->nr * fsize(o), sizeof(real)); o->S2 = (real *)calloc((size_t)o->nr * fsize(o), sizeof(real)); }
+    for (int r = 0; r < o->nr; r++) {
+        rfe_make_map(o, r, 0, o->S1 + (size_t)r * fsize(o));
+        rfe_make_map(o, r, 1, o->S2 + (size_t)r * fsize(o));
+    }
+}
+
+void SUF(sft_oracle_get_rfe_maps)(void *h, int r, real *s1, real *s2) {
+    oracle_t *o = (oracle_t *)h;
+    memcpy(s1, o->S1 + (size_t)r * fsize(o), fsize(o) * sizeof(real));
+    memcpy(s2, o->S2 + (size_t)r * fsize(o), fsize(o) * sizeof(real));
+}
+
+/* The source advance S(B, h) at time t (reading U29): when t has reached the time of the second map, map 2 becomes map
+ * 1 and a new map 2 is drawn (:207); then B <- B + h [(1 - alpha) S1 + alpha S2], alpha = (t - t1)/tau (Eq. 15),
+ * i.e. forward Euler with the source frozen at the start of the advance. */
+static void rfe_advance(oracle_t *o, double t, double h) {
+    size_t n = fsize(o);
+    while (t >= o->rfe_t1 + o->rfe_tau) {
+        for (int r = 0; r < o->nr; r++) {
+            memcpy(o->S1 + r * n, o->S2 + r * n, n * sizeof(real));
+            rfe_make_map(o, r, o->rfe_next, o->S2 + r * n);
+        }
+        o->rfe_next++;
+        o->rfe_t1 += o->rfe_tau;
+    }
+    real a = (real)((t - o->rfe_t1) / o->rfe_tau), hh = (real)h;   /* tau = inf: alpha = 0 */
+    for (int r = 0; r < o->nr; r++) {
+        real *B = field(o, r);
+        const real *s1 = o->S1 + r * n, *s2 = o->S2 + r * n;
+        for (size_t i = 0; i < n; i++) B[i] = B[i] + hh * (((real)1 - a) * s1[i] + a * s2[i]);
+    }
+}
+
 /* ------------------------------------------------------------------- step */
 
 /* Step 8: n_steps of B^{n+1} = D(A(B^n)) (Eq. 21 :308-313, S omitted).
@@ -716,9 +828,9 @@ int SUF(sft_oracle_step_ex)(void *h, int n_steps, double dt, int adv_flux, int a
         if (s < 2) return -1;
     }
     for (int n = 0; n < n_steps; n++) {
+        /* Eq. 21: A, D, S.  Eq. 22 (Strang): S(dt/2), A(dt/2), D(dt), A(dt/2), S(dt/2). */
+        if (o->rfe_model && split) rfe_advance(o, o->time, 0.5 * dt);
         for (int r = 0; r < o->nr; r++) {
-            /* split 0: Eq. 21 (:308-313) A(dt) then D(dt).  split 1: Strang, Eq. 22 (:317-326) with S omitted:
-             * A(dt/2), D(dt), A(dt/2). */
             real *start = NULL;
             if (split && adv_flux != 0 && o->B0[r] > 0.0) {   /* reading U23: one set of attenuated speeds per step */
                 start = (real *)malloc(fsize(o) * sizeof(real));
@@ -733,6 +845,11 @@ int SUF(sft_oracle_step_ex)(void *h, int n_steps, double dt, int adv_flux, int a
             o->att_src = NULL;
             free(start);
         }
+        if (o->rfe_model) {
+            if (split) rfe_advance(o, o->time + 0.5 * dt, 0.5 * dt);
+            else rfe_advance(o, o->time, dt);
+        }
+        o->time += dt;
     }
     return s;
 }

@@ -102,6 +102,30 @@ class Oracle:
         f(self.h, int(r), self._rp(a), self._rp(out), flux_mode, float(b0_gauss))
         return out
 
+    def set_rfe(self, model, flux_per_hr, tau_hours=float("inf"), seed=0):
+        """Random flux emergence (Sec. 2.4): model 0 off / 1 Eq. 13 / 2 Eq. 14; flux_per_hr in G radius_cm^2 / hr."""
+        f = self._f("sft_oracle_set_rfe")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_int, C.c_double, C.c_double, C.c_uint64]
+        f(self.h, int(model), float(flux_per_hr), float(tau_hours), int(seed))
+
+    def get_rfe_maps(self, r):
+        s1 = np.empty((self.nt + 2, self.np_), dtype=self.dtype)
+        s2 = np.empty_like(s1)
+        f = self._f("sft_oracle_get_rfe_maps")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        f(self.h, int(r), self._rp(s1), self._rp(s2))
+        return s1, s2
+
+    def philox(self, ctr, key):
+        c = (C.c_uint32 * 4)(*ctr); k = (C.c_uint32 * 2)(*key); out = (C.c_uint32 * 4)()
+        f = self._f("sft_oracle_philox")
+        f.restype = None
+        f.argtypes = [C.POINTER(C.c_uint32)] * 3
+        f(c, k, out)
+        return list(out)
+
     def set_map(self, r, m):
         m = np.ascontiguousarray(m, dtype=self.dtype)
         assert m.shape == (self.nt, self.np_)

@@ -211,3 +211,95 @@ def test_attenuation_slows_strong_field_only():
     assert free > 0.3
     assert abs(drift(1.0, 500.0) / free - 1.0) < 2e-3
     assert drift(2000.0, 500.0) < 0.5 * free
+
+
+# ---------------------------------------------------------------- random flux emergence, Sec. 2.4, 8(f)-2
+
+def test_philox_known_answer_vectors():
+    """The counter-based generator behind the per-cell normals is Philox4x32-10; its published known-answer vectors
+    (tests/golden/paper_values.txt, from the reference implementation of Salmon et al. 2011) pin every constant,
+    the round count and the word order."""
+    import os
+    from helpers import ROOT
+    o = Oracle(8, 16, [[0.0] * 7])
+    n = 0
+    for line in open(os.path.join(ROOT, "tests", "golden", "paper_values.txt")):
+        p = line.split()
+        if p and p[0] == "philox_kat":
+            w = [int(x, 16) for x in p[1:]]
+            assert o.philox(w[0:4], w[4:6]) == w[6:10], line
+            n += 1
+    assert n == 3
+
+
+def _rfe_oracle(model, nt=90, nphi=180, tau=float("inf"), flux=100e21, seed=7, nr=1):
+    o = Oracle(nt, nphi, [[0.0] * 7] * nr, radius_cm=6.96e10)
+    o.set_rfe(model, flux, tau, seed)
+    return o
+
+
+def test_rfe_maps_statistics_balance_and_latitude_dependence():
+    """Eq. 12-14 (:171-197): mean |S dA| per cell = Phi/hr / N_cells (model 1) and mean |S| = Phi/hr / (4 pi R^2)
+    (model 2), before balancing; after balancing the net flux of a map is zero to round-off (:207) and the scaling
+    changed the unsigned flux by O(1/sqrt(N)) only.  Model 1 has |S| ~ 1 / sin(theta) (:189), model 2 none (:199)."""
+    nt, nphi, flux, R = 90, 180, 100e21, 6.96e10
+    th, ph, dth, dph = grid(nt, nphi)
+    dA = (cell_areas(nt, nphi) * R * R)[1:-1]
+    for model in (1, 2):
+        o = _rfe_oracle(model, nt, nphi, flux=flux)
+        s1, s2 = o.get_rfe_maps(0)
+        assert not np.array_equal(s1, s2) and np.all(s1[0] == 0) and np.all(s1[-1] == 0)
+        for S in (s1[1:-1], s2[1:-1]):
+            net, uns = (S * dA).sum(), np.abs(S * dA).sum()
+            assert abs(net) < 1e-12 * uns                                    # balanced
+            if model == 1:
+                assert abs(uns / flux - 1) < 0.03                           # N = 16200 cells: ~0.6 % sampling error + balancing
+                lat_ratio = np.abs(S[4]).mean() / np.abs(S[nt // 2]).mean()  # row 5 (theta = 9.9 deg) against the equator
+                assert abs(lat_ratio * math.sin(5 * dth) - 1) < 0.25
+            else:
+                assert abs(np.abs(S).mean() * 4 * math.pi * R * R / flux - 1) < 0.03
+                assert abs(np.abs(S[4]).mean() / np.abs(S[nt // 2]).mean() - 1) < 0.25
+            # the underlying normals: zero mean, unit variance, Gaussian tails (after removing the known amplitude)
+            Y = S * dA if model == 1 else S
+            Y = Y / (np.abs(Y).mean() * math.sqrt(math.pi / 2))
+            assert abs(Y.mean()) < 0.03 and abs(Y.var() - 1) < 0.05 and abs((Y ** 4).mean() - 3) < 0.3
+            assert 0.25 < (np.abs(Y) > 1.0).mean() < 0.39                    # P(|Y| > 1) = 0.317
+
+
+def test_rfe_realized_unsigned_flux_rate_infinite_and_finite_lifetime():
+    """Fig. 3 (:209): source term only, zero initial map.  Infinite lifetime: the unsigned flux grows at the specified
+    Phi/hr and stays balanced; finite lifetime: it grows more slowly, because successive random maps cancel."""
+    flux, R = 100e21, 6.96e10
+    grow = {}
+    for tau in (float("inf"), 0.3):
+        o = _rfe_oracle(2, 60, 120, tau=tau, flux=flux)
+        o.step(20, 0.1, adv_flux=ADV_OFF, diff_time=DIFF_OFF)                # 2 hours
+        d = o.diagnostics()[0]
+        assert abs(d[0]) < 1e-12 * d[1]
+        grow[tau] = d[1] / 2.0
+    # quadrature of the diagnostics uses the same cell areas as Eq. 14's 4 pi R^2 up to O(dth^2)
+    assert abs(grow[float("inf")] / flux - 1) < 0.04
+    assert grow[0.3] < 0.6 * grow[float("inf")]
+
+
+def test_rfe_time_interpolation_and_map_rotation():
+    """Eq. 15 (:203): between t1 and t1 + tau the source is the linear interpolation of the two maps; at t1 + tau map 2
+    becomes map 1 and a new map is drawn.  Checked against the maps themselves with dt = tau / 4."""
+    tau, dt = 0.8, 0.2
+    o = _rfe_oracle(2, 12, 24, tau=tau, flux=1.0e22)
+    a1, a2 = o.get_rfe_maps(0)
+    exp = np.zeros_like(a1)
+    for n in range(4):
+        al = n * dt / tau
+        exp = exp + dt * ((1 - al) * a1 + al * a2)
+    o.step(4, dt, adv_flux=ADV_OFF, diff_time=DIFF_OFF)
+    assert rel_linf(o.get_full(0), exp) < 1e-14
+    o.step(1, dt, adv_flux=ADV_OFF, diff_time=DIFF_OFF)                       # t = tau: rotation, alpha = 0
+    b1, b2 = o.get_rfe_maps(0)
+    assert np.array_equal(b1, a2) and not np.array_equal(b2, a2) and not np.array_equal(b2, a1)
+    assert rel_linf(o.get_full(0), exp + dt * a2) < 1e-14
+    # different realizations and different seeds draw different maps; the same seed reproduces them
+    o2 = _rfe_oracle(2, 12, 24, tau=tau, flux=1.0e22, nr=2)
+    m0, m1 = o2.get_rfe_maps(0)[0], o2.get_rfe_maps(1)[0]
+    assert np.array_equal(m0, a1) and not np.array_equal(m1, a1)
+    assert not np.array_equal(_rfe_oracle(2, 12, 24, tau=tau, flux=1.0e22, seed=8).get_rfe_maps(0)[0], a1)
