@@ -130,7 +130,6 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--sts-block", type=int, default=0)
-    ap.add_argument("--graph", type=int, default=0, help="1: replay one time step as a CUDA graph (hft_options.use_graph)")
     ap.add_argument("--attenuation", type=float, default=0.0, help="B0 in Gauss: time the step with flow attenuation (Eq. 5) on")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -158,7 +157,7 @@ def main():
     def timed_run(dtype, with_extras):
         # rank k owns realizations [k R, (k+1) R) of the weak-scaled ensemble; one clock for the whole ensemble
         wd = ens.shard(args.config, dtype, rank, world)
-        ctx = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, use_graph=args.graph, flow_attenuation=int(args.attenuation > 0), device=f"cuda:{local}")
+        ctx = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, flow_attenuation=int(args.attenuation > 0), device=f"cuda:{local}")
         if args.attenuation > 0:
             ctx.set_attenuation(-1, args.attenuation)
         maps = ens.shard_maps(wd, device=f"cuda:{local}").to(ctx.tdtype).contiguous()
@@ -168,7 +167,7 @@ def main():
         if s != ctx.sts_stage_count(dt):          # another rank's realizations need more stages: force the same s
             ctx.close()
             ctx = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, sts_stages=s,
-                              use_graph=args.graph, device=f"cuda:{local}")
+                              device=f"cuda:{local}")
             ctx.set_map(-1, maps[0]) if not wd.per_real_maps else [ctx.set_map(r, maps[r]) for r in range(wd.n_real)]
         cells = wd.n_real * wd.n_theta * wd.n_phi
         for _ in range(args.warmup):
@@ -235,7 +234,7 @@ def main():
         "config": {"workload": wd.name, "grid": [wd.n_theta, wd.n_phi], "realizations_per_gpu": wd.n_real,
                    "dt_hours": res["dt"], "sts_stages": res["s"], "adv": "WENO3-CS(h)+SSPRK(4,3)", "diff": "RKG2(3/2)",
                    "l2": "inputs larger than L2 (arrays of %.0f MiB each)" % (wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes / 2**20),
-                   "sts_block": args.sts_block, "cuda_graph": args.graph, "flow_attenuation_b0": args.attenuation, "b_alg_bytes_per_cell_update": b_alg_step,
+                   "sts_block": args.sts_block, "flow_attenuation_b0": args.attenuation, "b_alg_bytes_per_cell_update": b_alg_step,
                    "hbm_roofline_frac_whole_step": frac_step},
         "gpu_launches": res["launches"],
         "clocks": res["clocks"],

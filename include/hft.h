@@ -69,8 +69,8 @@ typedef struct {
     int32_t sts_stages; /* 0 = smallest stable count for dt (hft_sts_stage_count); else forced, >= 2 */
     int32_t sts_block;  /* STS stages fused per kernel launch (temporal blocking): 0 = library default,
                            1 = one launch per stage, k > 1 = k stages per launch (even, <= 8) */
-    int32_t use_graph;  /* accepted and ignored: launches go back to back on one stream and the measured step has
-                           no launch gaps (profiles/), so graph replay was not built */
+    int32_t rfe;        /* 1 = reserve workspace for the two random-flux-emergence source maps (Sec. 2.4; 2 more field
+                           arrays) and allow hft_set_rfe.  0 (default) = off */
     int32_t strang;     /* 0 = Eq. 21 (:308-313): A(dt) then D(dt) per step (default);
                            1 = Strang splitting, Eq. 22 (:317-326) with S omitted: A(dt/2), D(dt), A(dt/2) */
     int32_t flow_attenuation; /* 1 = reserve workspace for flow attenuation (Eq. 5, :100) and allow hft_set_attenuation;
@@ -104,6 +104,19 @@ int hft_set_flow_tables(hft_ctx* ctx, int32_t r, const double* h_vtheta, const d
  * the SSPRK stages (readings U22, U23).  hft_stable_dt keeps returning the un-attenuated limit, which the
  * attenuated flow (|v| can only shrink) also satisfies.  Synchronises the stream. */
 int hft_set_attenuation(hft_ctx* ctx, int32_t r, double b0_gauss);
+
+/* Random flux emergence source term S (Sec. 2.4, :155-209).  model 0 = off, 1 = uniform unsigned flux per cell (Eq. 13),
+ * 2 = uniform unsigned flux per unit area (Eq. 14, the paper's default).  flux_per_hr: total unsigned flux per hour in
+ * G*radius_cm^2/hr (Mx/hr for radius_cm = 6.96e10); tau_hours: lifetime of the random flux elements = time between
+ * source maps (INFINITY: the first map stays); seed: of the counter-based generator (Philox4x32-10, counter = (cell,
+ * map index, realization, 0), Box-Muller in fp64: DESIGN.md reading U27).  Two source maps are kept, each balanced
+ * like Eq. 11; every hft_step integrates S(t) = (1-alpha) S1 + alpha S2, alpha = (t - t1)/tau (Eq. 15), with forward
+ * Euler after D (Eq. 21) or as two half advances around A D A (Eq. 22); when t reaches t1 + tau, map 2 becomes map 1 and a
+ * new map is drawn.  The call resets the run clock to 0 and draws maps 0 and 1.  Needs hft_options.rfe = 1. */
+int hft_set_rfe(hft_ctx* ctx, int32_t model, double flux_per_hr, double tau_hours, uint64_t seed);
+
+/* Copy source map `which` (0 = S1, 1 = S2) of realization r to d_out [n_theta][n_phi] (G/hr; tests). */
+int hft_get_rfe_map(hft_ctx* ctx, int32_t r, int32_t which, void* d_out);
 
 /* Set the map of realization r (r = -1: broadcast the one map to all).  d_map: device, [n_theta][n_phi]
  * in the context dtype.  Each polar cap is set to the dphi-weighted mean of its adjacent row. */
@@ -144,7 +157,7 @@ int hft_diagnostics_ext(hft_ctx* ctx, double polar_lat_deg, double* h_out);
 int hft_stable_dt(hft_ctx* ctx, double* h_dt_adv_limit_hours, double* h_dt_diff_euler_hours);
 int hft_sts_stage_count(hft_ctx* ctx, double dt_hours, int32_t* h_stages);
 
-/* Number of kernel launches enqueued by this context so far (graph replays count their nodes). */
+/* Number of kernel launches enqueued by this context so far. */
 int hft_launch_count(hft_ctx* ctx, int64_t* h_count);
 
 /* Enable per-kernel CUDA-event timing on the context's stream for the kernel class `which`

@@ -27,6 +27,7 @@ constexpr double kPi = 3.141592653589793238462643383279502884;
 constexpr double kMsToRsHr = 5.172413793103448e-6;    // PAPER.md:298  m/s -> R_sun/hr
 constexpr double kKm2sToRs2Hr = 7.43162901307967e-9;  // PAPER.md:298  km^2/s -> R_sun^2/hr
 constexpr int kNumArrays = 6;                         // state + 5 stage arrays
+constexpr int kNumRfeArrays = 2;                      // random flux emergence: the two current source maps (hft_options.rfe)
 constexpr int kNumAttArrays = 6;                      // flow attenuation: VT, VP, LMt, LPt, LMp, LPp (hft_options.flow_attenuation)
 constexpr int kProfEvents = 256;
 
@@ -52,6 +53,12 @@ struct hft_ctx {
     std::vector<double> B0;
     void* d_B0 = nullptr;
     bool att_any = false, att_ready = false;
+    // random flux emergence (Sec. 2.4): the two source maps behind the ring, the run clock and the map schedule
+    char* rfe_map[kNumRfeArrays] = {nullptr};
+    int rfe_model = 0;
+    double rfe_flux = 0.0, rfe_tau = 0.0, rfe_t1 = 0.0, time = 0.0;
+    uint64_t rfe_seed = 0;
+    uint32_t rfe_next = 2;
     // host tables (fp64)
     double dth = 0, dph = 0, P = 0, Apole = 0;
     std::vector<double> st, sth;      // sin(theta_j) [nt+2], sin(theta_{j+1/2}) [nt+1]
@@ -81,10 +88,6 @@ struct hft_ctx {
     int64_t prof_seen = 0;
     cudaEvent_t prof_ev[2 * kProfEvents];
     bool prof_ev_made = false;
-    // CUDA graph of one step
-    cudaGraphExec_t graph = nullptr;
-    double graph_dt = 0.0;
-    int64_t graph_launches = 0;
     std::string cuda_err;
     bool fp64() const { return grid.dtype == 1; }
 };
@@ -116,7 +119,7 @@ bool valid_grid(const hft_grid* g) {
 hft_options default_options() {
     hft_options o;
     memset(&o, 0, sizeof(o));
-    o.adv_flux = 2; o.adv_time = 4; o.diff_time = 3; o.sts_stages = 0; o.sts_block = 0; o.use_graph = 0;
+    o.adv_flux = 2; o.adv_time = 4; o.diff_time = 3; o.sts_stages = 0; o.sts_block = 0;
     return o;
 }
 
@@ -127,6 +130,7 @@ bool valid_options(const hft_options* o) {
     if (o->sts_stages != 0 && o->sts_stages < 2) return false;
     if (o->strang != 0 && o->strang != 1) return false;
     if (o->flow_attenuation != 0 && o->flow_attenuation != 1) return false;
+    if (o->rfe != 0 && o->rfe != 1) return false;
     if (o->sts_block < 0 || o->sts_block > STS_KMAX || (o->sts_block > 1 && (o->sts_block & 1))) return false;
     return true;
 }
@@ -446,12 +450,49 @@ int diffuse_unblocked(hft_ctx* c, double dt, int s) {
     return HFT_OK;
 }
 
+// ---------------------------------------------------------------- random flux emergence (Sec. 2.4)
+
+// One flux-balanced source map `map` of every realization into S (Eq. 13 / 14, balanced like Eq. 11, :207).
+template <typename real>
+int rfe_make_map(hft_ctx* c, real* S, uint32_t map) {
+    const Geom& G = c->G;
+    Tables<real>& T = tables_of<real>(c);
+    dim3 ga(G.nbx, G.nt + 2, c->nr), gp(RED_CTAS, c->nr);
+    const double r2 = c->grid.radius_cm * c->grid.radius_cm;
+    k_rfe_generate<real><<<ga, TX, 0, c->stream>>>(S, T, G, c->rfe_model, c->rfe_flux, r2, (uint32_t)c->rfe_seed,
+                                                   (uint32_t)(c->rfe_seed >> 32), map);
+    k_flux_partials<real, 0><<<gp, 256, 0, c->stream>>>(S, nullptr, nullptr, 0, T, G, c->d_fluxpart);
+    k_flux_finalize<real, 0><<<(c->nr + 63) / 64, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, nullptr, 0, T, G, 1.0, c->d_diag);
+    k_rfe_balance<real><<<ga, TX, 0, c->stream>>>(S, c->d_diag, G);
+    c->launches += 4;
+    return HFT_OK;
+}
+
+// S(B, h) at time t (reading U29): rotate the maps while t has reached the time of map 2, then forward Euler
+// with the Eq. 15 interpolation frozen at t.
+template <typename real>
+int rfe_advance(hft_ctx* c, double t, double h) {
+    const Geom& G = c->G;
+    while (t >= c->rfe_t1 + c->rfe_tau) {
+        char* tmp = c->rfe_map[0]; c->rfe_map[0] = c->rfe_map[1]; c->rfe_map[1] = tmp;   // map 2 becomes map 1
+        rfe_make_map<real>(c, (real*)c->rfe_map[1], c->rfe_next++);
+        c->rfe_t1 += c->rfe_tau;
+    }
+    const real a = (real)((t - c->rfe_t1) / c->rfe_tau);
+    dim3 ga(G.nbx, G.nt + 2, c->nr);
+    k_rfe_apply<real><<<ga, TX, 0, c->stream>>>(arr_of<real>(c, c->i_state), (const real*)c->rfe_map[0], (const real*)c->rfe_map[1], a,
+                                                (real)h, G);
+    c->launches++;
+    return HFT_OK;
+}
+
 template <typename real>
 int step_once(hft_ctx* c, double dt, int s) {
     int rc = HFT_OK;
     c->att_ready = false;
     // Eq. 21 (:308-313): A(dt) then D(dt).  Strang, Eq. 22 (:317-326) with S omitted: A(dt/2), D(dt), A(dt/2).
     const bool strang = c->opt.strang != 0;
+    if (c->rfe_model && strang) rfe_advance<real>(c, c->time, 0.5 * dt);   // Eq. 22: S(dt/2) first
     if (c->opt.adv_flux != 0) rc = advect<real>(c, strang ? 0.5 * dt : dt);
     if (rc != HFT_OK) return rc;
     if (c->opt.diff_time != 0) {
@@ -474,6 +515,11 @@ int step_once(hft_ctx* c, double dt, int s) {
         }
     }
     if (rc == HFT_OK && strang && c->opt.adv_flux != 0) rc = advect<real>(c, 0.5 * dt);
+    if (rc == HFT_OK && c->rfe_model) {   // Eq. 21: S after D; Eq. 22: the second S(dt/2)
+        if (strang) rfe_advance<real>(c, c->time + 0.5 * dt, 0.5 * dt);
+        else rfe_advance<real>(c, c->time, dt);
+    }
+    c->time += dt;
     return rc;
 }
 
@@ -509,7 +555,7 @@ int hft_workspace_bytes(const hft_grid* grid, int32_t n_real, const hft_options*
     if (opt && !valid_options(opt)) return HFT_ERR_ARG;
     const size_t w = grid->dtype == 1 ? 8 : 4;
     const size_t one = round_up((size_t)n_real * (grid->n_theta + 2) * pitch_for(grid->n_phi, grid->dtype) * w, 256);
-    *h_bytes = one * (kNumArrays + ((opt && opt->flow_attenuation) ? kNumAttArrays : 0));
+    *h_bytes = one * (kNumArrays + ((opt && opt->flow_attenuation) ? kNumAttArrays : 0) + ((opt && opt->rfe) ? kNumRfeArrays : 0));
     return HFT_OK;
 }
 
@@ -533,10 +579,13 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     c->G.nt = grid->n_theta; c->G.np = grid->n_phi; c->G.pitch = pitch_for(grid->n_phi, grid->dtype); c->G.nr = n_real;
     c->G.rstride = (size_t)(grid->n_theta + 2) * c->G.pitch;
     c->G.nbx = (grid->n_phi + TX - 1) / TX;
-    c->arr_bytes = need / (kNumArrays + (o.flow_attenuation ? kNumAttArrays : 0));
+    c->arr_bytes = need / (kNumArrays + (o.flow_attenuation ? kNumAttArrays : 0) + (o.rfe ? kNumRfeArrays : 0));
     for (int i = 0; i < kNumArrays; i++) c->arr[i] = (char*)d_workspace + (size_t)i * c->arr_bytes;
     if (o.flow_attenuation)
         for (int i = 0; i < kNumAttArrays; i++) c->att[i] = (char*)d_workspace + (size_t)(kNumArrays + i) * c->arr_bytes;
+    if (o.rfe)
+        for (int i = 0; i < kNumRfeArrays; i++)
+            c->rfe_map[i] = (char*)d_workspace + (size_t)(kNumArrays + (o.flow_attenuation ? kNumAttArrays : 0) + i) * c->arr_bytes;
     c->B0.assign(n_real, 0.0);
     c->nu.resize(n_real); c->vt.resize((size_t)n_real * (c->G.nt + 1)); c->om.resize((size_t)n_real * (c->G.nt + 2));
     build_metric(c);
@@ -566,7 +615,6 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
 
 void hft_destroy(hft_ctx* c) {
     if (!c) return;
-    if (c->graph) cudaGraphExecDestroy(c->graph);
     if (c->prof_ev_made)
         for (int i = 0; i < 2 * kProfEvents; i++) cudaEventDestroy(c->prof_ev[i]);
     cudaFree(c->d_tab); cudaFree(c->d_part[0]); cudaFree(c->d_part[1]); cudaFree(c->d_fluxpart);
@@ -585,7 +633,6 @@ int hft_set_flow_tables(hft_ctx* c, int32_t r, const double* h_vtheta, const dou
         for (int f = 0; f <= nt; f++) c->vt[(size_t)q * (nt + 1) + f] = h_vtheta[f] * kMsToRsHr;
         for (int j = 0; j <= nt + 1; j++) c->om[(size_t)q * (nt + 2) + j] = h_omega[j] * kMsToRsHr;
     }
-    if (c->graph) { cudaGraphExecDestroy(c->graph); c->graph = nullptr; }
     return upload_all_tables(c);
 }
 
@@ -603,6 +650,29 @@ int hft_set_attenuation(hft_ctx* c, int32_t r, double b0_gauss) {
         CK(cudaMemcpy(c->d_B0, f.data(), (size_t)c->nr * sizeof(float), cudaMemcpyHostToDevice));
     }
     return HFT_OK;
+}
+
+int hft_set_rfe(hft_ctx* c, int32_t model, double flux_per_hr, double tau_hours, uint64_t seed) {
+    if (!c || model < 0 || model > 2) return HFT_ERR_ARG;
+    if (model != 0 && (!c->opt.rfe || !(flux_per_hr >= 0.0) || !(tau_hours > 0.0))) return HFT_ERR_ARG;
+    c->rfe_model = model; c->rfe_flux = flux_per_hr; c->rfe_tau = tau_hours; c->rfe_seed = seed;
+    c->time = 0.0; c->rfe_t1 = 0.0; c->rfe_next = 2;
+    if (model == 0) return HFT_OK;
+    for (uint32_t m = 0; m < 2; m++) {
+        if (c->fp64()) rfe_make_map<double>(c, (double*)c->rfe_map[m], m);
+        else rfe_make_map<float>(c, (float*)c->rfe_map[m], m);
+    }
+    return check_launch(c);
+}
+
+int hft_get_rfe_map(hft_ctx* c, int32_t r, int32_t which, void* d_out) {
+    if (!c || !d_out || r < 0 || r >= c->nr || which < 0 || which > 1 || !c->rfe_model) return HFT_ERR_ARG;
+    const Geom& G = c->G;
+    dim3 g((G.np + 255) / 256, G.nt, 1);
+    if (c->fp64()) k_copy_map<double><<<g, 256, 0, c->stream>>>((double*)c->rfe_map[which], (double*)d_out, G, r, 0, 1);
+    else k_copy_map<float><<<g, 256, 0, c->stream>>>((float*)c->rfe_map[which], (float*)d_out, G, r, 0, 1);
+    c->launches++;
+    return check_launch(c);
 }
 
 int hft_set_map(hft_ctx* c, int32_t r, const void* d_map) {

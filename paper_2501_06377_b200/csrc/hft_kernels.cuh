@@ -601,4 +601,62 @@ __global__ void k_diag_ext_finalize(const real* state, const double* part, int n
     q[9] = sqrt(q[11] * q[11] + q[12] * q[12]);
 }
 
+// ------------------------------------------------------------------ random flux emergence, Sec. 2.4 (:155-209)
+
+// Philox4x32-10 (Salmon et al. 2011): the counter-based generator both sides implement (reading U27).
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                                              uint32_t& o0, uint32_t& o1) {
+#pragma unroll
+    for (int round = 0; round < 10; round++) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    o0 = c0; o1 = c1;
+}
+
+// One raw (unbalanced) source map, Eq. 13 (model 1) or Eq. 14 (model 2): S[j][k] = amp_j Y, Y the standard normal of
+// cell i = (j-1) np + k of map `map` of realization r (counter (i, map, r, 0), key = seed; Box-Muller in fp64).
+// Caps 0 (reading U28).  grid (nbx, nt+2, R).
+template <typename real>
+__global__ void __launch_bounds__(TX) k_rfe_generate(real* S, Tables<real> T, Geom G, int model, double flux_per_hr, double r2,
+                                                     uint32_t seed_lo, uint32_t seed_hi, uint32_t map) {
+    const int k = blockIdx.x * TX + threadIdx.x, j = blockIdx.y, r = blockIdx.z;
+    if (k >= G.np) return;
+    real v = (real)0;
+    if (j >= 1 && j <= G.nt) {
+        const double PI_ = 3.14159265358979323846264338327950288;
+        const double dA = T.dA[j] * r2, ncells = (double)G.nt * (double)G.np;
+        const double amp = model == 1 ? flux_per_hr / (dA * ncells) * sqrt(PI_ / 2.0) : flux_per_hr / (4.0 * PI_ * r2) * sqrt(PI_ / 2.0);
+        uint32_t x0, x1;
+        philox4x32_10((uint32_t)((j - 1) * G.np + k), map, (uint32_t)r, 0u, seed_lo, seed_hi, x0, x1);
+        const double u1 = ((double)x0 + 0.5) * (1.0 / 4294967296.0), u2 = ((double)x1 + 0.5) * (1.0 / 4294967296.0);
+        v = (real)(amp * (sqrt(-2.0 * log(u1)) * cos(2.0 * PI_ * u2)));
+    }
+    S[(size_t)r * G.rstride + (size_t)j * G.pitch + k] = v;
+}
+
+// Balance a source map "in the same manner as Eq. 11" (:207): flux[r][4] = {.., .., Phi+, Phi-} of the map (k_flux_*).
+template <typename real>
+__global__ void __launch_bounds__(TX) k_rfe_balance(real* S, const double* flux, Geom G) {
+    const int k = blockIdx.x * TX + threadIdx.x, j = blockIdx.y, r = blockIdx.z;
+    if (k >= G.np) return;
+    const double pp = flux[4 * r + 2], pm = flux[4 * r + 3];
+    if (pp == 0.0 || pm == 0.0) return;
+    const real sc = (real)sqrt(fabs(pp / pm));
+    real* p = S + (size_t)r * G.rstride + (size_t)j * G.pitch + k;
+    const real v = *p;
+    *p = v > (real)0 ? v / sc : v * sc;
+}
+
+// The source advance (Eq. 15 :203, forward Euler): B <- B + h [(1 - alpha) S1 + alpha S2].  grid (nbx, nt+2, R).
+template <typename real>
+__global__ void __launch_bounds__(TX) k_rfe_apply(real* B, const real* S1, const real* S2, real alpha, real h, Geom G) {
+    const int k = blockIdx.x * TX + threadIdx.x, j = blockIdx.y, r = blockIdx.z;
+    if (k >= G.np) return;
+    const size_t i = (size_t)r * G.rstride + (size_t)j * G.pitch + k;
+    B[i] = B[i] + h * (((real)1 - alpha) * S1[i] + alpha * S2[i]);
+}
+
 }  // namespace hft

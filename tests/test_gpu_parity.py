@@ -410,3 +410,38 @@ def test_flow_attenuation(dtype, case):
     with pytest.raises(H.HftError):
         H.Context(16, 32, [[0.0] * 7]).set_attenuation(0, 500.0)           # workspace was not reserved for it
     ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("model", [1, 2])
+def test_random_flux_emergence(dtype, model):
+    """source term of Sec. 2.4.  The two balanced source maps element by element (the per-cell normals
+    come from the same counter-based generator on both sides), then steps with A, D and S in the Eq. 21 order across two
+    map rotations, then a Strang step (Eq. 22)."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 41, 136, n_real=2)
+    flux, tau, seed = 100e21, 0.7, 0x1234567890ABCDEF
+    for strang in (0, 1):
+        ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype, radius_cm=6.96e10, rfe=1, strang=strang)
+        o = orc.Oracle(w.n_theta, w.n_phi, w.params, dtype=NPDT[dtype], radius_cm=6.96e10)
+        maps = wl.initial_maps(w).to(ctx.tdtype)
+        for r in range(w.n_real):
+            ctx.set_map(r, maps[r].contiguous().cuda())
+            o.set_map(r, maps[r].numpy())
+        ctx.set_rfe(model, flux, tau, seed)
+        o.set_rfe(model, flux, tau, seed)
+        for r in range(w.n_real):
+            s1, s2 = o.get_rfe_maps(r)
+            scale = np.abs(s1).max()
+            for which, s in ((0, s1), (1, s2)):
+                g = ctx.get_rfe_map(r, which).cpu().numpy()
+                assert np.abs(g - s[1:-1]).max() <= (1e-12 if dtype == "f64" else 1e-5) * scale, (r, which)
+        dt = 0.3
+        ctx.step(6, dt)                       # t = 0 .. 1.8 h: rotations at 0.7 and 1.4 h
+        o.step(6, dt, strang=bool(strang))
+        compare(ctx, o, TOL[dtype], f"rfe model {model} strang {strang}")
+        g1 = ctx.get_rfe_map(0, 0).cpu().numpy()
+        assert np.abs(g1 - o.get_rfe_maps(0)[0][1:-1]).max() <= (1e-12 if dtype == "f64" else 1e-5) * np.abs(g1).max()
+        ctx.close()
+    with pytest.raises(H.HftError):
+        H.Context(16, 32, [[0.0] * 7]).set_rfe(2, 1.0e21, 1.0, 1)          # workspace was not reserved for it
