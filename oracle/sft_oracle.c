@@ -72,6 +72,8 @@ typedef struct {
     double P;     /* polar prefactor, App. A :646 (exact form) */
     double Apole; /* polar cap area 2*pi*(1-cos(dth/2)), App. A :642 */
     double *nu;   /* [nr] diffusivity in R_sun^2/hr */
+    double *nuf;  /* [nr][nt+1] diffusivity at the theta-faces j+1/2 (the half grid of :288), R_sun^2/hr; = nu unless a
+                     latitude profile was set (nu(theta), grid-based nu_g of Eq. 7) */
     double *vt;   /* [nr][nt+1] v_theta at theta-faces, R_sun/hr (Eq. 4 :84) */
     double *om;   /* [nr][nt+2] Omega = v_phi/sin(theta) at rows, rad/hr (Eq. 3 :78) */
     real *B;      /* [nr][nt+2][np] state */
@@ -125,18 +127,43 @@ void *SUF(sft_oracle_create)(int nt, int np, int nr, const double *params /*[nr]
     o->st = (double *)calloc(nt + 2, sizeof(double));
     o->sth = (double *)calloc(nt + 1, sizeof(double));
     o->nu = (double *)calloc(nr, sizeof(double));
+    o->nuf = (double *)calloc((size_t)nr * (nt + 1), sizeof(double));
     o->vt = (double *)calloc((size_t)nr * (nt + 1), sizeof(double));
     o->om = (double *)calloc((size_t)nr * (nt + 2), sizeof(double));
     o->B = (real *)calloc((size_t)nr * (nt + 2) * np, sizeof(real));
     o->B0 = (double *)calloc(nr, sizeof(double));
     make_grid(o);
-    for (int r = 0; r < nr; r++) make_flow(o, r, params + 7 * r);
+    for (int r = 0; r < nr; r++) {
+        make_flow(o, r, params + 7 * r);
+        for (int f = 0; f <= nt; f++) o->nuf[(size_t)r * (nt + 1) + f] = o->nu[r];
+    }
     return o;
 }
 
 void SUF(sft_oracle_destroy)(void *h) {
     oracle_t *o = (oracle_t *)h;
-    free(o->st); free(o->sth); free(o->nu); free(o->vt); free(o->om); free(o->B); free(o->B0); free(o->S1); free(o->S2); free(o);
+    free(o->st); free(o->sth); free(o->nu); free(o->nuf); free(o->vt); free(o->om); free(o->B); free(o->B0); free(o->S1); free(o->S2); free(o);
+}
+
+/* Latitude-dependent diffusivity (Eq. 6 :109 with nu = nu(theta)): nu_face[f] in km^2/s at the theta-face f+1/2,
+ * f = 0..nt, for realization r (r < 0: all). */
+void SUF(sft_oracle_set_diffusivity_profile)(void *h, int r, const double *nu_face) {
+    oracle_t *o = (oracle_t *)h;
+    for (int q = 0; q < o->nr; q++)
+        if (r < 0 || q == r)
+            for (int f = 0; f <= o->nt; f++) o->nuf[(size_t)q * (o->nt + 1) + f] = nu_face[f] * KM2_S_TO_RS2_HR;
+}
+
+/* Grid-based diffusivity of the map smoother, Eq. 7 (:121): nu_g = alpha_nu [dtheta^2 + (dphi sin(theta))^2], evaluated
+ * where nu lives, at the theta-faces; alpha_nu in km^2/s per rad^2 (dtheta, dphi in radians). */
+void SUF(sft_oracle_set_grid_diffusivity)(void *h, int r, double alpha_nu) {
+    oracle_t *o = (oracle_t *)h;
+    for (int q = 0; q < o->nr; q++)
+        if (r < 0 || q == r)
+            for (int f = 0; f <= o->nt; f++) {
+                double dps = o->dph * o->sth[f];
+                o->nuf[(size_t)q * (o->nt + 1) + f] = alpha_nu * (o->dth * o->dth + dps * dps) * KM2_S_TO_RS2_HR;
+            }
 }
 
 /* Flow attenuation (Sec. 2.1.3, Eq. 5 :100): B0 in Gauss for realization r (r < 0: all); B0 <= 0 switches it off. */
@@ -227,12 +254,14 @@ void SUF(sft_oracle_set_full)(void *h, int r, const real *in) {
  * Row coefficients are formed in fp64 and rounded once to `real`. */
 static void diffusion_op(const oracle_t *o, int r, const real *B, real *out) {
     int nt = o->nt, np = o->np;
-    double nu = o->nu[r];
+    /* Eq. 28 (:450-458) with nu on the half grid and independent of phi: the theta-fluxes take nu at their face, the
+     * phi-term the mean of the two faces of the row, (nu_{j+1/2} + nu_{j-1/2})/2 */
+    const double *nuf = o->nuf + (size_t)r * (nt + 1);
     #pragma omp parallel for schedule(static)
     for (int j = 1; j <= nt; j++) {
-        real cp = (real)(nu * o->sth[j] / (o->st[j] * o->dth * o->dth));
-        real cm = (real)(nu * o->sth[j - 1] / (o->st[j] * o->dth * o->dth));
-        real cf = (real)(nu / (o->st[j] * o->st[j] * o->dph * o->dph));
+        real cp = (real)(nuf[j] * o->sth[j] / (o->st[j] * o->dth * o->dth));
+        real cm = (real)(nuf[j - 1] * o->sth[j - 1] / (o->st[j] * o->dth * o->dth));
+        real cf = (real)(0.5 * (nuf[j] + nuf[j - 1]) / (o->st[j] * o->st[j] * o->dph * o->dph));
         const real *Bc = B + (size_t)j * np, *Bn = Bc - np, *Bs = Bc + np; /* Bn = row j-1 (towards north), Bs = row j+1 */
         real *oc = out + (size_t)j * np;
         for (int k = 0; k < np; k++) {
@@ -242,14 +271,14 @@ static void diffusion_op(const oracle_t *o, int r, const real *B, real *out) {
             oc[k] = tth + tph;
         }
     }
-    double capc = o->P * (nu / o->dth) * o->dph;
+    double capN = o->P * (nuf[0] / o->dth) * o->dph, capS = o->P * (nuf[nt] / o->dth) * o->dph;
     kahan_t a = {0, 0}, b = {0, 0};
     for (int k = 0; k < np; k++) {
         kadd(&a, (double)(B[np + k] - B[0]));
         kadd(&b, (double)(B[(size_t)nt * np + k] - B[(size_t)(nt + 1) * np]));
     }
-    fill_row(out, np, (real)(capc * a.s));
-    fill_row(out + (size_t)(nt + 1) * np, np, (real)(capc * b.s));
+    fill_row(out, np, (real)(capN * a.s));
+    fill_row(out + (size_t)(nt + 1) * np, np, (real)(capS * b.s));
 }
 
 void SUF(sft_oracle_diffusion_op)(void *h, int r, const real *in, real *out) {
@@ -259,15 +288,19 @@ void SUF(sft_oracle_diffusion_op)(void *h, int r, const real *in, real *out) {
 /* Step 5: Euler limit.  Gershgorin: spectral radius <= 2 max|diag|, dt_expl = 2/rho =
  * 1 / max( max_j (c+_j + c-_j + 2 cphi_j), 2 pi P nu / dth ), with nu = max_r nu_r (reading U8). */
 static double diffusion_dt_expl(const oracle_t *o) {
-    double nu = 0.0;
-    for (int r = 0; r < o->nr; r++) if (o->nu[r] > nu) nu = o->nu[r];
-    double dmax = 2.0 * PI * o->P * nu / o->dth;
-    for (int j = 1; j <= o->nt; j++) {
-        double cp = nu * o->sth[j] / (o->st[j] * o->dth * o->dth);
-        double cm = nu * o->sth[j - 1] / (o->st[j] * o->dth * o->dth);
-        double cf = nu / (o->st[j] * o->st[j] * o->dph * o->dph);
-        double d = cp + cm + 2.0 * cf;
-        if (d > dmax) dmax = d;
+    double dmax = 0.0;
+    for (int r = 0; r < o->nr; r++) {
+        const double *nuf = o->nuf + (size_t)r * (o->nt + 1);
+        double dN = 2.0 * PI * o->P * nuf[0] / o->dth, dS = 2.0 * PI * o->P * nuf[o->nt] / o->dth;
+        if (dN > dmax) dmax = dN;
+        if (dS > dmax) dmax = dS;
+        for (int j = 1; j <= o->nt; j++) {
+            double cp = nuf[j] * o->sth[j] / (o->st[j] * o->dth * o->dth);
+            double cm = nuf[j - 1] * o->sth[j - 1] / (o->st[j] * o->dth * o->dth);
+            double cf = 0.5 * (nuf[j] + nuf[j - 1]) / (o->st[j] * o->st[j] * o->dph * o->dph);
+            double d = cp + cm + 2.0 * cf;
+            if (d > dmax) dmax = d;
+        }
     }
     return dmax > 0.0 ? 1.0 / dmax : INFINITY;
 }

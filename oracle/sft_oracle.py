@@ -85,6 +85,22 @@ class Oracle:
         f(self.h, r, _dp(vt), _dp(om))
 
     # -- state ------------------------------------------------------------------------------
+    def set_diffusivity_profile(self, r, nu_face_km2_s):
+        """nu(theta) at the theta-faces f+1/2, f = 0..nt, km^2/s (Eq. 6 with a latitude-dependent diffusivity)."""
+        a = np.ascontiguousarray(nu_face_km2_s, dtype=np.float64)
+        assert a.shape == (self.nt + 1,)
+        f = self._f("sft_oracle_set_diffusivity_profile")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
+        f(self.h, int(r), _dp(a))
+
+    def set_grid_diffusivity(self, r, alpha_nu):
+        """Eq. 7 (:121): nu_g = alpha_nu [dth^2 + (dph sin(theta))^2], alpha_nu in km^2/s per rad^2."""
+        f = self._f("sft_oracle_set_grid_diffusivity")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_int, C.c_double]
+        f(self.h, int(r), float(alpha_nu))
+
     def set_attenuation(self, r, b0_gauss):
         """Flow attenuation Eq. 5 (:100): saturation field B0 in Gauss for realization r (-1: all); <= 0 off."""
         f = self._f("sft_oracle_set_attenuation")

@@ -303,3 +303,92 @@ def test_rfe_time_interpolation_and_map_rotation():
     m0, m1 = o2.get_rfe_maps(0)[0], o2.get_rfe_maps(1)[0]
     assert np.array_equal(m0, a1) and not np.array_equal(m1, a1)
     assert not np.array_equal(_rfe_oracle(2, 12, 24, tau=tau, flux=1.0e22, seed=8).get_rfe_maps(0)[0], a1)
+
+
+# ---------------------------------------------------------------- latitude-dependent diffusivity, Eq. 6-7 (:109-121), 8(f)-4
+
+def test_diffusivity_profile_constant_is_the_scalar_path_bitwise():
+    nt, nphi = 20, 40
+    B = wl.bipolar_map(nt, nphi, 4, 21, sigma_deg=10.0).numpy()
+    a, b = Oracle(nt, nphi, [[432.1, 0, 0, 0, 0, 0, 0]]), Oracle(nt, nphi, [[1.0, 0, 0, 0, 0, 0, 0]])
+    b.set_diffusivity_profile(0, np.full(nt + 1, 432.1))
+    assert a.stable_dt()[1] == b.stable_dt()[1]
+    a.set_map(0, B); b.set_map(0, B)
+    f = a.get_full(0)
+    assert np.array_equal(a.diffusion_op(0, f), b.diffusion_op(0, f))
+    dt = 40 * a.stable_dt()[1]
+    a.step(2, dt, adv_flux=ADV_OFF); b.step(2, dt, adv_flux=ADV_OFF)
+    assert np.array_equal(a.get_full(0), b.get_full(0))
+
+
+def test_diffusivity_profile_manufactured_solutions_second_order():
+    """div(nu grad B) on the unit sphere in closed form for nu = nu0 (1 + a cos^2 theta):
+    B = cos(theta):           L = 2 a nu0 cos sin^2 - 2 nu0 (1 + a cos^2) cos                       (theta-term, nu at the faces)
+    B = sin(theta) cos(phi):  L = cos(phi) [ nu' cos + nu (cos^2 - sin^2)/sin - nu/sin ],  nu' = -2 a nu0 cos sin   (phi-term: nu at the row)
+    The discrete operator (Eq. 27-28 with nu on the half grid) must converge to both at 2nd order (measured
+    between 30 and 150 degrees colatitude)."""
+    from oracle.sft_oracle import Oracle as O
+    K = 7.43162901307967e-9
+    nu0, a = 500.0, 0.8
+    errs = {0: [], 1: []}
+    for nt in (31, 63, 127):
+        nphi = 2 * (nt + 1)
+        th, ph, dth, dph = grid(nt, nphi)
+        o = O(nt, nphi, [[0.0] * 7])
+        thf = (np.arange(nt + 1) + 0.5) * dth
+        o.set_diffusivity_profile(0, nu0 * (1 + a * np.cos(thf) ** 2))
+        nu = nu0 * K * (1 + a * np.cos(th) ** 2)
+        dnu = -2 * a * nu0 * K * np.cos(th) * np.sin(th)
+        s, c = np.sin(th), np.cos(th)
+        cases = [(c * np.ones_like(ph), (2 * a * nu0 * K * c * s ** 2 - 2 * nu * c) * np.ones_like(ph))]
+        with np.errstate(divide="ignore", invalid="ignore"):
+            L2 = np.cos(ph) * (dnu * c + nu * (c ** 2 - s ** 2) / s - nu / s)
+        cases.append((s * np.cos(ph), L2))
+        for i, (B, L) in enumerate(cases):
+            got = o.diffusion_op(0, B)
+            mid = (np.sin(th) > 0.5)[:, 0]       # next to the poles the m = 1 truncation error is O(h) on this grid for any nu
+            errs[i].append(np.abs(got[mid] - L[mid]).max() / np.abs(L[mid]).max())
+    for i in (0, 1):
+        assert errs[i][0] < 5e-3 and 3.3 < errs[i][0] / errs[i][1] < 4.7 and 3.3 < errs[i][1] / errs[i][2] < 4.7, errs
+
+
+def test_diffusivity_profile_conserves_and_is_self_adjoint():
+    """:448 'symmetric self-adjoint', :586 'flux-preserving': with nu(theta) the dA-weighted operator stays symmetric and
+    sum dA L(B) = 0 to round-off, caps included (the cap flux must use the same nu_{1/2} as row 1)."""
+    nt, nphi = 14, 24
+    rng = np.random.default_rng(4)
+    o = Oracle(nt, nphi, [[0.0] * 7])
+    o.set_diffusivity_profile(0, 100.0 + 900.0 * rng.random(nt + 1))
+    dA = cell_areas(nt, nphi)
+
+    def field():
+        f = rng.normal(size=(nt + 2, nphi)); f[0] = f[0, 0]; f[-1] = f[-1, 0]
+        return f
+    u, v = field(), field()
+    Lu, Lv = o.diffusion_op(0, u), o.diffusion_op(0, v)
+    scale = (dA * np.abs(Lu)).sum()
+    assert abs((dA * Lu).sum()) < 1e-13 * scale
+    assert abs((dA * v * Lu).sum() - (dA * u * Lv).sum()) < 1e-12 * (dA * np.abs(v * Lu)).sum()
+
+
+def test_grid_based_diffusivity_eq7_and_smoother():
+    """Eq. 7 (:121) evaluated independently with numpy and fed through the profile setter gives the same operator; as a
+    smoother (:586-594) one large STS step conserves the signed flux and lowers the unsigned flux and the extrema."""
+    nt, nphi, alpha = 40, 80, 2.0e6
+    o, p = Oracle(nt, nphi, [[0.0] * 7]), Oracle(nt, nphi, [[0.0] * 7])
+    o.set_grid_diffusivity(0, alpha)
+    dth, dph = math.pi / (nt + 1), 2 * math.pi / nphi
+    thf = (np.arange(nt + 1) + 0.5) * dth
+    p.set_diffusivity_profile(0, alpha * (dth ** 2 + (dph * np.sin(thf)) ** 2))
+    rng = np.random.default_rng(6)
+    B = wl.bipolar_map(nt, nphi, 10, 5).numpy() + rng.normal(0, 5.0, (nt, nphi))
+    o.set_map(0, B); p.set_map(0, B)
+    f = o.get_full(0)
+    assert rel_linf(o.diffusion_op(0, f), p.diffusion_op(0, f)) < 1e-14
+    assert abs(o.stable_dt()[1] / p.stable_dt()[1] - 1) < 1e-14
+    d0 = o.diagnostics()[0]
+    o.step(1, 60 * o.stable_dt()[1], adv_flux=ADV_OFF)
+    d1 = o.diagnostics()[0]
+    g = o.get_full(0)
+    assert abs(d1[0] - d0[0]) < 1e-13 * d0[1] and d1[1] < 0.9 * d0[1]
+    assert g.max() < f.max() and g.min() > f.min()
