@@ -97,6 +97,14 @@ void hft_destroy(hft_ctx* ctx);
  * j*dtheta, j = 0..n_theta+1, in m/s (i.e. the bracket of Eq. 3). */
 int hft_set_flow_tables(hft_ctx* ctx, int32_t r, const double* h_vtheta, const double* h_omega);
 
+/* Latitude-dependent diffusivity nu(theta) (Eq. 6 :109 with nu on the half grid of :288, phi-independent): h_nu_face
+ * [n_theta+1] in km^2/s at the theta-faces (j+1/2)*dtheta, j = 0..n_theta, for realization r (-1: all).  The theta-fluxes
+ * take nu at their face, the phi-term the mean of the row's two faces (Eq. 28 :450-458); hft_stable_dt and the STS stage
+ * count follow.  hft_set_grid_diffusivity sets the grid-based diffusivity of the map smoother, Eq. 7 (:121):
+ * nu_g = alpha_nu [dtheta^2 + (dphi sin(theta))^2], alpha_nu in km^2/s per rad^2.  Both synchronise the stream. */
+int hft_set_diffusivity_profile(hft_ctx* ctx, int32_t r, const double* h_nu_face);
+int hft_set_grid_diffusivity(hft_ctx* ctx, int32_t r, double alpha_nu);
+
 /* Flow attenuation (Sec. 2.1.3, Eq. 5 :100-103): v -> v [1 - tanh(|Br| / B0)] with the saturation field b0_gauss of
  * realization r (-1: all; the paper's default is 500 G); b0_gauss <= 0 switches it off for that realization.  Needs
  * hft_options.flow_attenuation = 1 at hft_create, else HFT_ERR_ARG.  |Br| at a face is the magnitude of the mean of the

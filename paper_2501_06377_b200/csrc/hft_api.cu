@@ -63,6 +63,7 @@ struct hft_ctx {
     double dth = 0, dph = 0, P = 0, Apole = 0;
     std::vector<double> st, sth;      // sin(theta_j) [nt+2], sin(theta_{j+1/2}) [nt+1]
     std::vector<double> nu;           // [R] R_sun^2/hr
+    std::vector<double> nuf;          // [R][nt+1] nu at the theta-faces (= nu unless a latitude profile was set; Eq. 6-7)
     std::vector<double> vt, om;       // [R][nt+1] R_sun/hr at faces, [R][nt+2] rad/hr at rows
     // device tables
     char* d_tab = nullptr;
@@ -179,7 +180,7 @@ void fill_tables(const hft_ctx* c, HostTab<real>& H) {
     H.pm.assign(n2, 0); H.pp.assign(n2, 0); H.c4.assign(4 * n2, 0);
     H.vtf.assign((size_t)R * (nt + 1), 0);
     H.sth.resize(nt + 1); H.rdt.assign(nt + 2, 0); H.rdp.assign(nt + 2, 0);
-    H.capc.resize(R); H.dA.resize(nt + 2);
+    H.capc.resize(2 * R); H.dA.resize(nt + 2);
     for (int f = 0; f <= nt; f++) H.sth[f] = (real)c->sth[f];
     for (int j = 1; j <= nt; j++) {
         H.rdt[j] = (real)(1.0 / (c->st[j] * c->dth));
@@ -188,17 +189,18 @@ void fill_tables(const hft_ctx* c, HostTab<real>& H) {
     }
     H.dA[0] = H.dA[nt + 1] = c->Apole;
     for (int r = 0; r < R; r++) {
-        const double nu = c->nu[r];
+        const double* nuf = &c->nuf[(size_t)r * (nt + 1)];
         const double* vt = &c->vt[(size_t)r * (nt + 1)];
         const double* om = &c->om[(size_t)r * (nt + 2)];
-        H.capc[r] = c->P * (nu / c->dth) * c->dph;
+        H.capc[2 * r] = c->P * (nuf[0] / c->dth) * c->dph;        // north: nu at face 1/2
+        H.capc[2 * r + 1] = c->P * (nuf[nt] / c->dth) * c->dph;   // south: nu at face nt+1/2
         for (int f = 0; f <= nt; f++) H.vtf[(size_t)r * (nt + 1) + f] = (real)vt[f];
         for (int j = 0; j <= nt + 1; j++) {
             const size_t i = (size_t)r * (nt + 2) + j;
-            if (j >= 1 && j <= nt) {  // Eq. 28 with constant nu, uniform spacing
-                H.cp[i] = (real)(nu * c->sth[j] / (c->st[j] * c->dth * c->dth));
-                H.cm[i] = (real)(nu * c->sth[j - 1] / (c->st[j] * c->dth * c->dth));
-                H.cf[i] = (real)(nu / (c->st[j] * c->st[j] * c->dph * c->dph));
+            if (j >= 1 && j <= nt) {  // Eq. 28, uniform spacing, nu = nu(theta) on the half grid (:288)
+                H.cp[i] = (real)(nuf[j] * c->sth[j] / (c->st[j] * c->dth * c->dth));
+                H.cm[i] = (real)(nuf[j - 1] * c->sth[j - 1] / (c->st[j] * c->dth * c->dth));
+                H.cf[i] = (real)(0.5 * (nuf[j] + nuf[j - 1]) / (c->st[j] * c->st[j] * c->dph * c->dph));
                 H.cd[i] = (real)((double)H.cp[i] + (double)H.cm[i] + 2.0 * (double)H.cf[i]);
                 H.c4[4 * i + 0] = H.cm[i]; H.c4[4 * i + 1] = H.cp[i]; H.c4[4 * i + 2] = H.cf[i]; H.c4[4 * i + 3] = H.cd[i];
             }
@@ -229,7 +231,7 @@ int upload_tables(hft_ctx* c, Tables<real>& T) {
     auto take = [&](size_t bytes) { size_t o = off; off = round_up(off + bytes, 256); return o; };
     size_t o_cp = take(n2), o_cm = take(n2), o_cf = take(n2), o_cd = take(n2), o_c4 = take(4 * n2), o_lm = take(n2), o_lp = take(n2), o_pm = take(n2), o_pp = take(n2);
     size_t o_vtf = take(n1), o_sth = take((nt + 1) * sizeof(real)), o_rdt = take((nt + 2) * sizeof(real)), o_rdp = take((nt + 2) * sizeof(real));
-    size_t o_capc = take(R * sizeof(double)), o_dA = take((nt + 2) * sizeof(double));
+    size_t o_capc = take(2 * R * sizeof(double)), o_dA = take((nt + 2) * sizeof(double));
     if (!c->d_tab) {
         c->tab_bytes = off;
         CK(cudaMalloc((void**)&c->d_tab, c->tab_bytes));
@@ -240,7 +242,7 @@ int upload_tables(hft_ctx* c, Tables<real>& T) {
     CK(up(o_lm, H.lm.data(), n2)); CK(up(o_lp, H.lp.data(), n2)); CK(up(o_pm, H.pm.data(), n2)); CK(up(o_pp, H.pp.data(), n2));
     CK(up(o_vtf, H.vtf.data(), n1)); CK(up(o_sth, H.sth.data(), (nt + 1) * sizeof(real)));
     CK(up(o_rdt, H.rdt.data(), (nt + 2) * sizeof(real))); CK(up(o_rdp, H.rdp.data(), (nt + 2) * sizeof(real)));
-    CK(up(o_capc, H.capc.data(), R * sizeof(double))); CK(up(o_dA, H.dA.data(), (nt + 2) * sizeof(double)));
+    CK(up(o_capc, H.capc.data(), 2 * R * sizeof(double))); CK(up(o_dA, H.dA.data(), (nt + 2) * sizeof(double)));
     CK(cudaStreamSynchronize(c->stream));  // H goes out of scope
     T.cp = (const real*)(d + o_cp); T.cm = (const real*)(d + o_cm); T.cf = (const real*)(d + o_cf); T.cd = (const real*)(d + o_cd); T.c4 = (const real*)(d + o_c4);
     T.lm = (const real*)(d + o_lm); T.lp = (const real*)(d + o_lp); T.pm = (const real*)(d + o_pm); T.pp = (const real*)(d + o_pp);
@@ -271,12 +273,16 @@ double adv_dt_limit(const hft_ctx* c) {
 
 // Gershgorin bound: rho <= 2 max|diag|; explicit Euler limit 2/rho, with nu = max_r nu_r (:448).
 double diff_dt_expl(const hft_ctx* c) {
-    double nu = 0.0;
-    for (double v : c->nu) nu = fmax(nu, v);
-    double d = 2.0 * kPi * c->P * nu / c->dth;  // cap row diagonal
-    for (int j = 1; j <= c->G.nt; j++) {
-        const double t = nu * (c->sth[j] + c->sth[j - 1]) / (c->st[j] * c->dth * c->dth) + 2.0 * nu / (c->st[j] * c->st[j] * c->dph * c->dph);
-        d = fmax(d, t);
+    const int nt = c->G.nt;
+    double d = 0.0;
+    for (int r = 0; r < c->nr; r++) {
+        const double* nuf = &c->nuf[(size_t)r * (nt + 1)];
+        d = fmax(d, fmax(2.0 * kPi * c->P * nuf[0] / c->dth, 2.0 * kPi * c->P * nuf[nt] / c->dth));  // cap row diagonals
+        for (int j = 1; j <= nt; j++) {
+            const double t = (nuf[j] * c->sth[j] + nuf[j - 1] * c->sth[j - 1]) / (c->st[j] * c->dth * c->dth) +
+                             (nuf[j] + nuf[j - 1]) / (c->st[j] * c->st[j] * c->dph * c->dph);
+            d = fmax(d, t);
+        }
     }
     return d > 0.0 ? 1.0 / d : INFINITY;
 }
@@ -587,9 +593,12 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
         for (int i = 0; i < kNumRfeArrays; i++)
             c->rfe_map[i] = (char*)d_workspace + (size_t)(kNumArrays + (o.flow_attenuation ? kNumAttArrays : 0) + i) * c->arr_bytes;
     c->B0.assign(n_real, 0.0);
-    c->nu.resize(n_real); c->vt.resize((size_t)n_real * (c->G.nt + 1)); c->om.resize((size_t)n_real * (c->G.nt + 2));
+    c->nu.resize(n_real); c->nuf.resize((size_t)n_real * (c->G.nt + 1)); c->vt.resize((size_t)n_real * (c->G.nt + 1)); c->om.resize((size_t)n_real * (c->G.nt + 2));
     build_metric(c);
-    for (int r = 0; r < n_real; r++) build_flow(c, r, h_params[r]);
+    for (int r = 0; r < n_real; r++) {
+        build_flow(c, r, h_params[r]);
+        for (int f = 0; f <= c->G.nt; f++) c->nuf[(size_t)r * (c->G.nt + 1) + f] = c->nu[r];
+    }
     int rc = HFT_OK;
     auto fail = [&](int code) { hft_destroy(c); return code; };
     cudaError_t e;
@@ -634,6 +643,29 @@ int hft_set_flow_tables(hft_ctx* c, int32_t r, const double* h_vtheta, const dou
         for (int j = 0; j <= nt + 1; j++) c->om[(size_t)q * (nt + 2) + j] = h_omega[j] * kMsToRsHr;
     }
     return upload_all_tables(c);
+}
+
+int hft_set_diffusivity_profile(hft_ctx* c, int32_t r, const double* h_nu_face) {
+    if (!c || !h_nu_face || r < -1 || r >= c->nr) return HFT_ERR_ARG;
+    const int nt = c->G.nt;
+    for (int f = 0; f <= nt; f++)
+        if (!(h_nu_face[f] >= 0.0)) return HFT_ERR_ARG;
+    for (int q = 0; q < c->nr; q++)
+        if (r < 0 || q == r)
+            for (int f = 0; f <= nt; f++) c->nuf[(size_t)q * (nt + 1) + f] = h_nu_face[f] * kKm2sToRs2Hr;
+    CK(cudaStreamSynchronize(c->stream));   // the tables may still be read by enqueued work
+    return upload_all_tables(c);
+}
+
+int hft_set_grid_diffusivity(hft_ctx* c, int32_t r, double alpha_nu) {
+    if (!c || r < -1 || r >= c->nr || !(alpha_nu >= 0.0)) return HFT_ERR_ARG;
+    const int nt = c->G.nt;
+    std::vector<double> p(nt + 1);
+    for (int f = 0; f <= nt; f++) {   // Eq. 7 (:121) where nu lives: at the theta-faces
+        const double dps = c->dph * c->sth[f];
+        p[f] = alpha_nu * (c->dth * c->dth + dps * dps);
+    }
+    return hft_set_diffusivity_profile(c, r, p.data());
 }
 
 int hft_set_attenuation(hft_ctx* c, int32_t r, double b0_gauss) {

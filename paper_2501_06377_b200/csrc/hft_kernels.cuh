@@ -23,7 +23,7 @@ struct Tables {            // device pointers, all [R][nt+2] unless noted
     const real* cf;        //            nu / (sin^2(theta_j) dph^2)                         Eq. 28 (:450, :458)
     const real* cd;        //            cp + cm + 2 cf  (minus the diagonal a_{j,k} of Eq. 28, :454)
     const real* c4;        // [R][nt+2][4] = (cm, cp, cf, cd) interleaved, zero on the cap rows (k_sts_pipe)
-    const double* capc;    // [R] P (nu/dth) dph : polar cap diffusion prefactor             App. A (:646)
+    const double* capc;    // [R][2] P (nu_face/dth) dph, north / south polar cap diffusion prefactor   App. A (:646)
     const real* lm;        // advection LLF: (v_{j-1/2} + alpha_j)/2                         B2 (:684)
     const real* lp;        //                (v_{j+1/2} - alpha_j)/2
     const real* vtf;       // [R][nt+1] v_theta at theta-faces (upwind faces)                Eq. 4 (:84)
@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(TX) k_sts_stage(StsArgs<real> A, Tables<real> 
         if (j == 0 || j == G.nt + 1) {
             const int pole = (j == 0) ? 0 : 1;
             double S = sum_partials(A.part_in + ((size_t)r * 2 + pole) * G.nbx, G.nbx);
-            L = (real)(T.capc[r] * (S - (double)G.np * (double)c));
+            L = (real)(T.capc[2 * r + pole] * (S - (double)G.np * (double)c));
         } else {
             real w = in[(size_t)j * G.pitch + kw], e = in[(size_t)j * G.pitch + ke];
             L = cp[j] * (s - c) - cm[j] * (c - n) + cf[j] * ((e - (real)2 * c) + w);

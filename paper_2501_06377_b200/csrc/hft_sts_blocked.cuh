@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(32 * STS_KMAX) k_sts_capseq(BlkArgs<real, K> A
     mF[0] = (double)A.F[capoff];
     const real* cp = T.cp + (size_t)r * (G.nt + 2);
     const real* cm = T.cm + (size_t)r * (G.nt + 2);
-    const double capc = T.capc[r] * (double)G.np;
+    const double capc = T.capc[2 * r + pole] * (double)G.np;
     double lc[K + 1], lp[K + 1], ln[K + 1];  // current level, previous level, new level
     for (int d = 0; d <= K; d++) { lc[d] = m0[d]; lp[d] = mp[d]; }
     for (int s = 1; s <= K; s++) {

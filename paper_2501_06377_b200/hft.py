@@ -18,7 +18,7 @@ if not os.path.exists(LIB_PATH):
                       "(the CUDA extension is required; there is no CPU fallback)")
 _lib = C.CDLL(LIB_PATH)
 
-EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_flow_tables", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
+EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
            "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_diagnostics", "hft_diagnostics_ext", "hft_stable_dt",
            "hft_sts_stage_count", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
            "hft_last_cuda_error"]
@@ -50,6 +50,8 @@ _lib.hft_create.argtypes = [C.POINTER(hft_grid), C.c_int32, C.POINTER(hft_params
 _lib.hft_destroy.argtypes = [C.c_void_p]
 _lib.hft_destroy.restype = None
 _lib.hft_set_flow_tables.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+_lib.hft_set_diffusivity_profile.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
+_lib.hft_set_grid_diffusivity.argtypes = [C.c_void_p, C.c_int32, C.c_double]
 _lib.hft_set_attenuation.argtypes = [C.c_void_p, C.c_int32, C.c_double]
 _lib.hft_set_rfe.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_uint64]
 _lib.hft_get_rfe_map.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
@@ -147,6 +149,15 @@ class Context:
         assert vt.shape == (self.n_theta + 1,) and om.shape == (self.n_theta + 2,)
         self._ck(_lib.hft_set_flow_tables(self._h, r, vt.ctypes.data_as(C.POINTER(C.c_double)),
                                           om.ctypes.data_as(C.POINTER(C.c_double))), "hft_set_flow_tables")
+
+    def set_diffusivity_profile(self, r, nu_face_km2_s):
+        a = np.ascontiguousarray(nu_face_km2_s, dtype=np.float64)
+        assert a.shape == (self.n_theta + 1,)
+        self._ck(_lib.hft_set_diffusivity_profile(self._h, int(r), a.ctypes.data_as(C.POINTER(C.c_double))),
+                 "hft_set_diffusivity_profile")
+
+    def set_grid_diffusivity(self, r, alpha_nu):
+        self._ck(_lib.hft_set_grid_diffusivity(self._h, int(r), float(alpha_nu)), "hft_set_grid_diffusivity")
 
     def set_attenuation(self, r, b0_gauss):
         self._ck(_lib.hft_set_attenuation(self._h, int(r), float(b0_gauss)), "hft_set_attenuation")

@@ -445,3 +445,47 @@ def test_random_flux_emergence(dtype, model):
         ctx.close()
     with pytest.raises(H.HftError):
         H.Context(16, 32, [[0.0] * 7]).set_rfe(2, 1.0e21, 1.0, 1)          # workspace was not reserved for it
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("block", [1, 0])
+def test_latitude_dependent_diffusivity(dtype, block):
+    """SURVEY.md 8(f)-4 (phi-independent part): nu(theta) profiles per realization and the grid-based nu_g of Eq. 7, through
+    both STS paths (the zonal-mean cap recurrence of the blocked kernel only needs phi-independent coefficients), with
+    advection on; then the map-smoother use (:586): diffusion only, one large step."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 72, 264, n_real=3)
+    ctx, o = make_pair(w, dtype, sts_block=block)
+    rng = np.random.default_rng(12)
+    thf = (np.arange(w.n_theta + 1) + 0.5) * math.pi / (w.n_theta + 1)
+    prof = [300.0 * (1 + 0.8 * np.cos(thf) ** 2), None, 200.0 + 400.0 * rng.random(w.n_theta + 1)]
+    for r, p in enumerate(prof):
+        if p is not None:
+            ctx.set_diffusivity_profile(r, p)
+            o.set_diffusivity_profile(r, p)
+    ga, gd = ctx.stable_dt()
+    oa, od = o.stable_dt()
+    assert abs(gd / od - 1) < 1e-14
+    dt, _, _ = wl.plan(w, ga, gd)
+    assert ctx.sts_stage_count(dt) == o.sts_stage_count(dt)
+    before = ctx.diagnostics()
+    ctx.step(3, dt)
+    o.step(3, dt)
+    compare(ctx, o, TOL[dtype], "nu(theta)")
+    after = ctx.diagnostics()
+    assert np.all(np.abs(after[:, 0] - before[:, 0]) <= (1e-12 if dtype == "f64" else 2e-5) * before[:, 1])
+    ctx.close()
+    # smoother: grid-based diffusivity, diffusion only
+    ctx = H.Context(w.n_theta, w.n_phi, w.params[:1], dtype=dtype, adv_flux=H.ADV_OFF, sts_block=block)
+    o = orc.Oracle(w.n_theta, w.n_phi, w.params[:1], dtype=NPDT[dtype])
+    m = (wl.bipolar_map(w.n_theta, w.n_phi, 12, 77) + torch.from_numpy(rng.normal(0, 5.0, (w.n_theta, w.n_phi)))).to(ctx.tdtype)
+    ctx.set_grid_diffusivity(0, 2.0e6)
+    o.set_grid_diffusivity(0, 2.0e6)
+    ctx.set_map(0, m.contiguous().cuda())
+    o.set_map(0, m.numpy())
+    _, gd = ctx.stable_dt()
+    assert abs(gd / o.stable_dt()[1] - 1) < 1e-14
+    ctx.step(1, 150 * gd)
+    o.step(1, 150 * gd, adv_flux=orc.ADV_OFF)
+    compare(ctx, o, TOL[dtype], "smoother")
+    ctx.close()
