@@ -489,3 +489,38 @@ def test_latitude_dependent_diffusivity(dtype, block):
     o.step(1, 150 * gd, adv_flux=orc.ADV_OFF)
     compare(ctx, o, TOL[dtype], "smoother")
     ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_degenerate_sizes_and_calls(dtype):
+    """Edge cases: the smallest grid the ABI accepts (8 x 8) and an odd ragged one (9 x 17, below every vector width, so
+    all stages take the un-blocked kernels); zero steps is a no-op; a zero map stays zero; a constant map is a fixed point
+    of diffusion."""
+    H = hft()
+    for nt, nphi in ((8, 8), (9, 17)):
+        w = wl.scaled(wl.config(1), nt, nphi)
+        rng = np.random.default_rng(nt)
+        m = torch.from_numpy(rng.normal(0, 10.0, (nt, nphi)))
+        ctx = H.Context(nt, nphi, w.params, dtype=dtype)
+        o = orc.Oracle(nt, nphi, w.params, dtype=NPDT[dtype])
+        ctx.set_map(0, m.to(ctx.tdtype).cuda())
+        o.set_map(0, m.to(ctx.tdtype).numpy())
+        ctx.step(0, 1.0)
+        compare(ctx, o, 1e-15 if dtype == "f64" else 1e-7, "zero steps")   # caps = row means: summation order
+        dt, _, _ = wl.plan(w, *ctx.stable_dt())
+        ctx.step(3, dt)
+        o.step(3, dt)
+        compare(ctx, o, TOL[dtype], f"{nt}x{nphi}")
+        z = torch.zeros(nt, nphi, dtype=ctx.tdtype, device="cuda")
+        ctx.set_map(0, z)
+        ctx.step(2, dt)
+        assert torch.equal(ctx.get_map(0), z)
+        ctx.close()
+        ctx = H.Context(nt, nphi, w.params, dtype=dtype, adv_flux=H.ADV_OFF)
+        cst = torch.full((nt, nphi), 3.25, dtype=ctx.tdtype, device="cuda")
+        ctx.set_map(0, cst)
+        ctx.step(2, dt)
+        assert (ctx.get_full(0) - 3.25).abs().max().item() <= (1e-13 if dtype == "f64" else 1e-5)
+        ctx.close()
+    with pytest.raises(H.HftError):
+        H.Context(7, 8, [[0.0] * 7])
