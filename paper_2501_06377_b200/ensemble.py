@@ -56,7 +56,7 @@ def _dev():
 def global_limits(dt_adv_limit: float, dt_diff_expl: float):
     """Ensemble-wide step-size limits: the minimum over ranks of each rank's limits (inf stays inf)."""
     dist = _dist()
-    if dist is None or dist.get_world_size() == 1:
+    if dist is None:
         return dt_adv_limit, dt_diff_expl
     t = torch.tensor([dt_adv_limit, dt_diff_expl], dtype=torch.float64, device=_dev())
     dist.all_reduce(t, op=dist.ReduceOp.MIN)
@@ -65,7 +65,7 @@ def global_limits(dt_adv_limit: float, dt_diff_expl: float):
 
 def max_over_ranks(x: float) -> float:
     dist = _dist()
-    if dist is None or dist.get_world_size() == 1:
+    if dist is None:
         return x
     t = torch.tensor([x], dtype=torch.float64, device=_dev())
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -75,7 +75,7 @@ def max_over_ranks(x: float) -> float:
 def gather_diagnostics(diag: np.ndarray) -> np.ndarray:
     """[n_real][4] per rank -> [world * n_real][4] on every rank, in global realization order."""
     dist = _dist()
-    if dist is None or dist.get_world_size() == 1:
+    if dist is None:
         return np.asarray(diag)
     t = torch.from_numpy(np.ascontiguousarray(diag, dtype=np.float64)).to(_dev())
     out = [torch.empty_like(t) for _ in range(dist.get_world_size())]
