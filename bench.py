@@ -197,18 +197,50 @@ def main():
         if with_extras and not args.no_e2e:
             host_in = maps.cpu().pin_memory()
             host_out = torch.empty_like(host_in).pin_memory()
-            dev_in, dev_out = torch.empty_like(maps), torch.empty_like(maps)
-            n_e2e = max(1, min(args.steps, 2))
+            dev_in = [torch.empty_like(maps), torch.empty_like(maps)]
+            dev_out = [torch.empty_like(maps), torch.empty_like(maps)]
+            n_e2e = max(1, args.steps)
+            # three streams, as a user of the C ABI would drive it: step i+1's maps come up and step i-1's result goes
+            # down while step i computes (PCIe is full duplex); every copy, the first host-to-device and the last
+            # device-to-host included, is inside the timed region
+            main, up, side = torch.cuda.current_stream(), torch.cuda.Stream(), torch.cuda.Stream()
             barrier()
             t0 = torch.cuda.Event(enable_timing=True); t1 = torch.cuda.Event(enable_timing=True)
             t0.record()
-            for _ in range(n_e2e):
-                dev_in.copy_(host_in, non_blocking=True)
+            up.wait_stream(main)
+
+            consumed, copied = [None, None], [None, None]
+
+            def upload(i):
+                with torch.cuda.stream(up):
+                    if consumed[i % 2] is not None:
+                        up.wait_event(consumed[i % 2])      # set_map of step i-2 has read this buffer
+                    dev_in[i % 2].copy_(host_in, non_blocking=True)
+                    ev = torch.cuda.Event()
+                    ev.record(up)
+                return ev
+
+            arrived = upload(0)
+            for i in range(n_e2e):
+                main.wait_event(arrived)
                 for r in range(wd.n_real):
-                    ctx.set_map(r, dev_in[r])
+                    ctx.set_map(r, dev_in[i % 2][r])
+                consumed[i % 2] = torch.cuda.Event()
+                consumed[i % 2].record(main)
+                if i + 1 < n_e2e:
+                    arrived = upload(i + 1)          # into the other input buffer
                 ctx.step(1, dt)
-                ctx.get_map(-1, out=dev_out)
-                host_out.copy_(dev_out, non_blocking=True)
+                if copied[i % 2] is not None:
+                    main.wait_event(copied[i % 2])    # the result of step i-2 has left this buffer
+                ctx.get_map(-1, out=dev_out[i % 2])
+                done = torch.cuda.Event()
+                done.record(main)
+                with torch.cuda.stream(side):
+                    side.wait_event(done)
+                    host_out.copy_(dev_out[i % 2], non_blocking=True)
+                    copied[i % 2] = torch.cuda.Event()
+                    copied[i % 2].record(side)
+            main.wait_stream(side)
             t1.record()
             barrier()
             ems = t0.elapsed_time(t1)
