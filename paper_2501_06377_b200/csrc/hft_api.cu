@@ -398,8 +398,8 @@ int advect(hft_ctx* c, double dt) {
         a.VT = att[0]; a.VP = att[1]; a.LMt = att[2]; a.LPt = att[3]; a.LMp = att[4]; a.LPp = att[5];
         bool armed;
         prof_begin(c, 2, armed);
-        if (c->att_any) k_adv_stage<real, true><<<g, TX, 0, c->stream>>>(a, T, G);
-        else k_adv_stage<real, false><<<g, TX, 0, c->stream>>>(a, T, G);
+        if (c->att_any) k_adv_stage_att<real><<<g, TX, 0, c->stream>>>(a, T, G);
+        else k_adv_stage<real><<<g, TX, 0, c->stream>>>(a, T, G);
         prof_end(c, armed, 1);
         k_adv_caps<real><<<gc, TX, 0, c->stream>>>(a, T, G);
         c->launches += 2;

@@ -191,7 +191,7 @@ struct AdvArgs {
     double* part;     // [R][2][nbx] phi-sums of the theta-flux at the faces next to the caps
     real ca, cb, cdt;
     int upwind_only;  // adv_flux == 1
-    // flow attenuation (Eq. 5 :100), k_adv_stage<real, true> only: field-shaped arrays [R][nt+2][pitch]
+    // flow attenuation (Eq. 5 :100), k_adv_stage_att only: field-shaped arrays [R][nt+2][pitch]
     const real* VT;   // attenuated v_theta at face j+1/2 (row j = 0..nt)
     const real* VP;   // attenuated v_phi at face k-1/2 (rows 1..nt)
     const real *LMt, *LPt;   // theta LLF half-speeds of cell (j,k): (v_{j-1/2} + alpha)/2, (v_{j+1/2} - alpha)/2
@@ -219,7 +219,7 @@ __device__ __forceinline__ real phi_face_flux(real bm2, real bm1, real b0, real 
     return weno3_side(pp * bp1, pp * b0, pp * bm1, eps);
 }
 
-template <typename real, bool ATT>
+template <typename real>
 __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> T, Geom G) {
     __shared__ double red[32];
     const int r = blockIdx.z;
@@ -240,36 +240,16 @@ __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> 
     auto ld = [&](int j) -> real { return in[(size_t)min(max(j, 0), nt + 1) * G.pitch + k0]; };
 
     real w0 = ld(j0 - 2), w1 = ld(j0 - 1), w2 = ld(j0), w3 = ld(j0 + 1);
-    // ATT: per-cell speeds of this column / this row instead of the per-row tables
-    auto att_theta = [&](int f, real bm1, real b0, real bp1, real bp2) -> real {
-        auto at = [&](const real* p, int j) -> real { return p[base + (size_t)j * G.pitch + k0]; };
-        if (A.upwind_only || f <= 1 || f >= nt - 1) return upwind(at(A.VT, f), b0, bp1);
-        real um = weno3_side(bm1 * at(A.LMt, f - 1), b0 * at(A.LMt, f), bp1 * at(A.LMt, f + 1), T.eps_t);
-        real up = weno3_side(bp2 * at(A.LPt, f + 2), bp1 * at(A.LPt, f + 1), b0 * at(A.LPt, f), T.eps_t);
-        return up + um;
-    };
-    // face between columns kc-1 and kc of row j; (bm2, bm1, b0, bp1) = columns kc-2 .. kc+1
-    auto att_phi = [&](int j, int kc2, int kc1, int kc, int kcp, real bm2, real bm1, real b0, real bp1) -> real {
-        const size_t ro = base + (size_t)j * G.pitch;
-        if (A.upwind_only) return upwind(A.VP[ro + kc], bm1, b0);
-        real um = weno3_side(bm2 * A.LMp[ro + kc2], bm1 * A.LMp[ro + kc1], b0 * A.LMp[ro + kc], T.eps_p);
-        real up = weno3_side(bp1 * A.LPp[ro + kcp], b0 * A.LPp[ro + kc], bm1 * A.LPp[ro + kc1], T.eps_p);
-        return up + um;
-    };
-    real Fn = ATT ? att_theta(j0 - 1, w0, w1, w2, w3)
-                  : theta_face_flux<real>(j0 - 1, w0, w1, w2, w3, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
+    real Fn = theta_face_flux<real>(j0 - 1, w0, w1, w2, w3, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
     double sumN = 0.0, sumS = 0.0;
     if (j0 == 1) sumN = live ? (double)Fn : 0.0;
     for (int j = j0; j < j1; j++) {
         real w4 = ld(j + 2);
-        real Fs = ATT ? att_theta(j, w1, w2, w3, w4)
-                      : theta_face_flux<real>(j, w1, w2, w3, w4, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
+        real Fs = theta_face_flux<real>(j, w1, w2, w3, w4, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
         const real* row = in + (size_t)j * G.pitch;
         real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1], bp2 = row[kp2];
-        real Fw = ATT ? att_phi(j, km2, km1, k0, kp1, bm2, bm1, w2, bp1)
-                      : phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, A.upwind_only);
-        real Fe = ATT ? att_phi(j, km1, k0, kp1, kp2, bm1, w2, bp1, bp2)
-                      : phi_face_flux<real>(bm1, w2, bp1, bp2, pm[j], pp[j], T.eps_p, A.upwind_only);
+        real Fw = phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, A.upwind_only);
+        real Fe = phi_face_flux<real>(bm1, w2, bp1, bp2, pm[j], pp[j], T.eps_p, A.upwind_only);
         real tend = (T.sth[j] * Fs - T.sth[j - 1] * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
         const size_t off = base + (size_t)j * G.pitch + k0;
         real o = A.cb * w2 - A.cdt * tend;
@@ -278,6 +258,87 @@ __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> 
         if (j == nt) sumS = live ? (double)Fs : 0.0;
         Fn = Fs;
         w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+    }
+    if (j0 == 1) {
+        double t = block_sum(sumN, red);
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbx + blockIdx.x] = t;
+    }
+    if (j0 <= nt && nt < j1) {
+        double t = block_sum(sumS, red);
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbx + blockIdx.x] = t;
+    }
+}
+
+// The same stage with flow attenuation (Eq. 5): per-cell LLF half-speeds (k_att_halfspeeds) instead of per-row tables,
+// both LLF parts live in phi.  A thread streams RPT rows of its column; B and the theta half-speeds move through
+// register windows (one new row of each per row-step), and ALL operands of a row are requested before its arithmetic
+// starts, so that the ~16 independent loads of a row overlap (the first version interleaved them with the WENO
+// arithmetic and stalled 9 issue slots per instruction on the scoreboard: profiles/r01_final_cfg3.md).
+template <typename real>
+__global__ void __launch_bounds__(TX) k_adv_stage_att(AdvArgs<real> A, Tables<real> T, Geom G) {
+    __shared__ double red[32];
+    const int r = blockIdx.z;
+    const int k = blockIdx.x * TX + threadIdx.x;
+    const bool live = k < G.np;
+    const int np = G.np, nt = G.nt;
+    const int k0 = live ? k : 0;
+    const int km1 = (k0 + np - 1) % np, km2 = (k0 + np - 2) % np, kp1 = (k0 + 1) % np, kp2 = (k0 + 2) % np;
+    const int j0 = 1 + blockIdx.y * RPT;
+    const int j1 = min(j0 + RPT, nt + 1);
+    const size_t base = (size_t)r * G.rstride;
+    const real* in = A.in + base;
+    auto col = [&](const real* p, int j) -> real { return p[base + (size_t)min(max(j, 0), nt + 1) * G.pitch + k0]; };
+    const bool uw = A.upwind_only != 0;
+
+    // theta-face flux at face f from B rows f-1..f+2 and the half-speeds LMt rows f-1..f+1, LPt rows f..f+2
+    auto theta_flux = [&](int f, real bm1, real b0, real bp1, real bp2, real m0, real m1, real m2, real p0, real p1, real p2) -> real {
+        if (uw || f <= 1 || f >= nt - 1) return upwind(col(A.VT, f), b0, bp1);
+        real um = weno3_side(bm1 * m0, b0 * m1, bp1 * m2, T.eps_t);
+        real up = weno3_side(bp2 * p2, bp1 * p1, b0 * p0, T.eps_t);
+        return up + um;
+    };
+    real w0 = col(A.in, j0 - 2), w1 = col(A.in, j0 - 1), w2 = col(A.in, j0), w3 = col(A.in, j0 + 1);
+    // windows for face f = j0 - 1: LMt rows f-1, f, f+1; LPt rows f, f+1, f+2
+    real m0 = col(A.LMt, j0 - 2), m1 = col(A.LMt, j0 - 1), m2 = col(A.LMt, j0);
+    real p0 = col(A.LPt, j0 - 1), p1 = col(A.LPt, j0), p2 = col(A.LPt, j0 + 1);
+    real Fn = theta_flux(j0 - 1, w0, w1, w2, w3, m0, m1, m2, p0, p1, p2);
+    double sumN = 0.0, sumS = 0.0;
+    if (j0 == 1) sumN = live ? (double)Fn : 0.0;
+    for (int j = j0; j < j1; j++) {
+        // ---- every load of this row first
+        const size_t ro = base + (size_t)j * G.pitch;
+        const real w4 = col(A.in, j + 2);
+        const real m3 = col(A.LMt, j + 1), p3 = col(A.LPt, j + 2);
+        const real* row = in + (size_t)j * G.pitch;
+        const real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1], bp2 = row[kp2];
+        real a_m2 = 0, a_m1 = 0, a_0 = 0, a_p1 = 0, b_m1 = 0, b_0 = 0, b_p1 = 0, b_p2 = 0, vw = 0, ve = 0;
+        if (uw) {
+            vw = A.VP[ro + k0]; ve = A.VP[ro + kp1];
+        } else {
+            a_m2 = A.LMp[ro + km2]; a_m1 = A.LMp[ro + km1]; a_0 = A.LMp[ro + k0]; a_p1 = A.LMp[ro + kp1];
+            b_m1 = A.LPp[ro + km1]; b_0 = A.LPp[ro + k0]; b_p1 = A.LPp[ro + kp1]; b_p2 = A.LPp[ro + kp2];
+        }
+        const real fnv = (A.ca != (real)0) ? A.fn[ro + k0] : (real)0;
+        // ---- then the arithmetic.  Face j (between rows j, j+1): LMt rows j-1..j+1 = (m1, m2, m3), LPt rows j..j+2 = (p1, p2, p3)
+        const real Fs = theta_flux(j, w1, w2, w3, w4, m1, m2, m3, p1, p2, p3);
+        real Fw, Fe;
+        if (uw) {
+            Fw = upwind(vw, bm1, w2);
+            Fe = upwind(ve, w2, bp1);
+        } else {
+            // face k-1/2: LM of cells k-2, k-1, k; LP of cells k+1, k, k-1.  face k+1/2: shifted by one column
+            Fw = weno3_side(bp1 * b_p1, w2 * b_0, bm1 * b_m1, T.eps_p) + weno3_side(bm2 * a_m2, bm1 * a_m1, w2 * a_0, T.eps_p);
+            Fe = weno3_side(bp2 * b_p2, bp1 * b_p1, w2 * b_0, T.eps_p) + weno3_side(bm1 * a_m1, w2 * a_0, bp1 * a_p1, T.eps_p);
+        }
+        const real tend = (T.sth[j] * Fs - T.sth[j - 1] * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
+        real o = A.cb * w2 - A.cdt * tend;
+        if (A.ca != (real)0) o = A.ca * fnv + o;
+        if (live) A.out[ro + k0] = o;
+        if (j == nt) sumS = live ? (double)Fs : 0.0;
+        Fn = Fs;
+        w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+        m0 = m1; m1 = m2; m2 = m3;
+        p0 = p1; p1 = p2; p2 = p3;
     }
     if (j0 == 1) {
         double t = block_sum(sumN, red);
