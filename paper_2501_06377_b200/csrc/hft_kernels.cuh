@@ -167,6 +167,19 @@ __global__ void __launch_bounds__(TX) k_polar_row_sums(const real* f, double* pa
 
 // WENO3-CS(h) one-sided face value (App. B :658-676, uniform grid: D = 1/2, 1/3, 2/3), written with one
 // division: u = (d0 p0 (eps+b1)^2 + d1 p1 (eps+b0)^2) / (d0 (eps+b1)^2 + d1 (eps+b0)^2).
+// num / den for den > 0 (a sum of squares here): hardware reciprocal seed (~20 bits) and two Newton steps, within
+// about an ulp of the IEEE quotient, without the slow path of the correctly rounded division (the WENO weights need 4 to 6
+// of these per cell and stage; the division was the largest single cost of the stage kernel).
+__device__ __forceinline__ double pos_div(double num, double den) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(den));
+    r = fma(fma(-den, r, 1.0), r, r);
+    r = fma(fma(-den, r, 1.0), r, r);
+    const double q = num * r;
+    return fma(fma(-den, q, num), r, q);
+}
+__device__ __forceinline__ float pos_div(float num, float den) { return __fdividef(num, den); }
+
 template <typename real>
 __device__ __forceinline__ real weno3_side(real far, real near, real other, real eps) {
     real p0 = (real)1.5 * near - (real)0.5 * far;
@@ -175,7 +188,7 @@ __device__ __forceinline__ real weno3_side(real far, real near, real other, real
     real e0 = eps + q0 * q0, e1 = eps + q1 * q1;
     real a0 = e1 * e1;               // proportional to w0 = (1/3)/e0^2   (times e0^2 e1^2 * 3)
     real a1 = (real)2 * (e0 * e0);   // proportional to w1 = (2/3)/e1^2
-    return (a0 * p0 + a1 * p1) / (a0 + a1);
+    return pos_div(a0 * p0 + a1 * p1, a0 + a1);
 }
 
 template <typename real>
