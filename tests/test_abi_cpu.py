@@ -78,3 +78,19 @@ def test_product_never_imports_the_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2501_06377_b200" not in src and "from paper_2501_06377_b200" not in src
             assert "hft.h" not in src and "csrc" not in src.replace("paper_2501_06377_b200/csrc/", "")
+
+
+def test_workspace_grows_with_the_optional_rows(lib):
+    """hft_options.flow_attenuation reserves 6 more field arrays, hft_options.rfe 2 more; invalid options are refused."""
+    from paper_2501_06377_b200 import hft
+    one = 4 * 66 * 128 * 8          # n_real x (n_theta + 2) x pitch x sizeof(double)
+    base = hft.workspace_bytes(64, 128, 4, "f64")
+    assert base == 6 * one
+    opt = hft.hft_options(2, 4, 3, 0, 0, 0, 0, 1)
+    assert hft.workspace_bytes(64, 128, 4, "f64", opt) == 12 * one
+    opt = hft.hft_options(2, 4, 3, 0, 0, 1, 1, 1)
+    assert hft.workspace_bytes(64, 128, 4, "f64", opt) == 14 * one
+    for bad in (hft.hft_options(5, 4, 3, 0, 0, 0, 0, 0), hft.hft_options(2, 2, 3, 0, 0, 0, 0, 0), hft.hft_options(2, 4, 3, 1, 0, 0, 0, 0),
+                hft.hft_options(2, 4, 3, 0, 3, 0, 0, 0), hft.hft_options(2, 4, 3, 0, 0, 2, 0, 0), hft.hft_options(2, 4, 3, 0, 0, 0, 0, 7)):
+        with pytest.raises(hft.HftError):
+            hft.workspace_bytes(64, 128, 4, "f64", bad)
