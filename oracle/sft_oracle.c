@@ -74,6 +74,9 @@ typedef struct {
     double *nu;   /* [nr] diffusivity in R_sun^2/hr */
     double *nuf;  /* [nr][nt+1] diffusivity at the theta-faces j+1/2 (the half grid of :288), R_sun^2/hr; = nu unless a
                      latitude profile was set (nu(theta), grid-based nu_g of Eq. 7) */
+    double **nuhh; /* [nr] -> NULL, or [nt+1][np] diffusivity nu(theta, phi) on the half-half grid (Eq. 27 :438-446: "nu is located
+                     on a staggered grid in both the theta and phi direction"): nuhh[f][k] at theta-face f+1/2, phi-face k+1/2
+                     (between columns k and k+1, periodic), R_sun^2/hr.  SURVEY 8(f)-4, reading U31 */
     double *vt;   /* [nr][nt+1] v_theta at theta-faces, R_sun/hr (Eq. 4 :84) */
     double *om;   /* [nr][nt+2] Omega = v_phi/sin(theta) at rows, rad/hr (Eq. 3 :78) */
     real *B;      /* [nr][nt+2][np] state */
@@ -128,6 +131,7 @@ void *SUF(sft_oracle_create)(int nt, int np, int nr, const double *params /*[nr]
     o->sth = (double *)calloc(nt + 1, sizeof(double));
     o->nu = (double *)calloc(nr, sizeof(double));
     o->nuf = (double *)calloc((size_t)nr * (nt + 1), sizeof(double));
+    o->nuhh = (double **)calloc(nr, sizeof(double *));
     o->vt = (double *)calloc((size_t)nr * (nt + 1), sizeof(double));
     o->om = (double *)calloc((size_t)nr * (nt + 2), sizeof(double));
     o->B = (real *)calloc((size_t)nr * (nt + 2) * np, sizeof(real));
@@ -142,6 +146,8 @@ void *SUF(sft_oracle_create)(int nt, int np, int nr, const double *params /*[nr]
 
 void SUF(sft_oracle_destroy)(void *h) {
     oracle_t *o = (oracle_t *)h;
+    for (int r = 0; r < o->nr; r++) free(o->nuhh[r]);
+    free(o->nuhh);
     free(o->st); free(o->sth); free(o->nu); free(o->nuf); free(o->vt); free(o->om); free(o->B); free(o->B0); free(o->S1); free(o->S2); free(o);
 }
 
@@ -152,6 +158,23 @@ void SUF(sft_oracle_set_diffusivity_profile)(void *h, int r, const double *nu_fa
     for (int q = 0; q < o->nr; q++)
         if (r < 0 || q == r)
             for (int f = 0; f <= o->nt; f++) o->nuf[(size_t)q * (o->nt + 1) + f] = nu_face[f] * KM2_S_TO_RS2_HR;
+}
+
+/* Spatially varying diffusivity nu(theta, phi) (Eq. 6 :109, Eq. 27-28 :438-460): nu_hh[f][k] in km^2/s on the half-half
+ * grid, f = 0..nt (theta-face f+1/2), k = 0..np-1 (phi-face k+1/2, between columns k and k+1), for realization r (r < 0:
+ * all).  NULL returns realization r to its latitude profile / scalar value. */
+void SUF(sft_oracle_set_diffusivity_map)(void *h, int r, const double *nu_hh) {
+    oracle_t *o = (oracle_t *)h;
+    size_t n = (size_t)(o->nt + 1) * o->np;
+    for (int q = 0; q < o->nr; q++)
+        if (r < 0 || q == r) {
+            free(o->nuhh[q]);
+            o->nuhh[q] = NULL;
+            if (nu_hh) {
+                o->nuhh[q] = (double *)malloc(n * sizeof(double));
+                for (size_t i = 0; i < n; i++) o->nuhh[q][i] = nu_hh[i] * KM2_S_TO_RS2_HR;
+            }
+        }
 }
 
 /* Grid-based diffusivity of the map smoother, Eq. 7 (:121): nu_g = alpha_nu [dtheta^2 + (dphi sin(theta))^2], evaluated
@@ -252,8 +275,49 @@ void SUF(sft_oracle_set_full)(void *h, int r, const real *in) {
  *   caps (App. A :624-648, F = nu dB/dtheta by central differences at the first half-mesh point):
  *     north: P (nu/dth) sum_k (B[1,k]-B[0]) dph ;  south: P (nu/dth) sum_k (B[nt,k]-B[nt+1]) dph
  * Row coefficients are formed in fp64 and rounded once to `real`. */
+/* Eq. 27 (:438-446) written out with nu(theta, phi) on the half-half grid and uniform spacing; the four off-diagonal
+ * coefficients are those of Eq. 28 (:450-458), the diagonal is minus their sum, i.e. the difference form below:
+ *   a_{j+1,k} = (nu_{j+1/2,k+1/2} + nu_{j+1/2,k-1/2}) sin(theta_{j+1/2}) / (2 dth^2 sin(theta_j))
+ *   a_{j-1,k} = (nu_{j-1/2,k+1/2} + nu_{j-1/2,k-1/2}) sin(theta_{j-1/2}) / (2 dth^2 sin(theta_j))
+ *   a_{j,k+1} = (nu_{j+1/2,k+1/2} + nu_{j-1/2,k+1/2}) / (2 dph^2 sin^2(theta_j))
+ *   a_{j,k-1} = (nu_{j+1/2,k-1/2} + nu_{j-1/2,k-1/2}) / (2 dph^2 sin^2(theta_j))
+ *   L(B)_{j,k} = a_{j+1,k} (B[j+1,k]-B[j,k]) - a_{j-1,k} (B[j,k]-B[j-1,k]) + a_{j,k+1} (B[j,k+1]-B[j,k]) - a_{j,k-1} (B[j,k]-B[j,k-1])
+ * Caps (App. A :624-648 with F = nu dB/dtheta at the first half-mesh point, nu averaged to the theta-face like a_{j+-1,k}):
+ *   north: P sum_k nu_{1/2,k} (B[1,k]-B[0]) / dth dph,  nu_{1/2,k} = (nu_{1/2,k+1/2} + nu_{1/2,k-1/2})/2;  south likewise.
+ * Coefficients are formed in fp64 and rounded once to `real` (reading U31). */
+static void diffusion_op_map(const oracle_t *o, int r, const real *B, real *out) {
+    int nt = o->nt, np = o->np;
+    const double *nu = o->nuhh[r];
+    #pragma omp parallel for schedule(static)
+    for (int j = 1; j <= nt; j++) {
+        const double *nS = nu + (size_t)j * np, *nN = nu + (size_t)(j - 1) * np; /* faces j+1/2 and j-1/2 */
+        const real *Bc = B + (size_t)j * np, *Bn = Bc - np, *Bs = Bc + np;
+        real *oc = out + (size_t)j * np;
+        for (int k = 0; k < np; k++) {
+            int kw = (k + np - 1) % np, ke = (k + 1) % np;
+            real as = (real)(0.5 * (nS[k] + nS[kw]) * o->sth[j] / (o->st[j] * o->dth * o->dth));
+            real an = (real)(0.5 * (nN[k] + nN[kw]) * o->sth[j - 1] / (o->st[j] * o->dth * o->dth));
+            real ae = (real)(0.5 * (nS[k] + nN[k]) / (o->st[j] * o->st[j] * o->dph * o->dph));
+            real aw = (real)(0.5 * (nS[kw] + nN[kw]) / (o->st[j] * o->st[j] * o->dph * o->dph));
+            real tth = as * (Bs[k] - Bc[k]) - an * (Bc[k] - Bn[k]);
+            real tph = ae * (Bc[ke] - Bc[k]) - aw * (Bc[k] - Bc[kw]);
+            oc[k] = tth + tph;
+        }
+    }
+    const double *n0 = nu, *n1 = nu + (size_t)nt * np;
+    kahan_t a = {0, 0}, b = {0, 0};
+    for (int k = 0; k < np; k++) {
+        int kw = (k + np - 1) % np;
+        kadd(&a, 0.5 * (n0[k] + n0[kw]) * (double)(B[np + k] - B[0]));
+        kadd(&b, 0.5 * (n1[k] + n1[kw]) * (double)(B[(size_t)nt * np + k] - B[(size_t)(nt + 1) * np]));
+    }
+    fill_row(out, np, (real)(o->P / o->dth * o->dph * a.s));
+    fill_row(out + (size_t)(nt + 1) * np, np, (real)(o->P / o->dth * o->dph * b.s));
+}
+
 static void diffusion_op(const oracle_t *o, int r, const real *B, real *out) {
     int nt = o->nt, np = o->np;
+    if (o->nuhh[r]) { diffusion_op_map(o, r, B, out); return; }
     /* Eq. 28 (:450-458) with nu on the half grid and independent of phi: the theta-fluxes take nu at their face, the
      * phi-term the mean of the two faces of the row, (nu_{j+1/2} + nu_{j-1/2})/2 */
     const double *nuf = o->nuf + (size_t)r * (nt + 1);
@@ -290,6 +354,30 @@ void SUF(sft_oracle_diffusion_op)(void *h, int r, const real *in, real *out) {
 static double diffusion_dt_expl(const oracle_t *o) {
     double dmax = 0.0;
     for (int r = 0; r < o->nr; r++) {
+        if (o->nuhh[r]) { /* nu(theta, phi): the same Gershgorin bound, max over every cell of -a_{j,k} of Eq. 28 (:454) */
+            int nt = o->nt, np = o->np;
+            const double *nu = o->nuhh[r];
+            double wN = 0.0, wS = 0.0;
+            for (int k = 0; k < np; k++) {
+                int kw = (k + np - 1) % np;
+                wN += 0.5 * (nu[k] + nu[kw]);
+                wS += 0.5 * (nu[(size_t)nt * np + k] + nu[(size_t)nt * np + kw]);
+            }
+            if (o->P * wN * o->dph / o->dth > dmax) dmax = o->P * wN * o->dph / o->dth;
+            if (o->P * wS * o->dph / o->dth > dmax) dmax = o->P * wS * o->dph / o->dth;
+            for (int j = 1; j <= nt; j++) {
+                const double *nS = nu + (size_t)j * np, *nN = nu + (size_t)(j - 1) * np;
+                for (int k = 0; k < np; k++) {
+                    int kw = (k + np - 1) % np;
+                    double d = 0.5 * (nS[k] + nS[kw]) * o->sth[j] / (o->st[j] * o->dth * o->dth)
+                             + 0.5 * (nN[k] + nN[kw]) * o->sth[j - 1] / (o->st[j] * o->dth * o->dth)
+                             + 0.5 * (nS[k] + nN[k]) / (o->st[j] * o->st[j] * o->dph * o->dph)
+                             + 0.5 * (nS[kw] + nN[kw]) / (o->st[j] * o->st[j] * o->dph * o->dph);
+                    if (d > dmax) dmax = d;
+                }
+            }
+            continue;
+        }
         const double *nuf = o->nuf + (size_t)r * (o->nt + 1);
         double dN = 2.0 * PI * o->P * nuf[0] / o->dth, dS = 2.0 * PI * o->P * nuf[o->nt] / o->dth;
         if (dN > dmax) dmax = dN;

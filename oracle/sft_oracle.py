@@ -94,6 +94,18 @@ class Oracle:
         f.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
         f(self.h, int(r), _dp(a))
 
+    def set_diffusivity_map(self, r, nu_hh_km2_s):
+        """nu(theta, phi) on the half-half grid [nt+1][np] in km^2/s (Eq. 27-28), or None to switch the map off."""
+        f = self._f("sft_oracle_set_diffusivity_map")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double)]
+        if nu_hh_km2_s is None:
+            f(self.h, r, None)
+            return
+        a = np.ascontiguousarray(nu_hh_km2_s, dtype=np.float64)
+        assert a.shape == (self.nt + 1, self.np_)
+        f(self.h, r, _dp(a))
+
     def set_grid_diffusivity(self, r, alpha_nu):
         """Eq. 7 (:121): nu_g = alpha_nu [dth^2 + (dph sin(theta))^2], alpha_nu in km^2/s per rad^2."""
         f = self._f("sft_oracle_set_grid_diffusivity")

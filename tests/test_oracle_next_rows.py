@@ -392,3 +392,129 @@ def test_grid_based_diffusivity_eq7_and_smoother():
     g = o.get_full(0)
     assert abs(d1[0] - d0[0]) < 1e-13 * d0[1] and d1[1] < 0.9 * d0[1]
     assert g.max() < f.max() and g.min() > f.min()
+
+
+# ---------------------------------------------------------------- nu(theta, phi) on the half-half grid, Eq. 27-28 (:438-460), 8(f)-4
+
+def _hh(nt, nphi):
+    """Angles of the half-half grid points [nt+1][nphi]: theta-face f+1/2, phi-face k+1/2."""
+    dth, dph = math.pi / (nt + 1), 2 * math.pi / nphi
+    return ((np.arange(nt + 1) + 0.5) * dth)[:, None], ((np.arange(nphi) + 0.5) * dph)[None, :]
+
+
+def _dia_matrix(nt, nphi, nu):
+    """The matrix of Eq. 28 (:450-458) assembled entry by entry on the uniform grid, plus the two polar-cap rows of App. A
+    (:624-648); unknowns: cap N, cells (j, k) row-major, cap S.  nu[f][k] at (f+1/2, k+1/2) in R_sun^2/hr."""
+    dth, dph = math.pi / (nt + 1), 2 * math.pi / nphi
+    n = nt * nphi + 2
+    A = np.zeros((n, n))
+    P = math.sin(dth / 2) / (2 * math.pi * (1 - math.cos(dth / 2)))
+
+    def idx(j, k):
+        return 0 if j == 0 else (n - 1 if j == nt + 1 else 1 + (j - 1) * nphi + k % nphi)
+    for j in range(1, nt + 1):
+        sj, sp, sm = math.sin(j * dth), math.sin((j + 0.5) * dth), math.sin((j - 0.5) * dth)
+        for k in range(nphi):
+            km = (k - 1) % nphi
+            npp, npm, nmp, nmm = nu[j, k], nu[j, km], nu[j - 1, k], nu[j - 1, km]     # nu_{j+-1/2, k+-1/2}
+            a_w = (npm + nmm) / (2 * dph * dph * sj ** 2)
+            a_e = (npp + nmp) / (2 * dph * dph * sj ** 2)
+            a_n = (nmp + nmm) * sm / (2 * dth * dth * sj)
+            a_s = (npp + npm) * sp / (2 * dth * dth * sj)
+            i = idx(j, k)
+            A[i, idx(j, k - 1)] += a_w; A[i, idx(j, k + 1)] += a_e
+            A[i, idx(j - 1, k)] += a_n; A[i, idx(j + 1, k)] += a_s
+            A[i, i] += -(a_w + a_e + a_n + a_s)
+    for k in range(nphi):
+        km = (k - 1) % nphi
+        for cap, row, f in ((0, 1, 0), (n - 1, nt, nt)):
+            c = P * 0.5 * (nu[f, k] + nu[f, km]) / dth * dph
+            A[cap, idx(row, k)] += c; A[cap, cap] -= c
+    return A
+
+
+def _flat(f):
+    return np.concatenate([[f[0, 0]], f[1:-1].ravel(), [f[-1, 0]]])
+
+
+def test_diffusivity_map_equals_the_dense_dia_matrix_of_eq28_on_8x16():
+    nt, nphi = 8, 16
+    rng = np.random.default_rng(11)
+    numap = 100.0 + 900.0 * rng.random((nt + 1, nphi))
+    o = Oracle(nt, nphi, [[0.0] * 7])
+    o.set_diffusivity_map(0, numap)
+    A = _dia_matrix(nt, nphi, numap * 7.43162901307967e-9)
+    f = rng.normal(size=(nt + 2, nphi)); f[0] = f[0, 0]; f[-1] = f[-1, 0]
+    got = o.diffusion_op(0, f)
+    assert np.all(got[0] == got[0, 0]) and np.all(got[-1] == got[-1, 0])
+    want = A @ _flat(f)
+    assert np.abs(_flat(got) - want).max() < 1e-13 * np.abs(want).max()
+    # Euler limit: the Gershgorin bound 1 / max|diag| of that matrix (:448)
+    assert abs(o.stable_dt()[1] * np.abs(np.diag(A)).max() - 1) < 1e-13
+    # :448 "symmetric self-adjoint" under the cell areas, constants in the null space
+    dA = _flat(cell_areas(nt, nphi)); dA[0] *= nphi; dA[-1] *= nphi
+    M = dA[:, None] * A
+    assert np.abs(M - M.T).max() < 1e-13 * np.abs(M).max()
+    assert np.abs(A.sum(axis=1)).max() < 1e-12 * np.abs(A).max()
+    # one RKG2 step of s stages = the stability polynomial of the dense matrix applied to Y0: here only that the step is
+    # stable at the limit and conserves the signed flux
+    o.set_full(0, f)
+    d0 = o.diagnostics()[0]
+    o.step(3, 14.0 * o.stable_dt()[1] * 0.999, adv_flux=ADV_OFF, sts_stages=8)
+    d1 = o.diagnostics()[0]
+    assert abs(d1[0] - d0[0]) < 1e-13 * d0[1] and np.abs(o.get_full(0)).max() <= np.abs(f).max()
+
+
+def test_diffusivity_map_reduces_to_profile_and_scalar():
+    nt, nphi = 20, 40
+    B = wl.bipolar_map(nt, nphi, 4, 21, sigma_deg=10.0).numpy()
+    thf, _ = _hh(nt, nphi)
+    prof = 300.0 * (1 + 0.7 * np.cos(thf[:, 0]) ** 2)
+    a, b = Oracle(nt, nphi, [[0.0] * 7]), Oracle(nt, nphi, [[0.0] * 7])
+    a.set_diffusivity_profile(0, prof)
+    b.set_diffusivity_map(0, np.repeat(prof[:, None], nphi, axis=1))
+    assert abs(a.stable_dt()[1] / b.stable_dt()[1] - 1) < 1e-14
+    a.set_map(0, B); b.set_map(0, B)
+    f = a.get_full(0)
+    assert rel_linf(b.diffusion_op(0, f), a.diffusion_op(0, f)) < 1e-14
+    dt = 40 * a.stable_dt()[1]
+    a.step(2, dt, adv_flux=ADV_OFF); b.step(2, dt, adv_flux=ADV_OFF)
+    assert rel_linf(b.get_full(0), a.get_full(0)) < 1e-13
+    b.set_diffusivity_map(0, None)      # back to the scalar value given at create (0 here): nothing moves
+    g = b.get_full(0)
+    b.step(1, 1.0, adv_flux=ADV_OFF, sts_stages=4)
+    assert np.array_equal(b.get_full(0), g)
+
+
+def test_diffusivity_map_manufactured_solution_second_order():
+    """nu = nu0 (1 + a x), B = x^2 - y^2 with (x, y, z) the unit vector: B is an l = 2 harmonic, so on the unit sphere
+    div_s(nu grad_s B) = nu lap_s B + grad_s nu . grad_s B = -6 nu B + [grad nu . grad B - (n . grad nu)(n . grad B)]
+                       = -6 nu0 (1 + a x)(x^2 - y^2) + 2 a nu0 x [1 - (x^2 - y^2)].
+    nu varies along phi, so a map shifted by half a cell in either direction would converge at first order only."""
+    K = 7.43162901307967e-9
+    nu0, a = 500.0, 0.6
+    errs = []
+    for nt in (31, 63, 127):
+        nphi = 2 * (nt + 1)
+        th, ph, dth, dph = grid(nt, nphi)
+        thf, phf = _hh(nt, nphi)
+        o = Oracle(nt, nphi, [[0.0] * 7])
+        o.set_diffusivity_map(0, nu0 * (1 + a * np.sin(thf) * np.cos(phf)))
+        x, y = np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph)
+        B = x * x - y * y
+        L = nu0 * K * (-6 * (1 + a * x) * B + 2 * a * x * (1 - B))
+        got = o.diffusion_op(0, B)
+        mid = (np.sin(th) > 0.5)[:, 0]      # next to the poles the truncation error of m = 1 terms is O(h) on this grid for any nu
+        errs.append(np.abs(got[mid] - L[mid]).max() / np.abs(L[mid]).max())
+    assert errs[0] < 2e-2 and 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs
+    # the same map entered half a cell off in phi is only first-order accurate: the test above can tell
+    nt = 63; nphi = 2 * (nt + 1)
+    th, ph, dth, dph = grid(nt, nphi)
+    thf, phf = _hh(nt, nphi)
+    o = Oracle(nt, nphi, [[0.0] * 7])
+    o.set_diffusivity_map(0, nu0 * (1 + a * np.sin(thf) * np.cos(phf - 0.5 * dph)))
+    x, y = np.sin(th) * np.cos(ph), np.sin(th) * np.sin(ph)
+    B = x * x - y * y
+    L = nu0 * K * (-6 * (1 + a * x) * B + 2 * a * x * (1 - B))
+    mid = (np.sin(th) > 0.5)[:, 0]
+    assert np.abs(o.diffusion_op(0, B)[mid] - L[mid]).max() / np.abs(L[mid]).max() > 3 * errs[1]
