@@ -132,6 +132,8 @@ def main():
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--sts-block", type=int, default=0)
     ap.add_argument("--attenuation", type=float, default=0.0, help="B0 in Gauss: time the step with flow attenuation (Eq. 5) on")
+    ap.add_argument("--nu-map", action="store_true",
+                    help="time the step with a spatially varying diffusivity nu(theta, phi) (Eq. 27-28): one launch per STS stage")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--also-f32", action="store_true", help="add a second timed run in fp32 to the JSON line")
@@ -158,17 +160,26 @@ def main():
     def timed_run(dtype, with_extras):
         # rank k owns realizations [k R, (k+1) R) of the weak-scaled ensemble; one clock for the whole ensemble
         wd = ens.shard(args.config, dtype, rank, world)
-        ctx = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, flow_attenuation=int(args.attenuation > 0), device=f"cuda:{local}")
-        if args.attenuation > 0:
-            ctx.set_attenuation(-1, args.attenuation)
+        def make_ctx(**kw):
+            c = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block,
+                            flow_attenuation=int(args.attenuation > 0), diffusivity_map=int(args.nu_map), device=f"cuda:{local}", **kw)
+            if args.attenuation > 0:
+                c.set_attenuation(-1, args.attenuation)
+            if args.nu_map:      # nu_r (1 + 0.3 sin(theta) cos(phi)) on the half-half grid: smooth, phi-dependent, per realization
+                thf = ((np.arange(wd.n_theta + 1) + 0.5) * np.pi / (wd.n_theta + 1))[:, None]
+                phf = ((np.arange(wd.n_phi) + 0.5) * 2 * np.pi / wd.n_phi)[None, :]
+                shape = 1.0 + 0.3 * np.sin(thf) * np.cos(phf)
+                for r in range(wd.n_real):
+                    c.set_diffusivity_map(r, wd.params[r][0] * shape)
+            return c
+        ctx = make_ctx()
         maps = ens.shard_maps(wd, device=f"cuda:{local}").to(ctx.tdtype).contiguous()
         ctx.set_map(-1, maps[0]) if not wd.per_real_maps else [ctx.set_map(r, maps[r]) for r in range(wd.n_real)]
         dt, n_cfg, per = wl.plan(wd, *ens.global_limits(*ctx.stable_dt()))
         s = int(ens.max_over_ranks(float(ctx.sts_stage_count(dt))))
         if s != ctx.sts_stage_count(dt):          # another rank's realizations need more stages: force the same s
             ctx.close()
-            ctx = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, sts_stages=s,
-                              device=f"cuda:{local}")
+            ctx = make_ctx(sts_stages=s)
             ctx.set_map(-1, maps[0]) if not wd.per_real_maps else [ctx.set_map(r, maps[r]) for r in range(wd.n_real)]
         cells = wd.n_real * wd.n_theta * wd.n_phi
         for _ in range(args.warmup):
@@ -258,7 +269,9 @@ def main():
     wbytes = 8 if args.dtype == "f64" else 4
     peak, peak_src = peaks()
     # algorithmic bytes: 4 array passes per STS stage, 9 per SSPRK(4,3) advection step
-    b_alg_step = (9 + 4 * res["s"]) * wbytes
+    # (with nu(theta, phi) a stage also reads the nu array once: 5 passes)
+    stage_passes = 5 if args.nu_map else 4
+    b_alg_step = (9 + stage_passes * res["s"]) * wbytes
     frac_step = res["value"] / world * b_alg_step / (peak * 1e9)
     out = {
         "metric": "cell-updates/s", "value": res["value"], "unit": "cell-updates/s", "n_gpus": world, "steps": args.steps,
@@ -267,7 +280,7 @@ def main():
         "config": {"workload": wd.name, "grid": [wd.n_theta, wd.n_phi], "realizations_per_gpu": wd.n_real,
                    "dt_hours": res["dt"], "sts_stages": res["s"], "adv": "WENO3-CS(h)+SSPRK(4,3)", "diff": "RKG2(3/2)",
                    "l2": "inputs larger than L2 (arrays of %.0f MiB each)" % (wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes / 2**20),
-                   "sts_block": args.sts_block, "flow_attenuation_b0": args.attenuation, "b_alg_bytes_per_cell_update": b_alg_step,
+                   "sts_block": args.sts_block, "flow_attenuation_b0": args.attenuation, "nu_map": bool(args.nu_map), "b_alg_bytes_per_cell_update": b_alg_step,
                    "hbm_roofline_frac_whole_step": frac_step},
         "gpu_launches": res["launches"],
         "clocks": res["clocks"],
@@ -279,10 +292,10 @@ def main():
         stages_per_launch = res["kernel_stages"]
         field_bytes = wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes
         sec = res["kernel_ms"] * 1e-3
-        ach = 4 * field_bytes * stages_per_launch / sec / 1e9
+        ach = stage_passes * field_bytes * stages_per_launch / sec / 1e9
         blocked = stages_per_launch > 1
         out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                           "kernel": "k_sts_pipe" if blocked else "k_sts_stage", "stages_per_launch": stages_per_launch,
+                           "kernel": "k_sts_pipe" if blocked else ("k_sts_stage_map" if args.nu_map else "k_sts_stage"), "stages_per_launch": stages_per_launch,
                            "avg_launch_ms": res["kernel_ms"], "sampled_launches": res["kernel_samples"], "peak_source": peak_src}
         if blocked:
             # a K-stage block moves 5 array passes (3 in, 2 out) however large K is; the

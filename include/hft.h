@@ -75,10 +75,12 @@ typedef struct {
                            1 = Strang splitting, Eq. 22 (:317-326) with S omitted: A(dt/2), D(dt), A(dt/2) */
     int32_t flow_attenuation; /* 1 = reserve workspace for flow attenuation (Eq. 5, :100) and allow hft_set_attenuation;
                                  6 more field arrays.  0 (default) = off */
+    int32_t diffusivity_map;  /* 1 = reserve workspace for a spatially varying diffusivity nu(theta, phi) (Eq. 27-28, :438-460;
+                                 1 more field array) and allow hft_set_diffusivity_map.  0 (default) = off */
 } hft_options;
 
 /* Bytes of device workspace hft_create needs for this grid / batch (state + 5 stage arrays, + 6 with
- * opt->flow_attenuation).  opt may be NULL (defaults). */
+ * opt->flow_attenuation, + 2 with opt->rfe, + 1 with opt->diffusivity_map).  opt may be NULL (defaults). */
 int hft_workspace_bytes(const hft_grid* grid, int32_t n_real, const hft_options* opt, size_t* h_bytes);
 
 /* Create a context.  d_workspace: caller-allocated device memory of at least hft_workspace_bytes,
@@ -104,6 +106,19 @@ int hft_set_flow_tables(hft_ctx* ctx, int32_t r, const double* h_vtheta, const d
  * nu_g = alpha_nu [dtheta^2 + (dphi sin(theta))^2], alpha_nu in km^2/s per rad^2.  Both synchronise the stream. */
 int hft_set_diffusivity_profile(hft_ctx* ctx, int32_t r, const double* h_nu_face);
 int hft_set_grid_diffusivity(hft_ctx* ctx, int32_t r, double alpha_nu);
+
+/* Spatially varying diffusivity nu(theta, phi) (Eq. 6 :109; Eq. 27-28 :438-460: nu on the grid staggered in both directions).
+ * h_nu_hh: HOST, [n_theta+1][n_phi] doubles in km^2/s; entry [f][k] is nu at colatitude (f+1/2)*dtheta and longitude
+ * (k+1/2)*dphi (between columns k and k+1; column n_phi-1 wraps to column 0), every value >= 0, for realization r (-1: all).
+ * Owned by the caller, consumed before the call returns (synchronises the stream).  Each theta-flux takes the mean of the two
+ * nu values on its face, each phi-flux likewise, the polar-cap fluxes of App. A (:624-648) the face means of row f = 0 / n_theta:
+ * exactly the coefficients a_{j+-1,k}, a_{j,k+-1} of Eq. 28, applied in difference form.  Once any realization has a map,
+ * every realization is advanced by the one-launch-per-stage kernel k_sts_stage_map (the others with their nu(theta) profile
+ * or scalar value): with phi-dependent coefficients the temporally blocked kernel does not apply.
+ * hft_stable_dt and the STS stage count use the Gershgorin bound max |a_{j,k}| over every cell of the map.  A later
+ * hft_set_diffusivity_profile / hft_set_grid_diffusivity for realization r replaces its map.  Needs
+ * hft_options.diffusivity_map = 1 at hft_create, else HFT_ERR_ARG. */
+int hft_set_diffusivity_map(hft_ctx* ctx, int32_t r, const double* h_nu_hh);
 
 /* Flow attenuation (Sec. 2.1.3, Eq. 5 :100-103): v -> v [1 - tanh(|Br| / B0)] with the saturation field b0_gauss of
  * realization r (-1: all; the paper's default is 500 G); b0_gauss <= 0 switches it off for that realization.  Needs

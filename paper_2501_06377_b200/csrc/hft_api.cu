@@ -18,6 +18,7 @@
 #include "hft_kernels.cuh"
 #include "hft_sts_blocked.cuh"
 #include "hft_sts_pipe.cuh"
+#include "hft_sts_map.cuh"
 
 using namespace hft;
 
@@ -29,6 +30,7 @@ constexpr double kKm2sToRs2Hr = 7.43162901307967e-9;  // PAPER.md:298  km^2/s ->
 constexpr int kNumArrays = 6;                         // state + 5 stage arrays
 constexpr int kNumRfeArrays = 2;                      // random flux emergence: the two current source maps (hft_options.rfe)
 constexpr int kNumAttArrays = 6;                      // flow attenuation: VT, VP, LMt, LPt, LMp, LPp (hft_options.flow_attenuation)
+constexpr int kNumMapArrays = 1;                      // nu(theta, phi) on the half-half grid (hft_options.diffusivity_map)
 constexpr int kProfEvents = 256;
 
 struct StsCoef {  // per-stage scalars of Sec. 3.7.2 schemes, index 0..s
@@ -59,6 +61,13 @@ struct hft_ctx {
     double rfe_flux = 0.0, rfe_tau = 0.0, rfe_t1 = 0.0, time = 0.0;
     uint64_t rfe_seed = 0;
     uint32_t rfe_next = 2;
+    // nu(theta, phi) (Eq. 27-28): the NU array behind the ring; per realization: "a map was set", the Gershgorin diagonal
+    // maximum of its matrix, and the two polar weight sums (device copy d_capw)
+    char* numap = nullptr;
+    bool map_any = false;
+    std::vector<char> map_set;
+    std::vector<double> map_diag, capw;
+    double* d_capw = nullptr;
     // host tables (fp64)
     double dth = 0, dph = 0, P = 0, Apole = 0;
     std::vector<double> st, sth;      // sin(theta_j) [nt+2], sin(theta_{j+1/2}) [nt+1]
@@ -124,6 +133,10 @@ hft_options default_options() {
     return o;
 }
 
+int extra_arrays(const hft_options* o) {
+    return o ? (o->flow_attenuation ? kNumAttArrays : 0) + (o->rfe ? kNumRfeArrays : 0) + (o->diffusivity_map ? kNumMapArrays : 0) : 0;
+}
+
 bool valid_options(const hft_options* o) {
     if (o->adv_flux < 0 || o->adv_flux > 2) return false;
     if (o->adv_time != 1 && o->adv_time != 3 && o->adv_time != 4) return false;
@@ -132,6 +145,7 @@ bool valid_options(const hft_options* o) {
     if (o->strang != 0 && o->strang != 1) return false;
     if (o->flow_attenuation != 0 && o->flow_attenuation != 1) return false;
     if (o->rfe != 0 && o->rfe != 1) return false;
+    if (o->diffusivity_map != 0 && o->diffusivity_map != 1) return false;
     if (o->sts_block < 0 || o->sts_block > STS_KMAX || (o->sts_block > 1 && (o->sts_block & 1))) return false;
     return true;
 }
@@ -276,6 +290,10 @@ double diff_dt_expl(const hft_ctx* c) {
     const int nt = c->G.nt;
     double d = 0.0;
     for (int r = 0; r < c->nr; r++) {
+        if (c->map_set[r]) {   // nu(theta, phi): max |a_{j,k}| over every cell and both caps, found when the map was set
+            d = fmax(d, c->map_diag[r]);
+            continue;
+        }
         const double* nuf = &c->nuf[(size_t)r * (nt + 1)];
         d = fmax(d, fmax(2.0 * kPi * c->P * nuf[0] / c->dth, 2.0 * kPi * c->P * nuf[nt] / c->dth));  // cap row diagonals
         for (int j = 1; j <= nt; j++) {
@@ -410,6 +428,74 @@ int advect(hft_ctx* c, double dt) {
     return HFT_OK;
 }
 
+// one diffusion step with nu(theta, phi) (Eq. 27-28; hft_set_diffusivity_map): one launch per stage, k_sts_stage_mapv
+// (16-byte vectors) when n_phi is a multiple of the vector width, else k_sts_stage_map (one column per thread)
+template <typename real, int MODE>
+void launch_map_stage(hft_ctx* c, const StsArgs<real>& a, MapArgs<real>& M, bool vec, int* nparts) {
+    const Geom& G = c->G;
+    Tables<real>& T = tables_of<real>(c);
+    if (vec) {
+        constexpr int C = 16 / (int)sizeof(real);
+        const int nbxv = (G.np / C + TX - 1) / TX;
+        dim3 g(nbxv, (G.nt + 2 + MAPV_RPT - 1) / MAPV_RPT, c->nr);
+        k_sts_stage_mapv<real, MODE><<<g, TX, 0, c->stream>>>(a, M, T, G);
+        *nparts = nbxv;
+    } else {
+        dim3 g(G.nbx, (G.nt + 2 + RPT - 1) / RPT, c->nr);
+        k_sts_stage_map<real, MODE><<<g, TX, 0, c->stream>>>(a, M, T, G);
+        *nparts = G.nbx;
+    }
+    c->launches++;
+}
+
+template <typename real>
+int diffuse_map(hft_ctx* c, double dt, int s) {
+    const Geom& G = c->G;
+    const int is = c->i_state;
+    real* Y0 = arr_of<real>(c, is);
+    real* F = arr_of<real>(c, (is + 1) % kNumArrays);
+    real* da = arr_of<real>(c, (is + 2) % kNumArrays);
+    real* db = arr_of<real>(c, (is + 3) % kNumArrays);
+    static const bool force_scalar = getenv("HFT_MAP_SCALAR") != nullptr;   // A/B timing of the one-column-per-thread kernel
+    const bool vec = !force_scalar && G.np % (16 / (int)sizeof(real)) == 0;
+    MapArgs<real> M;
+    M.NU = (const real*)c->numap; M.capw = c->d_capw; M.capP = c->P * c->dph / c->dth; M.rdth = (real)(1.0 / c->dth);
+    M.nparts_in = G.nbx;
+    dim3 gs(G.nbx, 2, c->nr);
+    k_polar_row_sums_map<real><<<gs, TX, 0, c->stream>>>(Y0, M.NU, c->d_part[0], G);
+    c->launches++;
+    StsArgs<real> a;
+    a.F = F; a.Y0 = Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
+    int np_out = 0;
+    if (c->opt.diff_time == 1) {  // explicit Euler (:474), new state written to `da`
+        a.in = Y0; a.d2 = da; a.part_in = c->d_part[0]; a.part_out = c->d_part[1]; a.a = (real)dt;
+        launch_map_stage<real, 3>(c, a, M, vec, &np_out);
+        c->i_state = (is + 2) % kNumArrays;
+        return HFT_OK;
+    }
+    const StsCoef& K = c->coef;
+    a.in = Y0; a.d2 = da; a.part_in = c->d_part[0]; a.part_out = c->d_part[1]; a.a = (real)K.a[1];
+    bool armed;
+    prof_begin(c, 1, armed);
+    launch_map_stage<real, 0>(c, a, M, vec, &np_out);
+    prof_end(c, armed, 1);
+    real *d1 = da, *d2 = db;
+    int pin = 1;
+    for (int j = 2; j <= s; j++) {
+        a.in = d1; a.d2 = d2; a.part_in = c->d_part[pin]; a.part_out = c->d_part[pin ^ 1];
+        a.mu = (real)K.mu[j]; a.nu = (real)K.nu[j]; a.a = (real)K.a[j]; a.g = (real)K.g[j];
+        a.use_d2 = j > 2;
+        M.nparts_in = np_out;
+        prof_begin(c, 1, armed);
+        if (j < s) launch_map_stage<real, 1>(c, a, M, vec, &np_out);
+        else launch_map_stage<real, 2>(c, a, M, vec, &np_out);
+        prof_end(c, armed, 1);
+        real* t = d1; d1 = d2; d2 = t;
+        pin ^= 1;
+    }
+    return HFT_OK;
+}
+
 // one diffusion step (D of Eq. 21), one launch per stage
 template <typename real>
 int diffuse_unblocked(hft_ctx* c, double dt, int s) {
@@ -421,6 +507,8 @@ int diffuse_unblocked(hft_ctx* c, double dt, int s) {
     real* da = arr_of<real>(c, (is + 2) % kNumArrays);
     real* db = arr_of<real>(c, (is + 3) % kNumArrays);
     dim3 g(G.nbx, (G.nt + 2 + RPT - 1) / RPT, c->nr);
+    const bool map = c->map_any;   // nu(theta, phi): same sequence with the k_sts_stage_map kernels and nu-weighted polar sums
+    if (map) return diffuse_map<real>(c, dt, s);
     launch_row_sums<real>(c, Y0, c->d_part[0]);
     StsArgs<real> a;
     a.F = F; a.Y0 = Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
@@ -503,7 +591,7 @@ int step_once(hft_ctx* c, double dt, int s) {
     if (rc != HFT_OK) return rc;
     if (c->opt.diff_time != 0) {
         const int kb = c->opt.sts_block == 0 ? sts_default_block(c->G, sizeof(real)) : c->opt.sts_block;
-        if (c->opt.diff_time >= 2 && kb > 1 && s > 2 * kb && sts_blocked_supported(c->G, sizeof(real))) {
+        if (!c->map_any && c->opt.diff_time >= 2 && kb > 1 && s > 2 * kb && sts_blocked_supported(c->G, sizeof(real))) {
             StsBlockedPlan<real> P;
             P.Y0 = arr_of<real>(c, c->i_state);
             for (int i = 0; i < 5; i++) P.buf[i] = arr_of<real>(c, (c->i_state + 1 + i) % kNumArrays);
@@ -527,6 +615,54 @@ int step_once(hft_ctx* c, double dt, int s) {
     }
     c->time += dt;
     return rc;
+}
+
+// nu(theta, phi) of realization q into the NU array: from h_map ([nt+1][np], R_sun^2/hr) or, if null, from the realization's
+// theta-face profile nuf (constant along phi).  Also the Gershgorin diagonal maximum of Eq. 28 (:454) over every cell and
+// both caps (fp64, from the given values) and the two polar weight sums (fp64, from the values as stored).
+template <typename real>
+int map_upload(hft_ctx* c, int q, const double* h_map) {
+    const int nt = c->G.nt, np = c->G.np;
+    std::vector<real> h((size_t)(nt + 1) * np);
+    const double* nuf = &c->nuf[(size_t)q * (nt + 1)];
+    for (int f = 0; f <= nt; f++)
+        for (int k = 0; k < np; k++) h[(size_t)f * np + k] = (real)(h_map ? h_map[(size_t)f * np + k] : nuf[f]);
+    double wN = 0.0, wS = 0.0;
+    for (int k = 0; k < np; k++) {
+        const int kw = (k + np - 1) % np;
+        wN += 0.5 * ((double)h[k] + (double)h[kw]);
+        wS += 0.5 * ((double)h[(size_t)nt * np + k] + (double)h[(size_t)nt * np + kw]);
+    }
+    c->capw[2 * q] = wN; c->capw[2 * q + 1] = wS;
+    c->map_set[q] = h_map != nullptr;
+    if (h_map) {
+        double wn = 0.0, ws = 0.0;
+        for (int k = 0; k < np; k++) {
+            const int kw = (k + np - 1) % np;
+            wn += 0.5 * (h_map[k] + h_map[kw]);
+            ws += 0.5 * (h_map[(size_t)nt * np + k] + h_map[(size_t)nt * np + kw]);
+        }
+        double d = fmax(c->P * wn * c->dph / c->dth, c->P * ws * c->dph / c->dth);
+        for (int j = 1; j <= nt; j++) {
+            const double *nS = h_map + (size_t)j * np, *nN = h_map + (size_t)(j - 1) * np;
+            const double gt = 1.0 / (c->st[j] * c->dth * c->dth), gp = 1.0 / (c->st[j] * c->st[j] * c->dph * c->dph);
+            for (int k = 0; k < np; k++) {
+                const int kw = (k + np - 1) % np;
+                d = fmax(d, 0.5 * (nS[k] + nS[kw]) * c->sth[j] * gt + 0.5 * (nN[k] + nN[kw]) * c->sth[j - 1] * gt +
+                                0.5 * (nS[k] + nN[k]) * gp + 0.5 * (nS[kw] + nN[kw]) * gp);
+            }
+        }
+        c->map_diag[q] = d;
+    }
+    CK(cudaMemcpy2DAsync(c->numap + (size_t)q * c->G.rstride * sizeof(real), (size_t)c->G.pitch * sizeof(real), h.data(),
+                         (size_t)np * sizeof(real), (size_t)np * sizeof(real), nt + 1, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(c->d_capw + 2 * q, &c->capw[2 * q], 2 * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CK(cudaStreamSynchronize(c->stream));   // h goes out of scope
+    return HFT_OK;
+}
+
+int map_upload_any(hft_ctx* c, int q, const double* h_map) {
+    return c->fp64() ? map_upload<double>(c, q, h_map) : map_upload<float>(c, q, h_map);
 }
 
 int check_launch(hft_ctx* c) {
@@ -561,7 +697,7 @@ int hft_workspace_bytes(const hft_grid* grid, int32_t n_real, const hft_options*
     if (opt && !valid_options(opt)) return HFT_ERR_ARG;
     const size_t w = grid->dtype == 1 ? 8 : 4;
     const size_t one = round_up((size_t)n_real * (grid->n_theta + 2) * pitch_for(grid->n_phi, grid->dtype) * w, 256);
-    *h_bytes = one * (kNumArrays + ((opt && opt->flow_attenuation) ? kNumAttArrays : 0) + ((opt && opt->rfe) ? kNumRfeArrays : 0));
+    *h_bytes = one * (kNumArrays + extra_arrays(opt));
     return HFT_OK;
 }
 
@@ -585,13 +721,16 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     c->G.nt = grid->n_theta; c->G.np = grid->n_phi; c->G.pitch = pitch_for(grid->n_phi, grid->dtype); c->G.nr = n_real;
     c->G.rstride = (size_t)(grid->n_theta + 2) * c->G.pitch;
     c->G.nbx = (grid->n_phi + TX - 1) / TX;
-    c->arr_bytes = need / (kNumArrays + (o.flow_attenuation ? kNumAttArrays : 0) + (o.rfe ? kNumRfeArrays : 0));
+    c->arr_bytes = need / (kNumArrays + extra_arrays(&o));
     for (int i = 0; i < kNumArrays; i++) c->arr[i] = (char*)d_workspace + (size_t)i * c->arr_bytes;
     if (o.flow_attenuation)
         for (int i = 0; i < kNumAttArrays; i++) c->att[i] = (char*)d_workspace + (size_t)(kNumArrays + i) * c->arr_bytes;
     if (o.rfe)
         for (int i = 0; i < kNumRfeArrays; i++)
             c->rfe_map[i] = (char*)d_workspace + (size_t)(kNumArrays + (o.flow_attenuation ? kNumAttArrays : 0) + i) * c->arr_bytes;
+    if (o.diffusivity_map)
+        c->numap = (char*)d_workspace + (size_t)(kNumArrays + (o.flow_attenuation ? kNumAttArrays : 0) + (o.rfe ? kNumRfeArrays : 0)) * c->arr_bytes;
+    c->map_set.assign(n_real, 0); c->map_diag.assign(n_real, 0.0); c->capw.assign(2 * (size_t)n_real, 0.0);
     c->B0.assign(n_real, 0.0);
     c->nu.resize(n_real); c->nuf.resize((size_t)n_real * (c->G.nt + 1)); c->vt.resize((size_t)n_real * (c->G.nt + 1)); c->om.resize((size_t)n_real * (c->G.nt + 2));
     build_metric(c);
@@ -611,6 +750,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
         (e = cudaMalloc((void**)&c->d_zmean, sts_zmean_bytes(c->G))) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_capseq, sts_capseq_bytes(c->G))) != cudaSuccess ||
         (e = cudaMalloc(&c->d_B0, (size_t)n_real * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&c->d_capw, (size_t)n_real * 2 * sizeof(double))) != cudaSuccess ||
         (e = cudaMallocHost((void**)&c->h_diag, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess) {
         cuda_fail(c, e, "cudaMalloc");
         return fail(HFT_ERR_NOMEM);
@@ -627,7 +767,7 @@ void hft_destroy(hft_ctx* c) {
     if (c->prof_ev_made)
         for (int i = 0; i < 2 * kProfEvents; i++) cudaEventDestroy(c->prof_ev[i]);
     cudaFree(c->d_tab); cudaFree(c->d_part[0]); cudaFree(c->d_part[1]); cudaFree(c->d_fluxpart);
-    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq); cudaFree(c->d_B0);
+    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq); cudaFree(c->d_B0); cudaFree(c->d_capw);
     if (c->h_diag) cudaFreeHost(c->h_diag);
     cudaFree(c->d_extpart); cudaFree(c->d_ext);
     if (c->h_ext) cudaFreeHost(c->h_ext);
@@ -654,7 +794,33 @@ int hft_set_diffusivity_profile(hft_ctx* c, int32_t r, const double* h_nu_face) 
         if (r < 0 || q == r)
             for (int f = 0; f <= nt; f++) c->nuf[(size_t)q * (nt + 1) + f] = h_nu_face[f] * kKm2sToRs2Hr;
     CK(cudaStreamSynchronize(c->stream));   // the tables may still be read by enqueued work
+    if (c->map_any)   // the realizations given a profile leave map mode's per-cell values for the profile's
+        for (int q = 0; q < c->nr; q++)
+            if (r < 0 || q == r) {
+                const int rc = map_upload_any(c, q, nullptr);
+                if (rc != HFT_OK) return rc;
+            }
     return upload_all_tables(c);
+}
+
+int hft_set_diffusivity_map(hft_ctx* c, int32_t r, const double* h_nu_hh) {
+    if (!c || !h_nu_hh || r < -1 || r >= c->nr || !c->opt.diffusivity_map) return HFT_ERR_ARG;
+    const int nt = c->G.nt, np = c->G.np;
+    const size_t n = (size_t)(nt + 1) * np;
+    std::vector<double> m(n);
+    for (size_t i = 0; i < n; i++) {
+        if (!(h_nu_hh[i] >= 0.0)) return HFT_ERR_ARG;
+        m[i] = h_nu_hh[i] * kKm2sToRs2Hr;
+    }
+    CK(cudaStreamSynchronize(c->stream));   // NU may still be read by enqueued work
+    for (int q = 0; q < c->nr; q++) {
+        const bool mine = r < 0 || q == r;
+        if (!mine && c->map_any) continue;   // already holds its own map or profile
+        const int rc = map_upload_any(c, q, mine ? m.data() : nullptr);
+        if (rc != HFT_OK) return rc;
+    }
+    c->map_any = true;
+    return HFT_OK;
 }
 
 int hft_set_grid_diffusivity(hft_ctx* c, int32_t r, double alpha_nu) {

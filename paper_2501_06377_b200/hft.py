@@ -18,7 +18,7 @@ if not os.path.exists(LIB_PATH):
                       "(the CUDA extension is required; there is no CPU fallback)")
 _lib = C.CDLL(LIB_PATH)
 
-EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
+EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_diffusivity_map", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
            "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_diagnostics", "hft_diagnostics_ext", "hft_stable_dt",
            "hft_sts_stage_count", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
            "hft_last_cuda_error"]
@@ -41,7 +41,8 @@ class hft_params(C.Structure):
 
 class hft_options(C.Structure):
     _fields_ = [("adv_flux", C.c_int32), ("adv_time", C.c_int32), ("diff_time", C.c_int32), ("sts_stages", C.c_int32),
-                ("sts_block", C.c_int32), ("rfe", C.c_int32), ("strang", C.c_int32), ("flow_attenuation", C.c_int32)]
+                ("sts_block", C.c_int32), ("rfe", C.c_int32), ("strang", C.c_int32), ("flow_attenuation", C.c_int32),
+                ("diffusivity_map", C.c_int32)]
 
 
 _lib.hft_workspace_bytes.argtypes = [C.POINTER(hft_grid), C.c_int32, C.POINTER(hft_options), C.POINTER(C.c_size_t)]
@@ -52,6 +53,7 @@ _lib.hft_destroy.restype = None
 _lib.hft_set_flow_tables.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.hft_set_diffusivity_profile.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
 _lib.hft_set_grid_diffusivity.argtypes = [C.c_void_p, C.c_int32, C.c_double]
+_lib.hft_set_diffusivity_map.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
 _lib.hft_set_attenuation.argtypes = [C.c_void_p, C.c_int32, C.c_double]
 _lib.hft_set_rfe.argtypes = [C.c_void_p, C.c_int32, C.c_double, C.c_double, C.c_uint64]
 _lib.hft_get_rfe_map.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
@@ -95,7 +97,7 @@ class Context:
     """hft_create ... hft_destroy.  Maps are torch CUDA tensors [n_theta][n_phi] of the context dtype."""
 
     def __init__(self, n_theta, n_phi, params, dtype="f64", radius_cm=1.0, adv_flux=ADV_WENO3, adv_time=TIME_SSPRK43,
-                 diff_time=DIFF_RKG2, sts_stages=0, sts_block=0, rfe=0, strang=0, flow_attenuation=0, device="cuda:0", stream=None):
+                 diff_time=DIFF_RKG2, sts_stages=0, sts_block=0, rfe=0, strang=0, flow_attenuation=0, diffusivity_map=0, device="cuda:0", stream=None):
         if not torch.cuda.is_available():
             raise HftError("no CUDA device: the hot path has no CPU fallback")
         self.device = torch.device(device)
@@ -107,7 +109,8 @@ class Context:
         self._h = C.c_void_p()
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-            opt = hft_options(adv_flux, adv_time, diff_time, sts_stages, sts_block, int(rfe), int(strang), int(flow_attenuation))
+            opt = hft_options(adv_flux, adv_time, diff_time, sts_stages, sts_block, int(rfe), int(strang), int(flow_attenuation),
+                              int(diffusivity_map))
             nbytes = workspace_bytes(n_theta, n_phi, self.n_real, dtype, opt)
             self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             grid = hft_grid(self.n_theta, self.n_phi, 1 if dtype == "f64" else 0, 0, float(radius_cm))
@@ -155,6 +158,12 @@ class Context:
         assert a.shape == (self.n_theta + 1,)
         self._ck(_lib.hft_set_diffusivity_profile(self._h, int(r), a.ctypes.data_as(C.POINTER(C.c_double))),
                  "hft_set_diffusivity_profile")
+
+    def set_diffusivity_map(self, r, nu_hh_km2_s):
+        a = np.ascontiguousarray(nu_hh_km2_s, dtype=np.float64)
+        assert a.shape == (self.n_theta + 1, self.n_phi)
+        self._ck(_lib.hft_set_diffusivity_map(self._h, int(r), a.ctypes.data_as(C.POINTER(C.c_double))),
+                 "hft_set_diffusivity_map")
 
     def set_grid_diffusivity(self, r, alpha_nu):
         self._ck(_lib.hft_set_grid_diffusivity(self._h, int(r), float(alpha_nu)), "hft_set_grid_diffusivity")

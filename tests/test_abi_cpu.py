@@ -90,7 +90,10 @@ def test_workspace_grows_with_the_optional_rows(lib):
     assert hft.workspace_bytes(64, 128, 4, "f64", opt) == 12 * one
     opt = hft.hft_options(2, 4, 3, 0, 0, 1, 1, 1)
     assert hft.workspace_bytes(64, 128, 4, "f64", opt) == 14 * one
+    opt = hft.hft_options(2, 4, 3, 0, 0, 1, 1, 1, 1)
+    assert hft.workspace_bytes(64, 128, 4, "f64", opt) == 15 * one
     for bad in (hft.hft_options(5, 4, 3, 0, 0, 0, 0, 0), hft.hft_options(2, 2, 3, 0, 0, 0, 0, 0), hft.hft_options(2, 4, 3, 1, 0, 0, 0, 0),
-                hft.hft_options(2, 4, 3, 0, 3, 0, 0, 0), hft.hft_options(2, 4, 3, 0, 0, 2, 0, 0), hft.hft_options(2, 4, 3, 0, 0, 0, 0, 7)):
+                hft.hft_options(2, 4, 3, 0, 3, 0, 0, 0), hft.hft_options(2, 4, 3, 0, 0, 2, 0, 0), hft.hft_options(2, 4, 3, 0, 0, 0, 0, 7),
+                hft.hft_options(2, 4, 3, 0, 0, 0, 0, 0, 2)):
         with pytest.raises(hft.HftError):
             hft.workspace_bytes(64, 128, 4, "f64", bad)

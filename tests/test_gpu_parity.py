@@ -492,6 +492,73 @@ def test_latitude_dependent_diffusivity(dtype, block):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("case", ["rkg2_adv", "rkl2", "euler"])
+@pytest.mark.parametrize("nphi", [264, 263])
+def test_diffusivity_map_theta_phi(dtype, case, nphi):
+    """nu(theta, phi) on the half-half grid (Eq. 27-28): realization 0 a smooth map, 1 keeps its scalar
+    value, 2 a rough random map; ragged grids: 264 columns take the 16-byte-vector kernel k_sts_stage_mapv (part-filled
+    warps, 75 + 2 rows = 4 row blocks + tail), 263 columns the one-column-per-thread kernel k_sts_stage_map.  Then the
+    gpu fp32 result against the fp64 oracle, a map replaced by a profile, and the constant map against the table path."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 75, nphi, n_real=3)
+    opt = dict(diffusivity_map=1)
+    kw = {}
+    if case == "rkl2":
+        opt.update(adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKL2); kw.update(adv_flux=orc.ADV_OFF, diff_time=orc.DIFF_RKL2)
+    if case == "euler":
+        opt.update(adv_flux=H.ADV_OFF, diff_time=H.DIFF_EULER); kw.update(adv_flux=orc.ADV_OFF, diff_time=orc.DIFF_EULER)
+    ctx, o = make_pair(w, dtype, **opt)
+    o64 = orc.Oracle(w.n_theta, w.n_phi, w.params, dtype=np.float64)
+    for r in range(3):
+        o64.set_full(r, o.get_full(r).astype(np.float64))
+    rng = np.random.default_rng(31)
+    thf = ((np.arange(w.n_theta + 1) + 0.5) * math.pi / (w.n_theta + 1))[:, None]
+    phf = ((np.arange(w.n_phi) + 0.5) * 2 * math.pi / w.n_phi)[None, :]
+    maps = {0: 400.0 * (1 + 0.5 * np.sin(thf) * np.cos(phf) + 0.3 * np.cos(thf) ** 2 * np.sin(3 * phf)),
+            2: 100.0 + 500.0 * rng.random((w.n_theta + 1, w.n_phi))}
+    for r, m in maps.items():
+        ctx.set_diffusivity_map(r, m); o.set_diffusivity_map(r, m); o64.set_diffusivity_map(r, m)
+    ga, gd = ctx.stable_dt()
+    oa, od = o.stable_dt()
+    assert abs(gd / od - 1) < 1e-13
+    if case == "euler":
+        dt, n = 0.9 * gd, 25
+    else:
+        dt, n = (wl.plan(w, ga, gd)[0] if case == "rkg2_adv" else 300.0 * gd), 3
+        assert ctx.sts_stage_count(dt) == o.sts_stage_count(dt, kw.get("diff_time", orc.DIFF_RKG2))
+    before = ctx.diagnostics()
+    ctx.step(n, dt); o.step(n, dt, **kw); o64.step(n, dt, **kw)
+    compare(ctx, o, TOL[dtype], "nu(theta,phi) " + case)
+    compare(ctx, o64, TOL[dtype], "nu(theta,phi) vs fp64 oracle " + case)
+    after = ctx.diagnostics()
+    assert np.all(np.abs(after[:, 0] - before[:, 0]) <= (1e-12 if dtype == "f64" else 2e-5) * before[:, 1])
+    # realization 2 leaves its map for a profile; realization 0 keeps its map
+    prof = 200.0 + 300.0 * rng.random(w.n_theta + 1)
+    ctx.set_diffusivity_profile(2, prof); o.set_diffusivity_map(2, None); o.set_diffusivity_profile(2, prof)
+    assert abs(ctx.stable_dt()[1] / o.stable_dt()[1] - 1) < 1e-13
+    ctx.step(1, dt); o.step(1, dt, **kw)
+    compare(ctx, o, TOL[dtype], "map then profile " + case)
+    ctx.close()
+    # a constant map is the table path (blocked kernel) up to round-off
+    if case == "rkl2":
+        a, oa_ = make_pair(w, dtype, adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKL2)
+        b, _ = make_pair(w, dtype, diffusivity_map=1, adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKL2)
+        for r in range(3):
+            b.set_diffusivity_map(r, np.full((w.n_theta + 1, w.n_phi), w.params[r][0]))
+        assert abs(a.stable_dt()[1] / b.stable_dt()[1] - 1) < 1e-13
+        dt = 300.0 * a.stable_dt()[1]
+        a.step(2, dt); b.step(2, dt)
+        for r in range(3):
+            assert rel_linf(b.get_full(r).cpu().numpy(), a.get_full(r).cpu().numpy()) <= TOL[dtype]
+        a.close(); b.close()
+    # the option is required
+    c = H.Context(16, 32, w.params[:1], dtype=dtype)
+    with pytest.raises(H.HftError):
+        c.set_diffusivity_map(0, np.ones((17, 32)))
+    c.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_degenerate_sizes_and_calls(dtype):
     """Edge cases: the smallest grid the ABI accepts (8 x 8) and an odd ragged one (9 x 17, below every vector width, so
     all stages take the un-blocked kernels); zero steps is a no-op; a zero map stays zero; a constant map is a fixed point
