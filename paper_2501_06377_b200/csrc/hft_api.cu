@@ -366,14 +366,6 @@ void prof_end(hft_ctx* c, bool armed, int stages) {
     c->prof_n++;
 }
 
-template <typename real>
-int launch_row_sums(hft_ctx* c, const real* f, double* part) {
-    dim3 g(c->G.nbx, 2, c->nr);
-    k_polar_row_sums<real><<<g, TX, 0, c->stream>>>(f, part, c->G);
-    c->launches++;
-    return HFT_OK;
-}
-
 // one advection step (A of Eq. 21): SSPRK stages, each = stage kernel + cap kernel
 template <typename real>
 int advect(hft_ctx* c, double dt) {
@@ -428,9 +420,10 @@ int advect(hft_ctx* c, double dt) {
     return HFT_OK;
 }
 
-// one diffusion step with nu(theta, phi) (Eq. 27-28; hft_set_diffusivity_map): one launch per stage, k_sts_stage_mapv
-// (16-byte vectors) when n_phi is a multiple of the vector width, else k_sts_stage_map (one column per thread)
-template <typename real, int MODE>
+// one diffusion step, one launch per stage.  MAP: nu(theta, phi) (Eq. 27-28; hft_set_diffusivity_map), else the per-row
+// coefficient tables.  k_sts_stage_mapv (16-byte vectors) when n_phi is a multiple of the vector width, else the
+// one-column-per-thread kernels k_sts_stage_map / k_sts_stage
+template <typename real, int MODE, bool MAP = true>
 void launch_map_stage(hft_ctx* c, const StsArgs<real>& a, MapArgs<real>& M, bool vec, int* nparts) {
     const Geom& G = c->G;
     Tables<real>& T = tables_of<real>(c);
@@ -438,8 +431,12 @@ void launch_map_stage(hft_ctx* c, const StsArgs<real>& a, MapArgs<real>& M, bool
         constexpr int C = 16 / (int)sizeof(real);
         const int nbxv = (G.np / C + TX - 1) / TX;
         dim3 g(nbxv, (G.nt + 2 + MAPV_RPT - 1) / MAPV_RPT, c->nr);
-        k_sts_stage_mapv<real, MODE><<<g, TX, 0, c->stream>>>(a, M, T, G);
+        k_sts_stage_mapv<real, MODE, MAP><<<g, TX, 0, c->stream>>>(a, M, T, G);
         *nparts = nbxv;
+    } else if (!MAP) {
+        dim3 g(G.nbx, (G.nt + 2 + RPT - 1) / RPT, c->nr);
+        k_sts_stage<real, MODE><<<g, TX, 0, c->stream>>>(a, T, G);
+        *nparts = G.nbx;
     } else {
         dim3 g(G.nbx, (G.nt + 2 + RPT - 1) / RPT, c->nr);
         k_sts_stage_map<real, MODE><<<g, TX, 0, c->stream>>>(a, M, T, G);
@@ -448,8 +445,8 @@ void launch_map_stage(hft_ctx* c, const StsArgs<real>& a, MapArgs<real>& M, bool
     c->launches++;
 }
 
-template <typename real>
-int diffuse_map(hft_ctx* c, double dt, int s) {
+template <typename real, bool MAP>
+int diffuse_stagewise(hft_ctx* c, double dt, int s) {
     const Geom& G = c->G;
     const int is = c->i_state;
     real* Y0 = arr_of<real>(c, is);
@@ -462,14 +459,15 @@ int diffuse_map(hft_ctx* c, double dt, int s) {
     M.NU = (const real*)c->numap; M.capw = c->d_capw; M.capP = c->P * c->dph / c->dth; M.rdth = (real)(1.0 / c->dth);
     M.nparts_in = G.nbx;
     dim3 gs(G.nbx, 2, c->nr);
-    k_polar_row_sums_map<real><<<gs, TX, 0, c->stream>>>(Y0, M.NU, c->d_part[0], G);
+    if (MAP) k_polar_row_sums_map<real><<<gs, TX, 0, c->stream>>>(Y0, M.NU, c->d_part[0], G);
+    else k_polar_row_sums<real><<<gs, TX, 0, c->stream>>>(Y0, c->d_part[0], G);
     c->launches++;
     StsArgs<real> a;
     a.F = F; a.Y0 = Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
     int np_out = 0;
     if (c->opt.diff_time == 1) {  // explicit Euler (:474), new state written to `da`
         a.in = Y0; a.d2 = da; a.part_in = c->d_part[0]; a.part_out = c->d_part[1]; a.a = (real)dt;
-        launch_map_stage<real, 3>(c, a, M, vec, &np_out);
+        launch_map_stage<real, 3, MAP>(c, a, M, vec, &np_out);
         c->i_state = (is + 2) % kNumArrays;
         return HFT_OK;
     }
@@ -477,7 +475,7 @@ int diffuse_map(hft_ctx* c, double dt, int s) {
     a.in = Y0; a.d2 = da; a.part_in = c->d_part[0]; a.part_out = c->d_part[1]; a.a = (real)K.a[1];
     bool armed;
     prof_begin(c, 1, armed);
-    launch_map_stage<real, 0>(c, a, M, vec, &np_out);
+    launch_map_stage<real, 0, MAP>(c, a, M, vec, &np_out);
     prof_end(c, armed, 1);
     real *d1 = da, *d2 = db;
     int pin = 1;
@@ -487,8 +485,8 @@ int diffuse_map(hft_ctx* c, double dt, int s) {
         a.use_d2 = j > 2;
         M.nparts_in = np_out;
         prof_begin(c, 1, armed);
-        if (j < s) launch_map_stage<real, 1>(c, a, M, vec, &np_out);
-        else launch_map_stage<real, 2>(c, a, M, vec, &np_out);
+        if (j < s) launch_map_stage<real, 1, MAP>(c, a, M, vec, &np_out);
+        else launch_map_stage<real, 2, MAP>(c, a, M, vec, &np_out);
         prof_end(c, armed, 1);
         real* t = d1; d1 = d2; d2 = t;
         pin ^= 1;
@@ -499,49 +497,7 @@ int diffuse_map(hft_ctx* c, double dt, int s) {
 // one diffusion step (D of Eq. 21), one launch per stage
 template <typename real>
 int diffuse_unblocked(hft_ctx* c, double dt, int s) {
-    const Geom& G = c->G;
-    Tables<real>& T = tables_of<real>(c);
-    const int is = c->i_state;
-    real* Y0 = arr_of<real>(c, is);
-    real* F = arr_of<real>(c, (is + 1) % kNumArrays);
-    real* da = arr_of<real>(c, (is + 2) % kNumArrays);
-    real* db = arr_of<real>(c, (is + 3) % kNumArrays);
-    dim3 g(G.nbx, (G.nt + 2 + RPT - 1) / RPT, c->nr);
-    const bool map = c->map_any;   // nu(theta, phi): same sequence with the k_sts_stage_map kernels and nu-weighted polar sums
-    if (map) return diffuse_map<real>(c, dt, s);
-    launch_row_sums<real>(c, Y0, c->d_part[0]);
-    StsArgs<real> a;
-    a.F = F; a.Y0 = Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
-    if (c->opt.diff_time == 1) {  // explicit Euler (:474), new state written to `da`
-        a.in = Y0; a.d2 = da; a.part_in = c->d_part[0]; a.part_out = c->d_part[1]; a.a = (real)dt;
-        k_sts_stage<real, 3><<<g, TX, 0, c->stream>>>(a, T, G);
-        c->launches++;
-        c->i_state = (is + 2) % kNumArrays;
-        return HFT_OK;
-    }
-    const StsCoef& K = c->coef;
-    // stage 1: F = L(Y0), delta_1 = mut_1 dt F
-    a.in = Y0; a.d2 = da; a.part_in = c->d_part[0]; a.part_out = c->d_part[1]; a.a = (real)K.a[1];
-    bool armed;
-    prof_begin(c, 1, armed);
-    k_sts_stage<real, 0><<<g, TX, 0, c->stream>>>(a, T, G);
-    prof_end(c, armed, 1);
-    c->launches++;
-    real *d1 = da, *d2 = db;
-    int pin = 1;
-    for (int j = 2; j <= s; j++) {
-        a.in = d1; a.d2 = d2; a.part_in = c->d_part[pin]; a.part_out = c->d_part[pin ^ 1];
-        a.mu = (real)K.mu[j]; a.nu = (real)K.nu[j]; a.a = (real)K.a[j]; a.g = (real)K.g[j];
-        a.use_d2 = j > 2;
-        prof_begin(c, 1, armed);
-        if (j < s) k_sts_stage<real, 1><<<g, TX, 0, c->stream>>>(a, T, G);
-        else k_sts_stage<real, 2><<<g, TX, 0, c->stream>>>(a, T, G);
-        prof_end(c, armed, 1);
-        c->launches++;
-        real* t = d1; d1 = d2; d2 = t;
-        pin ^= 1;
-    }
-    return HFT_OK;
+    return c->map_any ? diffuse_stagewise<real, true>(c, dt, s) : diffuse_stagewise<real, false>(c, dt, s);
 }
 
 // ---------------------------------------------------------------- random flux emergence (Sec. 2.4)

@@ -109,7 +109,9 @@ __global__ void __launch_bounds__(TX) k_sts_stage_map(StsArgs<real> A, MapArgs<r
 
 constexpr int MAPV_RPT = 16;   // rows streamed per thread of the vector kernel
 
-template <typename real, int MODE>
+// MAP = false: the same 16-byte-vector stage kernel with the per-row coefficient tables of k_sts_stage (scalar nu or
+// nu(theta)), identical arithmetic to k_sts_stage; NU / capw are not read, the polar sums are unweighted.
+template <typename real, int MODE, bool MAP = true>
 __global__ void __launch_bounds__(TX) k_sts_stage_mapv(StsArgs<real> A, MapArgs<real> M, Tables<real> T, Geom G) {
     constexpr int C = 16 / (int)sizeof(real);
     __shared__ double red[32];
@@ -133,20 +135,25 @@ __global__ void __launch_bounds__(TX) k_sts_stage_mapv(StsArgs<real> A, MapArgs<
     for (int q = 0; q < C; q++) { n[q] = (real)0; nN[q] = (real)0; }
     if (j0 > 0) {
         vload<real, C>(n, in + (size_t)(j0 - 1) * G.pitch + cc);
-        vload<real, C>(nN, nu + (size_t)(j0 - 1) * G.pitch + cc);   // face j0 - 1/2
+        if (MAP) vload<real, C>(nN, nu + (size_t)(j0 - 1) * G.pitch + cc);   // face j0 - 1/2
     }
     vload<real, C>(c, in + (size_t)j0 * G.pitch + cc);
-    nNw = __shfl_up_sync(full, nN[C - 1], 1);
-    if (edgeW && j0 > 0) nNw = nu[(size_t)(j0 - 1) * G.pitch + cw];
+    if (MAP) {
+        nNw = __shfl_up_sync(full, nN[C - 1], 1);
+        if (edgeW && j0 > 0) nNw = nu[(size_t)(j0 - 1) * G.pitch + cw];
+    }
+    const real* cpt = T.cp + (size_t)r * (G.nt + 2);
+    const real* cmt = T.cm + (size_t)r * (G.nt + 2);
+    const real* cft = T.cf + (size_t)r * (G.nt + 2);
     double sumN = 0.0, sumS = 0.0;
     for (int j = j0; j < j1; j++) {
         const size_t off = base + (size_t)j * G.pitch + cc;
-        real s[C], nS[C], nSw, out[C], Lv[C];
+        real s[C], nS[C], nSw = (real)0, out[C], Lv[C];
 #pragma unroll
         for (int q = 0; q < C; q++) { s[q] = (real)0; nS[q] = (real)0; }
         if (j < G.nt + 1) {
             vload<real, C>(s, in + (size_t)(j + 1) * G.pitch + cc);
-            vload<real, C>(nS, nu + (size_t)j * G.pitch + cc);   // face j + 1/2
+            if (MAP) vload<real, C>(nS, nu + (size_t)j * G.pitch + cc);   // face j + 1/2
         }
         real d2v[C], Fv[C];
 #pragma unroll
@@ -155,18 +162,31 @@ __global__ void __launch_bounds__(TX) k_sts_stage_mapv(StsArgs<real> A, MapArgs<
             if (A.use_d2) vload<real, C>(d2v, A.d2 + off);
             vload<real, C>(Fv, A.F + off);
         }
-        nSw = __shfl_up_sync(full, nS[C - 1], 1);
-        if (edgeW && j < G.nt + 1) nSw = nu[(size_t)j * G.pitch + cw];
+        if (MAP) {
+            nSw = __shfl_up_sync(full, nS[C - 1], 1);
+            if (edgeW && j < G.nt + 1) nSw = nu[(size_t)j * G.pitch + cw];
+        }
         if (j == 0 || j == G.nt + 1) {
             const int pole = (j == 0) ? 0 : 1;
             double S = sum_partials(A.part_in + ((size_t)r * 2 + pole) * G.nbx, M.nparts_in);
-            const real L = (real)(M.capP * (S - M.capw[2 * r + pole] * (double)c[0]));
+            const real L = MAP ? (real)(M.capP * (S - M.capw[2 * r + pole] * (double)c[0]))
+                               : (real)(T.capc[2 * r + pole] * (S - (double)G.np * (double)c[0]));
 #pragma unroll
             for (int q = 0; q < C; q++) Lv[q] = L;
         } else {
             real w0 = __shfl_up_sync(full, c[C - 1], 1), e0 = __shfl_down_sync(full, c[0], 1);
             if (edgeW) w0 = in[(size_t)j * G.pitch + cw];
             if (edgeE) e0 = in[(size_t)j * G.pitch + ce];
+            if (!MAP) {
+                const real cp = cpt[j], cm = cmt[j], cf = cft[j];
+#pragma unroll
+                for (int q = 0; q < C; q++) {
+                    const real w = q == 0 ? w0 : c[q > 0 ? q - 1 : 0];
+                    const real e = q == C - 1 ? e0 : c[q < C - 1 ? q + 1 : 0];
+                    Lv[q] = cp * (s[q] - c[q]) - cm * (c[q] - n[q]) + cf * ((e - (real)2 * c[q]) + w);
+                }
+            }
+            if (MAP) {
             const real gt = T.rdt[j] * M.rdth, gp = T.rdp[j] * T.rdp[j];
             const real gs = T.sth[j] * gt, gn = T.sth[j - 1] * gt;
 #pragma unroll
@@ -180,6 +200,7 @@ __global__ void __launch_bounds__(TX) k_sts_stage_mapv(StsArgs<real> A, MapArgs<
                 const real ae = half * (nS[q] + nN[q]) * gp;
                 const real aw = half * (nSq_w + nNq_w) * gp;
                 Lv[q] = (as * (s[q] - c[q]) - an * (c[q] - n[q])) + (ae * (e - c[q]) - aw * (c[q] - w));
+            }
             }
         }
 #pragma unroll
@@ -202,7 +223,7 @@ __global__ void __launch_bounds__(TX) k_sts_stage_mapv(StsArgs<real> A, MapArgs<
             for (int q = 0; q < C; q++) {
                 const real a = (j == 1) ? nN[q] : nS[q];
                 const real b = (j == 1) ? (q == 0 ? nNw : nN[q > 0 ? q - 1 : 0]) : (q == 0 ? nSw : nS[q > 0 ? q - 1 : 0]);
-                t += 0.5 * ((double)a + (double)b) * (double)out[q];
+                t += MAP ? 0.5 * ((double)a + (double)b) * (double)out[q] : (double)out[q];
             }
             if (!live) t = 0.0;
             if (j == 1) sumN = t;
