@@ -295,7 +295,7 @@ def main():
         ach = stage_passes * field_bytes * stages_per_launch / sec / 1e9
         blocked = stages_per_launch > 1
         out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                           "kernel": "k_sts_pipe" if blocked else ("k_sts_stage_map" if args.nu_map else "k_sts_stage"), "stages_per_launch": stages_per_launch,
+                           "kernel": "k_sts_pipe" if blocked else ("k_sts_stage_mapv<MAP=true>" if args.nu_map else "k_sts_stage_mapv<MAP=false>"), "stages_per_launch": stages_per_launch,
                            "avg_launch_ms": res["kernel_ms"], "sampled_launches": res["kernel_samples"], "peak_source": peak_src}
         if blocked:
             # a K-stage block moves 5 array passes (3 in, 2 out) however large K is; the
