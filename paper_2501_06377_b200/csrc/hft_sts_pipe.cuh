@@ -29,6 +29,7 @@
 #include <stdint.h>
 
 #include "hft_sts_blocked.cuh"
+#include "hft_sts_map.cuh"
 
 namespace hft {
 
@@ -316,12 +317,19 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
     const int K = P.kb, s = P.s;
     real* F = P.buf[0];
     real* b[4] = {P.buf[1], P.buf[2], P.buf[3], P.buf[4]};
-    dim3 g1(G.nbx, (G.nt + 2 + RPT - 1) / RPT, G.nr), gs(G.nbx, 2, G.nr);
+    // stage 1 and an odd remainder stage run one stage per launch in the 16-byte-vector kernel (n_phi is a multiple of the
+    // vector width whenever the blocked path is taken); its polar partials come in nbxv pieces per row
+    constexpr int CV = 16 / (int)sizeof(real);
+    const int nbxv = (G.np / CV + TX - 1) / TX;
+    dim3 g1(nbxv, (G.nt + 2 + MAPV_RPT - 1) / MAPV_RPT, G.nr), gs(G.nbx, 2, G.nr);
     k_polar_row_sums<real><<<gs, TX, 0, P.stream>>>(P.Y0, P.part[0], G);
+    MapArgs<real> M;
+    M.NU = nullptr; M.capw = nullptr; M.capP = 0.0; M.rdth = (real)0; M.nparts_in = G.nbx;
     StsArgs<real> a;
     a.F = F; a.Y0 = P.Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
     a.in = P.Y0; a.d2 = b[0]; a.part_in = P.part[0]; a.part_out = P.part[1]; a.a = (real)P.a[1];
-    k_sts_stage<real, 0><<<g1, TX, 0, P.stream>>>(a, T, G);
+    k_sts_stage_mapv<real, 0, false><<<g1, TX, 0, P.stream>>>(a, M, T, G);
+    M.nparts_in = nbxv;
     *launches += 2;
     const int rem = (s - 1) % K;
     // the remainder: one un-blocked stage if it is odd, then (pipe only) ONE shorter block of rem - (rem & 1) stages
@@ -335,7 +343,7 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
         a.in = b[icur]; a.d2 = b[iprev]; a.part_in = P.part[pin]; a.part_out = P.part[pin ^ 1];
         a.mu = (real)P.mu[j]; a.nu = (real)P.nu[j]; a.a = (real)P.a[j]; a.g = (real)P.g[j];
         a.use_d2 = has_prev;
-        k_sts_stage<real, 1><<<g1, TX, 0, P.stream>>>(a, T, G);
+        k_sts_stage_mapv<real, 1, false><<<g1, TX, 0, P.stream>>>(a, M, T, G);
         *launches += 1;
         int t = icur; icur = iprev; iprev = t;
         has_prev = true;
