@@ -318,7 +318,9 @@ def main():
                            "hbm_roofline_frac_whole_step": r32["value"] / world * (9 + 4 * r32["s"]) * 4 / (peak * 1e9)}
     if rank == 0:
         if not args.no_cpu_baseline:
-            n_or = 24 if wd.n_theta >= 1024 else 200        # ~10-30 s of oracle work on the box's host cores
+            # ~10-30 s of oracle work on the box's host cores (the float build of the oracle runs ~12x slower per step than
+            # the double build on this workload -- subnormal operands, no flush-to-zero -- so its sample is shorter)
+            n_or = (24 if args.dtype == "f64" else 3) if wd.n_theta >= 1024 else 200
             rate, el, thr = oracle_sample(wd, args.dtype, n_or, res["dt"], res["s"])
             out["cpu_baseline"] = {"value": rate, "unit": "cell-updates/s", "cores": thr, "kind": "oracle",
                                    "sample": f"1 of {wd.n_real} realizations x {n_or} steps of the full grid ({el:.1f} s)"}
