@@ -165,12 +165,9 @@ def main():
                             flow_attenuation=int(args.attenuation > 0), diffusivity_map=int(args.nu_map), device=f"cuda:{local}", **kw)
             if args.attenuation > 0:
                 c.set_attenuation(-1, args.attenuation)
-            if args.nu_map:      # nu_r (1 + 0.3 sin(theta) cos(phi)) on the half-half grid: smooth, phi-dependent, per realization
-                thf = ((np.arange(wd.n_theta + 1) + 0.5) * np.pi / (wd.n_theta + 1))[:, None]
-                phf = ((np.arange(wd.n_phi) + 0.5) * 2 * np.pi / wd.n_phi)[None, :]
-                shape = 1.0 + 0.3 * np.sin(thf) * np.cos(phf)
+            if args.nu_map:      # nu_r (1 + 0.3 sin(theta) cos(phi)) on the half-half grid, per realization (workloads.diffusivity_map)
                 for r in range(wd.n_real):
-                    c.set_diffusivity_map(r, wd.params[r][0] * shape)
+                    c.set_diffusivity_map(r, wl.diffusivity_map(wd, r))
             return c
         ctx = make_ctx()
         maps = ens.shard_maps(wd, device=f"cuda:{local}").to(ctx.tdtype).contiguous()

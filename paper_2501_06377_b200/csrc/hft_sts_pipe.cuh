@@ -293,12 +293,15 @@ int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& 
     // runs in waves of `slots` CTAs; take the count that minimises waves x row-steps per segment
     int nseg = 1;
     long best = -1;
-    for (int n = 1; n <= 32 && (G.nt + 2) / n >= 4 * K; n++) {
+    // (a small batch leaves most of the 148 SMs idle: short segments, down to K rows each, then cost nothing although
+    // they re-stream more rows than they own -- cfg 1, one 512x1024 realization, runs 22 strips x 32 segments)
+    for (int n = 1; n <= 64 && (G.nt + 2) / n >= K; n++) {
         const long rows = (G.nt + 2 + n - 1) / n + 2 * K;
         const long waves = ((long)ctas_x * n * G.nr + slots - 1) / slots;
         if (best < 0 || waves * rows < best) { best = waves * rows; nseg = n; }
     }
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
+    nseg = (G.nt + 2 + a.rows_per_seg - 1) / a.rows_per_seg;   // no empty segment
     dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
     k_sts_capseq<real, K><<<gc, 32 * STS_KMAX, 0, P.stream>>>(a, T, G, P.capseq);
     bool armed = false;

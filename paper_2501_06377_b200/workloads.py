@@ -125,6 +125,15 @@ def plan(w: Workload, dt_adv_limit: float, dt_diff_expl: float):
     return dt, n, 0
 
 
+def diffusivity_map(w: Workload, r: int):
+    """Synthetic spatially varying diffusivity of realization r on the half-half grid [n_theta+1][n_phi], km^2/s
+    (bench.py --nu-map and the full-size parity test): eta_r (1 + 0.3 sin(theta) cos(phi)) -- smooth, phi-dependent,
+    positive; entry [f][k] at colatitude (f+1/2) dtheta, longitude (k+1/2) dphi.  numpy float64."""
+    thf = ((np.arange(w.n_theta + 1) + 0.5) * math.pi / (w.n_theta + 1))[:, None]
+    phf = ((np.arange(w.n_phi) + 0.5) * 2.0 * math.pi / w.n_phi)[None, :]
+    return float(w.params[r][0]) * (1.0 + 0.3 * np.sin(thf) * np.cos(phf))
+
+
 def colatitudes(n_theta, device="cpu"):
     return torch.arange(1, n_theta + 1, dtype=torch.float64, device=device) * (math.pi / (n_theta + 1))
 

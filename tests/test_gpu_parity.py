@@ -199,6 +199,39 @@ def test_config3_full_size_sampled_realizations(dtype):
     ctx.close()
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("path", ["nu_map", "unblocked"])
+def test_config3_full_size_stage_by_stage_paths(dtype, path):
+    """The two one-launch-per-stage paths at BASELINE config 3's full size in the launch configurations bench.py times
+    (`--nu-map`: nu(theta, phi) of workloads.diffusivity_map; `--sts-block 1`), one step; the oracle checks a sampled
+    realization; all 64 conserve flux."""
+    H = hft()
+    w = wl.config(3, dtype)
+    opt = dict(diffusivity_map=1) if path == "nu_map" else dict(sts_block=1)
+    ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype, **opt)
+    maps = wl.initial_maps(w, device="cuda").to(ctx.tdtype)
+    for r in range(w.n_real):
+        ctx.set_map(r, maps[r].contiguous())
+        if path == "nu_map":
+            ctx.set_diffusivity_map(r, wl.diffusivity_map(w, r))
+    dt, _, _ = wl.plan(w, *ctx.stable_dt())
+    s = ctx.sts_stage_count(dt)
+    before = ctx.diagnostics()
+    ctx.step(1, dt)
+    after = ctx.diagnostics()
+    cons = 1e-12 if dtype == "f64" else 2e-5
+    assert np.all(np.abs(after[:, 0] - before[:, 0]) <= cons * before[:, 1])
+    r = 42 if dtype == "f64" else 21
+    o = orc.Oracle(w.n_theta, w.n_phi, w.params[r:r + 1], dtype=NPDT[dtype])
+    o.set_map(0, maps[r].cpu().numpy())
+    if path == "nu_map":
+        o.set_diffusivity_map(0, wl.diffusivity_map(w, r))
+    o.step(1, dt, sts_stages=s)
+    e = rel_linf(ctx.get_full(r).cpu().numpy(), o.get_full(0))
+    assert e <= TOL[dtype], (r, e)
+    ctx.close()
+
+
 def test_config2_full_size_sampled_realizations():
     """BASELINE config 2 at full size (1024x2048, 8 realizations with eta = 250..600, v0 = 10..20, shared map),
     2 of its 31 steps; the oracle checks realizations 0 and 7 (smallest and largest diffusivity) one by one."""
