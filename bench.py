@@ -122,6 +122,47 @@ def run_reference(args, w):
         "gpu_launches": 0}))
 
 
+def run_paper_case(args):
+    """The two validation runs the paper prints wall times for (RTX 3090 Ti), on this GPU:
+    `diffusion`: Eq. 19 field, nu = 500 km^2/s, 512x1024 file grid, ONE 672 h step of RKG2(3/2) (PAPER.md:476: 0.55 s, HH 6.3e-5);
+    `advdiff`:   the same field with rigid rotation v_phi = 1.80766 km/s sin(theta), WENO3 + SSPRK(4,3) + RKG2, dt = 0.62 h
+                 over 672 h (Table 1 :337-344: 21.1 s, HH 4.8e-5).
+    Context lines, not the bench metric: another machine's numbers, the paper's grid (510 x 1023 regular cells, odd n_phi)."""
+    from paper_2501_06377_b200 import hft
+    torch.cuda.set_device(0)
+    nt, nphi = (510, 1023) if not args.paper_grid_even else (510, 1024)
+    u = wl.soccer_ball_full(nt, nphi)
+    rot = 1.80766e3 if args.paper_case == "advdiff" else 0.0
+    ctx = hft.Context(nt, nphi, [[500.0, rot, 0, 0, 0, 0, 0]], dtype=args.dtype,
+                      adv_flux=hft.ADV_WENO3 if rot else hft.ADV_OFF, sts_block=args.sts_block)
+    ut = torch.from_numpy(u).to(ctx.tdtype).cuda().contiguous()
+    n = round(672.0 / 0.62) if rot else 1
+    dt = 672.0 / n
+    s = ctx.sts_stage_count(dt)
+    times = []
+    for rep in range(1 + max(1, args.steps)):          # first repetition = warm-up
+        ctx.set_full(0, ut)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0 = ctx.launch_count()
+        e0.record()
+        ctx.step(n, dt)
+        e1.record()
+        torch.cuda.synchronize()
+        times.append(e0.elapsed_time(e1) * 1e-3)
+        launches = ctx.launch_count() - l0
+    got = ctx.get_full(0).double().cpu().numpy()
+    exact = u * math.exp(-42.0 * 500.0 * 7.43162901307967e-9 * 672.0)      # l(l+1) = 42, nu in R_sun^2/hr (PAPER.md:298)
+    hh = math.sqrt(((got[1:-1] - exact[1:-1]) ** 2).sum() / (np.abs(got[1:-1]) * np.abs(exact[1:-1])).sum())   # Eq. 18 (:246)
+    ctx.close()
+    paper = {"diffusion": {"seconds": 0.55, "hh": 6.3e-5, "hardware": "RTX 3090 Ti", "cite": "PAPER.md:476"},
+             "advdiff": {"seconds": 21.1, "hh": 4.8e-5, "hardware": "RTX 3090 Ti", "cite": "PAPER.md:337-344 (Table 1)"}}[args.paper_case]
+    print(json.dumps({"paper_case": args.paper_case, "metric": "seconds per run", "value": min(times[1:]), "unit": "s",
+                      "higher_is_better": False, "dtype": args.dtype, "grid": [nt, nphi], "steps_per_run": n, "dt_hours": dt,
+                      "sts_stages": s, "gpu_launches": launches, "hh_error_vs_analytic": hh, "runs_timed": len(times) - 1,
+                      "paper": paper, "note": "context only: the paper's number is another machine's"}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -134,10 +175,16 @@ def main():
     ap.add_argument("--attenuation", type=float, default=0.0, help="B0 in Gauss: time the step with flow attenuation (Eq. 5) on")
     ap.add_argument("--nu-map", action="store_true",
                     help="time the step with a spatially varying diffusivity nu(theta, phi) (Eq. 27-28): one launch per STS stage")
+    ap.add_argument("--paper-case", choices=["diffusion", "advdiff"], default=None,
+                    help="time one of the two validation runs the paper prints wall times for (context, not the bench metric)")
+    ap.add_argument("--paper-grid-even", action="store_true", help="--paper-case on 510 x 1024 instead of the paper's 510 x 1023")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--also-f32", action="store_true", help="add a second timed run in fp32 to the JSON line")
     args = ap.parse_args()
+    if args.paper_case:
+        run_paper_case(args)
+        return
     w = wl.config(args.config, args.dtype)
     if args.impl == "reference":
         run_reference(args, w)

@@ -546,8 +546,8 @@ int step_once(hft_ctx* c, double dt, int s) {
     if (c->opt.adv_flux != 0) rc = advect<real>(c, strang ? 0.5 * dt : dt);
     if (rc != HFT_OK) return rc;
     if (c->opt.diff_time != 0) {
-        const int kb = c->opt.sts_block == 0 ? sts_default_block(c->G, sizeof(real)) : c->opt.sts_block;
-        if (!c->map_any && c->opt.diff_time >= 2 && kb > 1 && s > 2 * kb && sts_blocked_supported(c->G, sizeof(real))) {
+        const int kb = c->opt.sts_block == 0 ? sts_default_block(c->G, sizeof(real), c->sts_pipe != 0) : c->opt.sts_block;
+        if (!c->map_any && c->opt.diff_time >= 2 && kb > 1 && s > 2 * kb && sts_blocked_supported(c->G, sizeof(real), c->sts_pipe != 0)) {
             StsBlockedPlan<real> P;
             P.Y0 = arr_of<real>(c, c->i_state);
             for (int i = 0; i < 5; i++) P.buf[i] = arr_of<real>(c, (c->i_state + 1 + i) % kNumArrays);

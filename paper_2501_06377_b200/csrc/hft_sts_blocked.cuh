@@ -83,6 +83,16 @@ __global__ void __launch_bounds__(32 * STS_KMAX) k_sts_capseq(BlkArgs<real, K> A
         const bool lower = i < K;   // prev and F are needed on rows 1..K-1 only
         double a = 0.0, b = 0.0, c = 0.0;
         for (int k = lane * C; k < G.np; k += 32 * C) {
+            if (k + C > G.np) {   // n_phi not a multiple of C: the last columns of the row one by one
+                for (int kk = k; kk < G.np; kk++) {
+                    a += (double)A.cur[off + kk];
+                    if (lower) {
+                        if (A.has_prev) b += (double)A.prev[off + kk];
+                        c += (double)A.F[off + kk];
+                    }
+                }
+                break;
+            }
             real v[C];
             vload<real, C>(v, A.cur + off + k);
 #pragma unroll
@@ -273,11 +283,13 @@ template <typename real> struct BlkCfg;
 template <> struct BlkCfg<double> { static constexpr int C = 2; };
 template <> struct BlkCfg<float> { static constexpr int C = 4; };
 
-inline bool sts_blocked_supported(const Geom& G, size_t wbytes) {
+// pipe: k_sts_pipe takes any n_phi (lanes behind the seam move their columns one by one); the first-generation
+// k_sts_blocked needs n_phi to be a multiple of the vector width
+inline bool sts_blocked_supported(const Geom& G, size_t wbytes, bool pipe = true) {
     const int C = wbytes == 8 ? 2 : 4;
-    return (G.np % C) == 0 && G.np >= 32 * C && G.nt >= 2 * STS_KMAX;
+    return (pipe || (G.np % C) == 0) && G.np >= 32 * C && G.nt >= 2 * STS_KMAX;
 }
-inline int sts_default_block(const Geom& G, size_t wbytes) { return sts_blocked_supported(G, wbytes) ? 8 : 1; }
+inline int sts_default_block(const Geom& G, size_t wbytes, bool pipe = true) { return sts_blocked_supported(G, wbytes, pipe) ? 8 : 1; }
 inline size_t sts_zmean_bytes(const Geom&) { return 256; }
 inline size_t sts_capseq_bytes(const Geom& G) { return (size_t)G.nr * 2 * STS_KMAX * sizeof(double) + 256; }
 inline int sts_blocked_init(const Geom&, bool) { return 0; }

@@ -78,7 +78,9 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 __device__ __forceinline__ double fma_r(double a, double b, double c) { return fma(a, b, c); }
 __device__ __forceinline__ float fma_r(float a, float b, float c) { return fmaf(a, b, c); }
 
-template <typename real, int K>
+// SPLIT = false: n_phi is a multiple of C, every lane moves its C columns as one 16-byte vector (the hot instantiation).
+// SPLIT = true:  any n_phi; lanes that are misaligned or straddle the seam move their columns one by one.
+template <typename real, int K, bool SPLIT>
 struct PipeWarp {
     using P = PipeCfg<real, K>;
     static constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, NF = P::NF, ROW = P::ROW, NCS = P::NCS;
@@ -97,16 +99,30 @@ struct PipeWarp {
     real sa, sadd;                   // this lane's product: fma(sa, raw, sadd)
     int cl;                          // this lane's level - 1
     int nt, pitch, ja, jb, lane;
-    bool wr;
+    // a lane whose C columns are 16-byte aligned and do not straddle the periodic seam moves them as one vector; with
+    // n_phi not a multiple of C the lanes behind the seam of the first / last strip are misaligned and move their
+    // columns one by one (dq = element offsets relative to the lane's first column, wmask = elements this lane writes)
+    bool simple;
+    int dq[C];
+    int wmask;
 
     __device__ __forceinline__ PipeWarp(const BlkArgs<real, K>& A_) : A(A_) {}
 
     __device__ __forceinline__ void prefetch(int row, int slot) {
         if (row <= nt + 1) {
             const size_t o = (size_t)row * pitch;
-            cp_async16(smem_u32(s_cur + slot * ROW), gcur + o);
-            cp_async16(smem_u32(s_prev + slot * ROW), gprev + o);
-            cp_async16(smem_u32(s_F + slot * ROW), gF + o);
+            if (!SPLIT || simple) {
+                cp_async16(smem_u32(s_cur + slot * ROW), gcur + o);
+                cp_async16(smem_u32(s_prev + slot * ROW), gprev + o);
+                cp_async16(smem_u32(s_F + slot * ROW), gF + o);
+            } else {
+#pragma unroll
+                for (int q = 0; q < C; q++) {
+                    cp_async_small(smem_u32(s_cur + slot * ROW + q), gcur + o + dq[q]);
+                    cp_async_small(smem_u32(s_prev + slot * ROW + q), gprev + o + dq[q]);
+                    cp_async_small(smem_u32(s_F + slot * ROW + q), gF + o + dq[q]);
+                }
+            }
         }
         // the raw row coefficient behind this lane's product of row-step row+1 rides in the same group, so it has
         // landed when the data of `row` has (an LDG issued three row-steps ahead still stalled 17 % of the warp
@@ -182,17 +198,30 @@ struct PipeWarp {
         if (cl < K) s_coef[((PH + 1) % NCS) * (K * 4) + lane] = fma_r(sa, raw_next, sadd);
         // row jo = t-K of levels K and K-1 (level K-1 row t-K is its centre: slot (PH-(K-1)-1) mod 3)
         const int jo = t - K;
-        if (wr && jo >= ja && jo < jb) {
+        if (wmask && jo >= ja && jo < jb) {
             const size_t o = (size_t)jo * pitch;
-            if (A.last) {
-                real y[C];
-                vload<real, C>(y, gY0 + o);
+            if (!SPLIT || (simple && wmask == (1 << C) - 1)) {
+                if (A.last) {
+                    real y[C];
+                    vload<real, C>(y, gY0 + o);
 #pragma unroll
-                for (int q = 0; q < C; q++) y[q] += outK[q];
-                vstore<real, C>(gY0 + o, y);
+                    for (int q = 0; q < C; q++) y[q] += outK[q];
+                    vstore<real, C>(gY0 + o, y);
+                } else {
+                    vstore<real, C>(gocur + o, outK);
+                    vstore<real, C>(goprev + o, u[K - 1][pmod(PH - K, 3)]);
+                }
             } else {
-                vstore<real, C>(gocur + o, outK);
-                vstore<real, C>(goprev + o, u[K - 1][pmod(PH - K, 3)]);
+#pragma unroll
+                for (int q = 0; q < C; q++)
+                    if (wmask >> q & 1) {
+                        if (A.last) {
+                            gY0[o + dq[q]] += outK[q];
+                        } else {
+                            gocur[o + dq[q]] = outK[q];
+                            goprev[o + dq[q]] = u[K - 1][pmod(PH - K, 3)][q];
+                        }
+                    }
             }
         }
     }
@@ -204,7 +233,7 @@ struct PipeWarp {
     }
 };
 
-template <typename real, int K>
+template <typename real, int K, bool SPLIT = false>
 __global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const __grid_constant__ BlkArgs<real, K> A, Tables<real> T, Geom G) {
     using P = PipeCfg<real, K>;
     constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, ROW = P::ROW;
@@ -213,7 +242,7 @@ __global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const _
     const int strip = blockIdx.x * PIPE_WARPS + wrp;
     if (strip >= A.nstrips) return;   // warp-uniform; the kernel has no block-level barrier
     const int r = blockIdx.z, nt = G.nt, np = G.np;
-    PipeWarp<real, K> W(A);
+    PipeWarp<real, K, SPLIT> W(A);
     W.nt = nt; W.pitch = G.pitch; W.lane = lane;
     W.ja = blockIdx.y * A.rows_per_seg;
     W.jb = min(W.ja + A.rows_per_seg, nt + 2);
@@ -221,7 +250,16 @@ __global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const _
     const int uc = strip * P::WOUT - P::HALO + lane * C;   // unwrapped first column of this lane
     int col = uc % np;
     if (col < 0) col += np;
-    W.wr = (lane * C >= P::HALO) && (lane * C < P::HALO + P::WOUT) && (uc < np);
+    W.simple = (col % C == 0) && (col + C <= np);
+    W.wmask = 0;
+#pragma unroll
+    for (int q = 0; q < C; q++) {
+        int cq = col + q;
+        if (cq >= np) cq -= np;
+        W.dq[q] = cq - col;
+        if ((lane * C >= P::HALO) && (lane * C < P::HALO + P::WOUT) && (uc + q < np)) W.wmask |= 1 << q;
+    }
+    if (!SPLIT) W.wmask = ((lane * C >= P::HALO) && (lane * C < P::HALO + P::WOUT) && (uc < np)) ? (1 << C) - 1 : 0;
     const size_t base = (size_t)r * G.rstride + col;
     W.gcur = A.cur + base; W.gprev = A.prev + base; W.gF = A.F + base;
     W.gocur = A.ocur + base; W.goprev = A.oprev + base; W.gY0 = A.Y0 + base;
@@ -265,18 +303,18 @@ __global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const _
 
 // ------------------------------------------------------------------ host side
 
-template <typename real, int K>
-int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
-                    real* ocur, real* oprev, bool last, int64_t* launches) {
+template <typename real, int K, bool SPLIT>
+int sts_pipe_launch_impl(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
+                         real* ocur, real* oprev, bool last, int64_t* launches) {
     using PC = PipeCfg<real, K>;
     static int slots = 0;   // CTAs resident on the whole device
     const int smem = PIPE_WARPS * PC::WARP_BYTES;
     if (!slots) {
-        cudaError_t e = cudaFuncSetAttribute(k_sts_pipe<real, K>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(k_sts_pipe<real, K, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return -1;
         int dev = 0, sms = 0, per_sm = 0;
         if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sts_pipe<real, K>, PIPE_WARPS * 32, smem) != cudaSuccess || per_sm < 1)
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sts_pipe<real, K, SPLIT>, PIPE_WARPS * 32, smem) != cudaSuccess || per_sm < 1)
             return -1;
         slots = sms * per_sm;
     }
@@ -306,10 +344,17 @@ int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& 
     k_sts_capseq<real, K><<<gc, 32 * STS_KMAX, 0, P.stream>>>(a, T, G, P.capseq);
     bool armed = false;
     P.prof_begin(P.user, &armed);
-    k_sts_pipe<real, K><<<g, PIPE_WARPS * 32, smem, P.stream>>>(a, T, G);
+    k_sts_pipe<real, K, SPLIT><<<g, PIPE_WARPS * 32, smem, P.stream>>>(a, T, G);
     P.prof_end(P.user, armed, K);
     *launches += 2;
     return 0;
+}
+
+template <typename real, int K>
+int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
+                    real* ocur, real* oprev, bool last, int64_t* launches) {
+    if (G.np % PipeCfg<real, K>::C == 0) return sts_pipe_launch_impl<real, K, false>(P, T, G, j0, cur, prev, ocur, oprev, last, launches);
+    return sts_pipe_launch_impl<real, K, true>(P, T, G, j0, cur, prev, ocur, oprev, last, launches);
 }
 
 // One STS step: stage 1, the (s-1) mod K remainder stages (pipe: one un-blocked stage if odd, then one shorter block;
@@ -320,8 +365,8 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
     const int K = P.kb, s = P.s;
     real* F = P.buf[0];
     real* b[4] = {P.buf[1], P.buf[2], P.buf[3], P.buf[4]};
-    // stage 1 and an odd remainder stage run one stage per launch in the 16-byte-vector kernel (n_phi is a multiple of the
-    // vector width whenever the blocked path is taken); its polar partials come in nbxv pieces per row
+    // stage 1 and an odd remainder stage run one stage per launch, in the 16-byte-vector kernel when n_phi is a multiple of
+    // the vector width (its polar partials come in nbxv pieces per row), else in the one-column-per-thread kernel
     constexpr int CV = 16 / (int)sizeof(real);
     const int nbxv = (G.np / CV + TX - 1) / TX;
     dim3 g1(nbxv, (G.nt + 2 + MAPV_RPT - 1) / MAPV_RPT, G.nr), gs(G.nbx, 2, G.nr);
@@ -331,7 +376,10 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
     StsArgs<real> a;
     a.F = F; a.Y0 = P.Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
     a.in = P.Y0; a.d2 = b[0]; a.part_in = P.part[0]; a.part_out = P.part[1]; a.a = (real)P.a[1];
-    k_sts_stage_mapv<real, 0, false><<<g1, TX, 0, P.stream>>>(a, M, T, G);
+    const bool vec = G.np % CV == 0;
+    dim3 g1s(G.nbx, (G.nt + 2 + RPT - 1) / RPT, G.nr);
+    if (vec) k_sts_stage_mapv<real, 0, false><<<g1, TX, 0, P.stream>>>(a, M, T, G);
+    else k_sts_stage<real, 0><<<g1s, TX, 0, P.stream>>>(a, T, G);
     M.nparts_in = nbxv;
     *launches += 2;
     const int rem = (s - 1) % K;
@@ -346,7 +394,8 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
         a.in = b[icur]; a.d2 = b[iprev]; a.part_in = P.part[pin]; a.part_out = P.part[pin ^ 1];
         a.mu = (real)P.mu[j]; a.nu = (real)P.nu[j]; a.a = (real)P.a[j]; a.g = (real)P.g[j];
         a.use_d2 = has_prev;
-        k_sts_stage_mapv<real, 1, false><<<g1, TX, 0, P.stream>>>(a, M, T, G);
+        if (vec) k_sts_stage_mapv<real, 1, false><<<g1, TX, 0, P.stream>>>(a, M, T, G);
+        else k_sts_stage<real, 1><<<g1s, TX, 0, P.stream>>>(a, T, G);
         *launches += 1;
         int t = icur; icur = iprev; iprev = t;
         has_prev = true;

@@ -134,6 +134,17 @@ def diffusivity_map(w: Workload, r: int):
     return float(w.params[r][0]) * (1.0 + 0.3 * np.sin(thf) * np.cos(phf))
 
 
+def soccer_ball_full(n_theta, n_phi):
+    """The paper's validation field, Eq. 19: Y_6^0 + sqrt(14/11) Y_6^5 (real harmonics), scaled to
+    max |.| = 1, on the internal grid incl. the two pole rows: numpy float64 [n_theta+2][n_phi].  An l = 6 eigenfunction
+    of the surface Laplacian: under diffusion alone it decays as exp(-42 nu t)."""
+    from scipy.special import sph_harm_y
+    th = (np.arange(n_theta + 2) * math.pi / (n_theta + 1))[:, None]
+    ph = (np.arange(n_phi) * 2.0 * math.pi / n_phi)[None, :]
+    u = sph_harm_y(6, 0, th, ph).real + math.sqrt(14.0 / 11.0) * math.sqrt(2.0) * sph_harm_y(6, 5, th, ph).real
+    return np.ascontiguousarray(u / np.abs(u).max())
+
+
 def colatitudes(n_theta, device="cpu"):
     return torch.arange(1, n_theta + 1, dtype=torch.float64, device=device) * (math.pi / (n_theta + 1))
 

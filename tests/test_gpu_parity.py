@@ -139,12 +139,15 @@ def test_small_ragged_multi_realization(dtype, case):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("block", [2, 4, 6, 8])
 @pytest.mark.parametrize("s_forced", [0, 41])
-def test_sts_block_sizes_ragged(dtype, block, s_forced):
+@pytest.mark.parametrize("nphi", [328, 327, 329, 330])
+def test_sts_block_sizes_ragged(dtype, block, s_forced, nphi):
     """Every temporal-blocking depth K of the STS kernel (hft_options.sts_block) on a grid with ragged strips, a
     phi seam inside a strip and theta segments: s = 42 -> (s-1) mod K remainder stages un-blocked; s_forced = 41
-    -> (s-1) mod 8 = 0, the block that starts from delta_0 = 0."""
+    -> (s-1) mod 8 = 0, the block that starts from delta_0 = 0.  n_phi = 327, 329, 330 are not multiples of the
+    16-byte vector width (2 doubles / 4 floats): the lanes behind the seam move their columns one by one, a vector
+    may straddle the seam (the paper's own grids have odd n_phi in this API: 512 x 1024 files = 510 x 1023 cells)."""
     H = hft()
-    w = wl.scaled(wl.config(3), 150, 328, n_real=2)
+    w = wl.scaled(wl.config(3), 150, nphi, n_real=2)
     ctx, o = make_pair(w, dtype, adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKG2, sts_block=block, sts_stages=s_forced)
     _, dif = o.stable_dt()
     dt = 250.0 * dif
@@ -589,6 +592,31 @@ def test_diffusivity_map_theta_phi(dtype, case, nphi):
     with pytest.raises(H.HftError):
         c.set_diffusivity_map(0, np.ones((17, 32)))
     c.close()
+
+
+@pytest.mark.parametrize("scheme,name", [("rkl2", "hh_rkl2_diffusion"), ("rkg2", "hh_rkg2_diffusion")])
+@pytest.mark.parametrize("nphi", [1023, 1024])
+def test_paper_printed_hh_errors_on_the_gpu(scheme, name, nphi):
+    """diffusion only, Eq. 19 field, 512x1024 file grid (= 510 x 1023 regular cells), nu = 500 km^2/s, ONE 672 h
+    super-time step: HH (Eq. 18) against the analytic decay = 8.0e-5 (RKL2), 6.3e-5 (RKG2).  The CUDA path reproduces the
+    two printed digits on the paper's grid (odd n_phi: one-column kernels, one launch per stage) and, within 2 %, on
+    510 x 1024 (temporally blocked kernel, ~4.7 k stages in one step)."""
+    from helpers import golden, grid, hh_metric, soccer_ball
+    H = hft()
+    nt = 510
+    th, ph, _, _ = grid(nt, nphi)
+    u = soccer_ball(th, ph)
+    ctx = H.Context(nt, nphi, [[500.0, 0, 0, 0, 0, 0, 0]], dtype="f64", adv_flux=H.ADV_OFF,
+                    diff_time=H.DIFF_RKL2 if scheme == "rkl2" else H.DIFF_RKG2)
+    ctx.set_full(0, torch.from_numpy(np.ascontiguousarray(u)).cuda())
+    s = ctx.sts_stage_count(672.0)
+    assert 3500 < s < 5200
+    ctx.step(1, 672.0)
+    got = ctx.get_full(0).cpu().numpy()
+    exact = u * math.exp(-42.0 * 500.0 * golden("km2_s_to_rs2_hr") * 672.0)
+    hh = hh_metric(got[1:-1], exact[1:-1])
+    assert abs(hh / golden(name) - 1) < 0.02, (name, nphi, hh)
+    ctx.close()
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
