@@ -73,7 +73,7 @@ struct BlkArgs {
 template <typename real, int K>
 __global__ void __launch_bounds__(32 * STS_KMAX) k_sts_capseq(BlkArgs<real, K> A, Tables<real> T, Geom G, double* capseq) {
     constexpr int C = 16 / (int)sizeof(real);
-    __shared__ double m0[K + 1], mp[K + 1], mF[K + 1];
+    __shared__ double m0[K + 1], mp[K + 1], mF[K + 1], s_out[K + 1], s_in[K + 1];
     const int pole = blockIdx.x, r = blockIdx.y;
     const int lane = threadIdx.x & 31, i = (threadIdx.x >> 5) + 1;
     const size_t base = (size_t)r * G.rstride;
@@ -82,17 +82,12 @@ __global__ void __launch_bounds__(32 * STS_KMAX) k_sts_capseq(BlkArgs<real, K> A
         const size_t off = base + (size_t)rowidx(i) * G.pitch;
         const bool lower = i < K;   // prev and F are needed on rows 1..K-1 only
         double a = 0.0, b = 0.0, c = 0.0;
-        for (int k = lane * C; k < G.np; k += 32 * C) {
-            if (k + C > G.np) {   // n_phi not a multiple of C: the last columns of the row one by one
-                for (int kk = k; kk < G.np; kk++) {
-                    a += (double)A.cur[off + kk];
-                    if (lower) {
-                        if (A.has_prev) b += (double)A.prev[off + kk];
-                        c += (double)A.F[off + kk];
-                    }
-                }
-                break;
-            }
+        // whole 16-byte vectors, four iterations of independent loads in flight per lane (one dependent L2 round trip per
+        // iteration made this kernel 10-16 us: a quarter of a step on a single 512x1024 realization)
+        const int nvec = G.np / C;   // whole vectors in a row
+#pragma unroll 4
+        for (int iv = lane; iv < nvec; iv += 32) {
+            const int k = iv * C;
             real v[C];
             vload<real, C>(v, A.cur + off + k);
 #pragma unroll
@@ -108,17 +103,32 @@ __global__ void __launch_bounds__(32 * STS_KMAX) k_sts_capseq(BlkArgs<real, K> A
                 for (int q = 0; q < C; q++) c += (double)v[q];
             }
         }
+        // n_phi not a multiple of C: the last columns of the row one by one
+        for (int kk = nvec * C + lane; kk < G.np; kk += 32) {
+            a += (double)A.cur[off + kk];
+            if (lower) {
+                if (A.has_prev) b += (double)A.prev[off + kk];
+                c += (double)A.F[off + kk];
+            }
+        }
         a = warp_sum(a); b = warp_sum(b); c = warp_sum(c);
         if (lane == 0) { m0[i] = a / (double)G.np; mp[i] = b / (double)G.np; mF[i] = c / (double)G.np; }
     }
-    __syncthreads();
-    if (threadIdx.x != 0) return;
-    const size_t capoff = base + (size_t)rowidx(0) * G.pitch;
-    m0[0] = (double)A.cur[capoff];
-    mp[0] = A.has_prev ? (double)A.prev[capoff] : 0.0;
-    mF[0] = (double)A.F[capoff];
     const real* cp = T.cp + (size_t)r * (G.nt + 2);
     const real* cm = T.cm + (size_t)r * (G.nt + 2);
+    if (lane == 1 && i <= K) {   // theta coefficients of row i: towards the equator / towards the pole
+        const int j = rowidx(i);
+        s_out[i] = (double)(pole == 0 ? cp[j] : cm[j]);
+        s_in[i] = (double)(pole == 0 ? cm[j] : cp[j]);
+    }
+    if (threadIdx.x == 2) {      // the cap itself
+        const size_t capoff = base + (size_t)rowidx(0) * G.pitch;
+        m0[0] = (double)A.cur[capoff];
+        mp[0] = A.has_prev ? (double)A.prev[capoff] : 0.0;
+        mF[0] = (double)A.F[capoff];
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
     const double capc = T.capc[2 * r + pole] * (double)G.np;
     double lc[K + 1], lp[K + 1], ln[K + 1];  // current level, previous level, new level
     for (int d = 0; d <= K; d++) { lc[d] = m0[d]; lp[d] = mp[d]; }
@@ -126,9 +136,7 @@ __global__ void __launch_bounds__(32 * STS_KMAX) k_sts_capseq(BlkArgs<real, K> A
         const double mu = (double)A.mu[s - 1], nu = (double)A.nu[s - 1], a = (double)A.a[s - 1], g = (double)A.g[s - 1];
         ln[0] = mu * lc[0] + nu * lp[0] + a * (capc * (lc[1] - lc[0])) + g * mF[0];
         for (int d = 1; d <= K - s; d++) {
-            const int j = rowidx(d);
-            const double c_out = (double)(pole == 0 ? cp[j] : cm[j]);  // towards the equator
-            const double c_in = (double)(pole == 0 ? cm[j] : cp[j]);   // towards the pole
+            const double c_out = s_out[d], c_in = s_in[d];
             ln[d] = mu * lc[d] + nu * lp[d] + a * (c_out * (lc[d + 1] - lc[d]) - c_in * (lc[d] - lc[d - 1])) + g * mF[d];
         }
         capseq[((size_t)r * 2 + pole) * K + (s - 1)] = ln[0];
