@@ -1,4 +1,5 @@
-"""Build the C-ABI CUDA library in-tree: csrc/*.cu -> paper_2501_06377_b200/libhft.so (sm_100a only).
+"""Build the C-ABI CUDA library in-tree: csrc/*.cu (three translation units, compiled in parallel) ->
+paper_2501_06377_b200/libhft.so (sm_100a only).
 
     python -m paper_2501_06377_b200.build [--force] [--verbose]
 
@@ -31,12 +32,21 @@ def up_to_date():
 def build(force=False, verbose=False):
     if not force and up_to_date():
         return LIB
-    cmd = [NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-           "-shared", "-Xcompiler", "-fPIC", "-I", INCLUDE, "-o", LIB + ".tmp"]
+    flags = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC", "-I", INCLUDE]
     if verbose:
-        cmd += ["-Xptxas", "-v"]
-    cmd += sources()
-    subprocess.run(cmd, check=True)
+        flags += ["-Xptxas", "-v"]
+    # one nvcc -c per translation unit, in parallel, then one link
+    objdir = os.path.join(HERE, "build_obj")
+    os.makedirs(objdir, exist_ok=True)
+    procs = []
+    for src in sources():
+        obj = os.path.join(objdir, os.path.basename(src)[:-3] + ".o")
+        procs.append((src, obj, subprocess.Popen([NVCC] + flags + ["-c", src, "-o", obj])))
+    for src, obj, p in procs:
+        if p.wait() != 0:
+            raise subprocess.CalledProcessError(p.returncode, [NVCC, "-c", src])
+    subprocess.run([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", LIB + ".tmp"] + [obj for _, obj, _ in procs],
+                   check=True)
     os.replace(LIB + ".tmp", LIB)
     return LIB
 

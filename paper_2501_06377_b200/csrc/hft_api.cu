@@ -20,6 +20,11 @@
 #include "hft_sts_pipe.cuh"
 #include "hft_sts_map.cuh"
 
+// The temporally blocked STS step (all k_sts_pipe / k_sts_blocked instantiations) is compiled in its own translation units,
+// one per precision (hft_sts_f64.cu, hft_sts_f32.cu), so that the three units build in parallel.
+extern template int hft::sts_blocked_step<double>(hft::StsBlockedPlan<double>&, hft::Tables<double>&, const hft::Geom&, int, int64_t*);
+extern template int hft::sts_blocked_step<float>(hft::StsBlockedPlan<float>&, hft::Tables<float>&, const hft::Geom&, int, int64_t*);
+
 using namespace hft;
 
 namespace {
