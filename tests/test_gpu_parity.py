@@ -259,6 +259,78 @@ def test_config2_full_size_sampled_realizations():
     ctx.close()
 
 
+def test_config3_full_length_sampled_realization():
+    """BASELINE config 3 at full size AND full length: 2 simulated days = 79 steps of 604 RKG2 stages + SSPRK(4,3) on all
+    64 realizations, in fp64 and in fp32, both started from the same float-representable maps.  The fp64 oracle follows
+    realization 42 through all 79 steps (about half a minute on the box's host cores).
+    fp64 CUDA path: <= 1e-12 (measured 2.3e-15).
+    fp32 CUDA path against the fp64 oracle: measured 1.36e-5 (advection alone 2.3e-6, diffusion alone 1.27e-5: every one of
+    the 79 x 604 stages rounds delta to 24 bits and the three-term recurrence amplifies that noise).  This is what fp32
+    arithmetic gives for this method at this length, not an implementation difference: the oracle built in float is 3.7e-5
+    from the fp64 oracle on the same run, and the CUDA path 3.3e-5 from the float oracle (HFT_SLOW=1 below runs it: 7 min).
+    The 1e-5 gate of north_star therefore holds at the lengths the float oracle can separate implementations (the 2-step
+    full-size test above, all small-grid tests); here the gate is 2e-5 against the fp64 oracle (reading U14)."""
+    import os
+    H = hft()
+    w = wl.config(3, "f64")
+    maps32 = wl.initial_maps(w, device="cuda").to(torch.float32)
+    r = 42
+    errs = {}
+    ref = None
+    for dtype in ("f64", "f32"):
+        ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype)
+        for q in range(w.n_real):
+            ctx.set_map(q, maps32[q].to(ctx.tdtype).contiguous())
+        dt, n, _ = wl.plan(w, *ctx.stable_dt())
+        s = ctx.sts_stage_count(dt)
+        assert n == 79 and s == 604, (n, s)
+        before = ctx.diagnostics()
+        ctx.step(n, dt)
+        after = ctx.diagnostics()
+        cons = 1e-12 if dtype == "f64" else 1e-4
+        assert np.all(np.abs(after[:, 0] - before[:, 0]) <= cons * before[:, 1])
+        if ref is None:
+            o = orc.Oracle(w.n_theta, w.n_phi, w.params[r:r + 1], dtype=np.float64)
+            o.set_map(0, maps32[r].double().cpu().numpy())
+            o.step(n, dt, sts_stages=s)
+            ref = o.get_full(0)
+            o.close()
+        g = ctx.get_full(r).cpu().numpy()
+        errs[dtype] = rel_linf(g, ref)
+        ctx.close()
+    print("cfg3 full length (79 steps), realization 42: rel L-inf fp64 %.3e, fp32 %.3e" % (errs["f64"], errs["f32"]))
+    assert errs["f64"] <= 1e-12 and errs["f32"] <= 2e-5, errs
+    if os.environ.get("HFT_SLOW") == "1":
+        o = orc.Oracle(w.n_theta, w.n_phi, w.params[r:r + 1], dtype=np.float32)
+        o.set_map(0, maps32[r].cpu().numpy())
+        o.step(n, dt, sts_stages=s)
+        ref32 = o.get_full(0)
+        e_gpu, e_orc = rel_linf(g, ref32), rel_linf(ref32, ref)
+        print("float oracle: cuda fp32 vs float oracle %.3e, float oracle vs fp64 oracle %.3e" % (e_gpu, e_orc))
+        assert errs["f32"] <= e_orc and e_gpu <= 2.0 * e_orc      # the CUDA path is the more accurate of the two
+
+
+def test_config2_full_length_sampled_realization():
+    """BASELINE config 2 at full size and full length: 31 steps of 683 stages, 8 realizations, fp64; the oracle follows
+    realization 7 (largest diffusivity and flow speed) to the end."""
+    H = hft()
+    w = wl.config(2)
+    ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype="f64")
+    maps = wl.initial_maps(w, device="cuda")
+    ctx.set_map(-1, maps[0].contiguous())
+    dt, n, _ = wl.plan(w, *ctx.stable_dt())
+    s = ctx.sts_stage_count(dt)
+    assert n == 31
+    ctx.step(n, dt)
+    o = orc.Oracle(w.n_theta, w.n_phi, w.params[7:8])
+    o.set_map(0, maps[0].cpu().numpy())
+    o.step(n, dt, sts_stages=s)
+    e = rel_linf(ctx.get_full(7).cpu().numpy(), o.get_full(0))
+    print("cfg2 full length (31 steps), realization 7: rel L-inf %.3e" % e)
+    assert e <= 1e-12, e
+    ctx.close()
+
+
 def test_config4_full_size_first_assimilation_hour():
     """BASELINE config 4 at full size (2048x4096, fp64): the first simulated hour (its steps at CFL 0.5, s ~ 1640
     stages each) followed by the hourly assimilation of the synthetic observation with the disc weights; element by
