@@ -304,7 +304,6 @@ def main():
                           "h2d_bytes_per_step": host_in.numel() * host_in.element_size(),
                           "d2h_bytes_per_step": host_out.numel() * host_out.element_size(), "steps": n_e2e}
             assert torch.isfinite(host_out).all()
-        kb_used = os.environ.get("HFT_STS_BLOCK_USED")
         ctx.close()
         return res
 
