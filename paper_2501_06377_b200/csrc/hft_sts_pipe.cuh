@@ -35,21 +35,39 @@ namespace hft {
 
 __host__ __device__ constexpr int pmod(int a, int m) { return ((a % m) + m) % m; }
 
-#ifndef HFT_PIPE_WARPS
-#define HFT_PIPE_WARPS 4
+// CTA shape per precision (overridable for experiments): warps (= strips) per CTA -- warps never synchronise with each
+// other -- and the resident CTAs per SM the register budget is set for.  fp64: 4 x 2 with the long body (206 registers);
+// 12 warps per SM with the short body need 4 % fewer cycles but draw more power, and under the 1000 W cap the clock drops by
+// more than that (122.5 against 120.7 ms per cfg 3 step).  fp32 (not power-limited): 4 x 3 with the short body at 168
+// registers, 12 warps per SM: 59.7 -> 53.6 ms per step (3 x 3: 56.5, 2 x 5: 54.0, 2 x 6: 53.9, 3 x 4: 56.8).
+template <typename real> struct PipeShape {
+#ifdef HFT_PIPE_WARPS
+    static constexpr int WARPS = HFT_PIPE_WARPS, MINB = HFT_PIPE_MINB;
+#else
+    static constexpr int WARPS = 4, MINB = sizeof(real) == 4 ? 3 : 2;
 #endif
-#ifndef HFT_PIPE_MINB
-#define HFT_PIPE_MINB 2
-#endif
-constexpr int PIPE_WARPS = HFT_PIPE_WARPS;   // warps (= strips) per CTA; warps never synchronise with each other
-constexpr int PIPE_MINB = HFT_PIPE_MINB;     // resident CTAs per SM the register budget is set for
+};
 
 template <typename real, int K>
 struct PipeCfg {
     static constexpr int C = 16 / (int)sizeof(real);          // columns per lane
     static constexpr int NF = K + 1;                          // F rows alive in registers
-    static constexpr int U = (NF % 3 == 0) ? NF : 3 * NF;     // row-steps per unrolled macro-iteration
-    static constexpr int D = NF;                              // ring depth in rows (divides U)
+    // Two loop bodies.  SHIFTF = false (fp64): the F slots rotate by unrolling lcm(3, K+1) = 9 row-steps, no register is
+    // ever moved.  SHIFTF = true (fp32): the body is 3 row-steps (the period of the level windows); the F rows live in a
+    // sliding window of K+3 register rows that is shifted down by 3 rows after every body (K short register moves per 3
+    // row-steps) and the slot of the shared-memory ring is a run-time offset -- a third of the straight-line code.  The
+    // long body stalls on instruction fetch (0.31 per issue in fp32, 0.19 in fp64); measured on cfg 3 the short body is
+    // 3 % faster in fp32 and 1.5 % slower in fp64 (where the extra moves and slot arithmetic cost more than the fetches).
+#if defined(HFT_PIPE_LONG_BODY)
+    static constexpr bool SHIFTF = false;
+#elif defined(HFT_PIPE_SHORT_BODY)
+    static constexpr bool SHIFTF = true;
+#else
+    static constexpr bool SHIFTF = sizeof(real) == 4;
+#endif
+    static constexpr int U = SHIFTF ? 3 : ((NF % 3 == 0) ? NF : 3 * NF);   // row-steps per unrolled macro-iteration
+    static constexpr int NFW = SHIFTF ? K + 3 : NF;
+    static constexpr int D = NF;                              // ring depth in rows
     static constexpr int DP = D - 2;                          // prefetch distance in rows
     static constexpr int ROW = 32 * C;                        // reals per ring row (512 B)
     static constexpr int NCS = 3;                             // coefficient ring slots (divides U)
@@ -84,10 +102,12 @@ template <typename real, int K, bool SPLIT>
 struct PipeWarp {
     using P = PipeCfg<real, K>;
     static constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, NF = P::NF, ROW = P::ROW, NCS = P::NCS;
+    static constexpr bool SHIFTF = P::SHIFTF;
 
     // registers
     real u[K][3][C];   // level l (0..K-1), row rho in slot rho mod 3 (relative to the macro-iteration origin)
-    real f[NF][C];     // F row rho in slot rho mod NF
+    real f[P::NFW][C]; // F row rho in slot rho mod NF; SHIFTF: row tb + x of the current body in slot x + K, x = -K..2
+    int rb;            // SHIFTF: shared-memory ring slot of row tb (0, 3, 6, .. < D)
     // per-warp constants
     const BlkArgs<real, K>& A;
     const real *gcur, *gprev, *gF;   // this lane's column of row 0 of the three inputs
@@ -143,12 +163,20 @@ struct PipeWarp {
     __device__ __forceinline__ void rowstep(int t) {
         cp_async_wait<DP - 1>();   // this lane's copies of row t have landed
         __syncwarp();              // the products written during the previous row-step are visible
-        constexpr int sl = PH % D;
+        int sl, slm1, slpf;        // ring slots of rows t, t-1 and t+DP
+        if constexpr (SHIFTF) {
+            sl = rb + PH; if (sl >= D) sl -= D;
+            slm1 = sl - 1; if (slm1 < 0) slm1 += D;
+            slpf = sl + DP; if (slpf >= D) slpf -= D;
+        } else {
+            sl = PH % D; slm1 = pmod(PH - 1, D); slpf = (PH + DP) % D;
+        }
+        constexpr int fnew = SHIFTF ? PH + K : PH % NF;
         vload<real, C>(u[0][PH % 3], s_cur + sl * ROW);
-        vload<real, C>(f[PH % NF], s_F + sl * ROW);
+        vload<real, C>(f[fnew], s_F + sl * ROW);
         real pl1[C];               // delta_{j0-1} row t-1: the "two levels back" operand of level 1
-        vload<real, C>(pl1, s_prev + pmod(PH - 1, D) * ROW);
-        prefetch(t + DP, (PH + DP) % D);   // overwrites the slot of row t-2, last read one row-step ago
+        vload<real, C>(pl1, s_prev + slm1 * ROW);
+        prefetch(t + DP, slpf);    // overwrites the slot of row t-2, last read one row-step ago
         const real raw_next = s_raw[sl * 32];   // this lane's own copy, arrived with the group of row t
         const real* cfs = s_coef + (PH % NCS) * (K * 4);
         real outK[C];
@@ -170,7 +198,7 @@ struct PipeWarp {
                 const real w = (q == 0) ? west : u[l - 1][sC][q > 0 ? q - 1 : 0];
                 const real e = (q == C - 1) ? east : u[l - 1][sC][q < C - 1 ? q + 1 : 0];
                 const real p2 = (l == 1) ? pl1[q] : u[l >= 2 ? l - 2 : 0][sC][q];   // level l-2 row t-l is ITS oldest: slot (PH-(l-2)-2) mod 3 = sC
-                real acc = gc * f[pmod(PH - l, NF)][q];
+                real acc = gc * f[SHIFTF ? PH - l + K : pmod(PH - l, NF)][q];
                 acc = fma_r(nuc, p2, acc);
                 acc = fma_r(Af, e + w, acc);
                 acc = fma_r(Ac, c, acc);
@@ -230,15 +258,24 @@ struct PipeWarp {
     __device__ __forceinline__ void macro(int tb) {
         rowstep<PH, GEN>(tb + PH);
         if constexpr (PH + 1 < U) macro<PH + 1, GEN>(tb);
+        else if constexpr (SHIFTF) {   // slide the F window down by the 3 rows of this body
+#pragma unroll
+            for (int i = 0; i < K; i++)
+#pragma unroll
+                for (int q = 0; q < C; q++) f[i][q] = f[i + 3][q];
+            rb += 3;
+            if (rb >= D) rb -= D;
+        }
     }
 };
 
 template <typename real, int K, bool SPLIT = false>
-__global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const __grid_constant__ BlkArgs<real, K> A, Tables<real> T, Geom G) {
+__global__ void __launch_bounds__(PipeShape<real>::WARPS * 32, PipeShape<real>::MINB) k_sts_pipe(const __grid_constant__ BlkArgs<real, K> A, Tables<real> T, Geom G) {
     using P = PipeCfg<real, K>;
     constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, ROW = P::ROW;
     extern __shared__ __align__(128) unsigned char pipe_smem[];
     const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
+    constexpr int PIPE_WARPS = PipeShape<real>::WARPS;
     const int strip = blockIdx.x * PIPE_WARPS + wrp;
     if (strip >= A.nstrips) return;   // warp-uniform; the kernel has no block-level barrier
     const int r = blockIdx.z, nt = G.nt, np = G.np;
@@ -285,9 +322,10 @@ __global__ void __launch_bounds__(PIPE_WARPS * 32, PIPE_MINB) k_sts_pipe(const _
 #pragma unroll
             for (int q = 0; q < C; q++) W.u[l][i][q] = (real)0;
 #pragma unroll
-    for (int i = 0; i < P::NF; i++)
+    for (int i = 0; i < P::NFW; i++)
 #pragma unroll
         for (int q = 0; q < C; q++) W.f[i][q] = (real)0;
+    W.rb = 0;
     // clear this warp's shared memory (the ring slot of "row t0-1" is read before it is ever written)
     for (int i = lane; i < P::WARP_REALS; i += 32) ws[i] = (real)0;
     __syncwarp();
@@ -308,6 +346,7 @@ int sts_pipe_launch_impl(const StsBlockedPlan<real>& P, Tables<real>& T, const G
                          real* ocur, real* oprev, bool last, int64_t* launches) {
     using PC = PipeCfg<real, K>;
     static int slots = 0;   // CTAs resident on the whole device
+    constexpr int PIPE_WARPS = PipeShape<real>::WARPS;
     const int smem = PIPE_WARPS * PC::WARP_BYTES;
     if (!slots) {
         cudaError_t e = cudaFuncSetAttribute(k_sts_pipe<real, K, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
