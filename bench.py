@@ -31,7 +31,7 @@ from paper_2501_06377_b200 import workloads as wl  # noqa: E402
 
 # per-launch DRAM bytes of k_sts_pipe<K = 8> from the committed ncu --set full captures (profiles/)
 NCU_TRAFFIC_BYTES = {(3, "f64"): 3.434079e9 + 2.121872e9,     # profiles/r01_final_cfg3.md
-                     (3, "f32"): 1.966273e9 + 1.046607e9}     # profiles/r01_pipe_cfg3_gen2.md
+                     (3, "f32"): 1.888619e9 + 1.046579e9}     # profiles/r01d_pipe_f32_3rowstep.md
 # FMA-class lane-operations per second measured on this pool's B200 with a register-only loop
 # (profiles/r01_pipe_cfg3_gen2.md): 64 DFMA / 128 FFMA lanes per clock per SM
 ALU_PEAK_FMA_PER_S = {"f64": 1.70e13, "f32": 3.53e13}
@@ -346,7 +346,7 @@ def main():
             # fp64 / fp32 FMA-class lane-operations / time against the FMA peak measured on this pool
             traffic = NCU_TRAFFIC_BYTES.get((args.config, args.dtype)) if stages_per_launch > 7 else None
             out["roofline"]["traffic"] = traffic
-            out["roofline"]["traffic_source"] = "ncu --set full dram__bytes_read+write.sum per launch (profiles/r01_final_cfg3.md, r01_pipe_cfg3_gen2.md)" if traffic else None
+            out["roofline"]["traffic_source"] = "ncu --set full dram__bytes_read+write.sum per launch (profiles/r01_final_cfg3.md, r01d_pipe_f32_3rowstep.md)" if traffic else None
             out["roofline"]["frac_of_blocked_traffic"] = 5 * field_bytes / sec / 1e9 / peak
             cols = 16 // wbytes * 32                           # columns per warp strip
             halo = 8                                           # K = 8 invalid columns per side
