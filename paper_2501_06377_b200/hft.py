@@ -97,7 +97,8 @@ class Context:
     """hft_create ... hft_destroy.  Maps are torch CUDA tensors [n_theta][n_phi] of the context dtype."""
 
     def __init__(self, n_theta, n_phi, params, dtype="f64", radius_cm=1.0, adv_flux=ADV_WENO3, adv_time=TIME_SSPRK43,
-                 diff_time=DIFF_RKG2, sts_stages=0, sts_block=0, rfe=0, strang=0, flow_attenuation=0, diffusivity_map=0, device="cuda:0", stream=None):
+                 diff_time=DIFF_RKG2, sts_stages=0, sts_block=0, rfe=0, strang=0, flow_attenuation=0, diffusivity_map=0, device="cuda:0", stream=None,
+                 workspace=None):
         if not torch.cuda.is_available():
             raise HftError("no CUDA device: the hot path has no CPU fallback")
         self.device = torch.device(device)
@@ -112,7 +113,12 @@ class Context:
             opt = hft_options(adv_flux, adv_time, diff_time, sts_stages, sts_block, int(rfe), int(strang), int(flow_attenuation),
                               int(diffusivity_map))
             nbytes = workspace_bytes(n_theta, n_phi, self.n_real, dtype, opt)
-            self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            if workspace is None:
+                workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            # caller-owned device memory (include/hft.h): a contiguous uint8 CUDA tensor of >= hft_workspace_bytes
+            assert workspace.is_cuda and workspace.dtype == torch.uint8 and workspace.is_contiguous()
+            self.workspace = workspace
+            nbytes = workspace.numel()
             grid = hft_grid(self.n_theta, self.n_phi, 1 if dtype == "f64" else 0, 0, float(radius_cm))
             pa = (hft_params * self.n_real)(*[hft_params(*row) for row in p])
             rc = _lib.hft_create(C.byref(grid), self.n_real, pa, C.byref(opt), C.c_void_p(self.workspace.data_ptr()),

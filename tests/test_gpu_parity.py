@@ -747,3 +747,55 @@ def test_degenerate_sizes_and_calls(dtype):
         ctx.close()
     with pytest.raises(H.HftError):
         H.Context(7, 8, [[0.0] * 7])
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("nt,nphi,opt", [(37, 256, {}), (37, 250, {}), (21, 131, {}), (40, 512, {"sts_block": 1}),
+                                          (37, 256, {"flow_attenuation": 1}), (37, 256, {"rfe": 1}), (24, 128, {"diffusivity_map": 1}),
+                                          (1024, 2048, {"n_real": 64})])
+def test_no_write_outside_caller_buffers(dtype, nt, nphi, opt):
+    """Every buffer is caller-owned (include/hft.h).  The workspace and the output of hft_get_map sit inside poisoned
+    allocations; after the whole path has run (set_map, advection + blocked / stage-by-stage STS with a remainder block,
+    both assimilation variants, both diagnostics, get_map) every guard byte on either side is untouched.  (compute-sanitizer
+    is not available on the GPU boxes; this is the bounds check that is.)"""
+    H = hft()
+    opt = dict(opt)
+    w = wl.scaled(wl.config(3), nt, nphi, n_real=opt.pop("n_real", 3))      # the last case is cfg 3 itself, as bench.py launches it
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    o = H.hft_options(H.ADV_WENO3, H.TIME_SSPRK43, H.DIFF_RKG2, 0, opt.get("sts_block", 0), opt.get("rfe", 0), 0,
+                      opt.get("flow_attenuation", 0), opt.get("diffusivity_map", 0))
+    need = H.workspace_bytes(nt, nphi, w.n_real, dtype, o)
+    G = 1 << 16
+    big = torch.full((G + need + G,), 0xA5, dtype=torch.uint8, device="cuda")
+    ctx = H.Context(nt, nphi, w.params, dtype=dtype, radius_cm=6.96e10, workspace=big[G:G + need], **opt)
+    if opt.get("flow_attenuation"):
+        ctx.set_attenuation(-1, 300.0)
+    if opt.get("diffusivity_map"):
+        th = (np.arange(nt + 1)[:, None] + 0.5) * math.pi / (nt + 1)
+        ph = (np.arange(nphi)[None, :] + 0.5) * 2 * math.pi / nphi
+        ctx.set_diffusivity_map(1, 400.0 * (1 + 0.3 * np.sin(th) * np.cos(ph)))
+    rng = torch.Generator(device="cuda").manual_seed(5)
+    maps = 50.0 * torch.randn((w.n_real, nt, nphi), generator=rng, device="cuda", dtype=tdt)
+    for r in range(w.n_real):
+        ctx.set_map(r, maps[r].contiguous())
+    if opt.get("rfe"):
+        ctx.set_rfe(1, 100e21, 0.3, 7)
+    dt, _, _ = wl.plan(w, *ctx.stable_dt())
+    for dt_k in (dt, 0.37 * dt):                      # two stage counts: different remainders of the K = 8 blocks
+        ctx.step(1 if nt >= 1024 else 2, dt_k)
+    obs = (maps + torch.randn(maps.shape, generator=rng, device="cuda", dtype=tdt)).contiguous()
+    wts = torch.rand(maps.shape, generator=rng, device="cuda", dtype=tdt).contiguous()
+    ctx.assimilate(obs, wts, 0)
+    ctx.assimilate(obs, wts, 1)
+    ctx.step(1, dt)
+    ctx.diagnostics()
+    ctx.diagnostics_ext(60.0)
+    cells = w.n_real * nt * nphi
+    outbig = torch.full((G + cells * maps.element_size() + G,), 0x5A, dtype=torch.uint8, device="cuda")
+    out = outbig[G:G + cells * maps.element_size()].view(tdt).view(w.n_real, nt, nphi)
+    ctx.get_map(-1, out)
+    torch.cuda.synchronize()
+    assert torch.isfinite(out).all()
+    assert bool((big[:G] == 0xA5).all()) and bool((big[G + need:] == 0xA5).all()), "write outside the workspace"
+    assert bool((outbig[:G] == 0x5A).all()) and bool((outbig[-G:] == 0x5A).all()), "write outside the get_map buffer"
+    ctx.close()
