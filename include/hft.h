@@ -13,7 +13,9 @@
  *
  * Conventions
  *   - Every function returns HFT_OK (0) or a negative hft_status; nothing throws across the ABI.
- *     hft_error_string() names a code.  A context is not thread-safe; there is no global state.
+ *     hft_error_string() names a code.  A context is not thread-safe.  The only process-wide state is internal and
+ *     guarded: per-device caches of kernel occupancy, and the owner of the constant-bank coefficient table of k_sts_upipe
+ *     (contexts that alternate on one device re-upload it, waiting for the device first).
  *   - "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.  All buffers are owned by the
  *     caller (e.g. allocated with PyTorch) and must stay valid until the stream work that uses them has
  *     completed; the context never frees them.  Calls enqueue work on the stream given to hft_create
@@ -77,6 +79,13 @@ typedef struct {
                                  6 more field arrays.  0 (default) = off */
     int32_t diffusivity_map;  /* 1 = reserve workspace for a spatially varying diffusivity nu(theta, phi) (Eq. 27-28, :438-460;
                                  1 more field array) and allow hft_set_diffusivity_map.  0 (default) = off */
+    int32_t f32_accumulate;   /* dtype fp32 only: 1 = the temporally blocked STS kernel keeps the state in fp32 in memory but does
+                                 the arithmetic of a block of stages in fp64 registers, rounding to fp32 only at the two stores per
+                                 block (the scheme integrated is Sec. 3.7.2 :470-476 unchanged).  0 (default) = fp32 arithmetic */
+    int32_t sts_kernel;       /* which temporally blocked kernel: 0 (default) = the library's choice; 1 = k_sts_pipe (per-realization
+                                 coefficient tables through shared memory; any batch); 2 = k_sts_upipe (one coefficient table
+                                 through the uniform datapath) whenever the batch shares one table up to the factor nu_r and it
+                                 fits the constant bank (n_theta <= 2048), else k_sts_pipe */
 } hft_options;
 
 /* Bytes of device workspace hft_create needs for this grid / batch (state + 5 stage arrays, + 6 with

@@ -10,6 +10,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <atomic>
+#include <cmath>
 #include <new>
 #include <string>
 #include <vector>
@@ -17,13 +19,13 @@
 #include "../../include/hft.h"
 #include "hft_kernels.cuh"
 #include "hft_sts_blocked.cuh"
-#include "hft_sts_pipe.cuh"
 #include "hft_sts_map.cuh"
+#include "hft_sts_step.cuh"
 
-// The temporally blocked STS step (all k_sts_pipe / k_sts_blocked instantiations) is compiled in its own translation units,
-// one per precision (hft_sts_f64.cu, hft_sts_f32.cu), so that the three units build in parallel.
-extern template int hft::sts_blocked_step<double>(hft::StsBlockedPlan<double>&, hft::Tables<double>&, const hft::Geom&, int, int64_t*);
-extern template int hft::sts_blocked_step<float>(hft::StsBlockedPlan<float>&, hft::Tables<float>&, const hft::Geom&, int, int64_t*);
+// The temporally blocked STS step (all k_sts_pipe / k_sts_upipe / k_sts_capseq instantiations) is compiled in its own
+// translation units (hft_sts_f64.cu, hft_sts_f32.cu, hft_sts_mixed.cu), so that the units build in parallel.
+extern template int hft::sts_blocked_step<double>(hft::StsBlockedPlan<double>&, hft::Tables<double>&, const hft::Geom&, int64_t*);
+extern template int hft::sts_blocked_step<float>(hft::StsBlockedPlan<float>&, hft::Tables<float>&, const hft::Geom&, int64_t*);
 
 using namespace hft;
 
@@ -40,7 +42,7 @@ constexpr int kProfEvents = 256;
 
 struct StsCoef {  // per-stage scalars of Sec. 3.7.2 schemes, index 0..s
     int scheme = 0, s = 0;
-    double dt = 0.0;
+    double dt = 0.0, w1 = 0.0;
     std::vector<double> mu, nu, a, g;  // mu_j, nu_j, mut_j*dt, mut_j*b_{j-1}*dt ; a[1] = mut_1*dt
 };
 
@@ -91,11 +93,21 @@ struct hft_ctx {
     double* d_diag = nullptr;                // [R][4]
     double* d_zmean = nullptr;               // blocked STS: zonal partial sums (see hft_sts_blocked.cuh)
     double* d_capseq = nullptr;              // blocked STS: cap values per stage
+    double* d_kappa = nullptr;               // k_sts_upipe: w1 dt nu_r per realization
     double* h_diag = nullptr;                // pinned
     double *d_extpart = nullptr, *d_ext = nullptr, *h_ext = nullptr;   // hft_diagnostics_ext, allocated on first use
     int64_t launches = 0;
-    int sts_pipe = 1;  // 1: k_sts_pipe, 0: first-generation k_sts_blocked (env HFT_STS_PIPE=0, for A/B timing)
     StsCoef coef;
+    // uniform-coefficient blocked kernel (hft_sts_upipe.cuh): the shared table sigma*(cm, cp, cf, -cd)/nu_r, its owner key
+    UPipePlan up;
+    std::vector<unsigned char> utab;   // [nt][32 bytes]
+    std::vector<double> nu_scale;      // [R]: nuf[r][f] = nu_scale[r] * nu_shape[f] when shape_common
+    std::vector<double> nu_shape;      // [nt+1]
+    bool shape_common = true;
+    uint64_t id = 0, tab_version = 1;  // tab_version: bumped whenever the diffusion tables change
+    uint64_t up_version = 0;           // tab_version/scheme/s/dt the table in `utab` was built for
+    int up_scheme = 0, up_s = 0;
+    double up_dt = 0.0;
     // sampled kernel timing
     int prof_which = 0;
     int prof_n = 0;
@@ -119,6 +131,12 @@ int cuda_fail(hft_ctx* c, cudaError_t e, const char* what) {
         if (e_ != cudaSuccess) return cuda_fail(c, e_, #call);    \
     } while (0)
 
+int check_launch(hft_ctx* c) {
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch");
+    return HFT_OK;
+}
+
 size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
 int pitch_for(int np, int dtype) {
@@ -128,7 +146,17 @@ int pitch_for(int np, int dtype) {
 
 bool valid_grid(const hft_grid* g) {
     return g && g->n_theta >= 8 && g->n_phi >= 8 && (g->dtype == 0 || g->dtype == 1) && g->reserved == 0 &&
-           g->n_theta <= (1 << 20) && g->n_phi <= (1 << 20) && g->radius_cm > 0.0;
+           g->n_theta + 2 <= 65535 && g->n_phi <= (1 << 20) && g->radius_cm > 0.0;   // rows ride in gridDim.y (16 bits)
+}
+
+bool valid_params(const hft_params* p, int n) {
+    for (int r = 0; r < n; r++) {
+        const double v[7] = {p[r].eta_km2_s, p[r].d0, p[r].d2, p[r].d4, p[r].m1, p[r].m3, p[r].m5};
+        for (double x : v)
+            if (!std::isfinite(x)) return false;
+        if (p[r].eta_km2_s < 0.0) return false;
+    }
+    return true;
 }
 
 hft_options default_options() {
@@ -152,6 +180,8 @@ bool valid_options(const hft_options* o) {
     if (o->rfe != 0 && o->rfe != 1) return false;
     if (o->diffusivity_map != 0 && o->diffusivity_map != 1) return false;
     if (o->sts_block < 0 || o->sts_block > STS_KMAX || (o->sts_block > 1 && (o->sts_block & 1))) return false;
+    if (o->f32_accumulate != 0 && o->f32_accumulate != 1) return false;
+    if (o->sts_kernel < 0 || o->sts_kernel > 2) return false;
     return true;
 }
 
@@ -336,6 +366,7 @@ void build_sts_coef(StsCoef& K, int scheme, int s, double dt) {
     };
     const double S = (double)s;
     const double w1 = scheme == 2 ? 4.0 / (S * S + S - 2.0) : 6.0 / ((S - 1.0) * (S + 4.0));
+    K.w1 = w1;
     K.a[1] = b(1) * w1 * dt;
     for (int j = 2; j <= s; j++) {
         const double x = (double)j;
@@ -347,6 +378,53 @@ void build_sts_coef(StsCoef& K, int scheme, int s, double dt) {
         K.a[j] = mut * dt;
         K.g[j] = mut * b(j - 1) * dt;
     }
+}
+
+// The shared coefficient table of k_sts_upipe (hft_sts_upipe.cuh): (cm, cp, cf, -cd)_j / nu_r for rows 1..nt, in the
+// arithmetic type of the kernel (fp64, or duplicated fp32 pairs), and kappa_r = w1 dt nu_r.  Usable when every
+// realization's diffusivity is nu_scale[r] * nu_shape(theta) and the table fits the constant bank; rebuilt when
+// (tables, scheme, s, dt) change.
+std::atomic<uint64_t> g_utab_key{1};
+
+int prepare_upipe(hft_ctx* c, int scheme, int s, double dt) {
+    UPipePlan& up = c->up;
+    if (c->up_version == c->tab_version && c->up_scheme == scheme && c->up_s == s && c->up_dt == dt) return HFT_OK;
+    c->up_version = c->tab_version; c->up_scheme = scheme; c->up_s = s; c->up_dt = dt;
+    up.ok = false;
+    const int nt = c->G.nt;
+    // default (0): k_sts_upipe only where it is the faster or the only kernel: fp32 storage with fp64 arithmetic
+    const bool want = c->opt.sts_kernel == 2 || (c->opt.sts_kernel == 0 && !c->fp64() && c->opt.f32_accumulate != 0);
+    if (!want || !c->shape_common || nt > UTAB_MAX_ROWS) return HFT_OK;
+    for (int r = 0; r < c->nr; r++)
+        if (!(c->nu_scale[r] >= 0.0) || !std::isfinite(c->nu_scale[r])) return HFT_OK;
+    const bool dbl = c->fp64() || c->opt.f32_accumulate != 0;
+    up.mixed = !c->fp64() && c->opt.f32_accumulate != 0;
+    c->utab.assign((size_t)nt * UTAB_ROW_BYTES, 0);
+    for (int j = 1; j <= nt; j++) {
+        const double cm = c->nu_shape[j - 1] * c->sth[j - 1] / (c->st[j] * c->dth * c->dth);
+        const double cp = c->nu_shape[j] * c->sth[j] / (c->st[j] * c->dth * c->dth);
+        const double cf = 0.5 * (c->nu_shape[j] + c->nu_shape[j - 1]) / (c->st[j] * c->st[j] * c->dph * c->dph);
+        unsigned char* row = &c->utab[(size_t)(j - 1) * UTAB_ROW_BYTES];
+        if (dbl) {
+            double v[4] = {cm, cp, cf, 0.0};
+            v[3] = -(v[0] + v[1] + 2.0 * v[2]);
+            memcpy(row, v, sizeof(v));
+        } else {
+            const float a = (float)cm, b = (float)cp, f = (float)cf;
+            const float d = -(float)((double)a + (double)b + 2.0 * (double)f);
+            const float v[8] = {a, a, b, b, f, f, d, d};
+            memcpy(row, v, sizeof(v));
+        }
+    }
+    std::vector<double> kap(c->nr);
+    for (int r = 0; r < c->nr; r++) kap[r] = c->coef.w1 * dt * c->nu_scale[r];
+    CK(cudaStreamSynchronize(c->stream));   // d_kappa may still be read by enqueued work
+    CK(cudaMemcpy(c->d_kappa, kap.data(), (size_t)c->nr * sizeof(double), cudaMemcpyHostToDevice));
+    up.h_table = c->utab.data();
+    up.d_kappa = c->d_kappa;
+    up.key = g_utab_key.fetch_add(1);
+    up.ok = true;
+    return HFT_OK;
 }
 
 // ---------------------------------------------------------------- launch helpers
@@ -458,8 +536,7 @@ int diffuse_stagewise(hft_ctx* c, double dt, int s) {
     real* F = arr_of<real>(c, (is + 1) % kNumArrays);
     real* da = arr_of<real>(c, (is + 2) % kNumArrays);
     real* db = arr_of<real>(c, (is + 3) % kNumArrays);
-    static const bool force_scalar = getenv("HFT_MAP_SCALAR") != nullptr;   // A/B timing of the one-column-per-thread kernel
-    const bool vec = !force_scalar && G.np % (16 / (int)sizeof(real)) == 0;
+    const bool vec = G.np % (16 / (int)sizeof(real)) == 0;
     MapArgs<real> M;
     M.NU = (const real*)c->numap; M.capw = c->d_capw; M.capP = c->P * c->dph / c->dth; M.rdth = (real)(1.0 / c->dth);
     M.nparts_in = G.nbx;
@@ -520,7 +597,7 @@ int rfe_make_map(hft_ctx* c, real* S, uint32_t map) {
     k_flux_finalize<real, 0><<<(c->nr + 63) / 64, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, nullptr, 0, T, G, 1.0, c->d_diag);
     k_rfe_balance<real><<<ga, TX, 0, c->stream>>>(S, c->d_diag, G);
     c->launches += 4;
-    return HFT_OK;
+    return check_launch(c);
 }
 
 // S(B, h) at time t (reading U29): rotate the maps while t has reached the time of map 2, then forward Euler
@@ -530,7 +607,8 @@ int rfe_advance(hft_ctx* c, double t, double h) {
     const Geom& G = c->G;
     while (t >= c->rfe_t1 + c->rfe_tau) {
         char* tmp = c->rfe_map[0]; c->rfe_map[0] = c->rfe_map[1]; c->rfe_map[1] = tmp;   // map 2 becomes map 1
-        rfe_make_map<real>(c, (real*)c->rfe_map[1], c->rfe_next++);
+        const int rc = rfe_make_map<real>(c, (real*)c->rfe_map[1], c->rfe_next++);
+        if (rc != HFT_OK) return rc;
         c->rfe_t1 += c->rfe_tau;
     }
     const real a = (real)((t - c->rfe_t1) / c->rfe_tau);
@@ -538,7 +616,7 @@ int rfe_advance(hft_ctx* c, double t, double h) {
     k_rfe_apply<real><<<ga, TX, 0, c->stream>>>(arr_of<real>(c, c->i_state), (const real*)c->rfe_map[0], (const real*)c->rfe_map[1], a,
                                                 (real)h, G);
     c->launches++;
-    return HFT_OK;
+    return check_launch(c);
 }
 
 template <typename real>
@@ -547,12 +625,12 @@ int step_once(hft_ctx* c, double dt, int s) {
     c->att_ready = false;
     // Eq. 21 (:308-313): A(dt) then D(dt).  Strang, Eq. 22 (:317-326) with S omitted: A(dt/2), D(dt), A(dt/2).
     const bool strang = c->opt.strang != 0;
-    if (c->rfe_model && strang) rfe_advance<real>(c, c->time, 0.5 * dt);   // Eq. 22: S(dt/2) first
-    if (c->opt.adv_flux != 0) rc = advect<real>(c, strang ? 0.5 * dt : dt);
+    if (c->rfe_model && strang) rc = rfe_advance<real>(c, c->time, 0.5 * dt);   // Eq. 22: S(dt/2) first
+    if (rc == HFT_OK && c->opt.adv_flux != 0) rc = advect<real>(c, strang ? 0.5 * dt : dt);
     if (rc != HFT_OK) return rc;
     if (c->opt.diff_time != 0) {
-        const int kb = c->opt.sts_block == 0 ? sts_default_block(c->G, sizeof(real), c->sts_pipe != 0) : c->opt.sts_block;
-        if (!c->map_any && c->opt.diff_time >= 2 && kb > 1 && s > 2 * kb && sts_blocked_supported(c->G, sizeof(real), c->sts_pipe != 0)) {
+        const int kb = c->opt.sts_block == 0 ? sts_default_block(c->G, sizeof(real)) : c->opt.sts_block;
+        if (!c->map_any && c->opt.diff_time >= 2 && kb > 1 && s > 2 * kb && sts_blocked_supported(c->G, sizeof(real))) {
             StsBlockedPlan<real> P;
             P.Y0 = arr_of<real>(c, c->i_state);
             for (int i = 0; i < 5; i++) P.buf[i] = arr_of<real>(c, (c->i_state + 1 + i) % kNumArrays);
@@ -562,8 +640,9 @@ int step_once(hft_ctx* c, double dt, int s) {
             P.prof_begin = [](void* u, bool* armed) { prof_begin((hft_ctx*)u, 1, *armed); };
             P.prof_end = [](void* u, bool armed, int stages) { prof_end((hft_ctx*)u, armed, stages); };
             P.user = c;
+            P.up = &c->up;
             int64_t n = 0;
-            rc = sts_blocked_step<real>(P, tables_of<real>(c), c->G, c->sts_pipe, &n) == 0 ? HFT_OK : HFT_ERR_CUDA;
+            rc = sts_blocked_step<real>(P, tables_of<real>(c), c->G, &n) == 0 ? HFT_OK : HFT_ERR_CUDA;
             c->launches += n;
         } else {
             rc = diffuse_unblocked<real>(c, dt, s);
@@ -571,8 +650,8 @@ int step_once(hft_ctx* c, double dt, int s) {
     }
     if (rc == HFT_OK && strang && c->opt.adv_flux != 0) rc = advect<real>(c, 0.5 * dt);
     if (rc == HFT_OK && c->rfe_model) {   // Eq. 21: S after D; Eq. 22: the second S(dt/2)
-        if (strang) rfe_advance<real>(c, c->time + 0.5 * dt, 0.5 * dt);
-        else rfe_advance<real>(c, c->time, dt);
+        if (strang) rc = rfe_advance<real>(c, c->time + 0.5 * dt, 0.5 * dt);
+        else rc = rfe_advance<real>(c, c->time, dt);
     }
     c->time += dt;
     return rc;
@@ -626,12 +705,6 @@ int map_upload_any(hft_ctx* c, int q, const double* h_map) {
     return c->fp64() ? map_upload<double>(c, q, h_map) : map_upload<float>(c, q, h_map);
 }
 
-int check_launch(hft_ctx* c) {
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(c, e, "kernel launch");
-    return HFT_OK;
-}
-
 }  // namespace
 
 // ===================================================================== C ABI
@@ -654,7 +727,7 @@ const char* hft_error_string(int code) {
 const char* hft_last_cuda_error(hft_ctx* ctx) { return ctx ? ctx->cuda_err.c_str() : ""; }
 
 int hft_workspace_bytes(const hft_grid* grid, int32_t n_real, const hft_options* opt, size_t* h_bytes) {
-    if (!valid_grid(grid) || n_real < 1 || !h_bytes) return HFT_ERR_ARG;
+    if (!valid_grid(grid) || n_real < 1 || n_real > 65535 || !h_bytes) return HFT_ERR_ARG;   // realizations ride in gridDim.z
     if (opt && !valid_options(opt)) return HFT_ERR_ARG;
     const size_t w = grid->dtype == 1 ? 8 : 4;
     const size_t one = round_up((size_t)n_real * (grid->n_theta + 2) * pitch_for(grid->n_phi, grid->dtype) * w, 256);
@@ -666,7 +739,8 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
                void* d_workspace, size_t workspace_bytes, void* cuda_stream, hft_ctx** out) {
     if (!out) return HFT_ERR_ARG;
     *out = nullptr;
-    if (!valid_grid(grid) || n_real < 1 || !h_params || !d_workspace) return HFT_ERR_ARG;
+    if (!valid_grid(grid) || n_real < 1 || n_real > 65535 || !h_params || !d_workspace) return HFT_ERR_ARG;
+    if (!valid_params(h_params, n_real)) return HFT_ERR_ARG;
     hft_options o = opt ? *opt : default_options();
     if (!valid_options(&o)) return HFT_ERR_ARG;
     size_t need = 0;
@@ -678,7 +752,6 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     hft_ctx* c = new (std::nothrow) hft_ctx();
     if (!c) return HFT_ERR_NOMEM;
     c->grid = *grid; c->opt = o; c->nr = n_real; c->stream = (cudaStream_t)cuda_stream;
-    if (const char* e = getenv("HFT_STS_PIPE")) c->sts_pipe = atoi(e) != 0;
     c->G.nt = grid->n_theta; c->G.np = grid->n_phi; c->G.pitch = pitch_for(grid->n_phi, grid->dtype); c->G.nr = n_real;
     c->G.rstride = (size_t)(grid->n_theta + 2) * c->G.pitch;
     c->G.nbx = (grid->n_phi + TX - 1) / TX;
@@ -695,9 +768,11 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     c->B0.assign(n_real, 0.0);
     c->nu.resize(n_real); c->nuf.resize((size_t)n_real * (c->G.nt + 1)); c->vt.resize((size_t)n_real * (c->G.nt + 1)); c->om.resize((size_t)n_real * (c->G.nt + 2));
     build_metric(c);
+    c->nu_scale.resize(n_real); c->nu_shape.assign(c->G.nt + 1, 1.0);
     for (int r = 0; r < n_real; r++) {
         build_flow(c, r, h_params[r]);
         for (int f = 0; f <= c->G.nt; f++) c->nuf[(size_t)r * (c->G.nt + 1) + f] = c->nu[r];
+        c->nu_scale[r] = c->nu[r];
     }
     int rc = HFT_OK;
     auto fail = [&](int code) { hft_destroy(c); return code; };
@@ -711,6 +786,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
         (e = cudaMalloc((void**)&c->d_zmean, sts_zmean_bytes(c->G))) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_capseq, sts_capseq_bytes(c->G))) != cudaSuccess ||
         (e = cudaMalloc(&c->d_B0, (size_t)n_real * sizeof(double))) != cudaSuccess ||
+        (e = cudaMalloc((void**)&c->d_kappa, (size_t)n_real * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_capw, (size_t)n_real * 2 * sizeof(double))) != cudaSuccess ||
         (e = cudaMallocHost((void**)&c->h_diag, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess) {
         cuda_fail(c, e, "cudaMalloc");
@@ -728,7 +804,7 @@ void hft_destroy(hft_ctx* c) {
     if (c->prof_ev_made)
         for (int i = 0; i < 2 * kProfEvents; i++) cudaEventDestroy(c->prof_ev[i]);
     cudaFree(c->d_tab); cudaFree(c->d_part[0]); cudaFree(c->d_part[1]); cudaFree(c->d_fluxpart);
-    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq); cudaFree(c->d_B0); cudaFree(c->d_capw);
+    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq); cudaFree(c->d_kappa); cudaFree(c->d_B0); cudaFree(c->d_capw);
     if (c->h_diag) cudaFreeHost(c->h_diag);
     cudaFree(c->d_extpart); cudaFree(c->d_ext);
     if (c->h_ext) cudaFreeHost(c->h_ext);
@@ -754,6 +830,14 @@ int hft_set_diffusivity_profile(hft_ctx* c, int32_t r, const double* h_nu_face) 
     for (int q = 0; q < c->nr; q++)
         if (r < 0 || q == r)
             for (int f = 0; f <= nt; f++) c->nuf[(size_t)q * (nt + 1) + f] = h_nu_face[f] * kKm2sToRs2Hr;
+    if (r < 0 || c->nr == 1) {   // one profile for the whole batch: nu_r(theta) = 1 * shape(theta)
+        for (int f = 0; f <= nt; f++) c->nu_shape[f] = h_nu_face[f] * kKm2sToRs2Hr;
+        for (int q = 0; q < c->nr; q++) c->nu_scale[q] = 1.0;
+        c->shape_common = true;
+    } else {
+        c->shape_common = false;   // per-realization profiles: per-realization tables (k_sts_pipe)
+    }
+    c->tab_version++;
     CK(cudaStreamSynchronize(c->stream));   // the tables may still be read by enqueued work
     if (c->map_any)   // the realizations given a profile leave map mode's per-cell values for the profile's
         for (int q = 0; q < c->nr; q++)
@@ -818,10 +902,10 @@ int hft_set_rfe(hft_ctx* c, int32_t model, double flux_per_hr, double tau_hours,
     c->time = 0.0; c->rfe_t1 = 0.0; c->rfe_next = 2;
     if (model == 0) return HFT_OK;
     for (uint32_t m = 0; m < 2; m++) {
-        if (c->fp64()) rfe_make_map<double>(c, (double*)c->rfe_map[m], m);
-        else rfe_make_map<float>(c, (float*)c->rfe_map[m], m);
+        const int rc = c->fp64() ? rfe_make_map<double>(c, (double*)c->rfe_map[m], m) : rfe_make_map<float>(c, (float*)c->rfe_map[m], m);
+        if (rc != HFT_OK) return rc;
     }
-    return check_launch(c);
+    return HFT_OK;
 }
 
 int hft_get_rfe_map(hft_ctx* c, int32_t r, int32_t which, void* d_out) {
@@ -899,6 +983,8 @@ int hft_step(hft_ctx* c, int32_t n_steps, double dt) {
         s = c->opt.sts_stages ? c->opt.sts_stages : need;
         if (s < need) return HFT_ERR_UNSTABLE;
         build_sts_coef(c->coef, c->opt.diff_time, s, dt);
+        const int rc = prepare_upipe(c, c->opt.diff_time, s, dt);
+        if (rc != HFT_OK) return rc;
     }
     for (int n = 0; n < n_steps; n++) {
         int rc = c->fp64() ? step_once<double>(c, dt, s) : step_once<float>(c, dt, s);

@@ -24,12 +24,15 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <map>
+#include <mutex>
+#include <utility>
+
 #include "hft_kernels.cuh"
 
 namespace hft {
 
 constexpr int STS_KMAX = 8;
-constexpr int BLK_WARPS = 4;  // warps per CTA: adjacent strips share their halo loads through L1
 
 template <typename real, int C> struct VecOf;
 template <> struct VecOf<double, 2> { typedef double2 type; };
@@ -144,163 +147,43 @@ __global__ void __launch_bounds__(32 * STS_KMAX) k_sts_capseq(BlkArgs<real, K> A
     }
 }
 
-// ------------------------------------------------------------------ main kernel
-template <typename real, int K, int C>
-__global__ void __launch_bounds__(BLK_WARPS * 32) k_sts_blocked(BlkArgs<real, K> A, Tables<real> T, Geom G) {
-    constexpr int HALO = (K + C - 1) / C * C;  // invalid columns per side, in whole 16-byte vectors
-    constexpr int WOUT = 32 * C - 2 * HALO;    // columns written per warp
-    const int lane = threadIdx.x & 31;
-    const int strip = blockIdx.x * BLK_WARPS + (threadIdx.x >> 5);
-    if (strip >= A.nstrips) return;  // warp-uniform; the kernel has no block-level barrier
-    const int r = blockIdx.z;
-    const int nt = G.nt, np = G.np;
-    const int ja = blockIdx.y * A.rows_per_seg;              // output rows [ja, jb)
-    const int jb = min(ja + A.rows_per_seg, nt + 2);
-    const int t0 = max(ja - K, 0);                           // first input row streamed
-    const int tend = jb - 1 + K;                             // last row-step (level K reaches row jb-1)
-    // columns of this lane: unwrapped index uc (may be < 0 or >= np), wrapped col
-    const int uc = strip * WOUT - HALO + lane * C;
-    int col = uc % np;
-    if (col < 0) col += np;
-    const bool wr = (lane * C >= HALO) && (lane * C < HALO + WOUT) && (uc < np);  // this lane's columns are written
-    const size_t base = (size_t)r * G.rstride + col;
-    const real* cpT = T.cp + (size_t)r * (nt + 2);
-    const real* cmT = T.cm + (size_t)r * (nt + 2);
-    const real* cfT = T.cf + (size_t)r * (nt + 2);
-    const real* cdT = T.cd + (size_t)r * (nt + 2);
-    const double* capN = A.capseq + ((size_t)r * 2 + 0) * K;
-    const double* capS = A.capseq + ((size_t)r * 2 + 1) * K;
-
-    real u[K][3][C];  // u[l][i]: level l, rows t-l-2+i (i = 0 oldest .. 2 newest)
-    real p[2][C];     // level -1, rows t-1, t
-    real f[K + 1][C]; // F rows t-i
-#pragma unroll
-    for (int l = 0; l < K; l++)
-#pragma unroll
-        for (int i = 0; i < 3; i++)
-#pragma unroll
-            for (int q = 0; q < C; q++) u[l][i][q] = (real)0;
-#pragma unroll
-    for (int i = 0; i < 2; i++)
-#pragma unroll
-        for (int q = 0; q < C; q++) p[i][q] = (real)0;
-#pragma unroll
-    for (int i = 0; i <= K; i++)
-#pragma unroll
-        for (int q = 0; q < C; q++) f[i][q] = (real)0;
-
-    // software prefetch: row t+1 is loaded while row t is processed
-    real nu0[C], np_[C], nf[C];
-#pragma unroll
-    for (int q = 0; q < C; q++) { nu0[q] = (real)0; np_[q] = (real)0; nf[q] = (real)0; }
-    {
-        const size_t off = base + (size_t)t0 * G.pitch;
-        vload<real, C>(nu0, A.cur + off);
-        if (A.has_prev) vload<real, C>(np_, A.prev + off);
-        vload<real, C>(nf, A.F + off);
-    }
-
-    for (int t = t0; t <= tend; t++) {
-        // shift the windows by one row
-#pragma unroll
-        for (int l = 0; l < K; l++)
-#pragma unroll
-            for (int q = 0; q < C; q++) { u[l][0][q] = u[l][1][q]; u[l][1][q] = u[l][2][q]; }
-#pragma unroll
-        for (int q = 0; q < C; q++) p[0][q] = p[1][q];
-#pragma unroll
-        for (int i = K; i >= 1; i--)
-#pragma unroll
-            for (int q = 0; q < C; q++) f[i][q] = f[i - 1][q];
-        // row t arrives (prefetched), row t+1 is requested
-#pragma unroll
-        for (int q = 0; q < C; q++) { u[0][2][q] = nu0[q]; p[1][q] = np_[q]; f[0][q] = nf[q]; }
-        if (t + 1 <= min(tend, nt + 1)) {
-            const size_t off = base + (size_t)(t + 1) * G.pitch;
-            vload<real, C>(nu0, A.cur + off);
-            if (A.has_prev) vload<real, C>(np_, A.prev + off);
-            vload<real, C>(nf, A.F + off);
-        }
-        real outK[C];
-#pragma unroll
-        for (int q = 0; q < C; q++) outK[q] = (real)0;
-        // levels 1..K: level l computes its row j = t - l from level l-1 rows j-1, j, j+1
-#pragma unroll
-        for (int l = 1; l <= K; l++) {
-            const int j = t - l;
-            real res[C];
-            if (j >= 1 && j <= nt) {
-                const real ca = A.a[l - 1];
-                const real An = ca * cmT[j], As = ca * cpT[j], Af = ca * cfT[j];
-                const real Ac = A.mu[l - 1] - ca * cdT[j];
-                const real nuc = A.nu[l - 1], gc = A.g[l - 1];
-                // phi neighbours of the row-j values of level l-1 (u[l-1][1]) from the adjacent lanes
-                real west = __shfl_up_sync(0xffffffffu, u[l - 1][1][C - 1], 1);
-                real east = __shfl_down_sync(0xffffffffu, u[l - 1][1][0], 1);
-#pragma unroll
-                for (int q = 0; q < C; q++) {
-                    const real c = u[l - 1][1][q];
-                    const real w = (q == 0) ? west : u[l - 1][1][q - 1];
-                    const real e = (q == C - 1) ? east : u[l - 1][1][q + 1];
-                    const real p2 = (l >= 2) ? u[(l >= 2) ? l - 2 : 0][0][q] : p[0][q];
-                    real acc = gc * f[l][q];
-                    acc = nuc * p2 + acc;
-                    acc = Af * (e + w) + acc;
-                    acc = Ac * c + acc;
-                    acc = An * u[l - 1][0][q] + acc;
-                    acc = As * u[l - 1][2][q] + acc;  // the only operand produced in this row-step: last in the chain
-                    res[q] = acc;
-                }
-            } else if (j == 0 || j == nt + 1) {
-                const real cv = (real)(j == 0 ? capN[l - 1] : capS[l - 1]);
-#pragma unroll
-                for (int q = 0; q < C; q++) res[q] = cv;
-            } else {
-#pragma unroll
-                for (int q = 0; q < C; q++) res[q] = (real)0;
-            }
-            if (l < K) {
-#pragma unroll
-                for (int q = 0; q < C; q++) u[(l < K) ? l : 0][2][q] = res[q];
-            } else {
-#pragma unroll
-                for (int q = 0; q < C; q++) outK[q] = res[q];
-            }
-        }
-        // write row jo = t - K of levels K and K-1
-        const int jo = t - K;
-        if (wr && jo >= ja && jo < jb) {
-            const size_t off = base + (size_t)jo * G.pitch;
-            if (A.last) {
-                real y[C];
-                vload<real, C>(y, A.Y0 + off);
-#pragma unroll
-                for (int q = 0; q < C; q++) y[q] += outK[q];
-                vstore<real, C>(A.Y0 + off, y);
-            } else {
-                vstore<real, C>(A.ocur + off, outK);
-                vstore<real, C>(A.oprev + off, u[K - 1][1]);
-            }
-        }
-    }
-}
-
 // ------------------------------------------------------------------ host side
 
 template <typename real> struct BlkCfg;
 template <> struct BlkCfg<double> { static constexpr int C = 2; };
 template <> struct BlkCfg<float> { static constexpr int C = 4; };
 
-// pipe: k_sts_pipe takes any n_phi (lanes behind the seam move their columns one by one); the first-generation
-// k_sts_blocked needs n_phi to be a multiple of the vector width
-inline bool sts_blocked_supported(const Geom& G, size_t wbytes, bool pipe = true) {
+// the blocked kernels take any n_phi (lanes behind the seam move their columns one by one)
+inline bool sts_blocked_supported(const Geom& G, size_t wbytes) {
     const int C = wbytes == 8 ? 2 : 4;
-    return (pipe || (G.np % C) == 0) && G.np >= 32 * C && G.nt >= 2 * STS_KMAX;
+    return G.np >= 32 * C && G.nt >= 2 * STS_KMAX;
 }
-inline int sts_default_block(const Geom& G, size_t wbytes, bool pipe = true) { return sts_blocked_supported(G, wbytes, pipe) ? 8 : 1; }
+inline int sts_default_block(const Geom& G, size_t wbytes) { return sts_blocked_supported(G, wbytes) ? 8 : 1; }
 inline size_t sts_zmean_bytes(const Geom&) { return 256; }
 inline size_t sts_capseq_bytes(const Geom& G) { return (size_t)G.nr * 2 * STS_KMAX * sizeof(double) + 256; }
 inline int sts_blocked_init(const Geom&, bool) { return 0; }
+
+// CTAs of `kernel` resident on the current device (SMs x occupancy), cached per (device, kernel); the first call for a
+// device also opts the kernel in to `smem` bytes of dynamic shared memory there.  < 1 on error.
+template <typename KernelT>
+int resident_ctas(KernelT kernel, int threads, int smem) {
+    static std::mutex m;
+    static std::map<std::pair<int, const void*>, int> cache;   // (kernels of one signature share this instantiation)
+    int dev = 0, sms = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    std::lock_guard<std::mutex> lk(m);
+    const auto key = std::make_pair(dev, (const void*)kernel);
+    const auto it = cache.find(key);
+    if (it != cache.end()) return it->second;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem) != cudaSuccess || per_sm < 1)
+        return -1;
+    cache[key] = sms * per_sm;
+    return sms * per_sm;
+}
+
+struct UPipePlan;   // hft_sts_upipe.cuh
 
 template <typename real>
 struct StsBlockedPlan {
@@ -315,34 +198,7 @@ struct StsBlockedPlan {
     void (*prof_begin)(void*, bool*);
     void (*prof_end)(void*, bool, int);
     void* user;
+    const UPipePlan* up;   // uniform-coefficient kernel (hft_sts_upipe.cuh) if up && up->ok, else k_sts_pipe
 };
-
-template <typename real, int K>
-void sts_blocked_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
-                        real* ocur, real* oprev, bool last, int64_t* launches) {
-    constexpr int C = BlkCfg<real>::C;
-    constexpr int WOUT = 32 * C - 2 * ((K + C - 1) / C * C);
-    BlkArgs<real, K> a;
-    a.cur = cur; a.prev = prev ? prev : cur; a.F = P.buf[0]; a.ocur = ocur; a.oprev = oprev; a.Y0 = P.Y0; a.capseq = P.capseq;
-    for (int i = 0; i < K; i++) {
-        a.mu[i] = (real)P.mu[j0 + 1 + i]; a.nu[i] = (real)P.nu[j0 + 1 + i];
-        a.a[i] = (real)P.a[j0 + 1 + i]; a.g[i] = (real)P.g[j0 + 1 + i];
-    }
-    a.has_prev = prev != nullptr; a.last = last;
-    a.nstrips = (G.np + WOUT - 1) / WOUT;
-    // theta segments: enough CTAs for ~4 waves of 148 SMs x resident CTAs, but segments of at least 64 rows
-    const int ctas_x = (a.nstrips + BLK_WARPS - 1) / BLK_WARPS;
-    int nseg = 1;
-    const long want = 148L * 8;
-    while ((long)ctas_x * nseg * G.nr < want && (G.nt + 2) / (nseg * 2) >= 64) nseg *= 2;
-    a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
-    dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
-    k_sts_capseq<real, K><<<gc, 32 * STS_KMAX, 0, P.stream>>>(a, T, G, P.capseq);
-    bool armed = false;
-    P.prof_begin(P.user, &armed);
-    k_sts_blocked<real, K, C><<<g, BLK_WARPS * 32, 0, P.stream>>>(a, T, G);
-    P.prof_end(P.user, armed, K);
-    *launches += 2;
-}
 
 }  // namespace hft

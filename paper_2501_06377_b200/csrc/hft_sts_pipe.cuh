@@ -3,7 +3,7 @@
 // (cp.async, several rows per warp in flight) for the three input streams, (iii) the per-(stage,row)
 // coefficient products formed once per warp row-step by the 32 lanes together instead of by every lane.
 //
-// Same decomposition as k_sts_blocked (hft_sts_blocked.cuh): a WARP owns a strip of
+// Decomposition (hft_sts_blocked.cuh): a WARP owns a strip of
 // 32*C phi-columns (one 16-byte vector per lane) and streams down the theta-rows; level l (= stage j0+l) lags
 // level l-1 by one row; phi-neighbours come from the adjacent lanes by shuffle; warps never synchronise with
 // each other.  What changed is the instruction stream (profiles/r01_cfg3_f64_first_pass.md: 523 warp
@@ -35,17 +35,13 @@ namespace hft {
 
 __host__ __device__ constexpr int pmod(int a, int m) { return ((a % m) + m) % m; }
 
-// CTA shape per precision (overridable for experiments): warps (= strips) per CTA -- warps never synchronise with each
+// CTA shape per precision: warps (= strips) per CTA -- warps never synchronise with each
 // other -- and the resident CTAs per SM the register budget is set for.  fp64: 4 x 2 with the long body (206 registers);
 // 12 warps per SM with the short body need 4 % fewer cycles but draw more power, and under the 1000 W cap the clock drops by
 // more than that (122.5 against 120.7 ms per cfg 3 step).  fp32 (not power-limited): 4 x 3 with the short body at 168
 // registers, 12 warps per SM: 59.7 -> 53.6 ms per step (3 x 3: 56.5, 2 x 5: 54.0, 2 x 6: 53.9, 3 x 4: 56.8).
 template <typename real> struct PipeShape {
-#ifdef HFT_PIPE_WARPS
-    static constexpr int WARPS = HFT_PIPE_WARPS, MINB = HFT_PIPE_MINB;
-#else
     static constexpr int WARPS = 4, MINB = sizeof(real) == 4 ? 3 : 2;
-#endif
 };
 
 template <typename real, int K>
@@ -58,13 +54,7 @@ struct PipeCfg {
     // row-steps) and the slot of the shared-memory ring is a run-time offset -- a third of the straight-line code.  The
     // long body stalls on instruction fetch (0.31 per issue in fp32, 0.19 in fp64); measured on cfg 3 the short body is
     // 3 % faster in fp32 and 1.5 % slower in fp64 (where the extra moves and slot arithmetic cost more than the fetches).
-#if defined(HFT_PIPE_LONG_BODY)
-    static constexpr bool SHIFTF = false;
-#elif defined(HFT_PIPE_SHORT_BODY)
-    static constexpr bool SHIFTF = true;
-#else
     static constexpr bool SHIFTF = sizeof(real) == 4;
-#endif
     static constexpr int U = SHIFTF ? 3 : ((NF % 3 == 0) ? NF : 3 * NF);   // row-steps per unrolled macro-iteration
     static constexpr int NFW = SHIFTF ? K + 3 : NF;
     static constexpr int D = NF;                              // ring depth in rows
@@ -345,18 +335,10 @@ template <typename real, int K, bool SPLIT>
 int sts_pipe_launch_impl(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int j0, const real* cur, const real* prev,
                          real* ocur, real* oprev, bool last, int64_t* launches) {
     using PC = PipeCfg<real, K>;
-    static int slots = 0;   // CTAs resident on the whole device
     constexpr int PIPE_WARPS = PipeShape<real>::WARPS;
     const int smem = PIPE_WARPS * PC::WARP_BYTES;
-    if (!slots) {
-        cudaError_t e = cudaFuncSetAttribute(k_sts_pipe<real, K, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-        if (e != cudaSuccess) return -1;
-        int dev = 0, sms = 0, per_sm = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sts_pipe<real, K, SPLIT>, PIPE_WARPS * 32, smem) != cudaSuccess || per_sm < 1)
-            return -1;
-        slots = sms * per_sm;
-    }
+    const int slots = resident_ctas(k_sts_pipe<real, K, SPLIT>, PIPE_WARPS * 32, smem);   // CTAs resident on this device
+    if (slots < 1) return -1;
     BlkArgs<real, K> a;
     a.cur = cur; a.prev = prev; a.F = P.buf[0]; a.ocur = ocur; a.oprev = oprev; a.Y0 = P.Y0; a.capseq = P.capseq;
     for (int i = 0; i < K; i++) {
@@ -394,90 +376,6 @@ int sts_pipe_launch(const StsBlockedPlan<real>& P, Tables<real>& T, const Geom& 
                     real* ocur, real* oprev, bool last, int64_t* launches) {
     if (G.np % PipeCfg<real, K>::C == 0) return sts_pipe_launch_impl<real, K, false>(P, T, G, j0, cur, prev, ocur, oprev, last, launches);
     return sts_pipe_launch_impl<real, K, true>(P, T, G, j0, cur, prev, ocur, oprev, last, launches);
-}
-
-// One STS step: stage 1, the (s-1) mod K remainder stages (pipe: one un-blocked stage if odd, then one shorter block;
-// first generation: one launch each), then (s-1)/K blocked launches of K stages.
-// pipe != 0: k_sts_pipe (default); pipe == 0: the first-generation k_sts_blocked (kept for comparison).
-template <typename real>
-int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, int pipe, int64_t* launches) {
-    const int K = P.kb, s = P.s;
-    real* F = P.buf[0];
-    real* b[4] = {P.buf[1], P.buf[2], P.buf[3], P.buf[4]};
-    // stage 1 and an odd remainder stage run one stage per launch, in the 16-byte-vector kernel when n_phi is a multiple of
-    // the vector width (its polar partials come in nbxv pieces per row), else in the one-column-per-thread kernel
-    constexpr int CV = 16 / (int)sizeof(real);
-    const int nbxv = (G.np / CV + TX - 1) / TX;
-    dim3 g1(nbxv, (G.nt + 2 + MAPV_RPT - 1) / MAPV_RPT, G.nr), gs(G.nbx, 2, G.nr);
-    k_polar_row_sums<real><<<gs, TX, 0, P.stream>>>(P.Y0, P.part[0], G);
-    MapArgs<real> M;
-    M.NU = nullptr; M.capw = nullptr; M.capP = 0.0; M.rdth = (real)0; M.nparts_in = G.nbx;
-    StsArgs<real> a;
-    a.F = F; a.Y0 = P.Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
-    a.in = P.Y0; a.d2 = b[0]; a.part_in = P.part[0]; a.part_out = P.part[1]; a.a = (real)P.a[1];
-    const bool vec = G.np % CV == 0;
-    dim3 g1s(G.nbx, (G.nt + 2 + RPT - 1) / RPT, G.nr);
-    if (vec) k_sts_stage_mapv<real, 0, false><<<g1, TX, 0, P.stream>>>(a, M, T, G);
-    else k_sts_stage<real, 0><<<g1s, TX, 0, P.stream>>>(a, T, G);
-    M.nparts_in = nbxv;
-    *launches += 2;
-    const int rem = (s - 1) % K;
-    // the remainder: one un-blocked stage if it is odd, then (pipe only) ONE shorter block of rem - (rem & 1) stages
-    int rem_single = rem;
-#ifndef HFT_FAST_BUILD
-    if (pipe) rem_single = rem & 1;
-#endif
-    int icur = 0, iprev = 1, pin = 1;
-    bool has_prev = false;
-    for (int j = 2; j <= 1 + rem_single; j++) {  // remainder stages, unblocked
-        a.in = b[icur]; a.d2 = b[iprev]; a.part_in = P.part[pin]; a.part_out = P.part[pin ^ 1];
-        a.mu = (real)P.mu[j]; a.nu = (real)P.nu[j]; a.a = (real)P.a[j]; a.g = (real)P.g[j];
-        a.use_d2 = has_prev;
-        if (vec) k_sts_stage_mapv<real, 1, false><<<g1, TX, 0, P.stream>>>(a, M, T, G);
-        else k_sts_stage<real, 1><<<g1s, TX, 0, P.stream>>>(a, T, G);
-        *launches += 1;
-        int t = icur; icur = iprev; iprev = t;
-        has_prev = true;
-        pin ^= 1;
-    }
-    int j0 = 1 + rem_single;  // stages done so far
-    while (j0 < s) {
-        const int kb = (rem - rem_single > 0 && j0 == 1 + rem_single) ? rem - rem_single : K;   // stages in this block
-        // outputs go to the two buffers that are not inputs
-        int o1 = -1, o2 = -1;
-        for (int q = 0; q < 4; q++)
-            if (q != icur && q != iprev) { if (o1 < 0) o1 = q; else o2 = q; }
-        const bool last = (j0 + kb == s);
-        if (pipe && !has_prev) {  // delta_0 = 0 is not stored: the pipe kernel reads it, so write it once
-            if (cudaMemsetAsync(b[iprev], 0, (size_t)G.nr * G.rstride * sizeof(real), P.stream) != cudaSuccess) return -1;
-            has_prev = true;
-        }
-        const real* prev = has_prev ? b[iprev] : nullptr;
-        int rc = 0;
-        if (pipe) {
-            switch (kb) {
-#ifndef HFT_FAST_BUILD   // experiment builds instantiate K = 8 only
-                case 2: rc = sts_pipe_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-                case 4: rc = sts_pipe_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-                case 6: rc = sts_pipe_launch<real, 6>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-#endif
-                default: rc = sts_pipe_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-            }
-        } else {
-            switch (kb) {
-#ifndef HFT_FAST_BUILD
-                case 2: sts_blocked_launch<real, 2>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-                case 4: sts_blocked_launch<real, 4>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-                case 6: sts_blocked_launch<real, 6>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-#endif
-                default: sts_blocked_launch<real, 8>(P, T, G, j0, b[icur], prev, b[o1], b[o2], last, launches); break;
-            }
-        }
-        if (rc != 0) return rc;
-        icur = o1; iprev = o2; has_prev = true;
-        j0 += kb;
-    }
-    return 0;
 }
 
 }  // namespace hft
