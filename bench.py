@@ -172,6 +172,8 @@ def main():
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--sts-block", type=int, default=0)
+    ap.add_argument("--sts-kernel", type=int, default=0, help="hft_options.sts_kernel: 0 library default, 1 k_sts_pipe, 2 k_sts_upipe")
+    ap.add_argument("--f32-accumulate", action="store_true", help="hft_options.f32_accumulate (fp32 storage, fp64 block arithmetic)")
     ap.add_argument("--attenuation", type=float, default=0.0, help="B0 in Gauss: time the step with flow attenuation (Eq. 5) on")
     ap.add_argument("--nu-map", action="store_true",
                     help="time the step with a spatially varying diffusivity nu(theta, phi) (Eq. 27-28): one launch per STS stage")
@@ -210,8 +212,8 @@ def main():
         # rank k owns realizations [k R, (k+1) R) of the weak-scaled ensemble; one clock for the whole ensemble
         wd = ens.shard(args.config, dtype, rank, world)
         def make_ctx(**kw):
-            c = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block,
-                            flow_attenuation=int(args.attenuation > 0), diffusivity_map=int(args.nu_map), device=f"cuda:{local}", **kw)
+            c = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, sts_kernel=args.sts_kernel,
+                            f32_accumulate=int(args.f32_accumulate and dtype == "f32"), flow_attenuation=int(args.attenuation > 0), diffusivity_map=int(args.nu_map), device=f"cuda:{local}", **kw)
             if args.attenuation > 0:
                 c.set_attenuation(-1, args.attenuation)
             if args.nu_map:      # nu_r (1 + 0.3 sin(theta) cos(phi)) on the half-half grid, per realization (workloads.diffusivity_map)

@@ -55,6 +55,29 @@ __device__ __forceinline__ void vstore(real* p, const real (&d)[C]) {
     *reinterpret_cast<typename VecOf<real, C>::type*>(p) = v;
 }
 
+// ------------------------------------------------------------------ compute-type traits: a "group" is what one FMA handles
+template <typename creal> struct UVec;
+template <> struct UVec<double> {
+    typedef double V;                       // one cell per FMA
+    static constexpr int W = 1;
+    static __device__ __forceinline__ V fma(V a, V b, V c) { return ::fma(a, b, c); }
+    static __device__ __forceinline__ V mul(V a, V b) { return a * b; }
+    static __device__ __forceinline__ V dup(double x) { return x; }
+    static __device__ __forceinline__ double get(const V& v, int) { return v; }
+    static __device__ __forceinline__ void set(V& v, int, double x) { v = x; }
+    static __host__ V hdup(double x) { return x; }
+};
+template <> struct UVec<float> {
+    typedef float2 V;                       // two cells per FFMA2
+    static constexpr int W = 2;
+    static __device__ __forceinline__ V fma(V a, V b, V c) { return __ffma2_rn(a, b, c); }
+    static __device__ __forceinline__ V mul(V a, V b) { return __fmul2_rn(a, b); }
+    static __device__ __forceinline__ V dup(float x) { return make_float2(x, x); }
+    static __device__ __forceinline__ float get(const V& v, int i) { return i == 0 ? v.x : v.y; }
+    static __device__ __forceinline__ void set(V& v, int i, float x) { if (i == 0) v.x = x; else v.y = x; }
+    static __host__ V hdup(double x) { return make_float2((float)x, (float)x); }
+};
+
 template <typename real, int K>
 struct BlkArgs {
     const real* cur;   // level 0  = delta_{j0}
@@ -65,6 +88,7 @@ struct BlkArgs {
     real* Y0;          // last block: Y0 += delta_s, ocur/oprev not written
     const double* capseq;  // [R][2][K] cap values of levels 1..K
     real mu[K], nu[K], a[K], g[K];  // scalars of stages j0+1 .. j0+K
+    typename UVec<real>::V nu2[K], g2[K];   // nu, g once more as FMA operands: {x, x} pairs in fp32 (FFMA2)
     int has_prev, last;
     int rows_per_seg, nstrips;
 };

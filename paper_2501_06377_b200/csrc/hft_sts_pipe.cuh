@@ -61,7 +61,9 @@ struct PipeCfg {
     static constexpr int DP = D - 2;                          // prefetch distance in rows
     static constexpr int ROW = 32 * C;                        // reals per ring row (512 B)
     static constexpr int NCS = 3;                             // coefficient ring slots (divides U)
-    static constexpr int WARP_REALS = 3 * D * ROW + NCS * K * 4 + D * 32;   // data rings, product ring, raw-coefficient ring
+    static constexpr int W = UVec<real>::W, NG = C / W;       // cells per FMA (fp32: 2, FFMA2), groups per lane
+    static constexpr int CS = K * 4 * W;                      // reals per coefficient slot: 4 products per level, fp32 as {p, p} pairs
+    static constexpr int WARP_REALS = 3 * D * ROW + NCS * CS + D * 32;   // data rings, product ring, raw-coefficient ring
     static constexpr int WARP_BYTES = WARP_REALS * (int)sizeof(real);
     static constexpr int HALO = (K + C - 1) / C * C;          // invalid columns per strip side, whole 16-byte vectors
     static constexpr int WOUT = 32 * C - 2 * HALO;            // columns written per warp
@@ -92,11 +94,14 @@ template <typename real, int K, bool SPLIT>
 struct PipeWarp {
     using P = PipeCfg<real, K>;
     static constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, NF = P::NF, ROW = P::ROW, NCS = P::NCS;
+    static constexpr int W = P::W, NG = P::NG, CS = P::CS;
     static constexpr bool SHIFTF = P::SHIFTF;
+    using UV = UVec<real>;
+    using V = typename UV::V;   // what one FMA handles: a double, or a float2 pair (packed FFMA2 / FMUL2 of sm_100)
 
     // registers
-    real u[K][3][C];   // level l (0..K-1), row rho in slot rho mod 3 (relative to the macro-iteration origin)
-    real f[P::NFW][C]; // F row rho in slot rho mod NF; SHIFTF: row tb + x of the current body in slot x + K, x = -K..2
+    V u[K][3][NG];     // level l (0..K-1), row rho in slot rho mod 3 (relative to the macro-iteration origin)
+    V f[P::NFW][NG];   // F row rho in slot rho mod NF; SHIFTF: row tb + x of the current body in slot x + K, x = -K..2
     int rb;            // SHIFTF: shared-memory ring slot of row tb (0, 3, 6, .. < D)
     // per-warp constants
     const BlkArgs<real, K>& A;
@@ -146,8 +151,13 @@ struct PipeWarp {
 
     // products used by row-step t
     __device__ __forceinline__ void gen_coef(int t, int slot) {
-        if (cl < K) s_coef[slot * (K * 4) + lane] = fma_r(sa, raw_of(t), sadd);
+        if (cl < K) put_coef(slot, fma_r(sa, raw_of(t), sadd));
     }
+    // this lane's product into its place of coefficient slot `slot` (fp32: both halves of the pair)
+    __device__ __forceinline__ void put_coef(int slot, real p) {
+        *reinterpret_cast<V*>(s_coef + slot * CS + lane * W) = UV::dup(p);
+    }
+    __device__ __forceinline__ static void vld(V (&d)[NG], const real* p) { vload<real, C>(*reinterpret_cast<real(*)[C]>(&d[0]), p); }
 
     template <int PH, bool GEN>
     __device__ __forceinline__ void rowstep(int t) {
@@ -162,82 +172,94 @@ struct PipeWarp {
             sl = PH % D; slm1 = pmod(PH - 1, D); slpf = (PH + DP) % D;
         }
         constexpr int fnew = SHIFTF ? PH + K : PH % NF;
-        vload<real, C>(u[0][PH % 3], s_cur + sl * ROW);
-        vload<real, C>(f[fnew], s_F + sl * ROW);
-        real pl1[C];               // delta_{j0-1} row t-1: the "two levels back" operand of level 1
-        vload<real, C>(pl1, s_prev + slm1 * ROW);
+        vld(u[0][PH % 3], s_cur + sl * ROW);
+        vld(f[fnew], s_F + sl * ROW);
+        V pl1[NG];                 // delta_{j0-1} row t-1: the "two levels back" operand of level 1
+        vld(pl1, s_prev + slm1 * ROW);
         prefetch(t + DP, slpf);    // overwrites the slot of row t-2, last read one row-step ago
         const real raw_next = s_raw[sl * 32];   // this lane's own copy, arrived with the group of row t
-        const real* cfs = s_coef + (PH % NCS) * (K * 4);
-        real outK[C];
+        const real* cfs = s_coef + (PH % NCS) * CS;
+        V outK[NG];
 #pragma unroll
         for (int l = 1; l <= K; l++) {
             // level l-1: newest row t-l+1 (s), centre t-l (c), oldest t-l-1 (n)
             const int sN = pmod(PH - (l - 1), 3), sC = pmod(PH - l, 3), sO = pmod(PH - l - 1, 3);
-            real cf4[4];
-            vload<real, C>(*reinterpret_cast<real(*)[C]>(&cf4[0]), cfs + (l - 1) * 4);
-            if constexpr (C < 4) vload<real, C>(*reinterpret_cast<real(*)[C]>(&cf4[4 - C]), cfs + (l - 1) * 4 + (4 - C));
-            const real An = cf4[0], As = cf4[1], Af = cf4[2], Ac = cf4[3];
-            const real nuc = A.nu[l - 1], gc = A.g[l - 1];
-            const real west = __shfl_up_sync(0xffffffffu, u[l - 1][sC][C - 1], 1);
-            const real east = __shfl_down_sync(0xffffffffu, u[l - 1][sC][0], 1);
-            real res[C];
+            V cf4[4];              // An, As, Af, Ac of this level and row: two broadcast LDS.128
+            vload<real, 2 * W>(*reinterpret_cast<real(*)[2 * W]>(&cf4[0]), cfs + (l - 1) * 4 * W);
+            vload<real, 2 * W>(*reinterpret_cast<real(*)[2 * W]>(&cf4[2]), cfs + (l - 1) * 4 * W + 2 * W);
+            const V An = cf4[0], As = cf4[1], Af = cf4[2], Ac = cf4[3];
+            const V nuc = A.nu2[l - 1], gc = A.g2[l - 1];
+            const real west = __shfl_up_sync(0xffffffffu, UV::get(u[l - 1][sC][NG - 1], W - 1), 1);
+            const real east = __shfl_down_sync(0xffffffffu, UV::get(u[l - 1][sC][0], 0), 1);
+            V res[NG];
 #pragma unroll
-            for (int q = 0; q < C; q++) {
-                const real c = u[l - 1][sC][q];
-                const real w = (q == 0) ? west : u[l - 1][sC][q > 0 ? q - 1 : 0];
-                const real e = (q == C - 1) ? east : u[l - 1][sC][q < C - 1 ? q + 1 : 0];
-                const real p2 = (l == 1) ? pl1[q] : u[l >= 2 ? l - 2 : 0][sC][q];   // level l-2 row t-l is ITS oldest: slot (PH-(l-2)-2) mod 3 = sC
-                real acc = gc * f[SHIFTF ? PH - l + K : pmod(PH - l, NF)][q];
-                acc = fma_r(nuc, p2, acc);
-                acc = fma_r(Af, e + w, acc);
-                acc = fma_r(Ac, c, acc);
-                acc = fma_r(An, u[l - 1][sO][q], acc);
-                acc = fma_r(As, u[l - 1][sN][q], acc);   // the only operand produced in this row-step
-                res[q] = acc;
+            for (int gI = 0; gI < NG; gI++) {
+                const V c = u[l - 1][sC][gI];
+                V S;               // e + w of every cell of the group (scalar adds; the FMAs are packed in fp32)
+#pragma unroll
+                for (int i = 0; i < W; i++) {
+                    const int q = gI * W + i;
+                    const real w = (q == 0) ? west : UV::get(u[l - 1][sC][(q > 0 ? q - 1 : 0) / W], (q > 0 ? q - 1 : 0) % W);
+                    const real e = (q == C - 1) ? east : UV::get(u[l - 1][sC][(q < C - 1 ? q + 1 : 0) / W], (q < C - 1 ? q + 1 : 0) % W);
+                    UV::set(S, i, e + w);
+                }
+                const V p2 = (l == 1) ? pl1[gI] : u[l >= 2 ? l - 2 : 0][sC][gI];   // level l-2 row t-l is ITS oldest: slot (PH-(l-2)-2) mod 3 = sC
+                V acc = UV::mul(gc, f[SHIFTF ? PH - l + K : pmod(PH - l, NF)][gI]);
+                acc = UV::fma(nuc, p2, acc);
+                acc = UV::fma(Af, S, acc);
+                acc = UV::fma(Ac, c, acc);
+                acc = UV::fma(An, u[l - 1][sO][gI], acc);
+                acc = UV::fma(As, u[l - 1][sN][gI], acc);   // the only operand produced in this row-step
+                res[gI] = acc;
             }
             if (GEN) {
                 const int j = t - l;
                 if (j == 0 || j == nt + 1) {
                     const real cv = (real)(j == 0 ? capN[l - 1] : capS[l - 1]);
 #pragma unroll
-                    for (int q = 0; q < C; q++) res[q] = cv;
+                    for (int gI = 0; gI < NG; gI++) res[gI] = UV::dup(cv);
                 }
             }
             if (l < K) {
 #pragma unroll
-                for (int q = 0; q < C; q++) u[l < K ? l : 0][sC][q] = res[q];   // level l newest = row t-l: slot (PH-l) mod 3 = sC
+                for (int gI = 0; gI < NG; gI++) u[l < K ? l : 0][sC][gI] = res[gI];   // level l newest = row t-l: slot (PH-l) mod 3 = sC
             } else {
 #pragma unroll
-                for (int q = 0; q < C; q++) outK[q] = res[q];
+                for (int gI = 0; gI < NG; gI++) outK[gI] = res[gI];
             }
         }
         // products for the next row-step (slot last read two row-steps ago)
-        if (cl < K) s_coef[((PH + 1) % NCS) * (K * 4) + lane] = fma_r(sa, raw_next, sadd);
+        if (cl < K) put_coef((PH + 1) % NCS, fma_r(sa, raw_next, sadd));
         // row jo = t-K of levels K and K-1 (level K-1 row t-K is its centre: slot (PH-(K-1)-1) mod 3)
         const int jo = t - K;
         if (wmask && jo >= ja && jo < jb) {
             const size_t o = (size_t)jo * pitch;
+            real oc[C], op[C];
+#pragma unroll
+            for (int q = 0; q < C; q++) {
+                oc[q] = UV::get(outK[q / W], q % W);
+                op[q] = UV::get(u[K - 1][pmod(PH - K, 3)][q / W], q % W);
+            }
             if (!SPLIT || (simple && wmask == (1 << C) - 1)) {
                 if (A.last) {
                     real y[C];
                     vload<real, C>(y, gY0 + o);
 #pragma unroll
-                    for (int q = 0; q < C; q++) y[q] += outK[q];
+                    for (int q = 0; q < C; q++) y[q] += oc[q];
                     vstore<real, C>(gY0 + o, y);
                 } else {
-                    vstore<real, C>(gocur + o, outK);
-                    vstore<real, C>(goprev + o, u[K - 1][pmod(PH - K, 3)]);
+                    vstore<real, C>(gocur + o, oc);
+                    vstore<real, C>(goprev + o, op);
                 }
             } else {
 #pragma unroll
                 for (int q = 0; q < C; q++)
                     if (wmask >> q & 1) {
                         if (A.last) {
-                            gY0[o + dq[q]] += outK[q];
+                            gY0[o + dq[q]] += oc[q];
                         } else {
-                            gocur[o + dq[q]] = outK[q];
-                            goprev[o + dq[q]] = u[K - 1][pmod(PH - K, 3)][q];
+                            gocur[o + dq[q]] = oc[q];
+                            goprev[o + dq[q]] = op[q];
                         }
                     }
             }
@@ -252,7 +274,7 @@ struct PipeWarp {
 #pragma unroll
             for (int i = 0; i < K; i++)
 #pragma unroll
-                for (int q = 0; q < C; q++) f[i][q] = f[i + 3][q];
+                for (int gI = 0; gI < NG; gI++) f[i][gI] = f[i + 3][gI];
             rb += 3;
             if (rb >= D) rb -= D;
         }
@@ -293,7 +315,7 @@ __global__ void __launch_bounds__(PipeShape<real>::WARPS * 32, PipeShape<real>::
     real* ws = reinterpret_cast<real*>(pipe_smem) + (size_t)wrp * P::WARP_REALS;
     W.s_cur = ws + lane * C; W.s_prev = W.s_cur + D * ROW; W.s_F = W.s_prev + D * ROW;
     W.s_coef = ws + 3 * D * ROW;
-    W.s_raw = W.s_coef + P::NCS * K * 4 + lane;
+    W.s_raw = W.s_coef + P::NCS * P::CS + lane;
     W.capN = A.capseq + ((size_t)r * 2 + 0) * K;
     W.capS = A.capseq + ((size_t)r * 2 + 1) * K;
     W.cl = lane >> 2;
@@ -310,11 +332,11 @@ __global__ void __launch_bounds__(PipeShape<real>::WARPS * 32, PipeShape<real>::
 #pragma unroll
         for (int i = 0; i < 3; i++)
 #pragma unroll
-            for (int q = 0; q < C; q++) W.u[l][i][q] = (real)0;
+            for (int gI = 0; gI < P::NG; gI++) W.u[l][i][gI] = UVec<real>::dup((real)0);
 #pragma unroll
     for (int i = 0; i < P::NFW; i++)
 #pragma unroll
-        for (int q = 0; q < C; q++) W.f[i][q] = (real)0;
+        for (int gI = 0; gI < P::NG; gI++) W.f[i][gI] = UVec<real>::dup((real)0);
     W.rb = 0;
     // clear this warp's shared memory (the ring slot of "row t0-1" is read before it is ever written)
     for (int i = lane; i < P::WARP_REALS; i += 32) ws[i] = (real)0;
@@ -344,6 +366,7 @@ int sts_pipe_launch_impl(const StsBlockedPlan<real>& P, Tables<real>& T, const G
     for (int i = 0; i < K; i++) {
         a.mu[i] = (real)P.mu[j0 + 1 + i]; a.nu[i] = (real)P.nu[j0 + 1 + i];
         a.a[i] = (real)P.a[j0 + 1 + i]; a.g[i] = (real)P.g[j0 + 1 + i];
+        a.nu2[i] = UVec<real>::hdup(P.nu[j0 + 1 + i]); a.g2[i] = UVec<real>::hdup(P.g[j0 + 1 + i]);
     }
     a.has_prev = 1; a.last = last;
     a.nstrips = (G.np + PC::WOUT - 1) / PC::WOUT;

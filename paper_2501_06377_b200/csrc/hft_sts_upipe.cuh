@@ -42,29 +42,6 @@
 
 namespace hft {
 
-// ------------------------------------------------------------------ compute-type traits: a "group" is what one FMA handles
-template <typename creal> struct UVec;
-template <> struct UVec<double> {
-    typedef double V;                       // one cell per FMA
-    static constexpr int W = 1;
-    static __device__ __forceinline__ V fma(V a, V b, V c) { return ::fma(a, b, c); }
-    static __device__ __forceinline__ V mul(V a, V b) { return a * b; }
-    static __device__ __forceinline__ V dup(double x) { return x; }
-    static __device__ __forceinline__ double get(const V& v, int) { return v; }
-    static __device__ __forceinline__ void set(V& v, int, double x) { v = x; }
-    static __host__ V hdup(double x) { return x; }
-};
-template <> struct UVec<float> {
-    typedef float2 V;                       // two cells per FFMA2
-    static constexpr int W = 2;
-    static __device__ __forceinline__ V fma(V a, V b, V c) { return __ffma2_rn(a, b, c); }
-    static __device__ __forceinline__ V mul(V a, V b) { return __fmul2_rn(a, b); }
-    static __device__ __forceinline__ V dup(float x) { return make_float2(x, x); }
-    static __device__ __forceinline__ float get(const V& v, int i) { return i == 0 ? v.x : v.y; }
-    static __device__ __forceinline__ void set(V& v, int i, float x) { if (i == 0) v.x = x; else v.y = x; }
-    static __host__ V hdup(double x) { return make_float2((float)x, (float)x); }
-};
-
 constexpr int UTAB_BYTES = 65536;           // the whole user constant bank
 constexpr int UTAB_ROW_BYTES = 32;          // 4 coefficients: 4 doubles, or 4 duplicated float pairs
 constexpr int UTAB_MAX_ROWS = UTAB_BYTES / UTAB_ROW_BYTES;
