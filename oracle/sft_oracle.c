@@ -34,6 +34,11 @@
  *                    of all 13 run-history numbers on 8x16
  *   attenuation      Eq. 5: with B0 = inf the variable-speed rule equals the table rule bit for bit; uniform field =>
  *                    flow scaled by 1 - tanh(|c|/B0); |B| >> B0 => nothing moves; flux conserved; strong spot drifts less
+ *   general rule     (tests/test_oracle_general_rule.py) sweep with speeds varying along the sweep: phi-mirror symmetry bit for
+ *                    bit (swaps LP <-> LM); brute force on 8x16 with faces keyed by half-integers, written from B2 (:684) and
+ *                    :689; alpha window: a speed spike at one face changes exactly the faces within 4 of it, a dip exactly
+ *                    LM_q / LP_{q-1}'s readers -- for the phi sweep and for the theta table rule
+ *   rotation         rows under differential rotation (Eq. 3) arrive with phase m Omega_j t, each row its own; error order >= 3
  *   PARITY UNPINNED against HipFT itself (no HipFT output in the container): which faces use upwind
  *   next to the poles (reading U6), the stage-count rule (U9), eps_w = coordinate spacing (U11), where |Br| is taken
  *   for a face speed and when the attenuated speeds are formed (U22, U23).
@@ -754,6 +759,16 @@ void SUF(sft_oracle_advection_tendency_general)(void *h, int r, const real *in, 
     o->B0[r] = keep;
     advection_tendency_general(o, in, out, flux_mode, VT, VP, Ft, Fp);
     free(Ft); free(Fp); free(VT); free(VP);
+}
+
+/* test hook: the general rule with ARBITRARY face speeds (pins of the phi sweep with phi-varying speeds and of the alpha
+ * window, tests/test_oracle_general_rule.py).  VT: [nt+1][np], VT[f][k] at theta-face f+1/2 of column k; VP: [nt+2][np],
+ * VP[j][k] at phi-face k-1/2 of row j (rows 1..nt used). */
+void SUF(sft_oracle_advection_tendency_faces)(void *h, const real *in, real *out, int flux_mode, const real *VT, const real *VP) {
+    oracle_t *o = (oracle_t *)h;
+    real *Ft = (real *)malloc((size_t)(o->nt + 1) * o->np * sizeof(real)), *Fp = (real *)calloc(fsize(o), sizeof(real));
+    advection_tendency_general(o, in, out, flux_mode, VT, VP, Ft, Fp);
+    free(Ft); free(Fp);
 }
 
 void SUF(sft_oracle_advection_tendency)(void *h, int r, const real *in, real *out, int flux_mode) {

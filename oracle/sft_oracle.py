@@ -130,6 +130,20 @@ class Oracle:
         f(self.h, int(r), self._rp(a), self._rp(out), flux_mode, float(b0_gauss))
         return out
 
+    def advection_tendency_faces(self, a, vt_faces, vp_faces, flux_mode=ADV_WENO3):
+        """F_A through the variable-face-speed rule with ARBITRARY face speeds (test hook): vt_faces [nt+1][np] at the
+        theta-faces f+1/2, vp_faces [nt+2][np] at the phi-faces k-1/2 (rows 1..nt used), both in R_sun/hr."""
+        a = np.ascontiguousarray(a, dtype=self.dtype)
+        vt = np.ascontiguousarray(vt_faces, dtype=self.dtype)
+        vp = np.ascontiguousarray(vp_faces, dtype=self.dtype)
+        assert a.shape == (self.nt + 2, self.np_) and vt.shape == (self.nt + 1, self.np_) and vp.shape == (self.nt + 2, self.np_)
+        out = np.zeros_like(a)
+        f = self._f("sft_oracle_advection_tendency_faces")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        f(self.h, self._rp(a), self._rp(out), flux_mode, self._rp(vt), self._rp(vp))
+        return out
+
     def set_rfe(self, model, flux_per_hr, tau_hours=float("inf"), seed=0):
         """Random flux emergence (Sec. 2.4): model 0 off / 1 Eq. 13 / 2 Eq. 14; flux_per_hr in G radius_cm^2 / hr."""
         f = self._f("sft_oracle_set_rfe")
