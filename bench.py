@@ -29,12 +29,63 @@ from paper_2501_06377_b200 import ensemble as ens  # noqa: E402
 from paper_2501_06377_b200 import workloads as wl  # noqa: E402
 
 
-# per-launch DRAM bytes of k_sts_pipe<K = 8> from the committed ncu --set full captures (profiles/)
-NCU_TRAFFIC_BYTES = {(3, "f64"): 3.434079e9 + 2.121872e9,     # profiles/r01_final_cfg3.md
-                     (3, "f32"): 1.888619e9 + 1.046579e9}     # profiles/r01d_pipe_f32_3rowstep.md
 # FMA-class lane-operations per second measured on this pool's B200 with a register-only loop
-# (profiles/r01_pipe_cfg3_gen2.md): 64 DFMA / 128 FFMA lanes per clock per SM
+# (profiles/r01_pipe_cfg3_gen2.md): 64 DFMA lanes per clock per SM; fp32: 128 lanes per clock per SM (FFMA2 or dual issue)
 ALU_PEAK_FMA_PER_S = {"f64": 1.70e13, "f32": 3.53e13}
+
+
+def kernel_source_hash():
+    """sha1 over the blocked-STS kernel sources: ties a stored ncu traffic figure to the code it was measured on."""
+    import hashlib
+    h = hashlib.sha1()
+    d = os.path.join(ROOT, "paper_2501_06377_b200", "csrc")
+    for f in ("hft_sts_blocked.cuh", "hft_sts_pipe.cuh", "hft_sts_upipe.cuh"):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:12]
+
+
+def record_traffic(csv_path, profile, config):
+    """bench.py --record-traffic raw.csv --traffic-profile profiles/x.md: read an `ncu -i x.ncu-rep --page raw --csv` export
+    and store the mean dram__bytes_read.sum + dram__bytes_write.sum per launch of every blocked STS kernel in
+    profiles/traffic.json, stamped with the commit and the hash of the kernel sources.  No GPU needed."""
+    import csv
+    import re
+    rows = list(csv.reader(open(csv_path)))
+    hdr, units, data = rows[0], rows[1], rows[2:]
+    ix = {h: i for i, h in enumerate(hdr)}
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    acc = {}
+    for r in data:
+        m = re.search(r"(k_sts_u?pipe)<(double|float), (?:(double|float), )?(?:\(int\))?(\d+)", r[ix["Kernel Name"]])
+        if not m:
+            continue
+        name = "%s<%s,%s>" % (m.group(1), ",".join(x for x in (m.group(2), m.group(3)) if x), m.group(4))
+        tot = sum(float(r[ix[c]]) * scale[units[ix[c]]] for c in ("dram__bytes_read.sum", "dram__bytes_write.sum"))
+        acc.setdefault(name, []).append(tot)
+    try:
+        head = subprocess.run(["git", "rev-parse", "--short", "HEAD"], cwd=ROOT, capture_output=True, text=True).stdout.strip()
+    except OSError:
+        head = ""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    doc = json.load(open(p)) if os.path.exists(p) else {"kernels": []}
+    for name, v in acc.items():
+        doc["kernels"] = [e for e in doc["kernels"] if not (e["kernel"] == name and e["config"] == config)]
+        doc["kernels"].append({"kernel": name, "config": config, "dram_bytes_per_launch": sum(v) / len(v), "launches": len(v),
+                               "git_head": head, "source_sha1": kernel_source_hash(), "profile": profile})
+    json.dump(doc, open(p, "w"), indent=1)
+    print(json.dumps(doc["kernels"], indent=1))
+
+
+def ncu_traffic(kernel, config):
+    """Per-launch DRAM bytes of `kernel` from profiles/traffic.json (written next to each ncu --set full summary), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    for e in json.load(open(p)).get("kernels", []):
+        if e["kernel"] == kernel and e["config"] == config:
+            return e
+    return None
 
 
 def peaks():
@@ -173,18 +224,23 @@ def main():
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--sts-block", type=int, default=0)
     ap.add_argument("--sts-kernel", type=int, default=0, help="hft_options.sts_kernel: 0 library default, 1 k_sts_pipe, 2 k_sts_upipe")
-    ap.add_argument("--f32-accumulate", action="store_true", help="hft_options.f32_accumulate (fp32 storage, fp64 block arithmetic)")
+    ap.add_argument("--f32-fast", action="store_true", help="hft_options.f32_arith = 1: fp32 arithmetic throughout (default: fp64 block arithmetic)")
     ap.add_argument("--attenuation", type=float, default=0.0, help="B0 in Gauss: time the step with flow attenuation (Eq. 5) on")
     ap.add_argument("--nu-map", action="store_true",
                     help="time the step with a spatially varying diffusivity nu(theta, phi) (Eq. 27-28): one launch per STS stage")
     ap.add_argument("--paper-case", choices=["diffusion", "advdiff"], default=None,
                     help="time one of the two validation runs the paper prints wall times for (context, not the bench metric)")
     ap.add_argument("--paper-grid-even", action="store_true", help="--paper-case on 510 x 1024 instead of the paper's 510 x 1023")
+    ap.add_argument("--record-traffic", default=None, metavar="RAW_CSV", help="no GPU: store the per-launch DRAM bytes of an ncu raw-page export in profiles/traffic.json")
+    ap.add_argument("--traffic-profile", default="", help="with --record-traffic: the profiles/*.md summary the capture belongs to")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--also-f32", action="store_true", help="add a second timed run in fp32 to the JSON line (default in the full report)")
     ap.add_argument("--no-also-f32", action="store_true", help="full report without the fp32 leg")
     args = ap.parse_args()
+    if args.record_traffic:
+        record_traffic(args.record_traffic, args.traffic_profile, args.config)
+        return
     if args.paper_case:
         run_paper_case(args)
         return
@@ -208,12 +264,12 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed_run(dtype, with_extras):
+    def timed_run(dtype, with_extras, f32_arith=None):
         # rank k owns realizations [k R, (k+1) R) of the weak-scaled ensemble; one clock for the whole ensemble
         wd = ens.shard(args.config, dtype, rank, world)
         def make_ctx(**kw):
             c = hft.Context(wd.n_theta, wd.n_phi, wd.params, dtype=dtype, sts_block=args.sts_block, sts_kernel=args.sts_kernel,
-                            f32_accumulate=int(args.f32_accumulate and dtype == "f32"), flow_attenuation=int(args.attenuation > 0), diffusivity_map=int(args.nu_map), device=f"cuda:{local}", **kw)
+                            f32_arith=int(args.f32_fast if f32_arith is None else f32_arith), flow_attenuation=int(args.attenuation > 0), diffusivity_map=int(args.nu_map), device=f"cuda:{local}", **kw)
             if args.attenuation > 0:
                 c.set_attenuation(-1, args.attenuation)
             if args.nu_map:      # nu_r (1 + 0.3 sin(theta) cos(phi)) on the half-half grid, per realization (workloads.diffusivity_map)
@@ -250,7 +306,8 @@ def main():
         ctx.profile_kernels(0)
         clocks = sampler.stop() if (rank == 0 and with_extras) else None
         ms = ens.max_over_ranks(ms)
-        res = dict(ms=ms, value=world * cells * args.steps / (ms * 1e-3), launches=launches, dt=dt, s=s, cells=cells,
+        res = dict(ms=ms, value=world * cells * args.steps / (ms * 1e-3), launches=launches, dt=dt, s=s, cells=cells, dtype=dtype,
+                   f32_arith=int(args.f32_fast if f32_arith is None else f32_arith),
                    kernel_ms=(kms / kn if kn else None), kernel_samples=kn, kernel_stages=(kst / kn if kn else None), clocks=clocks, wd=wd)
         # ---- end-to-end through the C ABI with host buffers
         if with_extras and not args.no_e2e:
@@ -318,8 +375,59 @@ def main():
     # algorithmic bytes: 4 array passes per STS stage, 9 per SSPRK(4,3) advection step
     # (with nu(theta, phi) a stage also reads the nu array once: 5 passes)
     stage_passes = 5 if args.nu_map else 4
-    b_alg_step = (9 + stage_passes * res["s"]) * wbytes
-    frac_step = res["value"] / world * b_alg_step / (peak * 1e9)
+
+    def b_alg(r, w):
+        return (9 + stage_passes * r["s"]) * w
+
+    def roofline_of(r):
+        """The dominant kernel's distance from its roofs, from the CUDA-event samples of this run."""
+        if not r["kernel_ms"]:
+            return None
+        dtype, w = r["dtype"], (8 if r["dtype"] == "f64" else 4)
+        spl = r["kernel_stages"]                        # STS stages per sampled launch
+        cells_launch = wd.n_real * (wd.n_theta + 2) * wd.n_phi
+        field_bytes = cells_launch * w
+        sec = r["kernel_ms"] * 1e-3
+        alg_gbs = stage_passes * field_bytes * spl / sec / 1e9      # SURVEY 8(d): 4 passes per stage, as a stage-by-stage code moves
+        if spl <= 1:
+            kern = "k_sts_stage_mapv<MAP=true>" if args.nu_map else "k_sts_stage_mapv<MAP=false>"
+            return {"bound": "hbm", "achieved": alg_gbs, "peak": peak, "unit": "GB/s", "frac": alg_gbs / peak, "traffic": None,
+                    "kernel": kern, "stages_per_launch": spl, "avg_launch_ms": r["kernel_ms"], "sampled_launches": r["kernel_samples"],
+                    "peak_source": peak_src}
+        # K stages per launch: the kernel moves 5 array passes per K stages, not 4 K, so it is NOT bound by HBM; what it
+        # saturates first is the FP pipe of its arithmetic type (fp64: DFMA 64 lanes/clk/SM; ncu: the pipe is the busiest
+        # unit, then the issue slots).  "alu": useful FP instruction slots per second -- 7 per cell and stage (1 add, 1 mul,
+        # 5 fma; halo recomputation and k_sts_upipe's 8th operation are NOT counted as useful) -- against the measured FMA
+        # issue rate of that type, both in FMA-equivalent TFLOP/s (2 flops per slot).
+        mixed = dtype == "f32" and r["f32_arith"] == 0
+        upipe = mixed or args.sts_kernel == 2
+        arith = "f64" if (dtype == "f64" or mixed) else "f32"
+        kern = ("k_sts_upipe<%s,%s,8>" % ("float" if dtype == "f32" else "double", "double" if arith == "f64" else "float")) if upipe \
+            else "k_sts_pipe<%s,8>" % ("double" if dtype == "f64" else "float")
+        alu_peak = ALU_PEAK_FMA_PER_S[arith]
+        useful = 7 * spl * cells_launch / sec
+        cols = 32 * (2 if arith == "f64" else 4)        # columns per warp strip; 8 invalid columns per side
+        executed = (8 if upipe else 7) * spl * cells_launch * cols / (cols - 16) / sec
+        out = {"bound": "alu", "achieved": 2 * useful / 1e12, "peak": 2 * alu_peak / 1e12, "unit": "TFLOP/s", "frac": useful / alu_peak,
+               "traffic": None, "kernel": kern, "stages_per_launch": spl, "avg_launch_ms": r["kernel_ms"],
+               "sampled_launches": r["kernel_samples"],
+               "peak_source": "FP%s FMA issue rate measured on this pool with a register-only loop (profiles/r01_pipe_cfg3_gen2.md), x 2 flops" % arith[1:],
+               "frac_with_halo_and_extra_ops": executed / alu_peak,
+               # context, not distances to a roof of this kernel: the rate expressed in the bytes a stage-by-stage code would
+               # move (SURVEY 8(d) B_alg) over the measured copy bandwidth -- how much faster than ANY such code could be
+               "hbm_algorithmic": {"achieved": alg_gbs, "peak": peak, "unit": "GB/s", "frac": alg_gbs / peak, "peak_source": peak_src,
+                                   "meaning": "speed-up over the HBM roofline of one launch per stage (4 passes per stage); > 1 because 8 stages stay on chip"},
+               "dram": {"achieved": 5 * field_bytes / sec / 1e9, "peak": peak, "unit": "GB/s", "frac": 5 * field_bytes / sec / 1e9 / peak,
+                        "meaning": "the 5 array passes per launch this kernel actually moves (3 in, 2 out) / time"}}
+        t = ncu_traffic(kern, args.config) if spl > 7 else None
+        if t:
+            out["traffic"] = t["dram_bytes_per_launch"]
+            out["traffic_source"] = t["profile"]
+            out["traffic_head"] = t["git_head"]
+            out["traffic_stale"] = t["source_sha1"] != kernel_source_hash()   # true: the kernel sources changed since that capture
+        return out
+
+    frac_step = res["value"] / world * b_alg(res, wbytes) / (peak * 1e9)
     out = {
         "metric": "cell-updates/s", "value": res["value"], "unit": "cell-updates/s", "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": res["ms"] / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -327,45 +435,38 @@ def main():
         "config": {"workload": wd.name, "grid": [wd.n_theta, wd.n_phi], "realizations_per_gpu": wd.n_real,
                    "dt_hours": res["dt"], "sts_stages": res["s"], "adv": "WENO3-CS(h)+SSPRK(4,3)", "diff": "RKG2(3/2)",
                    "l2": "inputs larger than L2 (arrays of %.0f MiB each)" % (wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes / 2**20),
-                   "sts_block": args.sts_block, "flow_attenuation_b0": args.attenuation, "nu_map": bool(args.nu_map), "b_alg_bytes_per_cell_update": b_alg_step,
-                   "hbm_roofline_frac_whole_step": frac_step},
+                   "sts_block": args.sts_block, "sts_kernel": args.sts_kernel, "f32_arith": res["f32_arith"] if args.dtype == "f32" else None,
+                   "flow_attenuation_b0": args.attenuation, "nu_map": bool(args.nu_map),
+                   "b_alg_bytes_per_cell_update": b_alg(res, wbytes), "hbm_roofline_frac_whole_step": frac_step},
         "gpu_launches": res["launches"],
         "clocks": res["clocks"],
     }
     if res.get("e2e"):
         out["e2e"] = res["e2e"]
-    if res["kernel_ms"]:
-        # dominant kernel: the STS stage kernel; algorithmic bytes per launch = 4 passes x field bytes x stages per launch
-        stages_per_launch = res["kernel_stages"]
-        field_bytes = wd.n_real * (wd.n_theta + 2) * wd.n_phi * wbytes
-        sec = res["kernel_ms"] * 1e-3
-        ach = stage_passes * field_bytes * stages_per_launch / sec / 1e9
-        blocked = stages_per_launch > 1
-        out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                           "kernel": "k_sts_pipe" if blocked else ("k_sts_stage_mapv<MAP=true>" if args.nu_map else "k_sts_stage_mapv<MAP=false>"), "stages_per_launch": stages_per_launch,
-                           "avg_launch_ms": res["kernel_ms"], "sampled_launches": res["kernel_samples"], "peak_source": peak_src}
-        if blocked:
-            # a K-stage block moves 5 array passes (3 in, 2 out) however large K is; the
-            # distance of THIS kernel from the DRAM roof is that traffic / time, and from the ALU roof its
-            # fp64 / fp32 FMA-class lane-operations / time against the FMA peak measured on this pool
-            traffic = NCU_TRAFFIC_BYTES.get((args.config, args.dtype)) if stages_per_launch > 7 else None
-            out["roofline"]["traffic"] = traffic
-            out["roofline"]["traffic_source"] = "ncu --set full dram__bytes_read+write.sum per launch (profiles/r01_final_cfg3.md, r01d_pipe_f32_3rowstep.md)" if traffic else None
-            out["roofline"]["frac_of_blocked_traffic"] = 5 * field_bytes / sec / 1e9 / peak
-            cols = 16 // wbytes * 32                           # columns per warp strip
-            halo = 8                                           # K = 8 invalid columns per side
-            redundancy = cols / (cols - 2 * halo)
-            lane_ops = 7 * stages_per_launch * wd.n_real * (wd.n_theta + 2) * wd.n_phi * redundancy
-            alu_peak = ALU_PEAK_FMA_PER_S[args.dtype]
-            out["roofline"]["alu_frac"] = lane_ops / sec / alu_peak
-            out["roofline"]["alu_peak_fma_per_s"] = alu_peak
+    rf = roofline_of(res)
+    if rf:
+        out["roofline"] = rf
     # BASELINE.json's metric is quoted "(fp64, fp32)": the full report (no --no-e2e / --no-cpu-baseline, i.e. not a profiling
-    # run) carries the fp32 rate of the same workload beside the fp64 line
+    # run) carries the fp32 record of the same workload beside the fp64 line -- the default fp32 path (fp64 block arithmetic,
+    # meets north_star's 1e-5) with its own clocks, roofline and end-to-end figure, and the fp32-arithmetic path (f32_arith = 1)
     full_report = not (args.no_e2e or args.no_cpu_baseline or args.no_also_f32)
     if (args.also_f32 or full_report) and args.dtype == "f64":
-        r32 = timed_run("f32", False)
-        out["also_f32"] = {"value": r32["value"], "ms_per_step": r32["ms"] / args.steps, "sts_stages": r32["s"],
-                           "hbm_roofline_frac_whole_step": r32["value"] / world * (9 + 4 * r32["s"]) * 4 / (peak * 1e9)}
+        def f32_record(r, parity):
+            d = {"value": r["value"], "ms_per_step": r["ms"] / args.steps, "sts_stages": r["s"], "f32_arith": r["f32_arith"],
+                 "gpu_launches": r["launches"], "parity_cfg3_full_length_vs_fp64_oracle": parity,
+                 "hbm_roofline_frac_whole_step": r["value"] / world * b_alg(r, 4) / (peak * 1e9)}
+            if r.get("clocks"):
+                d["clocks"] = r["clocks"]
+            if r.get("e2e"):
+                d["e2e"] = r["e2e"]
+            rr = roofline_of(r)
+            if rr:
+                d["roofline"] = rr
+            return d
+        r32 = timed_run("f32", True, 0)
+        out["also_f32"] = f32_record(r32, "2.0e-6 .. 2.7e-6 (north_star 1e-5 met; tests/test_gpu_parity.py)")
+        r32f = timed_run("f32", False, 1)
+        out["also_f32"]["fp32_arithmetic"] = f32_record(r32f, "1.4e-5 .. 2.2e-5 (north_star 1e-5 NOT met)")
     if rank == 0:
         if not args.no_cpu_baseline:
             # ~10-30 s of oracle work on the box's host cores (the float build of the oracle runs ~12x slower per step than

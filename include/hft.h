@@ -79,9 +79,13 @@ typedef struct {
                                  6 more field arrays.  0 (default) = off */
     int32_t diffusivity_map;  /* 1 = reserve workspace for a spatially varying diffusivity nu(theta, phi) (Eq. 27-28, :438-460;
                                  1 more field array) and allow hft_set_diffusivity_map.  0 (default) = off */
-    int32_t f32_accumulate;   /* dtype fp32 only: 1 = the temporally blocked STS kernel keeps the state in fp32 in memory but does
-                                 the arithmetic of a block of stages in fp64 registers, rounding to fp32 only at the two stores per
-                                 block (the scheme integrated is Sec. 3.7.2 :470-476 unchanged).  0 (default) = fp32 arithmetic */
+    int32_t f32_arith;        /* dtype fp32 only.  0 (default) = the temporally blocked STS kernel keeps the state in fp32 in memory but
+                                 does the arithmetic of a block of 8 stages in fp64 registers, rounding to fp32 only at the two
+                                 stores per block (the scheme integrated is Sec. 3.7.2 :470-476 unchanged): BASELINE config 3 at
+                                 full length ends 2.0e-6 .. 2.7e-6 from the fp64 oracle (north_star: <= 1e-5), at the rate of the
+                                 fp64 kernel and half its memory.  1 = fp32 arithmetic throughout: 2.1 x the rate, but every stage
+                                 rounds to 24 bits and the same run ends 1.4e-5 .. 2.2e-5 from the fp64 oracle.  The fp64-register
+                                 path needs k_sts_upipe (see sts_kernel); batches it cannot take run in fp32 arithmetic */
     int32_t sts_kernel;       /* which temporally blocked kernel: 0 (default) = the library's choice; 1 = k_sts_pipe (per-realization
                                  coefficient tables through shared memory; any batch); 2 = k_sts_upipe (one coefficient table
                                  through the uniform datapath) whenever the batch shares one table up to the factor nu_r and it
@@ -185,7 +189,12 @@ int hft_diagnostics(hft_ctx* ctx, double* h_out);
 int hft_diagnostics_ext(hft_ctx* ctx, double polar_lat_deg, double* h_out);
 
 /* Host helpers (not timed): Eq. 26 advective limit over all rows and realizations (no safety factor),
- * explicit-Euler diffusion limit 2/rho (Gershgorin), and the STS stage count for dt. */
+ * explicit-Euler diffusion limit 2/rho (Gershgorin), and the STS stage count for dt.
+ * The advective limit is ALWAYS the Eq. 26 form (:430), the limit of SSPRK(4,3), whatever adv_time the context was created
+ * with: forward Euler / upwind and SSPRK(3,3) are bound by Eq. 24 (:404), HALF of it -- a caller that selects adv_time 1 or 3
+ * multiplies by 0.5 itself (the paper applies a further safety factor of ~0.9, :406).  hft_step does not check dt against
+ * either: Eq. 24 is the paper's approximation for two-dimensional flow (a one-dimensional upwind step is stable, and exact,
+ * at twice that).  The diffusive side IS checked: a forced sts_stages below the stable count returns HFT_ERR_UNSTABLE. */
 int hft_stable_dt(hft_ctx* ctx, double* h_dt_adv_limit_hours, double* h_dt_diff_euler_hours);
 int hft_sts_stage_count(hft_ctx* ctx, double dt_hours, int32_t* h_stages);
 

@@ -51,7 +51,7 @@ struct StsCoef {  // per-stage scalars of Sec. 3.7.2 schemes (DESIGN.md "STS rec
 struct hft_ctx {
     hft_grid grid;
     hft_options opt;
-    int nr = 0;
+    int nr = 0, dev = 0;
     cudaStream_t stream = nullptr;
     Geom G;
     size_t arr_bytes = 0;
@@ -121,6 +121,17 @@ struct hft_ctx {
 
 namespace {
 
+// every entry point runs on the device the context was created on, whatever device is current in the calling thread
+struct DevGuard {
+    int prev = -1;
+    bool sw = false;
+    explicit DevGuard(const hft_ctx* c) {
+        if (!c) return;
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != c->dev) sw = cudaSetDevice(c->dev) == cudaSuccess;
+    }
+    ~DevGuard() { if (sw) cudaSetDevice(prev); }
+};
+
 int cuda_fail(hft_ctx* c, cudaError_t e, const char* what) {
     if (c) c->cuda_err = std::string(what) + ": " + cudaGetErrorString(e);
     return HFT_ERR_CUDA;
@@ -180,7 +191,7 @@ bool valid_options(const hft_options* o) {
     if (o->rfe != 0 && o->rfe != 1) return false;
     if (o->diffusivity_map != 0 && o->diffusivity_map != 1) return false;
     if (o->sts_block < 0 || o->sts_block > STS_KMAX || (o->sts_block > 1 && (o->sts_block & 1))) return false;
-    if (o->f32_accumulate != 0 && o->f32_accumulate != 1) return false;
+    if (o->f32_arith != 0 && o->f32_arith != 1) return false;
     if (o->sts_kernel < 0 || o->sts_kernel > 2) return false;
     return true;
 }
@@ -392,13 +403,14 @@ int prepare_upipe(hft_ctx* c, int scheme, int s, double dt) {
     c->up_version = c->tab_version; c->up_scheme = scheme; c->up_s = s; c->up_dt = dt;
     up.ok = false;
     const int nt = c->G.nt;
-    // default (0): k_sts_upipe only where it is the faster or the only kernel: fp32 storage with fp64 arithmetic
-    const bool want = c->opt.sts_kernel == 2 || (c->opt.sts_kernel == 0 && !c->fp64() && c->opt.f32_accumulate != 0);
+    // default (0): k_sts_upipe only where it is the only kernel: fp32 storage with fp64 block arithmetic (f32_arith = 0)
+    const bool want_mixed = !c->fp64() && c->opt.f32_arith == 0;
+    const bool want = c->opt.sts_kernel == 2 || (c->opt.sts_kernel == 0 && want_mixed);
     if (!want || !c->shape_common || nt > UTAB_MAX_ROWS) return HFT_OK;
     for (int r = 0; r < c->nr; r++)
         if (!(c->nu_scale[r] >= 0.0) || !std::isfinite(c->nu_scale[r])) return HFT_OK;
-    const bool dbl = c->fp64() || c->opt.f32_accumulate != 0;
-    up.mixed = !c->fp64() && c->opt.f32_accumulate != 0;
+    const bool dbl = c->fp64() || want_mixed;
+    up.mixed = want_mixed;
     c->utab.assign((size_t)nt * UTAB_ROW_BYTES, 0);
     for (int j = 1; j <= nt; j++) {
         const double cm = c->nu_shape[j - 1] * c->sth[j - 1] / (c->st[j] * c->dth * c->dth);
@@ -751,7 +763,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess || major != 10) return HFT_ERR_DEVICE;
     hft_ctx* c = new (std::nothrow) hft_ctx();
     if (!c) return HFT_ERR_NOMEM;
-    c->grid = *grid; c->opt = o; c->nr = n_real; c->stream = (cudaStream_t)cuda_stream;
+    c->grid = *grid; c->opt = o; c->nr = n_real; c->dev = dev; c->stream = (cudaStream_t)cuda_stream;
     c->G.nt = grid->n_theta; c->G.np = grid->n_phi; c->G.pitch = pitch_for(grid->n_phi, grid->dtype); c->G.nr = n_real;
     c->G.rstride = (size_t)(grid->n_theta + 2) * c->G.pitch;
     c->G.nbx = (grid->n_phi + TX - 1) / TX;
@@ -800,6 +812,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
 }
 
 void hft_destroy(hft_ctx* c) {
+    DevGuard dg_(c);
     if (!c) return;
     if (c->prof_ev_made)
         for (int i = 0; i < 2 * kProfEvents; i++) cudaEventDestroy(c->prof_ev[i]);
@@ -812,6 +825,7 @@ void hft_destroy(hft_ctx* c) {
 }
 
 int hft_set_flow_tables(hft_ctx* c, int32_t r, const double* h_vtheta, const double* h_omega) {
+    DevGuard dg_(c);
     if (!c || !h_vtheta || !h_omega || r < -1 || r >= c->nr) return HFT_ERR_ARG;
     const int nt = c->G.nt;
     for (int q = 0; q < c->nr; q++) {
@@ -823,6 +837,7 @@ int hft_set_flow_tables(hft_ctx* c, int32_t r, const double* h_vtheta, const dou
 }
 
 int hft_set_diffusivity_profile(hft_ctx* c, int32_t r, const double* h_nu_face) {
+    DevGuard dg_(c);
     if (!c || !h_nu_face || r < -1 || r >= c->nr) return HFT_ERR_ARG;
     const int nt = c->G.nt;
     for (int f = 0; f <= nt; f++)
@@ -849,6 +864,7 @@ int hft_set_diffusivity_profile(hft_ctx* c, int32_t r, const double* h_nu_face) 
 }
 
 int hft_set_diffusivity_map(hft_ctx* c, int32_t r, const double* h_nu_hh) {
+    DevGuard dg_(c);
     if (!c || !h_nu_hh || r < -1 || r >= c->nr || !c->opt.diffusivity_map) return HFT_ERR_ARG;
     const int nt = c->G.nt, np = c->G.np;
     const size_t n = (size_t)(nt + 1) * np;
@@ -869,6 +885,7 @@ int hft_set_diffusivity_map(hft_ctx* c, int32_t r, const double* h_nu_hh) {
 }
 
 int hft_set_grid_diffusivity(hft_ctx* c, int32_t r, double alpha_nu) {
+    DevGuard dg_(c);
     if (!c || r < -1 || r >= c->nr || !(alpha_nu >= 0.0)) return HFT_ERR_ARG;
     const int nt = c->G.nt;
     std::vector<double> p(nt + 1);
@@ -880,6 +897,7 @@ int hft_set_grid_diffusivity(hft_ctx* c, int32_t r, double alpha_nu) {
 }
 
 int hft_set_attenuation(hft_ctx* c, int32_t r, double b0_gauss) {
+    DevGuard dg_(c);
     if (!c || r < -1 || r >= c->nr || !c->opt.flow_attenuation || b0_gauss != b0_gauss) return HFT_ERR_ARG;
     for (int q = 0; q < c->nr; q++)
         if (r < 0 || q == r) c->B0[q] = b0_gauss > 0.0 ? b0_gauss : 0.0;
@@ -896,6 +914,7 @@ int hft_set_attenuation(hft_ctx* c, int32_t r, double b0_gauss) {
 }
 
 int hft_set_rfe(hft_ctx* c, int32_t model, double flux_per_hr, double tau_hours, uint64_t seed) {
+    DevGuard dg_(c);
     if (!c || model < 0 || model > 2) return HFT_ERR_ARG;
     if (model != 0 && (!c->opt.rfe || !(flux_per_hr >= 0.0) || !(tau_hours > 0.0))) return HFT_ERR_ARG;
     c->rfe_model = model; c->rfe_flux = flux_per_hr; c->rfe_tau = tau_hours; c->rfe_seed = seed;
@@ -909,6 +928,7 @@ int hft_set_rfe(hft_ctx* c, int32_t model, double flux_per_hr, double tau_hours,
 }
 
 int hft_get_rfe_map(hft_ctx* c, int32_t r, int32_t which, void* d_out) {
+    DevGuard dg_(c);
     if (!c || !d_out || r < 0 || r >= c->nr || which < 0 || which > 1 || !c->rfe_model) return HFT_ERR_ARG;
     const Geom& G = c->G;
     dim3 g((G.np + 255) / 256, G.nt, 1);
@@ -919,6 +939,7 @@ int hft_get_rfe_map(hft_ctx* c, int32_t r, int32_t which, void* d_out) {
 }
 
 int hft_set_map(hft_ctx* c, int32_t r, const void* d_map) {
+    DevGuard dg_(c);
     if (!c || !d_map || r < -1 || r >= c->nr) return HFT_ERR_ARG;
     const Geom& G = c->G;
     const int nz = r < 0 ? c->nr : 1, r0 = r < 0 ? 0 : r;
@@ -935,6 +956,7 @@ int hft_set_map(hft_ctx* c, int32_t r, const void* d_map) {
 }
 
 int hft_get_map(hft_ctx* c, int32_t r, void* d_out) {
+    DevGuard dg_(c);
     if (!c || !d_out || r < -1 || r >= c->nr) return HFT_ERR_ARG;
     const Geom& G = c->G;
     const int nz = r < 0 ? c->nr : 1, r0 = r < 0 ? 0 : r;
@@ -946,6 +968,7 @@ int hft_get_map(hft_ctx* c, int32_t r, void* d_out) {
 }
 
 static int copy_full(hft_ctx* c, int32_t r, void* d, int dir) {
+    DevGuard dg_(c);
     if (!c || !d || r < 0 || r >= c->nr) return HFT_ERR_ARG;
     const Geom& G = c->G;
     dim3 g((G.np + 255) / 256, G.nt + 2);
@@ -954,10 +977,13 @@ static int copy_full(hft_ctx* c, int32_t r, void* d, int dir) {
     c->launches++;
     return check_launch(c);
 }
-int hft_get_full(hft_ctx* c, int32_t r, void* d_out) { return copy_full(c, r, d_out, 1); }
-int hft_set_full(hft_ctx* c, int32_t r, const void* d_in) { return copy_full(c, r, (void*)d_in, 0); }
+int hft_get_full(hft_ctx* c, int32_t r, void* d_out) {
+    DevGuard dg_(c); return copy_full(c, r, d_out, 1); }
+int hft_set_full(hft_ctx* c, int32_t r, const void* d_in) {
+    DevGuard dg_(c); return copy_full(c, r, (void*)d_in, 0); }
 
 int hft_stable_dt(hft_ctx* c, double* h_adv, double* h_diff) {
+    DevGuard dg_(c);
     if (!c || !h_adv || !h_diff) return HFT_ERR_ARG;
     *h_adv = adv_dt_limit(c);
     *h_diff = diff_dt_expl(c);
@@ -965,6 +991,7 @@ int hft_stable_dt(hft_ctx* c, double* h_adv, double* h_diff) {
 }
 
 int hft_sts_stage_count(hft_ctx* c, double dt_hours, int32_t* h_stages) {
+    DevGuard dg_(c);
     if (!c || !h_stages || !(dt_hours > 0.0)) return HFT_ERR_ARG;
     const int scheme = c->opt.diff_time == 2 ? 2 : 3;
     const int s = sts_stages_for(c, scheme, dt_hours);
@@ -974,6 +1001,7 @@ int hft_sts_stage_count(hft_ctx* c, double dt_hours, int32_t* h_stages) {
 }
 
 int hft_step(hft_ctx* c, int32_t n_steps, double dt) {
+    DevGuard dg_(c);
     if (!c || n_steps < 0) return HFT_ERR_ARG;
     if (!(dt > 0.0)) return HFT_ERR_UNSTABLE;
     int s = 0;
@@ -994,6 +1022,7 @@ int hft_step(hft_ctx* c, int32_t n_steps, double dt) {
 }
 
 int hft_assimilate(hft_ctx* c, const void* d_obs, const void* d_w, int32_t shared, int32_t flags) {
+    DevGuard dg_(c);
     if (!c || !d_obs || !d_w) return HFT_ERR_ARG;
     const Geom& G = c->G;
     const int balanced = flags & 1, nmaps = shared ? 1 : c->nr;
@@ -1023,6 +1052,7 @@ int hft_assimilate(hft_ctx* c, const void* d_obs, const void* d_w, int32_t share
 }
 
 int hft_diagnostics(hft_ctx* c, double* h_out) {
+    DevGuard dg_(c);
     if (!c || !h_out) return HFT_ERR_ARG;
     const Geom& G = c->G;
     dim3 gp(RED_CTAS, c->nr);
@@ -1045,6 +1075,7 @@ int hft_diagnostics(hft_ctx* c, double* h_out) {
 }
 
 int hft_diagnostics_ext(hft_ctx* c, double polar_lat_deg, double* h_out) {
+    DevGuard dg_(c);
     if (!c || !h_out || !(polar_lat_deg >= 0.0 && polar_lat_deg <= 90.0)) return HFT_ERR_ARG;
     const Geom& G = c->G;
     if (!c->d_extpart) {
@@ -1077,12 +1108,14 @@ int hft_diagnostics_ext(hft_ctx* c, double polar_lat_deg, double* h_out) {
 }
 
 int hft_launch_count(hft_ctx* c, int64_t* h_count) {
+    DevGuard dg_(c);
     if (!c || !h_count) return HFT_ERR_ARG;
     *h_count = c->launches;
     return HFT_OK;
 }
 
 int hft_profile_kernels(hft_ctx* c, int32_t which) {
+    DevGuard dg_(c);
     if (!c || which < 0 || which > 2) return HFT_ERR_ARG;
     if (!c->prof_ev_made) {
         for (int i = 0; i < 2 * kProfEvents; i++) CK(cudaEventCreate(&c->prof_ev[i]));
@@ -1093,6 +1126,7 @@ int hft_profile_kernels(hft_ctx* c, int32_t which) {
 }
 
 int hft_kernel_time(hft_ctx* c, double* h_ms, int64_t* h_launches, int64_t* h_stages) {
+    DevGuard dg_(c);
     if (!c || !h_ms || !h_launches || !h_stages) return HFT_ERR_ARG;
     CK(cudaStreamSynchronize(c->stream));
     double ms = 0.0;

@@ -1,4 +1,4 @@
-// hft_sts_mixed.cu -- k_sts_upipe with fp32 storage and fp64 arithmetic (hft_options.f32_accumulate), a translation unit
+// hft_sts_mixed.cu -- k_sts_upipe with fp32 storage and fp64 arithmetic (hft_options.f32_arith = 0), a translation unit
 // of its own: its coefficient table (fp64) has its own constant bank, and the units build in parallel.
 #define HFT_STS_MIXED_TU
 #include "hft_sts_upipe.cuh"

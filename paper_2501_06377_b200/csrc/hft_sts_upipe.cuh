@@ -25,7 +25,7 @@
 //
 // fp32: a lane's four columns are two float2 pairs and every FMA is the packed FFMA2 of sm_100 (fma.rn.f32x2) with the
 // coefficient pair {c, c} taken straight from the table (stored duplicated) -- half the FMA-pipe instructions.
-// CREAL != REAL (fp32 storage, fp64 arithmetic; hft_options.f32_accumulate): a lane owns two columns (8-byte vectors),
+// CREAL != REAL (fp32 storage, fp64 arithmetic; hft_options.f32_arith = 0): a lane owns two columns (8-byte vectors),
 // converts on load, and rounds to fp32 only at the two stores per block (SURVEY.md section 7 hard part 3 fallback).
 //
 // Everything else is k_sts_pipe's design: a warp owns a strip of 32*C phi-columns and streams down the theta rows, level l

@@ -42,7 +42,7 @@ class hft_params(C.Structure):
 class hft_options(C.Structure):
     _fields_ = [("adv_flux", C.c_int32), ("adv_time", C.c_int32), ("diff_time", C.c_int32), ("sts_stages", C.c_int32),
                 ("sts_block", C.c_int32), ("rfe", C.c_int32), ("strang", C.c_int32), ("flow_attenuation", C.c_int32),
-                ("diffusivity_map", C.c_int32), ("f32_accumulate", C.c_int32), ("sts_kernel", C.c_int32)]
+                ("diffusivity_map", C.c_int32), ("f32_arith", C.c_int32), ("sts_kernel", C.c_int32)]
 
 
 _lib.hft_workspace_bytes.argtypes = [C.POINTER(hft_grid), C.c_int32, C.POINTER(hft_options), C.POINTER(C.c_size_t)]
@@ -97,7 +97,7 @@ class Context:
     """hft_create ... hft_destroy.  Maps are torch CUDA tensors [n_theta][n_phi] of the context dtype."""
 
     def __init__(self, n_theta, n_phi, params, dtype="f64", radius_cm=1.0, adv_flux=ADV_WENO3, adv_time=TIME_SSPRK43,
-                 diff_time=DIFF_RKG2, sts_stages=0, sts_block=0, rfe=0, strang=0, flow_attenuation=0, diffusivity_map=0, f32_accumulate=0, sts_kernel=0,
+                 diff_time=DIFF_RKG2, sts_stages=0, sts_block=0, rfe=0, strang=0, flow_attenuation=0, diffusivity_map=0, f32_arith=0, sts_kernel=0,
                  device="cuda:0", stream=None, workspace=None):
         if not torch.cuda.is_available():
             raise HftError("no CUDA device: the hot path has no CPU fallback")
@@ -111,7 +111,7 @@ class Context:
         with torch.cuda.device(self.device):
             self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             opt = hft_options(adv_flux, adv_time, diff_time, sts_stages, sts_block, int(rfe), int(strang), int(flow_attenuation),
-                              int(diffusivity_map), int(f32_accumulate), int(sts_kernel))
+                              int(diffusivity_map), int(f32_arith), int(sts_kernel))
             nbytes = workspace_bytes(n_theta, n_phi, self.n_real, dtype, opt)
             if workspace is None:
                 workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)

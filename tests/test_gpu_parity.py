@@ -140,15 +140,19 @@ def test_small_ragged_multi_realization(dtype, case):
 @pytest.mark.parametrize("block", [2, 4, 6, 8])
 @pytest.mark.parametrize("s_forced", [0, 41])
 @pytest.mark.parametrize("nphi", [328, 327, 329, 330])
-def test_sts_block_sizes_ragged(dtype, block, s_forced, nphi):
-    """Every temporal-blocking depth K of the STS kernel (hft_options.sts_block) on a grid with ragged strips, a
+@pytest.mark.parametrize("kern", ["pipe", "upipe", "default"])
+def test_sts_block_sizes_ragged(dtype, block, s_forced, nphi, kern):
+    """Both temporally blocked kernels -- k_sts_pipe (sts_kernel = 1), k_sts_upipe (2) in the state's own arithmetic, and
+    the library default (fp32: k_sts_upipe with fp64 block arithmetic) -- at
+    every temporal-blocking depth K of the STS kernel (hft_options.sts_block) on a grid with ragged strips, a
     phi seam inside a strip and theta segments: s = 42 -> (s-1) mod K remainder stages un-blocked; s_forced = 41
     -> (s-1) mod 8 = 0, the block that starts from delta_0 = 0.  n_phi = 327, 329, 330 are not multiples of the
     16-byte vector width (2 doubles / 4 floats): the lanes behind the seam move their columns one by one, a vector
     may straddle the seam (the paper's own grids have odd n_phi in this API: 512 x 1024 files = 510 x 1023 cells)."""
     H = hft()
     w = wl.scaled(wl.config(3), 150, nphi, n_real=2)
-    ctx, o = make_pair(w, dtype, adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKG2, sts_block=block, sts_stages=s_forced)
+    kw = {"pipe": dict(sts_kernel=1, f32_arith=1), "upipe": dict(sts_kernel=2, f32_arith=1), "default": {}}[kern]
+    ctx, o = make_pair(w, dtype, adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKG2, sts_block=block, sts_stages=s_forced, **kw)
     _, dif = o.stable_dt()
     dt = 250.0 * dif
     s = ctx.sts_stage_count(dt)
@@ -259,26 +263,24 @@ def test_config2_full_size_sampled_realizations():
     ctx.close()
 
 
-def test_config3_full_length_sampled_realization():
+def test_config3_full_length_sampled_realizations():
     """BASELINE config 3 at full size AND full length: 2 simulated days = 79 steps of 604 RKG2 stages + SSPRK(4,3) on all
-    64 realizations, in fp64 and in fp32, both started from the same float-representable maps.  The fp64 oracle follows
-    realization 42 through all 79 steps (about half a minute on the box's host cores).
-    fp64 CUDA path: <= 1e-12 (measured 2.3e-15).
-    fp32 CUDA path against the fp64 oracle: measured 1.36e-5 (advection alone 2.3e-6, diffusion alone 1.27e-5: every one of
-    the 79 x 604 stages rounds delta to 24 bits and the three-term recurrence amplifies that noise).  This is what fp32
-    arithmetic gives for this method at this length, not an implementation difference: the oracle built in float is 3.7e-5
-    from the fp64 oracle on the same run, and the CUDA path 3.3e-5 from the float oracle (HFT_SLOW=1 below runs it: 7 min).
-    The 1e-5 gate of north_star therefore holds at the lengths the float oracle can separate implementations (the 2-step
-    full-size test above, all small-grid tests); here the gate is 2e-5 against the fp64 oracle (reading U14)."""
+    64 realizations, started from the same float-representable maps in every precision.  The fp64 oracle follows
+    realizations 0, 21, 42, 63 (BASELINE.md section 3's plan) through all 79 steps, one by one.
+      fp64                                        <= 1e-12 (measured 2.3e-15 .. 3.9e-15)
+      fp32, default (fp64 block arithmetic)       <= 1e-5, north_star's gate (measured 2.0e-6 .. 2.7e-6)
+      fp32, f32_arith = 1 (fp32 arithmetic)       north_star's 1e-5 is NOT met: measured 1.4e-5 .. 2.2e-5.  Every one of the
+          79 x 604 stages rounds delta to 24 bits and the three-term recurrence amplifies that noise; the oracle built in
+          float is itself 3.7e-5 from the fp64 oracle on this run (HFT_SLOW=1 below runs it: 7 min).  The assertion below is
+          a regression bound on that known miss, not a claim of parity."""
     import os
     H = hft()
     w = wl.config(3, "f64")
     maps32 = wl.initial_maps(w, device="cuda").to(torch.float32)
-    r = 42
-    errs = {}
-    ref = None
-    for dtype in ("f64", "f32"):
-        ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype)
+    R = (0, 21, 42, 63)
+    errs, refs, g42 = {}, {}, None
+    for name, kw in (("f64", dict(dtype="f64")), ("f32", dict(dtype="f32")), ("f32_arith1", dict(dtype="f32", f32_arith=1))):
+        ctx = H.Context(w.n_theta, w.n_phi, w.params, **kw)
         for q in range(w.n_real):
             ctx.set_map(q, maps32[q].to(ctx.tdtype).contiguous())
         dt, n, _ = wl.plan(w, *ctx.stable_dt())
@@ -287,27 +289,31 @@ def test_config3_full_length_sampled_realization():
         before = ctx.diagnostics()
         ctx.step(n, dt)
         after = ctx.diagnostics()
-        cons = 1e-12 if dtype == "f64" else 1e-4
+        cons = 1e-12 if name == "f64" else 1e-4
         assert np.all(np.abs(after[:, 0] - before[:, 0]) <= cons * before[:, 1])
-        if ref is None:
-            o = orc.Oracle(w.n_theta, w.n_phi, w.params[r:r + 1], dtype=np.float64)
-            o.set_map(0, maps32[r].double().cpu().numpy())
-            o.step(n, dt, sts_stages=s)
-            ref = o.get_full(0)
-            o.close()
-        g = ctx.get_full(r).cpu().numpy()
-        errs[dtype] = rel_linf(g, ref)
+        if not refs:
+            for r in R:
+                o = orc.Oracle(w.n_theta, w.n_phi, w.params[r:r + 1], dtype=np.float64)
+                o.set_map(0, maps32[r].double().cpu().numpy())
+                o.step(n, dt, sts_stages=s)
+                refs[r] = o.get_full(0)
+                o.close()
+        errs[name] = [rel_linf(ctx.get_full(r).cpu().numpy(), refs[r]) for r in R]
+        if name == "f32_arith1":
+            g42 = ctx.get_full(42).cpu().numpy()
         ctx.close()
-    print("cfg3 full length (79 steps), realization 42: rel L-inf fp64 %.3e, fp32 %.3e" % (errs["f64"], errs["f32"]))
-    assert errs["f64"] <= 1e-12 and errs["f32"] <= 2e-5, errs
+    print("cfg3 full length (79 steps), realizations %s: rel L-inf %s" % (R, {k: ["%.2e" % e for e in v] for k, v in errs.items()}))
+    assert max(errs["f64"]) <= 1e-12, errs
+    assert max(errs["f32"]) <= 1e-5, errs                  # north_star's fp32 gate, met by the default fp32 path
+    assert max(errs["f32_arith1"]) <= 3e-5, errs           # fp32 arithmetic: north_star NOT met (1.4e-5 .. 2.2e-5); regression bound
     if os.environ.get("HFT_SLOW") == "1":
-        o = orc.Oracle(w.n_theta, w.n_phi, w.params[r:r + 1], dtype=np.float32)
-        o.set_map(0, maps32[r].cpu().numpy())
+        o = orc.Oracle(w.n_theta, w.n_phi, w.params[42:43], dtype=np.float32)
+        o.set_map(0, maps32[42].cpu().numpy())
         o.step(n, dt, sts_stages=s)
         ref32 = o.get_full(0)
-        e_gpu, e_orc = rel_linf(g, ref32), rel_linf(ref32, ref)
+        e_gpu, e_orc = rel_linf(g42, ref32), rel_linf(ref32, refs[42])
         print("float oracle: cuda fp32 vs float oracle %.3e, float oracle vs fp64 oracle %.3e" % (e_gpu, e_orc))
-        assert errs["f32"] <= e_orc and e_gpu <= 2.0 * e_orc      # the CUDA path is the more accurate of the two
+        assert errs["f32_arith1"][2] <= e_orc and e_gpu <= 2.0 * e_orc      # the CUDA path is the more accurate of the two
 
 
 def test_config2_full_length_sampled_realization():
@@ -356,15 +362,18 @@ def test_config4_full_size_first_assimilation_hour():
     ctx.close()
 
 
-@pytest.mark.skipif(__import__("os").environ.get("HFT_SLOW") != "1", reason="~8 min of oracle time; set HFT_SLOW=1 (result recorded in DESIGN.md)")
-def test_config4_full_length():
-    """BASELINE config 4 at full size and full length: 2048x4096, 1 simulated day = 24 x (3 steps of 1638 stages + the
-    hourly assimilation of the synthetic observation with the moving disc weights), fp64, element by element at the end."""
+def test_config4_full_size_assimilation_cycle():
+    """BASELINE config 4 at full size, 2048x4096 fp64: repeated hft_step <-> hft_assimilate.  By default the first 6 of the 24
+    assimilation hours (18 steps of 1638 stages + 6 blends of the synthetic observation with the moving disc weights, about
+    2 min of oracle time); HFT_SLOW=1 runs the full simulated day (72 steps + 24 assimilations, ~8 min).  Element by element
+    at the end."""
+    import os
+    hours = 24 if os.environ.get("HFT_SLOW") == "1" else 6
     w = wl.config(4)
     ctx, o = make_pair(w, "f64")
     dt, n, per = wl.plan(w, *ctx.stable_dt())
     t = 0.0
-    for hour in range(24):
+    for hour in range(hours):
         ctx.step(per, dt)
         o.step(per, dt)
         t += per * dt
@@ -372,8 +381,8 @@ def test_config4_full_length():
         wt = wl.assimilation_weights(w, t)
         ctx.assimilate(obs.cuda(), wt.cuda())
         o.assimilate(obs.numpy(), wt.numpy())
-    e = compare(ctx, o, 1e-12, "cfg4 full length")
-    print("cfg4 full length (72 steps + 24 assimilations): rel L-inf %.3e" % e)
+    e = compare(ctx, o, 1e-12, "cfg4 %d hours" % hours)
+    print("cfg4 (%d steps + %d assimilations): rel L-inf %.3e" % (hours * per, hours, e))
     dg, do = ctx.diagnostics(), o.diagnostics()
     assert np.allclose(dg, do, rtol=0, atol=1e-12 * do[:, 1].max())
     ctx.close()
@@ -448,6 +457,14 @@ def test_errors_are_reported():
         ctx.step(1, -1.0)
     assert ctx.launch_count() >= 0
     ctx.close()
+    # hft_create rejects what would fail later with a generic launch error or run anti-diffusion silently
+    for bad in ([[float("nan"), 0, 0, 0, 0, 0, 0]], [[-1.0, 0, 0, 0, 0, 0, 0]], [[500.0, float("inf"), 0, 0, 0, 0, 0]]):
+        with pytest.raises(H.HftError, match="invalid argument"):
+            H.Context(64, 128, bad)
+    with pytest.raises(H.HftError, match="invalid argument"):
+        H.workspace_bytes(65534, 128, 1, "f64", None)          # n_theta + 2 rows ride in gridDim.y (16 bits)
+    with pytest.raises(H.HftError, match="invalid argument"):
+        H.workspace_bytes(64, 128, 65536, "f64", None)         # realizations ride in gridDim.z
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
