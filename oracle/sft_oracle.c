@@ -74,8 +74,21 @@ typedef struct {
     double radius_cm;
     double *st;   /* sin(theta_j),        j = 0..nt+1 */
     double *sth;  /* sin(theta_{j+1/2}),  j = 0..nt   */
-    double P;     /* polar prefactor, App. A :646 (exact form) */
-    double Apole; /* polar cap area 2*pi*(1-cos(dth/2)), App. A :642 */
+    double P;     /* polar prefactor, App. A :646 (exact form); north cap (uniform grid: both) */
+    double Apole; /* polar cap area 2*pi*(1-cos(dth/2)), App. A :642; north cap (uniform grid: both) */
+    /* non-uniform theta grid ("logically-rectangular non-uniform"; reading U33).  On the default
+       uniform grid every entry of dthc / dthf holds the SAME double dth, so all expressions below evaluate as before. */
+    double *th;   /* theta_j,       j = 0..nt+1: the nodes where B_r lives; th[0] = 0, th[nt+1] = pi */
+    double *thf;  /* theta_{j+1/2}, j = 0..nt: the half grid, midway between the nodes */
+    double *dthc; /* Delta theta_j = theta_{j+1/2} - theta_{j-1/2}: width of cell j (Eq. 27, :354); caps: their half width */
+    double *dthf; /* Delta theta_{j+1/2} = theta_{j+1} - theta_j: node spacing across face j+1/2 (Eq. 27) */
+    double PN, PS, ApoleN, ApoleS;   /* per cap: P = sin(x)/(2 pi (1 - cos x)), A = 2 pi (1 - cos x), x = the cap's half width */
+    /* WENO3-CS(h) constants of App. B (:662-680) per theta-face f (cell i = f+1, face i-1/2), reading U12:
+       wm[f][0..4] = D^{c/cm}_{i-3/2}, D^{c/cm}_{i-1/2}, D^{c/cp}_{i-3/2}, D^{p/t}_{i-3/2}, D^{cm/t}_{i-3/2}   (u^-, from LM)
+       wp[f][0..4] = D^{c/cp}_{i-1/2}, D^{c/cp}_{i-3/2}, D^{c/cm}_{i-1/2}, D^{m/t}_{i-1/2}, D^{cp/t}_{i-1/2}   (u^+, from LP) */
+    double *wm, *wp;
+    double *params; /* [nr][7] as given to create (the flow tables are re-made when the grid changes) */
+    int uniform;
     double *nu;   /* [nr] diffusivity in R_sun^2/hr */
     double *nuf;  /* [nr][nt+1] diffusivity at the theta-faces j+1/2 (the half grid of :288), R_sun^2/hr; = nu unless a
                      latitude profile was set (nu(theta), grid-based nu_g of Eq. 7) */
@@ -101,16 +114,52 @@ typedef struct {
 /* Step 0 of DESIGN.md: grid metric.  1-cos(x) is evaluated as 2 sin^2(x/2) (identical function,
  * no cancellation); P*Apole == sin(dth/2) to round-off, which is what makes the cap update
  * cancel the theta-face term of row 1 (flux conservation). */
-static void make_grid(oracle_t *o) {
+static void make_grid(oracle_t *o, const double *theta_nodes) {
     int nt = o->nt;
     o->dth = PI / (double)(nt + 1);
     o->dph = 2.0 * PI / (double)o->np;
-    for (int j = 0; j <= nt + 1; j++) o->st[j] = sin((double)j * o->dth);
-    for (int j = 0; j <= nt; j++) o->sth[j] = sin(((double)j + 0.5) * o->dth);
-    double s4 = sin(0.25 * o->dth);
-    double one_minus_cos = 2.0 * s4 * s4;
-    o->Apole = 2.0 * PI * one_minus_cos;
-    o->P = sin(0.5 * o->dth) / (2.0 * PI * one_minus_cos);
+    o->uniform = theta_nodes == NULL;
+    if (o->uniform) {
+        for (int j = 0; j <= nt + 1; j++) { o->th[j] = (double)j * o->dth; o->dthc[j] = o->dth; }
+        for (int j = 0; j <= nt; j++) { o->thf[j] = ((double)j + 0.5) * o->dth; o->dthf[j] = o->dth; }
+        o->dthc[0] = o->dthc[nt + 1] = 0.5 * o->dth;
+    } else {
+        for (int j = 0; j <= nt + 1; j++) o->th[j] = theta_nodes[j];
+        for (int j = 0; j <= nt; j++) { o->thf[j] = 0.5 * (o->th[j] + o->th[j + 1]); o->dthf[j] = o->th[j + 1] - o->th[j]; }
+        for (int j = 1; j <= nt; j++) o->dthc[j] = o->thf[j] - o->thf[j - 1];
+        o->dthc[0] = o->thf[0] - o->th[0];
+        o->dthc[nt + 1] = o->th[nt + 1] - o->thf[nt];
+    }
+    for (int j = 0; j <= nt + 1; j++) o->st[j] = sin(o->th[j]);
+    for (int j = 0; j <= nt; j++) o->sth[j] = sin(o->thf[j]);
+    for (int pole = 0; pole < 2; pole++) {
+        double x = o->dthc[pole ? nt + 1 : 0];          /* half width of the cap */
+        double s4 = sin(0.5 * x);
+        double one_minus_cos = 2.0 * s4 * s4;
+        double A = 2.0 * PI * one_minus_cos, P = sin(x) / (2.0 * PI * one_minus_cos);
+        if (pole) { o->ApoleS = A; o->PS = P; } else { o->ApoleN = A; o->PN = P; }
+    }
+    o->Apole = o->ApoleN; o->P = o->PN;
+    /* App. B D-factors (Smit et al. 2005, :680) with Delta x_j = the cell widths dthc[j]; faces 2..nt-2 are WENO faces
+       (cells i-2..i+1 = f-1..f+2 are regular cells); on the uniform grid the textbook constants exactly */
+    for (int f = 0; f <= nt; f++) {
+        double *m = o->wm + 5 * f, *q = o->wp + 5 * f;
+        m[0] = m[1] = m[2] = q[0] = q[1] = q[2] = 0.5;
+        m[3] = q[3] = 1.0 / 3.0; m[4] = q[4] = 2.0 / 3.0;
+        if (o->uniform || f < 2 || f > nt - 2) continue;
+        int i = f + 1;
+        double xm2 = o->dthc[i - 2], xm1 = o->dthc[i - 1], x0 = o->dthc[i], xp1 = o->dthc[i + 1];
+        m[0] = xm1 / (xm1 + xm2);            /* D^{c/cm}_{i-3/2}: centre i-1 over (i-1, i-2) */
+        m[1] = x0 / (x0 + xm1);              /* D^{c/cm}_{i-1/2}: centre i   over (i, i-1)   */
+        m[2] = xm1 / (xm1 + x0);             /* D^{c/cp}_{i-3/2}: centre i-1 over (i-1, i)   */
+        m[3] = x0 / (xm2 + xm1 + x0);        /* D^{p/t}_{i-3/2}  */
+        m[4] = (xm1 + xm2) / (xm2 + xm1 + x0);   /* D^{cm/t}_{i-3/2} */
+        q[0] = x0 / (x0 + xp1);              /* D^{c/cp}_{i-1/2} */
+        q[1] = xm1 / (xm1 + x0);             /* D^{c/cp}_{i-3/2} */
+        q[2] = x0 / (x0 + xm1);              /* D^{c/cm}_{i-1/2} */
+        q[3] = xm1 / (xm1 + x0 + xp1);       /* D^{m/t}_{i-1/2}  */
+        q[4] = (x0 + xp1) / (xm1 + x0 + xp1);    /* D^{cp/t}_{i-1/2} */
+    }
 }
 
 /* params per realization: eta_km2_s, d0, d2, d4, m1, m3, m5 (Eq. 3, 4, 6; units m/s, km^2/s). */
@@ -119,12 +168,12 @@ static void make_flow(oracle_t *o, int r, const double *p) {
     o->nu[r] = p[0] * KM2_S_TO_RS2_HR;
     double d0 = p[1], d2 = p[2], d4 = p[3], m1 = p[4], m3 = p[5], m5 = p[6];
     for (int j = 0; j <= nt; j++) { /* Eq. 4 at the face angle */
-        double th = ((double)j + 0.5) * o->dth;
+        double th = o->thf[j];
         double c = cos(th), s = sin(th);
         o->vt[(size_t)r * (nt + 1) + j] = -(m1 * c + m3 * c * c * c + m5 * c * c * c * c * c) * s * M_S_TO_RS_HR;
     }
     for (int j = 0; j <= nt + 1; j++) { /* Eq. 3 divided by sin(theta) */
-        double c = cos((double)j * o->dth);
+        double c = cos(o->th[j]);
         o->om[(size_t)r * (nt + 2) + j] = (d0 + d2 * c * c + d4 * c * c * c * c) * M_S_TO_RS_HR;
     }
 }
@@ -141,7 +190,12 @@ void *SUF(sft_oracle_create)(int nt, int np, int nr, const double *params /*[nr]
     o->om = (double *)calloc((size_t)nr * (nt + 2), sizeof(double));
     o->B = (real *)calloc((size_t)nr * (nt + 2) * np, sizeof(real));
     o->B0 = (double *)calloc(nr, sizeof(double));
-    make_grid(o);
+    o->th = (double *)calloc(nt + 2, sizeof(double)); o->thf = (double *)calloc(nt + 1, sizeof(double));
+    o->dthc = (double *)calloc(nt + 2, sizeof(double)); o->dthf = (double *)calloc(nt + 1, sizeof(double));
+    o->wm = (double *)calloc(5 * (size_t)(nt + 1), sizeof(double)); o->wp = (double *)calloc(5 * (size_t)(nt + 1), sizeof(double));
+    o->params = (double *)malloc(7 * (size_t)nr * sizeof(double));
+    memcpy(o->params, params, 7 * (size_t)nr * sizeof(double));
+    make_grid(o, NULL);
     for (int r = 0; r < nr; r++) {
         make_flow(o, r, params + 7 * r);
         for (int f = 0; f <= nt; f++) o->nuf[(size_t)r * (nt + 1) + f] = o->nu[r];
@@ -153,7 +207,29 @@ void SUF(sft_oracle_destroy)(void *h) {
     oracle_t *o = (oracle_t *)h;
     for (int r = 0; r < o->nr; r++) free(o->nuhh[r]);
     free(o->nuhh);
+    free(o->th); free(o->thf); free(o->dthc); free(o->dthf); free(o->wm); free(o->wp); free(o->params);
     free(o->st); free(o->sth); free(o->nu); free(o->nuf); free(o->vt); free(o->om); free(o->B); free(o->B0); free(o->S1); free(o->S2); free(o);
+}
+
+/* Non-uniform theta grid (reading U33): theta[nt+2] = the nodes where B_r lives, theta[0] = 0, theta[nt+1] = pi,
+ * strictly increasing.  Re-makes the metric, the App. B constants and the analytic flow tables (custom flow tables and
+ * diffusivity profiles set before this call are kept as given: they are per face / per row, not functions of theta). */
+void SUF(sft_oracle_set_theta_nodes)(void *h, const double *theta) {
+    oracle_t *o = (oracle_t *)h;
+    make_grid(o, theta);
+    for (int r = 0; r < o->nr; r++) {
+        double nu_keep = o->nu[r];
+        make_flow(o, r, o->params + 7 * r);
+        o->nu[r] = nu_keep;
+    }
+}
+
+void SUF(sft_oracle_get_grid)(void *h, double *th /*[nt+2]*/, double *thf /*[nt+1]*/, double *dthc /*[nt+2]*/, double *dthf /*[nt+1]*/,
+                              double *caps /*[4]: PN, PS, ApoleN, ApoleS*/) {
+    oracle_t *o = (oracle_t *)h;
+    memcpy(th, o->th, sizeof(double) * (o->nt + 2)); memcpy(thf, o->thf, sizeof(double) * (o->nt + 1));
+    memcpy(dthc, o->dthc, sizeof(double) * (o->nt + 2)); memcpy(dthf, o->dthf, sizeof(double) * (o->nt + 1));
+    caps[0] = o->PN; caps[1] = o->PS; caps[2] = o->ApoleN; caps[3] = o->ApoleS;
 }
 
 /* Latitude-dependent diffusivity (Eq. 6 :109 with nu = nu(theta)): nu_face[f] in km^2/s at the theta-face f+1/2,
@@ -190,7 +266,7 @@ void SUF(sft_oracle_set_grid_diffusivity)(void *h, int r, double alpha_nu) {
         if (r < 0 || q == r)
             for (int f = 0; f <= o->nt; f++) {
                 double dps = o->dph * o->sth[f];
-                o->nuf[(size_t)q * (o->nt + 1) + f] = alpha_nu * (o->dth * o->dth + dps * dps) * KM2_S_TO_RS2_HR;
+                o->nuf[(size_t)q * (o->nt + 1) + f] = alpha_nu * (o->dthf[f] * o->dthf[f] + dps * dps) * KM2_S_TO_RS2_HR;
             }
 }
 
@@ -300,8 +376,8 @@ static void diffusion_op_map(const oracle_t *o, int r, const real *B, real *out)
         real *oc = out + (size_t)j * np;
         for (int k = 0; k < np; k++) {
             int kw = (k + np - 1) % np, ke = (k + 1) % np;
-            real as = (real)(0.5 * (nS[k] + nS[kw]) * o->sth[j] / (o->st[j] * o->dth * o->dth));
-            real an = (real)(0.5 * (nN[k] + nN[kw]) * o->sth[j - 1] / (o->st[j] * o->dth * o->dth));
+            real as = (real)(0.5 * (nS[k] + nS[kw]) * o->sth[j] / (o->st[j] * o->dthc[j] * o->dthf[j]));
+            real an = (real)(0.5 * (nN[k] + nN[kw]) * o->sth[j - 1] / (o->st[j] * o->dthc[j] * o->dthf[j - 1]));
             real ae = (real)(0.5 * (nS[k] + nN[k]) / (o->st[j] * o->st[j] * o->dph * o->dph));
             real aw = (real)(0.5 * (nS[kw] + nN[kw]) / (o->st[j] * o->st[j] * o->dph * o->dph));
             real tth = as * (Bs[k] - Bc[k]) - an * (Bc[k] - Bn[k]);
@@ -316,8 +392,8 @@ static void diffusion_op_map(const oracle_t *o, int r, const real *B, real *out)
         kadd(&a, 0.5 * (n0[k] + n0[kw]) * (double)(B[np + k] - B[0]));
         kadd(&b, 0.5 * (n1[k] + n1[kw]) * (double)(B[(size_t)nt * np + k] - B[(size_t)(nt + 1) * np]));
     }
-    fill_row(out, np, (real)(o->P / o->dth * o->dph * a.s));
-    fill_row(out + (size_t)(nt + 1) * np, np, (real)(o->P / o->dth * o->dph * b.s));
+    fill_row(out, np, (real)(o->PN / o->dthf[0] * o->dph * a.s));
+    fill_row(out + (size_t)(nt + 1) * np, np, (real)(o->PS / o->dthf[nt] * o->dph * b.s));
 }
 
 static void diffusion_op(const oracle_t *o, int r, const real *B, real *out) {
@@ -328,8 +404,8 @@ static void diffusion_op(const oracle_t *o, int r, const real *B, real *out) {
     const double *nuf = o->nuf + (size_t)r * (nt + 1);
     #pragma omp parallel for schedule(static)
     for (int j = 1; j <= nt; j++) {
-        real cp = (real)(nuf[j] * o->sth[j] / (o->st[j] * o->dth * o->dth));
-        real cm = (real)(nuf[j - 1] * o->sth[j - 1] / (o->st[j] * o->dth * o->dth));
+        real cp = (real)(nuf[j] * o->sth[j] / (o->st[j] * o->dthc[j] * o->dthf[j]));
+        real cm = (real)(nuf[j - 1] * o->sth[j - 1] / (o->st[j] * o->dthc[j] * o->dthf[j - 1]));
         real cf = (real)(0.5 * (nuf[j] + nuf[j - 1]) / (o->st[j] * o->st[j] * o->dph * o->dph));
         const real *Bc = B + (size_t)j * np, *Bn = Bc - np, *Bs = Bc + np; /* Bn = row j-1 (towards north), Bs = row j+1 */
         real *oc = out + (size_t)j * np;
@@ -340,7 +416,7 @@ static void diffusion_op(const oracle_t *o, int r, const real *B, real *out) {
             oc[k] = tth + tph;
         }
     }
-    double capN = o->P * (nuf[0] / o->dth) * o->dph, capS = o->P * (nuf[nt] / o->dth) * o->dph;
+    double capN = o->PN * (nuf[0] / o->dthf[0]) * o->dph, capS = o->PS * (nuf[nt] / o->dthf[nt]) * o->dph;
     kahan_t a = {0, 0}, b = {0, 0};
     for (int k = 0; k < np; k++) {
         kadd(&a, (double)(B[np + k] - B[0]));
@@ -368,14 +444,14 @@ static double diffusion_dt_expl(const oracle_t *o) {
                 wN += 0.5 * (nu[k] + nu[kw]);
                 wS += 0.5 * (nu[(size_t)nt * np + k] + nu[(size_t)nt * np + kw]);
             }
-            if (o->P * wN * o->dph / o->dth > dmax) dmax = o->P * wN * o->dph / o->dth;
-            if (o->P * wS * o->dph / o->dth > dmax) dmax = o->P * wS * o->dph / o->dth;
+            if (o->PN * wN * o->dph / o->dthf[0] > dmax) dmax = o->PN * wN * o->dph / o->dthf[0];
+            if (o->PS * wS * o->dph / o->dthf[o->nt] > dmax) dmax = o->PS * wS * o->dph / o->dthf[o->nt];
             for (int j = 1; j <= nt; j++) {
                 const double *nS = nu + (size_t)j * np, *nN = nu + (size_t)(j - 1) * np;
                 for (int k = 0; k < np; k++) {
                     int kw = (k + np - 1) % np;
-                    double d = 0.5 * (nS[k] + nS[kw]) * o->sth[j] / (o->st[j] * o->dth * o->dth)
-                             + 0.5 * (nN[k] + nN[kw]) * o->sth[j - 1] / (o->st[j] * o->dth * o->dth)
+                    double d = 0.5 * (nS[k] + nS[kw]) * o->sth[j] / (o->st[j] * o->dthc[j] * o->dthf[j])
+                             + 0.5 * (nN[k] + nN[kw]) * o->sth[j - 1] / (o->st[j] * o->dthc[j] * o->dthf[j - 1])
                              + 0.5 * (nS[k] + nN[k]) / (o->st[j] * o->st[j] * o->dph * o->dph)
                              + 0.5 * (nS[kw] + nN[kw]) / (o->st[j] * o->st[j] * o->dph * o->dph);
                     if (d > dmax) dmax = d;
@@ -384,12 +460,12 @@ static double diffusion_dt_expl(const oracle_t *o) {
             continue;
         }
         const double *nuf = o->nuf + (size_t)r * (o->nt + 1);
-        double dN = 2.0 * PI * o->P * nuf[0] / o->dth, dS = 2.0 * PI * o->P * nuf[o->nt] / o->dth;
+        double dN = 2.0 * PI * o->PN * nuf[0] / o->dthf[0], dS = 2.0 * PI * o->PS * nuf[o->nt] / o->dthf[o->nt];
         if (dN > dmax) dmax = dN;
         if (dS > dmax) dmax = dS;
         for (int j = 1; j <= o->nt; j++) {
-            double cp = nuf[j] * o->sth[j] / (o->st[j] * o->dth * o->dth);
-            double cm = nuf[j - 1] * o->sth[j - 1] / (o->st[j] * o->dth * o->dth);
+            double cp = nuf[j] * o->sth[j] / (o->st[j] * o->dthc[j] * o->dthf[j]);
+            double cm = nuf[j - 1] * o->sth[j - 1] / (o->st[j] * o->dthc[j] * o->dthf[j - 1]);
             double cf = 0.5 * (nuf[j] + nuf[j - 1]) / (o->st[j] * o->st[j] * o->dph * o->dph);
             double d = cp + cm + 2.0 * cf;
             if (d > dmax) dmax = d;
@@ -544,6 +620,24 @@ static real weno3_side(real far, real near, real other, real eps) {
     return (w0 * p0 + w1 * p1) / (w0 + w1);
 }
 
+/* The same face value on a non-uniform grid, App. B (:662-680) with the D-factors of Smit et al. (reading U12):
+ *   p0 = (1 + Dex) f_near - Dex f_far ; p1 = Da f_near + Db f_other
+ *   beta0 = 4 (Dex (f_near - f_far))^2 ; beta1 = 4 (Db (f_other - f_near))^2
+ *   w0 = d0/(eps+beta0)^2 ; w1 = d1/(eps+beta1)^2
+ * D = (Dex, Da, Db, d0, d1): for u^- the row wm[f] of make_grid, for u^+ the row wp[f].  With (1/2, 1/2, 1/2, 1/3, 2/3) every
+ * intermediate equals weno3_side's (scalings by powers of two are exact). */
+static real weno3_side_nu(real far, real near, real other, real eps, const double *D) {
+    real Dex = (real)D[0], Da = (real)D[1], Db = (real)D[2], d0 = (real)D[3], d1 = (real)D[4];
+    real p0 = ((real)1 + Dex) * near - Dex * far;
+    real p1 = Da * near + Db * other;
+    real t0 = Dex * (near - far), t1 = Db * (other - near);
+    real b0 = (real)4 * (t0 * t0);
+    real b1 = (real)4 * (t1 * t1);
+    real w0 = d0 / ((eps + b0) * (eps + b0));
+    real w1 = d1 / ((eps + b1) * (eps + b1));
+    return (w0 * p0 + w1 * p1) / (w0 + w1);
+}
+
 /* Steps 1-2: advection tendency F_A(B) = div_s(B v), :354, with
  *   theta-faces 1/2, 3/2, nt-1/2, nt+1/2 upwind (:388, reading U6), all others WENO3-CS(h) with
  *   LLF splitting (B2 :684): LP_i = B_i (v_{i+1/2} - alpha_i)/2, LM_i = B_i (v_{i-1/2} + alpha_i)/2,
@@ -583,8 +677,9 @@ static void advection_tendency(const oracle_t *o, int r, const real *B, real *ou
                 real LPp1 = (real)0.5 * B[(size_t)(i + 1) * np + k] * (vt[i + 1] - al[i + 1]);
                 real LP0  = (real)0.5 * B[(size_t)(i    ) * np + k] * (vt[i    ] - al[i    ]);
                 real LPm1 = (real)0.5 * B[(size_t)(i - 1) * np + k] * (vt[i - 1] - al[i - 1]);
-                real um = weno3_side(LMm2, LMm1, LM0, eps_t);
-                real up = weno3_side(LPp1, LP0, LPm1, eps_t);
+                real ef = (flux_mode == 3) ? eps_t : (real)o->dthf[f];   /* eps_w = h, the local spacing (:670) */
+                real um = weno3_side_nu(LMm2, LMm1, LM0, ef, o->wm + 5 * f);
+                real up = weno3_side_nu(LPp1, LP0, LPm1, ef, o->wp + 5 * f);
                 F = up + um;
             }
             Ft[(size_t)f * np + k] = F;
@@ -615,7 +710,7 @@ static void advection_tendency(const oracle_t *o, int r, const real *B, real *ou
     #pragma omp parallel for schedule(static)
     for (int j = 1; j <= nt; j++) {
         real sp = (real)o->sth[j], sm = (real)o->sth[j - 1];
-        real dt_den = (real)(o->st[j] * o->dth), dp_den = (real)(o->st[j] * o->dph);
+        real dt_den = (real)(o->st[j] * o->dthc[j]), dp_den = (real)(o->st[j] * o->dph);
         for (int k = 0; k < np; k++) {
             int kp1 = (k + 1) % np;
             real tth = (sp * Ft[(size_t)j * np + k] - sm * Ft[(size_t)(j - 1) * np + k]) / dt_den;
@@ -625,8 +720,8 @@ static void advection_tendency(const oracle_t *o, int r, const real *B, real *ou
     }
     kahan_t a = {0, 0}, b = {0, 0};
     for (int k = 0; k < np; k++) { kadd(&a, (double)Ft[k]); kadd(&b, (double)Ft[(size_t)nt * np + k]); }
-    fill_row(out, np, (real)(o->P * o->dph * a.s));
-    fill_row(out + (size_t)(nt + 1) * np, np, (real)(-(o->P * o->dph * b.s)));
+    fill_row(out, np, (real)(o->PN * o->dph * a.s));
+    fill_row(out + (size_t)(nt + 1) * np, np, (real)(-(o->PS * o->dph * b.s)));
     free(vt); free(al);
 }
 
@@ -696,7 +791,8 @@ static void advection_tendency_general(const oracle_t *o, const real *B, real *o
                 real LP0  = (real)0.5 * B[(size_t)(i    ) * np + k] * (VTF(i    ) - al[2]);
                 real LPm1 = (real)0.5 * B[(size_t)(i - 1) * np + k] * (VTF(i - 1) - al[1]);
                 #undef VTF
-                F = weno3_side(LPp1, LP0, LPm1, eps_t) + weno3_side(LMm2, LMm1, LM0, eps_t);
+                real ef = (flux_mode == 3) ? eps_t : (real)o->dthf[f];
+                F = weno3_side_nu(LPp1, LP0, LPm1, ef, o->wp + 5 * f) + weno3_side_nu(LMm2, LMm1, LM0, ef, o->wm + 5 * f);
             }
             Ft[(size_t)f * np + k] = F;
         }
@@ -732,7 +828,7 @@ static void advection_tendency_general(const oracle_t *o, const real *B, real *o
     #pragma omp parallel for schedule(static)
     for (int j = 1; j <= nt; j++) {
         real sp = (real)o->sth[j], sm = (real)o->sth[j - 1];
-        real dt_den = (real)(o->st[j] * o->dth), dp_den = (real)(o->st[j] * o->dph);
+        real dt_den = (real)(o->st[j] * o->dthc[j]), dp_den = (real)(o->st[j] * o->dph);
         for (int k = 0; k < np; k++) {
             int kp1 = (k + 1) % np;
             real tth = (sp * Ft[(size_t)j * np + k] - sm * Ft[(size_t)(j - 1) * np + k]) / dt_den;
@@ -742,8 +838,8 @@ static void advection_tendency_general(const oracle_t *o, const real *B, real *o
     }
     kahan_t a = {0, 0}, b = {0, 0};
     for (int k = 0; k < np; k++) { kadd(&a, (double)Ft[k]); kadd(&b, (double)Ft[(size_t)nt * np + k]); }
-    fill_row(out, np, (real)(o->P * o->dph * a.s));
-    fill_row(out + (size_t)(nt + 1) * np, np, (real)(-(o->P * o->dph * b.s)));
+    fill_row(out, np, (real)(o->PN * o->dph * a.s));
+    fill_row(out + (size_t)(nt + 1) * np, np, (real)(-(o->PS * o->dph * b.s)));
 }
 
 /* test hook: the general rule with the un-attenuated table speeds copied to every face must reproduce
@@ -832,7 +928,7 @@ static double advection_dt_limit(const oracle_t *o) {
         const double *vt = o->vt + (size_t)r * (o->nt + 1), *om = o->om + (size_t)r * (o->nt + 2);
         for (int j = 1; j <= o->nt; j++) {
             double a = fabs(vt[j - 1]) > fabs(vt[j]) ? fabs(vt[j - 1]) : fabs(vt[j]);
-            double rate = a / o->dth + fabs(om[j]) / o->dph;
+            double rate = a / o->dthc[j] + fabs(om[j]) / o->dph;
             if (rate > 0.0 && 1.0 / rate < best) best = 1.0 / rate;
         }
     }
@@ -884,7 +980,7 @@ static void rfe_make_map(const oracle_t *o, int r, uint32_t map, real *S) {
     double r2 = o->radius_cm * o->radius_cm, ncells = (double)nt * (double)np;
     memset(S, 0, fsize(o) * sizeof(real));
     for (int j = 1; j <= nt; j++) {
-        double dA = o->st[j] * o->dth * o->dph * r2;
+        double dA = o->st[j] * o->dthc[j] * o->dph * r2;
         double amp = o->rfe_model == 1 ? o->rfe_flux_per_hr / (dA * ncells) * sqrt(PI / 2.0)
                                        : o->rfe_flux_per_hr / (4.0 * PI * r2) * sqrt(PI / 2.0);
         for (int k = 0; k < np; k++)
@@ -892,7 +988,7 @@ static void rfe_make_map(const oracle_t *o, int r, uint32_t map, real *S) {
     }
     kahan_t pp = {0, 0}, pm = {0, 0};
     for (int j = 1; j <= nt; j++) {
-        double dA = o->st[j] * o->dth * o->dph;
+        double dA = o->st[j] * o->dthc[j] * o->dph;
         for (int k = 0; k < np; k++) {
             double v = (double)S[(size_t)j * np + k];
             if (v > 0) kadd(&pp, v * dA); else kadd(&pm, v * dA);
@@ -1024,15 +1120,15 @@ void SUF(sft_oracle_assimilate)(void *h, const real *obs, const real *w, int sha
         } else {
             kahan_t pp = {0, 0}, pm = {0, 0};
             real dN = wN * (obN - B[0]), dS = wS * (obS - B[(size_t)(nt + 1) * np]);
-            if (dN > (real)0) kadd(&pp, (double)dN * o->Apole); else kadd(&pm, (double)dN * o->Apole);
+            if (dN > (real)0) kadd(&pp, (double)dN * o->ApoleN); else kadd(&pm, (double)dN * o->ApoleN);
             for (int j = 1; j <= nt; j++) {
-                double dA = o->st[j] * o->dth * o->dph;
+                double dA = o->st[j] * o->dthc[j] * o->dph;
                 for (int k = 0; k < np; k++) {
                     real d = wt[(size_t)(j - 1) * np + k] * (ob[(size_t)(j - 1) * np + k] - B[(size_t)j * np + k]);
                     if (d > (real)0) kadd(&pp, (double)d * dA); else kadd(&pm, (double)d * dA);
                 }
             }
-            if (dS > (real)0) kadd(&pp, (double)dS * o->Apole); else kadd(&pm, (double)dS * o->Apole);
+            if (dS > (real)0) kadd(&pp, (double)dS * o->ApoleS); else kadd(&pm, (double)dS * o->ApoleS);
             real sc = (real)1;
             if (pp.s != 0.0 && pm.s != 0.0) sc = (real)sqrt(fabs(pp.s / pm.s));
             for (int j = 1; j <= nt; j++)
@@ -1062,16 +1158,16 @@ void SUF(sft_oracle_diagnostics)(void *h, double *out /*[nr][4]*/) {
         const real *B = field(o, r);
         kahan_t pp = {0, 0}, pm = {0, 0};
         double c0 = (double)B[0];
-        if (c0 > 0) kadd(&pp, c0 * o->Apole); else if (c0 < 0) kadd(&pm, c0 * o->Apole);
+        if (c0 > 0) kadd(&pp, c0 * o->ApoleN); else if (c0 < 0) kadd(&pm, c0 * o->ApoleN);
         for (int j = 1; j <= nt; j++) {
-            double dA = o->st[j] * o->dth * o->dph;
+            double dA = o->st[j] * o->dthc[j] * o->dph;
             for (int k = 0; k < np; k++) {
                 double v = (double)B[(size_t)j * np + k];
                 if (v > 0) kadd(&pp, v * dA); else if (v < 0) kadd(&pm, v * dA);
             }
         }
         double c1 = (double)B[(size_t)(nt + 1) * np];
-        if (c1 > 0) kadd(&pp, c1 * o->Apole); else if (c1 < 0) kadd(&pm, c1 * o->Apole);
+        if (c1 > 0) kadd(&pp, c1 * o->ApoleS); else if (c1 < 0) kadd(&pm, c1 * o->ApoleS);
         out[4 * r + 0] = (pp.s + pm.s) * r2;
         out[4 * r + 1] = (pp.s - pm.s) * r2;
         out[4 * r + 2] = pp.s * r2;
@@ -1099,8 +1195,8 @@ void SUF(sft_oracle_diagnostics_ext)(void *h, double lat_cut_deg, double *out /*
         double bmin = (double)B[0], bmax = (double)B[0], amin = fabs((double)B[0]);
         for (int j = 0; j <= nt + 1; j++) {
             int cap = (j == 0 || j == nt + 1);
-            double th = (double)j * o->dth;
-            double dA = cap ? o->Apole : o->st[j] * o->dth * o->dph;
+            double th = o->th[j];
+            double dA = cap ? (j == 0 ? o->ApoleN : o->ApoleS) : o->st[j] * o->dthc[j] * o->dph;
             int region = (th <= thc) ? 0 : (th >= PI - thc ? 1 : -1);
             int ncol = cap ? 1 : np;   /* a cap is one cell (stored replicated) */
             for (int k = 0; k < ncol; k++) {

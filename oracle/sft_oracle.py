@@ -84,6 +84,23 @@ class Oracle:
         f.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         f(self.h, r, _dp(vt), _dp(om))
 
+    def set_theta_nodes(self, theta):
+        """Non-uniform theta grid: theta[nt+2] = the B_r nodes, theta[0] = 0, theta[-1] = pi, increasing."""
+        a = np.ascontiguousarray(theta, dtype=np.float64)
+        assert a.shape == (self.nt + 2,) and a[0] == 0.0 and abs(a[-1] - np.pi) < 1e-15 and np.all(np.diff(a) > 0)
+        f = self._f("sft_oracle_set_theta_nodes")
+        f.restype = None
+        f.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+        f(self.h, _dp(a))
+
+    def grid_arrays(self):
+        th, thf, dthc, dthf, caps = np.zeros(self.nt + 2), np.zeros(self.nt + 1), np.zeros(self.nt + 2), np.zeros(self.nt + 1), np.zeros(4)
+        f = self._f("sft_oracle_get_grid")
+        f.restype = None
+        f.argtypes = [C.c_void_p] + [C.POINTER(C.c_double)] * 5
+        f(self.h, _dp(th), _dp(thf), _dp(dthc), _dp(dthf), _dp(caps))
+        return dict(th=th, thf=thf, dthc=dthc, dthf=dthf, PN=caps[0], PS=caps[1], ApoleN=caps[2], ApoleS=caps[3])
+
     # -- state ------------------------------------------------------------------------------
     def set_diffusivity_profile(self, r, nu_face_km2_s):
         """nu(theta) at the theta-faces f+1/2, f = 0..nt, km^2/s (Eq. 6 with a latitude-dependent diffusivity)."""
