@@ -106,6 +106,18 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params 
 
 void hft_destroy(hft_ctx* ctx);
 
+/* Non-uniform theta grid ("logically-rectangular non-uniform spherical surface grid"; Eq. 27-28 :438-460 with
+ * Delta theta_{j+-1/2}, Delta theta_j; :354; App. A :624-648; App. B :662-680).  h_theta[n_theta+2]: HOST, the colatitudes of
+ * the rows where B_r lives, strictly increasing, h_theta[0] = 0 and h_theta[n_theta+1] = pi (the two polar caps); user map row
+ * i is the cell at h_theta[i+1].  The half grid (flow speeds, fluxes, nu) lies midway between the nodes; Delta theta_{j+1/2} =
+ * theta_{j+1} - theta_j, Delta theta_j = theta_{j+1/2} - theta_{j-1/2}; each polar cap reaches to its first half-mesh point and
+ * takes the prefactor of App. A with its own half width; the WENO3-CS(h) constants are the D-factors of App. B with Delta x =
+ * the cell widths and eps_w = the local node spacing (readings U12, U33).  phi stays uniform.  Re-makes the
+ * metric, diffusion and analytic flow tables (Eq. 3-4 evaluated at the new angles): call it BEFORE hft_set_flow_tables; not
+ * allowed once a diffusivity map is set (HFT_ERR_ARG).  Every kernel, the temporally blocked ones included, runs unchanged:
+ * all coefficients stay phi-independent.  Synchronises the stream. */
+int hft_set_theta_nodes(hft_ctx* ctx, const double* h_theta);
+
 /* Replace the analytic flow of realization r (-1: all) by per-row tables (PAPER.md:90 custom flows,
  * phi-independent subset; needed for the App. C test :703): h_vtheta[n_theta+1] = v_theta at the
  * theta-faces (j+1/2)*dtheta, j = 0..n_theta, in m/s; h_omega[n_theta+2] = v_phi/sin(theta) at the rows

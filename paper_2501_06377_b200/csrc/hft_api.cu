@@ -76,8 +76,15 @@ struct hft_ctx {
     std::vector<double> map_diag, capw;
     double* d_capw = nullptr;
     // host tables (fp64)
-    double dth = 0, dph = 0, P = 0, Apole = 0;
+    double dth = 0, dph = 0, P = 0, Apole = 0;   // uniform spacings; P, Apole: north cap (uniform grid: both)
     std::vector<double> st, sth;      // sin(theta_j) [nt+2], sin(theta_{j+1/2}) [nt+1]
+    // theta grid (reading U33): nodes, half grid, cell widths (caps: half width), node spacing across the faces;
+    // on the default uniform grid dthc / dthf hold the one value dth
+    std::vector<double> th, thf, dthc, dthf;
+    double PN = 0, PS = 0, ApoleN = 0, ApoleS = 0;
+    std::vector<double> wm, wp;       // [nt+1][5] App. B D-factors per theta-face (oracle make_grid has the same list)
+    bool uniform = true;
+    std::vector<hft_params> params;   // as given to hft_create (the analytic flow tables follow the grid)
     std::vector<double> nu;           // [R] R_sun^2/hr
     std::vector<double> nuf;          // [R][nt+1] nu at the theta-faces (= nu unless a latitude profile was set; Eq. 6-7)
     std::vector<double> vt, om;       // [R][nt+1] R_sun/hr at faces, [R][nt+2] rad/hr at rows
@@ -199,17 +206,45 @@ bool valid_options(const hft_options* o) {
 // ---------------------------------------------------------------- host tables (fp64)
 
 // Grid metric (App. A :642-646).  1 - cos(x) is formed as 2 sin^2(x/2).
-void build_metric(hft_ctx* c) {
+void build_metric(hft_ctx* c, const double* theta_nodes) {
     const int nt = c->G.nt;
     c->dth = kPi / (double)(nt + 1);
     c->dph = 2.0 * kPi / (double)c->G.np;
-    c->st.resize(nt + 2);
-    c->sth.resize(nt + 1);
-    for (int j = 0; j <= nt + 1; j++) c->st[j] = sin(c->dth * (double)j);
-    for (int j = 0; j <= nt; j++) c->sth[j] = sin(c->dth * ((double)j + 0.5));
-    const double q = sin(c->dth * 0.25);
-    c->Apole = 2.0 * kPi * (2.0 * q * q);
-    c->P = sin(c->dth * 0.5) / c->Apole;
+    c->uniform = theta_nodes == nullptr;
+    c->st.resize(nt + 2); c->sth.resize(nt + 1);
+    c->th.resize(nt + 2); c->thf.resize(nt + 1); c->dthc.resize(nt + 2); c->dthf.resize(nt + 1);
+    if (c->uniform) {
+        for (int j = 0; j <= nt + 1; j++) { c->th[j] = c->dth * (double)j; c->dthc[j] = c->dth; }
+        for (int j = 0; j <= nt; j++) { c->thf[j] = c->dth * ((double)j + 0.5); c->dthf[j] = c->dth; }
+        c->dthc[0] = c->dthc[nt + 1] = 0.5 * c->dth;
+    } else {
+        for (int j = 0; j <= nt + 1; j++) c->th[j] = theta_nodes[j];
+        for (int j = 0; j <= nt; j++) { c->thf[j] = 0.5 * (c->th[j] + c->th[j + 1]); c->dthf[j] = c->th[j + 1] - c->th[j]; }
+        for (int j = 1; j <= nt; j++) c->dthc[j] = c->thf[j] - c->thf[j - 1];
+        c->dthc[0] = c->thf[0] - c->th[0];
+        c->dthc[nt + 1] = c->th[nt + 1] - c->thf[nt];
+    }
+    for (int j = 0; j <= nt + 1; j++) c->st[j] = sin(c->th[j]);
+    for (int j = 0; j <= nt; j++) c->sth[j] = sin(c->thf[j]);
+    for (int pole = 0; pole < 2; pole++) {   // App. A (:642-646) with the cap's own half width x
+        const double x = c->dthc[pole ? nt + 1 : 0], q = sin(0.5 * x);
+        const double A = 2.0 * kPi * (2.0 * q * q), P = sin(x) / A;
+        if (pole) { c->ApoleS = A; c->PS = P; } else { c->ApoleN = A; c->PN = P; }
+    }
+    c->Apole = c->ApoleN; c->P = c->PN;
+    // App. B (:662-680) D-factors per theta-face f (cell i = f+1, face i-1/2), Delta x = the cell widths; uniform: 1/2, 1/3, 2/3
+    c->wm.assign(5 * (size_t)(nt + 1), 0.5); c->wp.assign(5 * (size_t)(nt + 1), 0.5);
+    for (int f = 0; f <= nt; f++) {
+        double *m = &c->wm[5 * (size_t)f], *q = &c->wp[5 * (size_t)f];
+        m[3] = q[3] = 1.0 / 3.0; m[4] = q[4] = 2.0 / 3.0;
+        if (c->uniform || f < 2 || f > nt - 2) continue;
+        const int i = f + 1;
+        const double xm2 = c->dthc[i - 2], xm1 = c->dthc[i - 1], x0 = c->dthc[i], xp1 = c->dthc[i + 1];
+        m[0] = xm1 / (xm1 + xm2); m[1] = x0 / (x0 + xm1); m[2] = xm1 / (xm1 + x0);
+        m[3] = x0 / (xm2 + xm1 + x0); m[4] = (xm1 + xm2) / (xm2 + xm1 + x0);
+        q[0] = x0 / (x0 + xp1); q[1] = xm1 / (xm1 + x0); q[2] = x0 / (x0 + xm1);
+        q[3] = xm1 / (xm1 + x0 + xp1); q[4] = (x0 + xp1) / (xm1 + x0 + xp1);
+    }
 }
 
 // Analytic flows, Eq. 3-4 (:78-86), converted with :298.
@@ -217,18 +252,18 @@ void build_flow(hft_ctx* c, int r, const hft_params& p) {
     const int nt = c->G.nt;
     c->nu[r] = p.eta_km2_s * kKm2sToRs2Hr;
     for (int f = 0; f <= nt; f++) {
-        const double th = c->dth * ((double)f + 0.5), x = cos(th);
+        const double th = c->thf[f], x = cos(th);
         c->vt[(size_t)r * (nt + 1) + f] = -(p.m1 * x + p.m3 * x * x * x + p.m5 * x * x * x * x * x) * sin(th) * kMsToRsHr;
     }
     for (int j = 0; j <= nt + 1; j++) {
-        const double x = cos(c->dth * (double)j), x2 = x * x;
+        const double x = cos(c->th[j]), x2 = x * x;
         c->om[(size_t)r * (nt + 2) + j] = (p.d0 + p.d2 * x2 + p.d4 * x2 * x2) * kMsToRsHr;
     }
 }
 
 template <typename real>
 struct HostTab {
-    std::vector<real> cp, cm, cf, cd, c4, lm, lp, vtf, pm, pp, sth, rdt, rdp;
+    std::vector<real> cp, cm, cf, cd, c4, lm, lp, vtf, pm, pp, sth, rdt, rdp, rdf, wmp;
     std::vector<double> capc, dA;
 };
 
@@ -243,23 +278,30 @@ void fill_tables(const hft_ctx* c, HostTab<real>& H) {
     H.capc.resize(2 * R); H.dA.resize(nt + 2);
     for (int f = 0; f <= nt; f++) H.sth[f] = (real)c->sth[f];
     for (int j = 1; j <= nt; j++) {
-        H.rdt[j] = (real)(1.0 / (c->st[j] * c->dth));
+        H.rdt[j] = (real)(1.0 / (c->st[j] * c->dthc[j]));
         H.rdp[j] = (real)(1.0 / (c->st[j] * c->dph));
-        H.dA[j] = c->st[j] * c->dth * c->dph;
+        H.dA[j] = c->st[j] * c->dthc[j] * c->dph;
     }
-    H.dA[0] = H.dA[nt + 1] = c->Apole;
+    H.dA[0] = c->ApoleN; H.dA[nt + 1] = c->ApoleS;
+    H.rdf.resize(nt + 1);
+    H.wmp.assign(16 * (size_t)(nt + 1), 0);   // per face: wm[0..4], eps_w, 2 pad, wp[0..4], 3 pad
+    for (int f = 0; f <= nt; f++) {
+        H.rdf[f] = (real)(1.0 / c->dthf[f]);
+        for (int q = 0; q < 5; q++) { H.wmp[16 * (size_t)f + q] = (real)c->wm[5 * (size_t)f + q]; H.wmp[16 * (size_t)f + 8 + q] = (real)c->wp[5 * (size_t)f + q]; }
+        H.wmp[16 * (size_t)f + 5] = (real)c->dthf[f];   // eps_w = h, the local spacing (:670)
+    }
     for (int r = 0; r < R; r++) {
         const double* nuf = &c->nuf[(size_t)r * (nt + 1)];
         const double* vt = &c->vt[(size_t)r * (nt + 1)];
         const double* om = &c->om[(size_t)r * (nt + 2)];
-        H.capc[2 * r] = c->P * (nuf[0] / c->dth) * c->dph;        // north: nu at face 1/2
-        H.capc[2 * r + 1] = c->P * (nuf[nt] / c->dth) * c->dph;   // south: nu at face nt+1/2
+        H.capc[2 * r] = c->PN * (nuf[0] / c->dthf[0]) * c->dph;        // north: nu at face 1/2
+        H.capc[2 * r + 1] = c->PS * (nuf[nt] / c->dthf[nt]) * c->dph;   // south: nu at face nt+1/2
         for (int f = 0; f <= nt; f++) H.vtf[(size_t)r * (nt + 1) + f] = (real)vt[f];
         for (int j = 0; j <= nt + 1; j++) {
             const size_t i = (size_t)r * (nt + 2) + j;
             if (j >= 1 && j <= nt) {  // Eq. 28, uniform spacing, nu = nu(theta) on the half grid (:288)
-                H.cp[i] = (real)(nuf[j] * c->sth[j] / (c->st[j] * c->dth * c->dth));
-                H.cm[i] = (real)(nuf[j - 1] * c->sth[j - 1] / (c->st[j] * c->dth * c->dth));
+                H.cp[i] = (real)(nuf[j] * c->sth[j] / (c->st[j] * c->dthc[j] * c->dthf[j]));
+                H.cm[i] = (real)(nuf[j - 1] * c->sth[j - 1] / (c->st[j] * c->dthc[j] * c->dthf[j - 1]));
                 H.cf[i] = (real)(0.5 * (nuf[j] + nuf[j - 1]) / (c->st[j] * c->st[j] * c->dph * c->dph));
                 H.cd[i] = (real)((double)H.cp[i] + (double)H.cm[i] + 2.0 * (double)H.cf[i]);
                 H.c4[4 * i + 0] = H.cm[i]; H.c4[4 * i + 1] = H.cp[i]; H.c4[4 * i + 2] = H.cf[i]; H.c4[4 * i + 3] = H.cd[i];
@@ -292,6 +334,7 @@ int upload_tables(hft_ctx* c, Tables<real>& T) {
     size_t o_cp = take(n2), o_cm = take(n2), o_cf = take(n2), o_cd = take(n2), o_c4 = take(4 * n2), o_lm = take(n2), o_lp = take(n2), o_pm = take(n2), o_pp = take(n2);
     size_t o_vtf = take(n1), o_sth = take((nt + 1) * sizeof(real)), o_rdt = take((nt + 2) * sizeof(real)), o_rdp = take((nt + 2) * sizeof(real));
     size_t o_capc = take(2 * R * sizeof(double)), o_dA = take((nt + 2) * sizeof(double));
+    size_t o_rdf = take((nt + 1) * sizeof(real)), o_wmp = take(16 * (size_t)(nt + 1) * sizeof(real)), o_th = take((nt + 2) * sizeof(double));
     if (!c->d_tab) {
         c->tab_bytes = off;
         CK(cudaMalloc((void**)&c->d_tab, c->tab_bytes));
@@ -303,12 +346,16 @@ int upload_tables(hft_ctx* c, Tables<real>& T) {
     CK(up(o_vtf, H.vtf.data(), n1)); CK(up(o_sth, H.sth.data(), (nt + 1) * sizeof(real)));
     CK(up(o_rdt, H.rdt.data(), (nt + 2) * sizeof(real))); CK(up(o_rdp, H.rdp.data(), (nt + 2) * sizeof(real)));
     CK(up(o_capc, H.capc.data(), 2 * R * sizeof(double))); CK(up(o_dA, H.dA.data(), (nt + 2) * sizeof(double)));
+    CK(up(o_rdf, H.rdf.data(), (nt + 1) * sizeof(real))); CK(up(o_wmp, H.wmp.data(), 16 * (size_t)(nt + 1) * sizeof(real)));
+    CK(up(o_th, c->th.data(), (nt + 2) * sizeof(double)));
     CK(cudaStreamSynchronize(c->stream));  // H goes out of scope
     T.cp = (const real*)(d + o_cp); T.cm = (const real*)(d + o_cm); T.cf = (const real*)(d + o_cf); T.cd = (const real*)(d + o_cd); T.c4 = (const real*)(d + o_c4);
     T.lm = (const real*)(d + o_lm); T.lp = (const real*)(d + o_lp); T.pm = (const real*)(d + o_pm); T.pp = (const real*)(d + o_pp);
     T.vtf = (const real*)(d + o_vtf); T.sth = (const real*)(d + o_sth); T.rdt = (const real*)(d + o_rdt); T.rdp = (const real*)(d + o_rdp);
     T.capc = (const double*)(d + o_capc); T.dA = (const double*)(d + o_dA);
-    T.adv_capc = c->P * c->dph;
+    T.rdf = (const real*)(d + o_rdf); T.wmp = (const real*)(d + o_wmp); T.th = (const double*)(d + o_th);
+    T.adv_capc[0] = c->PN * c->dph; T.adv_capc[1] = c->PS * c->dph;
+    T.nonuniform = c->uniform ? 0 : 1;
     T.eps_t = (real)c->dth;
     T.eps_p = (real)c->dph;
     return HFT_OK;
@@ -325,7 +372,7 @@ double adv_dt_limit(const hft_ctx* c) {
     for (int r = 0; r < c->nr; r++)
         for (int j = 1; j <= nt; j++) {
             const double a = fmax(fabs(c->vt[(size_t)r * (nt + 1) + j - 1]), fabs(c->vt[(size_t)r * (nt + 1) + j]));
-            const double rate = a / c->dth + fabs(c->om[(size_t)r * (nt + 2) + j]) / c->dph;
+            const double rate = a / c->dthc[j] + fabs(c->om[(size_t)r * (nt + 2) + j]) / c->dph;
             if (rate > 0.0) best = fmin(best, 1.0 / rate);
         }
     return best;
@@ -341,9 +388,9 @@ double diff_dt_expl(const hft_ctx* c) {
             continue;
         }
         const double* nuf = &c->nuf[(size_t)r * (nt + 1)];
-        d = fmax(d, fmax(2.0 * kPi * c->P * nuf[0] / c->dth, 2.0 * kPi * c->P * nuf[nt] / c->dth));  // cap row diagonals
+        d = fmax(d, fmax(2.0 * kPi * c->PN * nuf[0] / c->dthf[0], 2.0 * kPi * c->PS * nuf[nt] / c->dthf[nt]));  // cap row diagonals
         for (int j = 1; j <= nt; j++) {
-            const double t = (nuf[j] * c->sth[j] + nuf[j - 1] * c->sth[j - 1]) / (c->st[j] * c->dth * c->dth) +
+            const double t = (nuf[j] * c->sth[j] / c->dthf[j] + nuf[j - 1] * c->sth[j - 1] / c->dthf[j - 1]) / (c->st[j] * c->dthc[j]) +
                              (nuf[j] + nuf[j - 1]) / (c->st[j] * c->st[j] * c->dph * c->dph);
             d = fmax(d, t);
         }
@@ -413,8 +460,8 @@ int prepare_upipe(hft_ctx* c, int scheme, int s, double dt) {
     up.mixed = want_mixed;
     c->utab.assign((size_t)nt * UTAB_ROW_BYTES, 0);
     for (int j = 1; j <= nt; j++) {
-        const double cm = c->nu_shape[j - 1] * c->sth[j - 1] / (c->st[j] * c->dth * c->dth);
-        const double cp = c->nu_shape[j] * c->sth[j] / (c->st[j] * c->dth * c->dth);
+        const double cm = c->nu_shape[j - 1] * c->sth[j - 1] / (c->st[j] * c->dthc[j] * c->dthf[j - 1]);
+        const double cp = c->nu_shape[j] * c->sth[j] / (c->st[j] * c->dthc[j] * c->dthf[j]);
         const double cf = 0.5 * (c->nu_shape[j] + c->nu_shape[j - 1]) / (c->st[j] * c->st[j] * c->dph * c->dph);
         unsigned char* row = &c->utab[(size_t)(j - 1) * UTAB_ROW_BYTES];
         if (dbl) {
@@ -550,7 +597,7 @@ int diffuse_stagewise(hft_ctx* c, double dt, int s) {
     real* db = arr_of<real>(c, (is + 3) % kNumArrays);
     const bool vec = G.np % (16 / (int)sizeof(real)) == 0;
     MapArgs<real> M;
-    M.NU = (const real*)c->numap; M.capw = c->d_capw; M.capP = c->P * c->dph / c->dth; M.rdth = (real)(1.0 / c->dth);
+    M.NU = (const real*)c->numap; M.capw = c->d_capw; M.capP[0] = c->PN * c->dph / c->dthf[0]; M.capP[1] = c->PS * c->dph / c->dthf[c->G.nt];
     M.nparts_in = G.nbx;
     dim3 gs(G.nbx, 2, c->nr);
     if (MAP) k_polar_row_sums_map<real><<<gs, TX, 0, c->stream>>>(Y0, M.NU, c->d_part[0], G);
@@ -694,13 +741,13 @@ int map_upload(hft_ctx* c, int q, const double* h_map) {
             wn += 0.5 * (h_map[k] + h_map[kw]);
             ws += 0.5 * (h_map[(size_t)nt * np + k] + h_map[(size_t)nt * np + kw]);
         }
-        double d = fmax(c->P * wn * c->dph / c->dth, c->P * ws * c->dph / c->dth);
+        double d = fmax(c->PN * wn * c->dph / c->dthf[0], c->PS * ws * c->dph / c->dthf[nt]);
         for (int j = 1; j <= nt; j++) {
             const double *nS = h_map + (size_t)j * np, *nN = h_map + (size_t)(j - 1) * np;
-            const double gt = 1.0 / (c->st[j] * c->dth * c->dth), gp = 1.0 / (c->st[j] * c->st[j] * c->dph * c->dph);
+            const double gtc = 1.0 / (c->st[j] * c->dthc[j]), gp = 1.0 / (c->st[j] * c->st[j] * c->dph * c->dph);
             for (int k = 0; k < np; k++) {
                 const int kw = (k + np - 1) % np;
-                d = fmax(d, 0.5 * (nS[k] + nS[kw]) * c->sth[j] * gt + 0.5 * (nN[k] + nN[kw]) * c->sth[j - 1] * gt +
+                d = fmax(d, 0.5 * (nS[k] + nS[kw]) * c->sth[j] * gtc / c->dthf[j] + 0.5 * (nN[k] + nN[kw]) * c->sth[j - 1] * gtc / c->dthf[j - 1] +
                                 0.5 * (nS[k] + nN[k]) * gp + 0.5 * (nS[kw] + nN[kw]) * gp);
             }
         }
@@ -779,7 +826,8 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     c->map_set.assign(n_real, 0); c->map_diag.assign(n_real, 0.0); c->capw.assign(2 * (size_t)n_real, 0.0);
     c->B0.assign(n_real, 0.0);
     c->nu.resize(n_real); c->nuf.resize((size_t)n_real * (c->G.nt + 1)); c->vt.resize((size_t)n_real * (c->G.nt + 1)); c->om.resize((size_t)n_real * (c->G.nt + 2));
-    build_metric(c);
+    build_metric(c, nullptr);
+    c->params.assign(h_params, h_params + n_real);
     c->nu_scale.resize(n_real); c->nu_shape.assign(c->G.nt + 1, 1.0);
     for (int r = 0; r < n_real; r++) {
         build_flow(c, r, h_params[r]);
@@ -822,6 +870,24 @@ void hft_destroy(hft_ctx* c) {
     cudaFree(c->d_extpart); cudaFree(c->d_ext);
     if (c->h_ext) cudaFreeHost(c->h_ext);
     delete c;
+}
+
+int hft_set_theta_nodes(hft_ctx* c, const double* h_theta) {
+    DevGuard dg_(c);
+    if (!c || !h_theta || c->map_any) return HFT_ERR_ARG;
+    const int nt = c->G.nt;
+    if (h_theta[0] != 0.0 || fabs(h_theta[nt + 1] - kPi) > 1e-14) return HFT_ERR_ARG;
+    for (int j = 0; j <= nt; j++)
+        if (!(h_theta[j + 1] > h_theta[j])) return HFT_ERR_ARG;
+    CK(cudaStreamSynchronize(c->stream));   // the tables may still be read by enqueued work
+    build_metric(c, h_theta);
+    for (int r = 0; r < c->nr; r++) {
+        const double nu = c->nu[r];
+        build_flow(c, r, c->params[r]);      // Eq. 3-4 at the new angles (custom flow tables are set after this call)
+        c->nu[r] = nu;
+    }
+    c->tab_version++;
+    return upload_all_tables(c);
 }
 
 int hft_set_flow_tables(hft_ctx* c, int32_t r, const double* h_vtheta, const double* h_omega) {
@@ -891,7 +957,7 @@ int hft_set_grid_diffusivity(hft_ctx* c, int32_t r, double alpha_nu) {
     std::vector<double> p(nt + 1);
     for (int f = 0; f <= nt; f++) {   // Eq. 7 (:121) where nu lives: at the theta-faces
         const double dps = c->dph * c->sth[f];
-        p[f] = alpha_nu * (c->dth * c->dth + dps * dps);
+        p[f] = alpha_nu * (c->dthf[f] * c->dthf[f] + dps * dps);
     }
     return hft_set_diffusivity_profile(c, r, p.data());
 }
@@ -1093,12 +1159,12 @@ int hft_diagnostics_ext(hft_ctx* c, double polar_lat_deg, double* h_out) {
     const double thc = (90.0 - polar_lat_deg) * kPi / 180.0;
     if (c->fp64()) {
         double* S = (double*)c->arr[c->i_state];
-        k_diag_ext_partials<double><<<gp, 256, 0, c->stream>>>(S, c->Td, G, c->dth, c->dph, thc, c->d_extpart);
-        k_diag_ext_finalize<double><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_extpart, RED_CTAS, c->Td, G, c->dth, thc, scale, c->d_ext);
+        k_diag_ext_partials<double><<<gp, 256, 0, c->stream>>>(S, c->Td, G, c->dph, thc, c->d_extpart);
+        k_diag_ext_finalize<double><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_extpart, RED_CTAS, c->Td, G, thc, scale, c->d_ext);
     } else {
         float* S = (float*)c->arr[c->i_state];
-        k_diag_ext_partials<float><<<gp, 256, 0, c->stream>>>(S, c->Tf, G, c->dth, c->dph, thc, c->d_extpart);
-        k_diag_ext_finalize<float><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_extpart, RED_CTAS, c->Tf, G, c->dth, thc, scale, c->d_ext);
+        k_diag_ext_partials<float><<<gp, 256, 0, c->stream>>>(S, c->Tf, G, c->dph, thc, c->d_extpart);
+        k_diag_ext_finalize<float><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_extpart, RED_CTAS, c->Tf, G, thc, scale, c->d_ext);
     }
     c->launches += 2;
     CK(cudaMemcpyAsync(c->h_ext, c->d_ext, (size_t)c->nr * EXT_NOUT * sizeof(double), cudaMemcpyDeviceToHost, c->stream));

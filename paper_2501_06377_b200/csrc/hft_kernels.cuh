@@ -32,8 +32,12 @@ struct Tables {            // device pointers, all [R][nt+2] unless noted
     const real* sth;       // [nt+1] sin(theta_{j+1/2})                                      :354
     const real* rdt;       // [nt+2] 1/(sin(theta_j) dth)
     const real* rdp;       // [nt+2] 1/(sin(theta_j) dph)
-    const double* dA;      // [nt+2] quadrature weights: sin(theta_j) dth dph; caps: A_pole   :225-230, App. A
-    double adv_capc;       // P dph                                                          App. A (:646)
+    const double* dA;      // [nt+2] quadrature weights: sin(theta_j) dth_j dph; caps: A_pole   :225-230, App. A
+    const real* rdf;       // [nt+1] 1 / (theta_{j+1} - theta_j): node spacing across theta-face j+1/2      Eq. 27
+    const real* wmp;       // [nt+1][16] per theta-face: App. B D-factors of u^- (0..4), eps_w (5), of u^+ (8..12)   :662-680
+    const double* th;      // [nt+2] theta_j
+    double adv_capc[2];    // P dph, north / south cap                                       App. A (:646)
+    int nonuniform;        // 0: uniform theta grid -- the WENO constants are 1/2, 1/3, 2/3 and eps_w = eps_t
     real eps_t, eps_p;     // WENO3-CS(h) eps_w = dth, dph                                    :670
 };
 
@@ -191,6 +195,21 @@ __device__ __forceinline__ real weno3_side(real far, real near, real other, real
     return pos_div(a0 * p0 + a1 * p1, a0 + a1);
 }
 
+// The same on a non-uniform grid, App. B (:662-680): D = (Dex, Da, Db, d0, d1) of this face and side (Tables::wmp).
+//   p0 = (1 + Dex) near - Dex far, p1 = Da near + Db other, beta0 = 4 (Dex (near - far))^2, beta1 = 4 (Db (other - near))^2,
+//   w0 = d0 / (eps + beta0)^2, w1 = d1 / (eps + beta1)^2; one division: multiply through by (eps+beta0)^2 (eps+beta1)^2.
+template <typename real>
+__device__ __forceinline__ real weno3_side_nu(real far, real near, real other, real eps, const real* D) {
+    const real Dex = D[0], Da = D[1], Db = D[2], d0 = D[3], d1 = D[4];
+    real p0 = near + Dex * (near - far);
+    real p1 = Da * near + Db * other;
+    real q0 = (real)2 * Dex * (near - far), q1 = (real)2 * Db * (other - near);
+    real e0 = eps + q0 * q0, e1 = eps + q1 * q1;
+    real a0 = d0 * (e1 * e1);
+    real a1 = d1 * (e0 * e0);
+    return pos_div(a0 * p0 + a1 * p1, a0 + a1);
+}
+
 template <typename real>
 __device__ __forceinline__ real upwind(real v, real bm, real bp) {
     return v > (real)0 ? v * bm : (v < (real)0 ? v * bp : (real)0);
@@ -215,8 +234,14 @@ struct AdvArgs {
 // Faces 1/2, 3/2, nt-1/2, nt+1/2 (f <= 1 or f >= nt-1) are upwind (:388); the others WENO3-CS(h) with LLF (B2).
 template <typename real>
 __device__ __forceinline__ real theta_face_flux(int f, real bm1, real b0, real bp1, real bp2, const real* lm,
-                                                const real* lp, const real* vtf, int nt, real eps, int upwind_only) {
+                                                const real* lp, const real* vtf, int nt, real eps, int upwind_only,
+                                                const real* wmp /* null: uniform grid */) {
     if (upwind_only || f <= 1 || f >= nt - 1) return upwind(vtf[f], b0, bp1);
+    if (wmp) {   // non-uniform theta grid: this face's D-factors and eps_w = its node spacing
+        const real* D = wmp + 16 * (size_t)f;
+        return weno3_side_nu(bp2 * lp[f + 2], bp1 * lp[f + 1], b0 * lp[f], D[5], D + 8) +
+               weno3_side_nu(bm1 * lm[f - 1], b0 * lm[f], bp1 * lm[f + 1], D[5], D);
+    }
     real um = weno3_side(bm1 * lm[f - 1], b0 * lm[f], bp1 * lm[f + 1], eps);   // right-moving part, from LM
     real up = weno3_side(bp2 * lp[f + 2], bp1 * lp[f + 1], b0 * lp[f], eps);   // left-moving part, from LP
     return up + um;
@@ -253,12 +278,13 @@ __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> 
     auto ld = [&](int j) -> real { return in[(size_t)min(max(j, 0), nt + 1) * G.pitch + k0]; };
 
     real w0 = ld(j0 - 2), w1 = ld(j0 - 1), w2 = ld(j0), w3 = ld(j0 + 1);
-    real Fn = theta_face_flux<real>(j0 - 1, w0, w1, w2, w3, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
+    const real* wmp = T.nonuniform ? T.wmp : nullptr;
+    real Fn = theta_face_flux<real>(j0 - 1, w0, w1, w2, w3, lm, lp, vtf, nt, T.eps_t, A.upwind_only, wmp);
     double sumN = 0.0, sumS = 0.0;
     if (j0 == 1) sumN = live ? (double)Fn : 0.0;
     for (int j = j0; j < j1; j++) {
         real w4 = ld(j + 2);
-        real Fs = theta_face_flux<real>(j, w1, w2, w3, w4, lm, lp, vtf, nt, T.eps_t, A.upwind_only);
+        real Fs = theta_face_flux<real>(j, w1, w2, w3, w4, lm, lp, vtf, nt, T.eps_t, A.upwind_only, wmp);
         const real* row = in + (size_t)j * G.pitch;
         real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1], bp2 = row[kp2];
         real Fw = phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, A.upwind_only);
@@ -306,6 +332,10 @@ __global__ void __launch_bounds__(TX) k_adv_stage_att(AdvArgs<real> A, Tables<re
     // theta-face flux at face f from B rows f-1..f+2 and the half-speeds LMt rows f-1..f+1, LPt rows f..f+2
     auto theta_flux = [&](int f, real bm1, real b0, real bp1, real bp2, real m0, real m1, real m2, real p0, real p1, real p2) -> real {
         if (uw || f <= 1 || f >= nt - 1) return upwind(col(A.VT, f), b0, bp1);
+        if (T.nonuniform) {
+            const real* D = T.wmp + 16 * (size_t)f;
+            return weno3_side_nu(bp2 * p2, bp1 * p1, b0 * p0, D[5], D + 8) + weno3_side_nu(bm1 * m0, b0 * m1, bp1 * m2, D[5], D);
+        }
         real um = weno3_side(bm1 * m0, b0 * m1, bp1 * m2, T.eps_t);
         real up = weno3_side(bp2 * p2, bp1 * p1, b0 * p0, T.eps_t);
         return up + um;
@@ -373,7 +403,7 @@ __global__ void __launch_bounds__(TX) k_adv_caps(AdvArgs<real> A, Tables<real> T
     const int j = pole == 0 ? 0 : G.nt + 1;
     const size_t off = (size_t)r * G.rstride + (size_t)j * G.pitch;
     double S = sum_partials(A.part + ((size_t)r * 2 + pole) * G.nbx, G.nbx);
-    real tend = (real)((pole == 0 ? 1.0 : -1.0) * (T.adv_capc * S));
+    real tend = (real)((pole == 0 ? 1.0 : -1.0) * (T.adv_capc[pole] * S));
     real o = A.cb * A.in[off] - A.cdt * tend;
     if (A.ca != (real)0) o = A.ca * A.fn[off] + o;
     A.out[off + k] = o;
@@ -599,7 +629,7 @@ __device__ __forceinline__ double block_min(double v, double* smem /*[32]*/) {
 // Rows 1..nt: polar-region fluxes (cells with theta_j <= thc or >= pi - thc), the dipole integrands of Eq. 16-17 and
 // min / max / min|B|.  part[r][cta][EXT_NPART]; grid (RED_CTAS, R), block 256.  Row sums in fp64, weights per row.
 template <typename real>
-__global__ void __launch_bounds__(256) k_diag_ext_partials(const real* state, Tables<real> T, Geom G, double dth, double dph,
+__global__ void __launch_bounds__(256) k_diag_ext_partials(const real* state, Tables<real> T, Geom G, double dph,
                                                            double thc, double* part) {
     __shared__ double red[32];
     const int r = blockIdx.y;
@@ -607,7 +637,7 @@ __global__ void __launch_bounds__(256) k_diag_ext_partials(const real* state, Ta
     double acc[7] = {0, 0, 0, 0, 0, 0, 0};
     double vmin = 1.0e300, vmax = -1.0e300, amin = 1.0e300;
     for (int j = 1 + blockIdx.x; j <= G.nt; j += gridDim.x) {
-        const double th = (double)j * dth, dA = T.dA[j];
+        const double th = T.th[j], dA = T.dA[j];
         const int region = th <= thc ? 0 : (th >= 3.14159265358979323846264338327950288 - thc ? 1 : -1);
         double rp = 0.0, rm = 0.0, rc = 0.0, rs = 0.0;
         for (int k = threadIdx.x; k < G.np; k += blockDim.x) {
@@ -637,7 +667,7 @@ __global__ void __launch_bounds__(256) k_diag_ext_partials(const real* state, Ta
 // One thread per realization: partials in index order, then the two caps (one cell each: sin(theta) = 0, so they
 // enter D, the polar fluxes / areas and the extrema only) and the region areas.
 template <typename real>
-__global__ void k_diag_ext_finalize(const real* state, const double* part, int nparts, Tables<real> T, Geom G, double dth,
+__global__ void k_diag_ext_finalize(const real* state, const double* part, int nparts, Tables<real> T, Geom G,
                                     double thc, double scale, double* out) {
     const int r = blockIdx.x * blockDim.x + threadIdx.x;
     if (r >= G.nr) return;
@@ -651,13 +681,13 @@ __global__ void k_diag_ext_finalize(const real* state, const double* part, int n
     }
     double area[2] = {0.0, 0.0};
     for (int j = 1; j <= G.nt; j++) {
-        const double th = (double)j * dth;
+        const double th = T.th[j];
         if (th <= thc) area[0] += T.dA[j] * (double)G.np;
         else if (th >= PI_ - thc) area[1] += T.dA[j] * (double)G.np;
     }
     for (int pole = 0; pole < 2; pole++) {
         const double v = (double)state[(size_t)r * G.rstride + (size_t)(pole == 0 ? 0 : G.nt + 1) * G.pitch];
-        const double th = pole == 0 ? 0.0 : (double)(G.nt + 1) * dth, dA = T.dA[0];
+        const double th = pole == 0 ? 0.0 : PI_, dA = T.dA[pole == 0 ? 0 : G.nt + 1];
         const int region = th <= thc ? 0 : (th >= PI_ - thc ? 1 : -1);
         if (region >= 0) {
             if (v > 0.0) acc[2 * region] += v * dA; else if (v < 0.0) acc[2 * region + 1] += v * dA;

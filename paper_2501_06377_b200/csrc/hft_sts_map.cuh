@@ -27,8 +27,7 @@ template <typename real>
 struct MapArgs {
     const real* NU;       // [R][nt+2][pitch], rows 0..nt used
     const double* capw;   // [R][2] sum_k (NU[f][k] + NU[f][k-1])/2 for f = 0 and f = nt, in fp64 from the stored values
-    double capP;          // P dph / dth
-    real rdth;            // 1 / dth
+    double capP[2];       // P dph / (theta_1 - theta_0), north / south cap
     int nparts_in;        // polar partial sums per row in part_in (the writer's CTAs along phi)
 };
 
@@ -71,12 +70,12 @@ __global__ void __launch_bounds__(TX) k_sts_stage_map(StsArgs<real> A, MapArgs<r
         if (j == 0 || j == G.nt + 1) {
             const int pole = (j == 0) ? 0 : 1;
             double S = sum_partials(A.part_in + ((size_t)r * 2 + pole) * G.nbx, M.nparts_in);
-            L = (real)(M.capP * (S - M.capw[2 * r + pole] * (double)c));
+            L = (real)(M.capP[pole] * (S - M.capw[2 * r + pole] * (double)c));
         } else {
             real w = in[(size_t)j * G.pitch + kw], e = in[(size_t)j * G.pitch + ke];
-            const real gt = T.rdt[j] * M.rdth, gp = T.rdp[j] * T.rdp[j];
-            const real as = half * (nSk + nSw) * (T.sth[j] * gt);
-            const real an = half * (nNk + nNw) * (T.sth[j - 1] * gt);
+            const real gp = T.rdp[j] * T.rdp[j];
+            const real as = half * (nSk + nSw) * (T.sth[j] * (T.rdt[j] * T.rdf[j]));
+            const real an = half * (nNk + nNw) * (T.sth[j - 1] * (T.rdt[j] * T.rdf[j - 1]));
             const real ae = half * (nSk + nNk) * gp;
             const real aw = half * (nSw + nNw) * gp;
             L = (as * (s - c) - an * (c - n)) + (ae * (e - c) - aw * (c - w));
@@ -169,7 +168,7 @@ __global__ void __launch_bounds__(TX) k_sts_stage_mapv(StsArgs<real> A, MapArgs<
         if (j == 0 || j == G.nt + 1) {
             const int pole = (j == 0) ? 0 : 1;
             double S = sum_partials(A.part_in + ((size_t)r * 2 + pole) * G.nbx, M.nparts_in);
-            const real L = MAP ? (real)(M.capP * (S - M.capw[2 * r + pole] * (double)c[0]))
+            const real L = MAP ? (real)(M.capP[pole] * (S - M.capw[2 * r + pole] * (double)c[0]))
                                : (real)(T.capc[2 * r + pole] * (S - (double)G.np * (double)c[0]));
 #pragma unroll
             for (int q = 0; q < C; q++) Lv[q] = L;
@@ -187,8 +186,8 @@ __global__ void __launch_bounds__(TX) k_sts_stage_mapv(StsArgs<real> A, MapArgs<
                 }
             }
             if (MAP) {
-            const real gt = T.rdt[j] * M.rdth, gp = T.rdp[j] * T.rdp[j];
-            const real gs = T.sth[j] * gt, gn = T.sth[j - 1] * gt;
+            const real gp = T.rdp[j] * T.rdp[j];
+            const real gs = T.sth[j] * (T.rdt[j] * T.rdf[j]), gn = T.sth[j - 1] * (T.rdt[j] * T.rdf[j - 1]);
 #pragma unroll
             for (int q = 0; q < C; q++) {
                 const real nSq_w = q == 0 ? nSw : nS[q > 0 ? q - 1 : 0];

@@ -39,7 +39,7 @@ int sts_blocked_step(StsBlockedPlan<real>& P, Tables<real>& T, const Geom& G, in
     dim3 g1(nbxv, (G.nt + 2 + MAPV_RPT - 1) / MAPV_RPT, G.nr), gs(G.nbx, 2, G.nr);
     k_polar_row_sums<real><<<gs, TX, 0, P.stream>>>(P.Y0, P.part[0], G);
     MapArgs<real> M;
-    M.NU = nullptr; M.capw = nullptr; M.capP = 0.0; M.rdth = (real)0; M.nparts_in = G.nbx;
+    M.NU = nullptr; M.capw = nullptr; M.capP[0] = M.capP[1] = 0.0; M.nparts_in = G.nbx;
     StsArgs<real> a;
     a.F = F; a.Y0 = P.Y0; a.mu = 0; a.nu = 0; a.g = 0; a.use_d2 = 0;
     a.in = P.Y0; a.d2 = b[0]; a.part_in = P.part[0]; a.part_out = P.part[1]; a.a = (real)P.a[1];

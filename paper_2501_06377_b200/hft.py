@@ -18,7 +18,7 @@ if not os.path.exists(LIB_PATH):
                       "(the CUDA extension is required; there is no CPU fallback)")
 _lib = C.CDLL(LIB_PATH)
 
-EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_diffusivity_map", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
+EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_theta_nodes", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_diffusivity_map", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
            "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_diagnostics", "hft_diagnostics_ext", "hft_stable_dt",
            "hft_sts_stage_count", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
            "hft_last_cuda_error"]
@@ -51,6 +51,7 @@ _lib.hft_create.argtypes = [C.POINTER(hft_grid), C.c_int32, C.POINTER(hft_params
 _lib.hft_destroy.argtypes = [C.c_void_p]
 _lib.hft_destroy.restype = None
 _lib.hft_set_flow_tables.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+_lib.hft_set_theta_nodes.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
 _lib.hft_set_diffusivity_profile.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
 _lib.hft_set_grid_diffusivity.argtypes = [C.c_void_p, C.c_int32, C.c_double]
 _lib.hft_set_diffusivity_map.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_double)]
@@ -152,6 +153,11 @@ class Context:
             pass
 
     # -- C-ABI calls (same names) ----------------------------------------------------------
+    def set_theta_nodes(self, theta):
+        a = np.ascontiguousarray(theta, dtype=np.float64)
+        assert a.shape == (self.n_theta + 2,)
+        self._ck(_lib.hft_set_theta_nodes(self._h, a.ctypes.data_as(C.POINTER(C.c_double))), "hft_set_theta_nodes")
+
     def set_flow_tables(self, r, vtheta_m_s, omega_m_s):
         vt = np.ascontiguousarray(vtheta_m_s, dtype=np.float64)
         om = np.ascontiguousarray(omega_m_s, dtype=np.float64)

@@ -163,6 +163,71 @@ def test_sts_block_sizes_ragged(dtype, block, s_forced, nphi, kern):
     ctx.close()
 
 
+def _stretched_nodes(nt, a=0.2):
+    xi = np.arange(nt + 2) * math.pi / (nt + 1)
+    th = xi + a * np.sin(2 * xi)
+    th[0], th[-1] = 0.0, math.pi
+    return th
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("path", ["default", "pipe", "upipe", "unblocked", "attenuated", "nu_map"])
+def test_nonuniform_theta_grid(dtype, path):
+    """the non-uniform theta grid (Eq. 27-28 with the printed spacings, App. A per-cap
+    prefactors, App. B D-factors; readings U12, U33) through every STS path -- both temporally blocked kernels, one launch
+    per stage, nu(theta, phi) -- with WENO3 advection, flow attenuation, assimilation and all diagnostics, on a ragged
+    stretched grid (cells differ by a factor 2.3 in width), 3 realizations."""
+    H = hft()
+    w = wl.scaled(wl.config(3), 75, 264, n_real=3)
+    w.params = np.array(w.params, dtype=np.float64)
+    w.params[:, 0] *= 12.0                            # eta x 12: s ~ 35 stages at CFL 0.5, enough for the blocked kernels
+    kw = {"default": {}, "pipe": dict(sts_kernel=1, f32_arith=1), "upipe": dict(sts_kernel=2, f32_arith=1), "unblocked": dict(sts_block=1),
+          "attenuated": dict(flow_attenuation=1), "nu_map": dict(diffusivity_map=1)}[path]
+    ctx, o = make_pair(w, dtype, **kw)
+    th = _stretched_nodes(w.n_theta)
+    ctx.set_theta_nodes(th)
+    o.set_theta_nodes(th)
+    # set_map averaged the caps on the old grid: same on both sides; re-set the maps so that both start from the same state
+    maps = wl.initial_maps(w).to(torch.float64 if dtype == "f64" else torch.float32)
+    for r in range(w.n_real):
+        ctx.set_map(r, maps[r].contiguous().cuda())
+        o.set_map(r, maps[r].numpy())
+    if path == "attenuated":
+        ctx.set_attenuation(-1, 30.0)
+        for r in range(w.n_real):
+            o.set_attenuation(r, 30.0)
+    if path == "nu_map":
+        for r in range(w.n_real):
+            m = wl.diffusivity_map(w, r)
+            ctx.set_diffusivity_map(r, m)
+            o.set_diffusivity_map(r, m)
+    ga, gd = ctx.stable_dt()
+    oa, od = o.stable_dt()
+    assert abs(ga / oa - 1) < 1e-13 and abs(gd / od - 1) < 1e-13
+    dt = 0.5 * ga
+    s = ctx.sts_stage_count(dt)
+    assert s == o.sts_stage_count(dt) and s > 20
+    before = ctx.diagnostics()
+    ctx.step(3, dt)
+    o.step(3, dt)
+    compare(ctx, o, TOL[dtype], "non-uniform " + path)
+    after = ctx.diagnostics()
+    assert np.all(np.abs(after[:, 0] - before[:, 0]) <= (1e-12 if dtype == "f64" else 2e-5) * before[:, 1])
+    wt = wl.assimilation_weights(w, 3 * dt)
+    obs = torch.from_numpy(o.get_map(0)).clone() + wl.emergence_map(w, 0).to(maps.dtype)
+    ctx.assimilate(obs.contiguous().cuda(), wt.to(maps.dtype).cuda(), flags=1)
+    o.assimilate(obs.numpy(), wt.to(maps.dtype).numpy(), flags=1)
+    compare(ctx, o, TOL[dtype], "non-uniform assimilation")
+    dg, do = ctx.diagnostics(), o.diagnostics()
+    assert np.allclose(dg, do, rtol=0, atol=(1e-12 if dtype == "f64" else 1e-5) * do[:, 1].max())
+    eg, eo = ctx.diagnostics_ext(55.0), o.diagnostics_ext(55.0)
+    tol, bmax = (1e-12 if dtype == "f64" else 2e-5), np.abs(eo[:, 6:8]).max()
+    assert np.allclose(eg[:, 0:4], eo[:, 0:4], rtol=0, atol=tol * do[:, 1].max())
+    assert np.allclose(eg[:, 4:6], eo[:, 4:6], rtol=1e-13, atol=0)                    # region areas: geometry only
+    assert np.allclose(eg[:, 6:13], eo[:, 6:13], rtol=0, atol=tol * bmax)
+    ctx.close()
+
+
 @pytest.mark.parametrize("block", [1, 0])
 def test_config1_full_length(block):
     """BASELINE config 1: 512x1024, 40 pairs, flows of reading U17, eta = 500, 16 steps of 1.5 h, s = 217."""
