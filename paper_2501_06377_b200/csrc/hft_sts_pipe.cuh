@@ -96,6 +96,7 @@ struct PipeWarp {
     static constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, NF = P::NF, ROW = P::ROW, NCS = P::NCS;
     static constexpr int W = P::W, NG = P::NG, CS = P::CS;
     static constexpr bool SHIFTF = P::SHIFTF;
+    static constexpr bool HOIST_SHFL = true;
     using UV = UVec<real>;
     using V = typename UV::V;   // what one FMA handles: a double, or a float2 pair (packed FFMA2 / FMUL2 of sm_100)
 
@@ -180,6 +181,18 @@ struct PipeWarp {
         const real raw_next = s_raw[sl * 32];   // this lane's own copy, arrived with the group of row t
         const real* cfs = s_coef + (PH % NCS) * CS;
         V outK[NG];
+        // phi-neighbours of every level first: level l reads row t-l of level l-1, which the PREVIOUS row-step produced, so
+        // all 2K shuffles of a row-step are independent of its arithmetic (issued where they are used, their (e + w) adds
+        // waited on the shuffle: 10 % of the warp samples, profiles/r02_blocked_kernels.md)
+        real wv[K], ev[K];
+        if constexpr (HOIST_SHFL) {
+#pragma unroll
+            for (int l = 1; l <= K; l++) {
+                const int sC = pmod(PH - l, 3);
+                wv[l - 1] = __shfl_up_sync(0xffffffffu, UV::get(u[l - 1][sC][NG - 1], W - 1), 1);
+                ev[l - 1] = __shfl_down_sync(0xffffffffu, UV::get(u[l - 1][sC][0], 0), 1);
+            }
+        }
 #pragma unroll
         for (int l = 1; l <= K; l++) {
             // level l-1: newest row t-l+1 (s), centre t-l (c), oldest t-l-1 (n)
@@ -189,8 +202,8 @@ struct PipeWarp {
             vload<real, 2 * W>(*reinterpret_cast<real(*)[2 * W]>(&cf4[2]), cfs + (l - 1) * 4 * W + 2 * W);
             const V An = cf4[0], As = cf4[1], Af = cf4[2], Ac = cf4[3];
             const V nuc = A.nu2[l - 1], gc = A.g2[l - 1];
-            const real west = __shfl_up_sync(0xffffffffu, UV::get(u[l - 1][sC][NG - 1], W - 1), 1);
-            const real east = __shfl_down_sync(0xffffffffu, UV::get(u[l - 1][sC][0], 0), 1);
+            const real west = HOIST_SHFL ? wv[l - 1] : __shfl_up_sync(0xffffffffu, UV::get(u[l - 1][sC][NG - 1], W - 1), 1);
+            const real east = HOIST_SHFL ? ev[l - 1] : __shfl_down_sync(0xffffffffu, UV::get(u[l - 1][sC][0], 0), 1);
             V res[NG];
 #pragma unroll
             for (int gI = 0; gI < NG; gI++) {
