@@ -186,6 +186,11 @@ int hft_step(hft_ctx* ctx, int32_t n_steps, double dt_hours);
  * (Eq. 10-11).  Caps are blended with the row means of obs and w (reading U18). */
 int hft_assimilate(hft_ctx* ctx, const void* d_obs, const void* d_weights, int32_t shared, int32_t flags);
 
+/* hft_assimilate followed by hft_diagnostics of the blended state, fused: the blend kernel accumulates Phi+ / Phi- of the values
+ * it writes, so the state is read once instead of twice (north_star's "fused assimilation/diagnostics kernel"; SURVEY.md 8(a)
+ * row A8).  h_out[n_real][4] as hft_diagnostics.  Synchronises the stream. */
+int hft_assimilate_diagnostics(hft_ctx* ctx, const void* d_obs, const void* d_weights, int32_t shared, int32_t flags, double* h_out);
+
 /* Flux diagnostics (:225-230): h_out[n_real][4] = {signed, unsigned, Phi+, Phi-} in G*radius_cm^2.
  * Synchronises the stream. */
 int hft_diagnostics(hft_ctx* ctx, double* h_out);

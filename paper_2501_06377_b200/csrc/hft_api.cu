@@ -1087,34 +1087,52 @@ int hft_step(hft_ctx* c, int32_t n_steps, double dt) {
     return check_launch(c);
 }
 
-int hft_assimilate(hft_ctx* c, const void* d_obs, const void* d_w, int32_t shared, int32_t flags) {
-    DevGuard dg_(c);
-    if (!c || !d_obs || !d_w) return HFT_ERR_ARG;
+}  // extern "C"
+
+// Eq. 8 / Eq. 10-11 blend; with h_diag the flux integrals of the blended state come out of the same pass (k_assim_blend_diag)
+template <typename real>
+static int assimilate_impl(hft_ctx* c, const real* obs, const real* w, int32_t shared, int32_t flags, double* h_diag) {
     const Geom& G = c->G;
+    Tables<real>& T = tables_of<real>(c);
     const int balanced = flags & 1, nmaps = shared ? 1 : c->nr;
     dim3 gm(2, nmaps), gb(G.nbx, G.nt + 2, c->nr), gp(RED_CTAS, c->nr);
     const int fin_blocks = (c->nr + 63) / 64;
-    if (c->fp64()) {
-        double* S = (double*)c->arr[c->i_state];
-        k_assim_cap_means<double><<<gm, 256, 0, c->stream>>>((const double*)d_obs, (const double*)d_w, G, c->d_capinfo);
-        if (balanced) {
-            k_flux_partials<double, 1><<<gp, 256, 0, c->stream>>>(S, (const double*)d_obs, (const double*)d_w, shared, c->Td, G, c->d_fluxpart);
-            k_flux_finalize<double, 1><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, c->d_capinfo, shared, c->Td, G, 1.0, c->d_scale);
-            c->launches += 2;
-        }
-        k_assim_blend<double><<<gb, TX, 0, c->stream>>>(S, (const double*)d_obs, (const double*)d_w, shared, c->d_capinfo, c->d_scale, balanced, G);
-    } else {
-        float* S = (float*)c->arr[c->i_state];
-        k_assim_cap_means<float><<<gm, 256, 0, c->stream>>>((const float*)d_obs, (const float*)d_w, G, c->d_capinfo);
-        if (balanced) {
-            k_flux_partials<float, 1><<<gp, 256, 0, c->stream>>>(S, (const float*)d_obs, (const float*)d_w, shared, c->Tf, G, c->d_fluxpart);
-            k_flux_finalize<float, 1><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, c->d_capinfo, shared, c->Tf, G, 1.0, c->d_scale);
-            c->launches += 2;
-        }
-        k_assim_blend<float><<<gb, TX, 0, c->stream>>>(S, (const float*)d_obs, (const float*)d_w, shared, c->d_capinfo, c->d_scale, balanced, G);
+    real* S = (real*)c->arr[c->i_state];
+    k_assim_cap_means<real><<<gm, 256, 0, c->stream>>>(obs, w, G, c->d_capinfo);
+    if (balanced) {
+        k_flux_partials<real, 1><<<gp, 256, 0, c->stream>>>(S, obs, w, shared, T, G, c->d_fluxpart);
+        k_flux_finalize<real, 1><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, c->d_capinfo, shared, T, G, 1.0, c->d_scale);
+        c->launches += 2;
     }
-    c->launches += 2;
-    return check_launch(c);
+    if (!h_diag) {
+        k_assim_blend<real><<<gb, TX, 0, c->stream>>>(S, obs, w, shared, c->d_capinfo, c->d_scale, balanced, G);
+        c->launches += 2;
+        return check_launch(c);
+    }
+    const double scale = c->grid.radius_cm * c->grid.radius_cm;
+    k_assim_blend_diag<real><<<gp, 256, 0, c->stream>>>(S, obs, w, shared, c->d_capinfo, c->d_scale, balanced, T, G, c->d_fluxpart);
+    k_flux_finalize<real, 0><<<fin_blocks, 64, 0, c->stream>>>(S, c->d_fluxpart, RED_CTAS, nullptr, 0, T, G, scale, c->d_diag);
+    c->launches += 3;
+    CK(cudaMemcpyAsync(c->h_diag, c->d_diag, (size_t)c->nr * 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    memcpy(h_diag, c->h_diag, (size_t)c->nr * 4 * sizeof(double));
+    return HFT_OK;
+}
+
+extern "C" {
+
+int hft_assimilate(hft_ctx* c, const void* d_obs, const void* d_w, int32_t shared, int32_t flags) {
+    DevGuard dg_(c);
+    if (!c || !d_obs || !d_w) return HFT_ERR_ARG;
+    return c->fp64() ? assimilate_impl<double>(c, (const double*)d_obs, (const double*)d_w, shared, flags, nullptr)
+                     : assimilate_impl<float>(c, (const float*)d_obs, (const float*)d_w, shared, flags, nullptr);
+}
+
+int hft_assimilate_diagnostics(hft_ctx* c, const void* d_obs, const void* d_w, int32_t shared, int32_t flags, double* h_out) {
+    DevGuard dg_(c);
+    if (!c || !d_obs || !d_w || !h_out) return HFT_ERR_ARG;
+    return c->fp64() ? assimilate_impl<double>(c, (const double*)d_obs, (const double*)d_w, shared, flags, h_out)
+                     : assimilate_impl<float>(c, (const float*)d_obs, (const float*)d_w, shared, flags, h_out);
 }
 
 int hft_diagnostics(hft_ctx* c, double* h_out) {

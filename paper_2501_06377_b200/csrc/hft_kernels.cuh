@@ -553,7 +553,7 @@ __global__ void __launch_bounds__(256) k_assim_cap_means(const real* obs, const 
     }
 }
 
-// Finalize flux integrals: add the caps (area dA[0] = dA[nt+1] = A_pole), sum the CTA partials in index order.
+// Finalize flux integrals: add the caps (areas dA[0], dA[nt+1]), sum the CTA partials in index order.
 // WHAT 0: out[r][4] = {signed, unsigned, Phi+, Phi-} * scale.   WHAT 1: out[r] = sqrt|Phi+/Phi-| (1 if either is 0).
 template <typename real, int WHAT>
 __global__ void k_flux_finalize(const real* state, const double* part, int nparts, const double* capinfo, int shared,
@@ -568,7 +568,7 @@ __global__ void k_flux_finalize(const real* state, const double* part, int npart
             const double* ci = capinfo + ((size_t)(shared ? 0 : r) * 2 + pole) * 2;
             v = (real)ci[1] * ((real)ci[0] - v);
         }
-        double c = (double)v * T.dA[0];
+        double c = (double)v * T.dA[pole == 0 ? 0 : G.nt + 1];
         if (v > (real)0) pp += c; else pm += c;
     }
     if (WHAT == 0) {
@@ -606,6 +606,51 @@ __global__ void __launch_bounds__(TX) k_assim_blend(real* state, const real* obs
         real d = F * (Bd - B);
         d = (d > (real)0) ? d / sc : d * sc;
         *p = B + d;
+    }
+}
+
+// The blend and the flux integrals of the blended state in ONE pass (north_star's "fused assimilation/diagnostics kernel";
+// "fused into A7 when called together").  grid (RED_CTAS, R), block 256: a CTA owns the rows
+// blockIdx.x, blockIdx.x + RED_CTAS, ... of 0..nt+1, blends them exactly as k_assim_blend does and accumulates Phi+ / Phi- of
+// the NEW values of rows 1..nt (row sums in fp64, then x dA_j) into part[r][cta][2]; k_flux_finalize<WHAT = 0> adds the caps
+// from the blended state.  The balanced form still needs its scale factor first (Eq. 11 needs Phi+- of the whole increment).
+template <typename real>
+__global__ void __launch_bounds__(256) k_assim_blend_diag(real* state, const real* obs, const real* wgt, int shared,
+                                                          const double* capinfo, const double* scale, int balanced,
+                                                          Tables<real> T, Geom G, double* part) {
+    __shared__ double red[32];
+    const int r = blockIdx.y;
+    real* f = state + (size_t)r * G.rstride;
+    const size_t mapoff = shared ? 0 : (size_t)r * G.nt * G.np;
+    const real sc = balanced ? (real)scale[r] : (real)1;
+    double pp = 0.0, pm = 0.0;
+    for (int j = blockIdx.x; j <= G.nt + 1; j += gridDim.x) {
+        const bool cap = j == 0 || j == G.nt + 1;
+        const double* ci = capinfo + ((size_t)(shared ? 0 : r) * 2 + (j == 0 ? 0 : 1)) * 2;
+        double rp = 0.0, rm = 0.0;
+        for (int k = threadIdx.x; k < G.np; k += blockDim.x) {
+            real Bd, F;
+            if (cap) { Bd = (real)ci[0]; F = (real)ci[1]; }
+            else { const size_t m = mapoff + (size_t)(j - 1) * G.np + k; Bd = obs[m]; F = wgt[m]; }
+            const real B = f[(size_t)j * G.pitch + k];
+            real v;
+            if (!balanced) {
+                v = F * Bd + ((real)1 - F) * B;
+            } else {
+                real d = F * (Bd - B);
+                d = (d > (real)0) ? d / sc : d * sc;
+                v = B + d;
+            }
+            f[(size_t)j * G.pitch + k] = v;
+            if (!cap) { if (v > (real)0) rp += (double)v; else rm += (double)v; }
+        }
+        if (!cap) { pp += rp * T.dA[j]; pm += rm * T.dA[j]; }
+    }
+    const double tp = block_sum(pp, red);
+    const double tm = block_sum(pm, red);
+    if (threadIdx.x == 0) {
+        part[((size_t)r * gridDim.x + blockIdx.x) * 2 + 0] = tp;
+        part[((size_t)r * gridDim.x + blockIdx.x) * 2 + 1] = tm;
     }
 }
 

@@ -19,7 +19,7 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 
 EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_theta_nodes", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_diffusivity_map", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
-           "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_diagnostics", "hft_diagnostics_ext", "hft_stable_dt",
+           "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_assimilate_diagnostics", "hft_diagnostics", "hft_diagnostics_ext", "hft_stable_dt",
            "hft_sts_stage_count", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
            "hft_last_cuda_error"]
 
@@ -64,6 +64,7 @@ _lib.hft_get_full.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
 _lib.hft_set_full.argtypes = [C.c_void_p, C.c_int32, C.c_void_p]
 _lib.hft_step.argtypes = [C.c_void_p, C.c_int32, C.c_double]
 _lib.hft_assimilate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32]
+_lib.hft_assimilate_diagnostics.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_double)]
 _lib.hft_diagnostics.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
 _lib.hft_diagnostics_ext.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
 _lib.hft_stable_dt.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -219,6 +220,14 @@ class Context:
         lead = 1 if shared else self.n_real
         self._ck(_lib.hft_assimilate(self._h, self._map_ptr(obs, lead), self._map_ptr(weights, lead), int(shared),
                                      int(flags)), "hft_assimilate")
+
+    def assimilate_diagnostics(self, obs, weights, flags=0):
+        shared = obs.dim() == 2 or (obs.shape[0] == 1 and self.n_real > 1)
+        lead = 1 if shared else self.n_real
+        out = np.zeros((self.n_real, 4))
+        self._ck(_lib.hft_assimilate_diagnostics(self._h, self._map_ptr(obs, lead), self._map_ptr(weights, lead), int(shared),
+                                                 int(flags), out.ctypes.data_as(C.POINTER(C.c_double))), "hft_assimilate_diagnostics")
+        return out
 
     def diagnostics(self):
         out = np.zeros((self.n_real, 4))

@@ -454,6 +454,49 @@ def test_config4_full_size_assimilation_cycle():
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("flags", [0, 1])
+def test_fused_assimilation_diagnostics(dtype, flags):
+    """hft_assimilate_diagnostics = hft_assimilate + hft_diagnostics in one pass over the state (north_star's fused
+    assimilation/diagnostics kernel): the blended state must be bit-identical to the two-call sequence, the diagnostics equal
+    to it up to summation order, and both must match the oracle; plain (Eq. 8) and flux-balanced (Eq. 10-11) blend, shared
+    and per-realization observations, ragged grid."""
+    H = hft()
+    w = wl.scaled(wl.config(4), 61, 200, t_end_hours=3.0)
+    w.params = np.repeat(w.params, 3, axis=0)
+    w.params[1, 0], w.params[2, 0] = 350.0, 650.0
+    w.n_real = 3
+    ctx, o = make_pair(w, dtype)
+    ctx2, _ = make_pair(w, dtype)
+    dt, _, per = wl.plan(w, *ctx.stable_dt())
+    for c in (ctx, ctx2):
+        c.step(1, dt)
+    o.step(1, dt)
+    td = torch.float64 if dtype == "f64" else torch.float32
+    wt = wl.assimilation_weights(w, dt).to(td)
+    obs1 = (torch.from_numpy(o.get_map(0)) + wl.emergence_map(w, 0).to(td)).contiguous()
+    dg = ctx.assimilate_diagnostics(obs1.cuda(), wt.cuda(), flags=flags)
+    ctx2.assimilate(obs1.cuda(), wt.cuda(), flags=flags)
+    d2 = ctx2.diagnostics()
+    o.assimilate(obs1.numpy(), wt.numpy(), flags=flags)
+    do = o.diagnostics()
+    for r in range(w.n_real):
+        assert torch.equal(ctx.get_full(r), ctx2.get_full(r))
+    tol = 1e-12 if dtype == "f64" else 1e-5
+    assert np.allclose(dg, d2, rtol=0, atol=1e-13 * do[:, 1].max())
+    assert np.allclose(dg, do, rtol=0, atol=tol * do[:, 1].max())
+    compare(ctx, o, TOL[dtype], "fused blend")
+    # per-realization observations
+    obsR = torch.stack([torch.from_numpy(o.get_map(r)) + wl.emergence_map(w, 1 + r).to(td) for r in range(w.n_real)]).contiguous()
+    wtR = torch.stack([wl.assimilation_weights(w, dt * (2 + r)).to(td) for r in range(w.n_real)]).contiguous()
+    dg = ctx.assimilate_diagnostics(obsR.cuda(), wtR.cuda(), flags=flags)
+    o.assimilate(obsR.numpy(), wtR.numpy(), flags=flags)
+    assert np.allclose(dg, o.diagnostics(), rtol=0, atol=tol * do[:, 1].max())
+    compare(ctx, o, TOL[dtype], "fused blend, per-realization maps")
+    ctx.close()
+    ctx2.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_assimilation_and_diagnostics(dtype):
     """Config 4 recipe on a small grid: steps, hourly blend with disc weights, per-realization and shared
     observations, flux-balanced variant, diagnostics."""
