@@ -215,6 +215,11 @@ int hft_diagnostics_ext(hft_ctx* ctx, double polar_lat_deg, double* h_out);
 int hft_stable_dt(hft_ctx* ctx, double* h_dt_adv_limit_hours, double* h_dt_diff_euler_hours);
 int hft_sts_stage_count(hft_ctx* ctx, double dt_hours, int32_t* h_stages);
 
+/* Wait for everything this context has enqueued and report it: hft_step and the other asynchronous calls return once their
+ * kernels are QUEUED, so a fault inside a kernel surfaces at the next synchronising call; calling hft_synchronize after a
+ * step attributes it to that step (HFT_ERR_CUDA, text in hft_last_cuda_error). */
+int hft_synchronize(hft_ctx* ctx);
+
 /* Number of kernel launches enqueued by this context so far. */
 int hft_launch_count(hft_ctx* ctx, int64_t* h_count);
 

@@ -530,7 +530,7 @@ int advect(hft_ctx* c, double dt) {
         sts.push_back({B, S, A, 2.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0});
         sts.push_back({A, nullptr, B, 0.0, 1.0, 0.5});
     }
-    dim3 g(G.nbx, (G.nt + RPT - 1) / RPT, c->nr), gc(G.nbx, 2, c->nr);
+    dim3 g(G.nbxa, (G.nt + RPT - 1) / RPT, c->nr), gc(G.nbx, 2, c->nr);
     real* att[kNumAttArrays] = {nullptr};
     if (c->att_any) {
         for (int i = 0; i < kNumAttArrays; i++) att[i] = (real*)c->att[i];
@@ -814,6 +814,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     c->G.nt = grid->n_theta; c->G.np = grid->n_phi; c->G.pitch = pitch_for(grid->n_phi, grid->dtype); c->G.nr = n_real;
     c->G.rstride = (size_t)(grid->n_theta + 2) * c->G.pitch;
     c->G.nbx = (grid->n_phi + TX - 1) / TX;
+    c->G.nbxa = (grid->n_phi + ADV_COLS - 1) / ADV_COLS;
     c->arr_bytes = need / (kNumArrays + extra_arrays(&o));
     for (int i = 0; i < kNumArrays; i++) c->arr[i] = (char*)d_workspace + (size_t)i * c->arr_bytes;
     if (o.flow_attenuation)
@@ -837,7 +838,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     int rc = HFT_OK;
     auto fail = [&](int code) { hft_destroy(c); return code; };
     cudaError_t e;
-    const size_t partb = (size_t)n_real * 2 * c->G.nbx * sizeof(double);
+    const size_t partb = (size_t)n_real * 2 * c->G.nbxa * sizeof(double);   // nbxa >= nbx
     if ((e = cudaMalloc((void**)&c->d_part[0], partb)) != cudaSuccess || (e = cudaMalloc((void**)&c->d_part[1], partb)) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_fluxpart, (size_t)n_real * RED_CTAS * 2 * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_capinfo, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess ||
@@ -1189,6 +1190,13 @@ int hft_diagnostics_ext(hft_ctx* c, double polar_lat_deg, double* h_out) {
     CK(cudaStreamSynchronize(c->stream));
     memcpy(h_out, c->h_ext, (size_t)c->nr * EXT_NOUT * sizeof(double));
     return HFT_OK;
+}
+
+int hft_synchronize(hft_ctx* c) {
+    DevGuard dg_(c);
+    if (!c) return HFT_ERR_ARG;
+    CK(cudaStreamSynchronize(c->stream));   // an asynchronous fault of the kernels enqueued so far surfaces here
+    return check_launch(c);
 }
 
 int hft_launch_count(hft_ctx* c, int64_t* h_count) {

@@ -14,6 +14,10 @@
 namespace hft {
 
 constexpr int TX = 128;  // threads per CTA = columns per CTA (one column per thread)
+// Advection stage kernels: a warp owns 31 output columns; lane 31 computes only the phi-face flux of the column after them, so
+// that every lane finds the flux of its EAST face in the lane to its right: each phi-face WENO value is evaluated once
+// instead of twice (the kernels are bound by that arithmetic, not by memory)
+constexpr int ADV_COLS = (TX / 32) * 31;
 constexpr int RPT = 8;   // rows per thread (column strip streamed in registers)
 
 template <typename real>
@@ -45,6 +49,7 @@ struct Geom {
     int nt, np, pitch, nr;
     size_t rstride;  // (nt+2)*pitch
     int nbx;         // ceil(np / TX): CTAs along phi == number of polar partial sums per row
+    int nbxa;        // ceil(np / ADV_COLS): the same for the advection stage kernels
 };
 
 // ------------------------------------------------------------------ reductions (fixed order => deterministic)
@@ -261,11 +266,12 @@ template <typename real>
 __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> T, Geom G) {
     __shared__ double red[32];
     const int r = blockIdx.z;
-    const int k = blockIdx.x * TX + threadIdx.x;
-    const bool live = k < G.np;
+    const int lane = threadIdx.x & 31;
+    const int k = (blockIdx.x * (TX / 32) + (threadIdx.x >> 5)) * 31 + lane;   // lane 31: the first column of the next warp
     const int np = G.np, nt = G.nt;
-    const int k0 = live ? k : 0;
-    const int km1 = (k0 + np - 1) % np, km2 = (k0 + np - 2) % np, kp1 = (k0 + 1) % np, kp2 = (k0 + 2) % np;
+    const bool live = lane < 31 && k < np;          // this lane writes column k
+    const int k0 = k % np;
+    const int km1 = (k0 + np - 1) % np, km2 = (k0 + np - 2) % np, kp1 = (k0 + 1) % np;
     const int j0 = 1 + blockIdx.y * RPT;            // rows 1..nt only; caps are done by k_adv_caps
     const int j1 = min(j0 + RPT, nt + 1);
     const size_t base = (size_t)r * G.rstride;
@@ -286,9 +292,9 @@ __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> 
         real w4 = ld(j + 2);
         real Fs = theta_face_flux<real>(j, w1, w2, w3, w4, lm, lp, vtf, nt, T.eps_t, A.upwind_only, wmp);
         const real* row = in + (size_t)j * G.pitch;
-        real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1], bp2 = row[kp2];
+        real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1];
         real Fw = phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, A.upwind_only);
-        real Fe = phi_face_flux<real>(bm1, w2, bp1, bp2, pm[j], pp[j], T.eps_p, A.upwind_only);
+        real Fe = __shfl_down_sync(0xffffffffu, Fw, 1);   // face k+1/2 = the west face of column k+1 (same operands, same bits)
         real tend = (T.sth[j] * Fs - T.sth[j - 1] * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
         const size_t off = base + (size_t)j * G.pitch + k0;
         real o = A.cb * w2 - A.cdt * tend;
@@ -300,11 +306,11 @@ __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> 
     }
     if (j0 == 1) {
         double t = block_sum(sumN, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbx + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbxa + blockIdx.x] = t;
     }
     if (j0 <= nt && nt < j1) {
         double t = block_sum(sumS, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbx + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbxa + blockIdx.x] = t;
     }
 }
 
@@ -317,11 +323,12 @@ template <typename real>
 __global__ void __launch_bounds__(TX) k_adv_stage_att(AdvArgs<real> A, Tables<real> T, Geom G) {
     __shared__ double red[32];
     const int r = blockIdx.z;
-    const int k = blockIdx.x * TX + threadIdx.x;
-    const bool live = k < G.np;
+    const int lane = threadIdx.x & 31;
+    const int k = (blockIdx.x * (TX / 32) + (threadIdx.x >> 5)) * 31 + lane;   // lane 31: the first column of the next warp
     const int np = G.np, nt = G.nt;
-    const int k0 = live ? k : 0;
-    const int km1 = (k0 + np - 1) % np, km2 = (k0 + np - 2) % np, kp1 = (k0 + 1) % np, kp2 = (k0 + 2) % np;
+    const bool live = lane < 31 && k < np;
+    const int k0 = k % np;
+    const int km1 = (k0 + np - 1) % np, km2 = (k0 + np - 2) % np, kp1 = (k0 + 1) % np;
     const int j0 = 1 + blockIdx.y * RPT;
     const int j1 = min(j0 + RPT, nt + 1);
     const size_t base = (size_t)r * G.rstride;
@@ -353,26 +360,25 @@ __global__ void __launch_bounds__(TX) k_adv_stage_att(AdvArgs<real> A, Tables<re
         const real w4 = col(A.in, j + 2);
         const real m3 = col(A.LMt, j + 1), p3 = col(A.LPt, j + 2);
         const real* row = in + (size_t)j * G.pitch;
-        const real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1], bp2 = row[kp2];
-        real a_m2 = 0, a_m1 = 0, a_0 = 0, a_p1 = 0, b_m1 = 0, b_0 = 0, b_p1 = 0, b_p2 = 0, vw = 0, ve = 0;
+        const real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1];
+        real a_m2 = 0, a_m1 = 0, a_0 = 0, b_m1 = 0, b_0 = 0, b_p1 = 0, vw = 0;
         if (uw) {
-            vw = A.VP[ro + k0]; ve = A.VP[ro + kp1];
+            vw = A.VP[ro + k0];
         } else {
-            a_m2 = A.LMp[ro + km2]; a_m1 = A.LMp[ro + km1]; a_0 = A.LMp[ro + k0]; a_p1 = A.LMp[ro + kp1];
-            b_m1 = A.LPp[ro + km1]; b_0 = A.LPp[ro + k0]; b_p1 = A.LPp[ro + kp1]; b_p2 = A.LPp[ro + kp2];
+            a_m2 = A.LMp[ro + km2]; a_m1 = A.LMp[ro + km1]; a_0 = A.LMp[ro + k0];
+            b_m1 = A.LPp[ro + km1]; b_0 = A.LPp[ro + k0]; b_p1 = A.LPp[ro + kp1];
         }
         const real fnv = (A.ca != (real)0) ? A.fn[ro + k0] : (real)0;
         // ---- then the arithmetic.  Face j (between rows j, j+1): LMt rows j-1..j+1 = (m1, m2, m3), LPt rows j..j+2 = (p1, p2, p3)
         const real Fs = theta_flux(j, w1, w2, w3, w4, m1, m2, m3, p1, p2, p3);
-        real Fw, Fe;
+        real Fw;
         if (uw) {
             Fw = upwind(vw, bm1, w2);
-            Fe = upwind(ve, w2, bp1);
         } else {
-            // face k-1/2: LM of cells k-2, k-1, k; LP of cells k+1, k, k-1.  face k+1/2: shifted by one column
+            // face k-1/2: LM of cells k-2, k-1, k; LP of cells k+1, k, k-1
             Fw = weno3_side(bp1 * b_p1, w2 * b_0, bm1 * b_m1, T.eps_p) + weno3_side(bm2 * a_m2, bm1 * a_m1, w2 * a_0, T.eps_p);
-            Fe = weno3_side(bp2 * b_p2, bp1 * b_p1, w2 * b_0, T.eps_p) + weno3_side(bm1 * a_m1, w2 * a_0, bp1 * a_p1, T.eps_p);
         }
+        const real Fe = __shfl_down_sync(0xffffffffu, Fw, 1);   // face k+1/2 = the west face of column k+1
         const real tend = (T.sth[j] * Fs - T.sth[j - 1] * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
         real o = A.cb * w2 - A.cdt * tend;
         if (A.ca != (real)0) o = A.ca * fnv + o;
@@ -385,11 +391,11 @@ __global__ void __launch_bounds__(TX) k_adv_stage_att(AdvArgs<real> A, Tables<re
     }
     if (j0 == 1) {
         double t = block_sum(sumN, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbx + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbxa + blockIdx.x] = t;
     }
     if (j0 <= nt && nt < j1) {
         double t = block_sum(sumS, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbx + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbxa + blockIdx.x] = t;
     }
 }
 
@@ -402,7 +408,7 @@ __global__ void __launch_bounds__(TX) k_adv_caps(AdvArgs<real> A, Tables<real> T
     if (k >= G.np) return;
     const int j = pole == 0 ? 0 : G.nt + 1;
     const size_t off = (size_t)r * G.rstride + (size_t)j * G.pitch;
-    double S = sum_partials(A.part + ((size_t)r * 2 + pole) * G.nbx, G.nbx);
+    double S = sum_partials(A.part + ((size_t)r * 2 + pole) * G.nbxa, G.nbxa);
     real tend = (real)((pole == 0 ? 1.0 : -1.0) * (T.adv_capc[pole] * S));
     real o = A.cb * A.in[off] - A.cdt * tend;
     if (A.ca != (real)0) o = A.ca * A.fn[off] + o;

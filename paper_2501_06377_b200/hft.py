@@ -20,7 +20,7 @@ _lib = C.CDLL(LIB_PATH)
 
 EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_theta_nodes", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_diffusivity_map", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
            "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_assimilate_diagnostics", "hft_diagnostics", "hft_diagnostics_ext", "hft_stable_dt",
-           "hft_sts_stage_count", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
+           "hft_sts_stage_count", "hft_synchronize", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
            "hft_last_cuda_error"]
 
 ADV_OFF, ADV_UPWIND, ADV_WENO3 = 0, 1, 2
@@ -70,6 +70,7 @@ _lib.hft_diagnostics_ext.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_doubl
 _lib.hft_stable_dt.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.hft_sts_stage_count.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_int32)]
 _lib.hft_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
+_lib.hft_synchronize.argtypes = [C.c_void_p]
 _lib.hft_profile_kernels.argtypes = [C.c_void_p, C.c_int32]
 _lib.hft_kernel_time.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
 _lib.hft_error_string.argtypes = [C.c_int]
@@ -249,6 +250,9 @@ class Context:
         s = C.c_int32()
         self._ck(_lib.hft_sts_stage_count(self._h, float(dt_hours), C.byref(s)), "hft_sts_stage_count")
         return s.value
+
+    def synchronize(self):
+        self._ck(_lib.hft_synchronize(self._h), "hft_synchronize")
 
     def launch_count(self):
         n = C.c_int64()

@@ -564,6 +564,8 @@ def test_errors_are_reported():
     with pytest.raises(H.HftError):
         ctx.step(1, -1.0)
     assert ctx.launch_count() >= 0
+    ctx.step(1, dtd)
+    ctx.synchronize()                            # where an asynchronous kernel fault of that step would be reported
     ctx.close()
     # hft_create rejects what would fail later with a generic launch error or run anti-diffusion silently
     for bad in ([[float("nan"), 0, 0, 0, 0, 0, 0]], [[-1.0, 0, 0, 0, 0, 0, 0]], [[500.0, float("inf"), 0, 0, 0, 0, 0]]):
