@@ -399,6 +399,19 @@ def main():
         # unit, then the issue slots).  "alu": useful FP instruction slots per second -- 7 per cell and stage (1 add, 1 mul,
         # 5 fma; halo recomputation and k_sts_upipe's 8th operation are NOT counted as useful) -- against the measured FMA
         # issue rate of that type, both in FMA-equivalent TFLOP/s (2 flops per slot).
+        if args.nu_map:     # k_sts_mpipe: 4 stages per launch, 14 FP operations per cell and stage (10 for Eq. 27 with the face
+            # conductances, 4 for the recurrence), 6 array passes per launch (3 fields + nu in, 2 out), 4 halo columns per side
+            cols = 32 * (2 if dtype == "f64" else 4)
+            useful = 14 * spl * cells_launch / sec
+            alu_peak = ALU_PEAK_FMA_PER_S[dtype]
+            return {"bound": "alu", "achieved": 2 * useful / 1e12, "peak": 2 * alu_peak / 1e12, "unit": "TFLOP/s", "frac": useful / alu_peak,
+                    "traffic": None, "kernel": "k_sts_mpipe<%s,4>" % ("double" if dtype == "f64" else "float"), "stages_per_launch": spl,
+                    "avg_launch_ms": r["kernel_ms"], "sampled_launches": r["kernel_samples"],
+                    "frac_with_halo": useful * cols / (cols - 8) / alu_peak,
+                    "hbm_algorithmic": {"achieved": alg_gbs, "peak": peak, "unit": "GB/s", "frac": alg_gbs / peak, "peak_source": peak_src,
+                                        "meaning": "speed-up over the HBM roofline of one launch per stage (5 passes per stage with nu(theta, phi))"},
+                    "dram": {"achieved": 6 * field_bytes / sec / 1e9, "peak": peak, "unit": "GB/s", "frac": 6 * field_bytes / sec / 1e9 / peak,
+                             "meaning": "the 6 array passes per launch this kernel moves (3 fields + nu in, 2 out) / time"}}
         mixed = dtype == "f32" and r["f32_arith"] == 0
         upipe = mixed or args.sts_kernel == 2
         arith = "f64" if (dtype == "f64" or mixed) else "f32"

@@ -21,6 +21,7 @@
 #include "hft_sts_blocked.cuh"
 #include "hft_sts_map.cuh"
 #include "hft_sts_step.cuh"
+#include "hft_sts_mpipe.cuh"
 
 // The temporally blocked STS step (all k_sts_pipe / k_sts_upipe / k_sts_capseq instantiations) is compiled in its own
 // translation units (hft_sts_f64.cu, hft_sts_f32.cu, hft_sts_mixed.cu), so that the units build in parallel.
@@ -101,6 +102,7 @@ struct hft_ctx {
     double* d_zmean = nullptr;               // blocked STS: zonal partial sums (see hft_sts_blocked.cuh)
     double* d_capseq = nullptr;              // blocked STS: cap values per stage
     double* d_kappa = nullptr;               // k_sts_upipe: w1 dt nu_r per realization
+    double* d_mscratch = nullptr;            // k_sts_mcapseq: polar-band level buffers, allocated on first use
     double* h_diag = nullptr;                // pinned
     double *d_extpart = nullptr, *d_ext = nullptr, *h_ext = nullptr;   // hft_diagnostics_ext, allocated on first use
     int64_t launches = 0;
@@ -703,6 +705,30 @@ int step_once(hft_ctx* c, double dt, int s) {
             int64_t n = 0;
             rc = sts_blocked_step<real>(P, tables_of<real>(c), c->G, &n) == 0 ? HFT_OK : HFT_ERR_CUDA;
             c->launches += n;
+        } else if (c->map_any && c->opt.diff_time >= 2 && c->opt.sts_block != 1 && s > 2 * MPIPE_K &&
+                   sts_mblocked_supported(c->G, sizeof(real))) {
+            // nu(theta, phi): K = 4 stages per launch, cap values from the polar band (hft_sts_mpipe.cuh)
+            if (!c->d_mscratch) {
+                const cudaError_t e = cudaMalloc((void**)&c->d_mscratch, sts_mscratch_bytes(c->G));
+                if (e != cudaSuccess) { cuda_fail(c, e, "cudaMalloc(polar band scratch)"); return HFT_ERR_NOMEM; }
+            }
+            StsBlockedPlan<real> P;
+            P.Y0 = arr_of<real>(c, c->i_state);
+            for (int i = 0; i < 5; i++) P.buf[i] = arr_of<real>(c, (c->i_state + 1 + i) % kNumArrays);
+            P.mu = c->coef.mu.data(); P.nu = c->coef.nu.data(); P.a = c->coef.a.data(); P.g = c->coef.g.data();
+            P.s = s; P.kb = MPIPE_K; P.stream = c->stream;
+            P.part = c->d_part; P.zmean = c->d_zmean; P.capseq = c->d_capseq;
+            P.prof_begin = [](void* u, bool* armed) { prof_begin((hft_ctx*)u, 1, *armed); };
+            P.prof_end = [](void* u, bool armed, int stages) { prof_end((hft_ctx*)u, armed, stages); };
+            P.user = c;
+            P.up = nullptr;
+            MapArgs<real> M;
+            M.NU = (const real*)c->numap; M.capw = c->d_capw;
+            M.capP[0] = c->PN * c->dph / c->dthf[0]; M.capP[1] = c->PS * c->dph / c->dthf[c->G.nt];
+            M.nparts_in = c->G.nbx;
+            int64_t n = 0;
+            rc = sts_mblocked_step<real>(P, M, tables_of<real>(c), c->G, c->d_mscratch, &n) == 0 ? HFT_OK : HFT_ERR_CUDA;
+            c->launches += n;
         } else {
             rc = diffuse_unblocked<real>(c, dt, s);
         }
@@ -866,7 +892,7 @@ void hft_destroy(hft_ctx* c) {
     if (c->prof_ev_made)
         for (int i = 0; i < 2 * kProfEvents; i++) cudaEventDestroy(c->prof_ev[i]);
     cudaFree(c->d_tab); cudaFree(c->d_part[0]); cudaFree(c->d_part[1]); cudaFree(c->d_fluxpart);
-    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq); cudaFree(c->d_kappa); cudaFree(c->d_B0); cudaFree(c->d_capw);
+    cudaFree(c->d_capinfo); cudaFree(c->d_scale); cudaFree(c->d_diag); cudaFree(c->d_zmean); cudaFree(c->d_capseq); cudaFree(c->d_kappa); cudaFree(c->d_mscratch); cudaFree(c->d_B0); cudaFree(c->d_capw);
     if (c->h_diag) cudaFreeHost(c->h_diag);
     cudaFree(c->d_extpart); cudaFree(c->d_ext);
     if (c->h_ext) cudaFreeHost(c->h_ext);

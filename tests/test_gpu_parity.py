@@ -272,14 +272,16 @@ def test_config3_full_size_sampled_realizations(dtype):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
-@pytest.mark.parametrize("path", ["nu_map", "unblocked"])
+@pytest.mark.parametrize("path", ["nu_map", "nu_map_stagewise", "unblocked"])
 def test_config3_full_size_stage_by_stage_paths(dtype, path):
-    """The two one-launch-per-stage paths at BASELINE config 3's full size in the launch configurations bench.py times
-    (`--nu-map`: nu(theta, phi) of workloads.diffusivity_map; `--sts-block 1`), one step; the oracle checks a sampled
-    realization; all 64 conserve flux."""
+    """The nu(theta, phi) paths and the one-launch-per-stage path at BASELINE config 3's full size in the launch configurations
+    bench.py times (`--nu-map`: nu(theta, phi) of workloads.diffusivity_map through the temporally blocked k_sts_mpipe with the
+    polar band k_sts_mcapseq; the same with `--sts-block 1`: one launch per stage; `--sts-block 1` alone), one step; the oracle
+    checks a sampled realization; all 64 conserve flux."""
     H = hft()
     w = wl.config(3, dtype)
-    opt = dict(diffusivity_map=1) if path == "nu_map" else dict(sts_block=1)
+    opt = {"nu_map": dict(diffusivity_map=1), "nu_map_stagewise": dict(diffusivity_map=1, sts_block=1), "unblocked": dict(sts_block=1)}[path]
+    path = "nu_map" if path.startswith("nu_map") else path
     ctx = H.Context(w.n_theta, w.n_phi, w.params, dtype=dtype, **opt)
     maps = wl.initial_maps(w, device="cuda").to(ctx.tdtype)
     for r in range(w.n_real):
@@ -752,14 +754,17 @@ def test_latitude_dependent_diffusivity(dtype, block):
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("case", ["rkg2_adv", "rkl2", "euler"])
 @pytest.mark.parametrize("nphi", [264, 263])
-def test_diffusivity_map_theta_phi(dtype, case, nphi):
+@pytest.mark.parametrize("block", [0, 1])
+def test_diffusivity_map_theta_phi(dtype, case, nphi, block):
     """nu(theta, phi) on the half-half grid (Eq. 27-28): realization 0 a smooth map, 1 keeps its scalar
-    value, 2 a rough random map; ragged grids: 264 columns take the 16-byte-vector kernel k_sts_stage_mapv (part-filled
+    value, 2 a rough random map; ragged grids: 264 columns take the temporally blocked k_sts_mpipe + polar band k_sts_mcapseq
+    (block = 0, when the step has more than 8 stages) or the 16-byte-vector kernel k_sts_stage_mapv one stage per launch
+    (block = 1; part-filled
     warps, 75 + 2 rows = 4 row blocks + tail), 263 columns the one-column-per-thread kernel k_sts_stage_map.  Then the
     gpu fp32 result against the fp64 oracle, a map replaced by a profile, and the constant map against the table path."""
     H = hft()
     w = wl.scaled(wl.config(3), 75, nphi, n_real=3)
-    opt = dict(diffusivity_map=1)
+    opt = dict(diffusivity_map=1, sts_block=block)
     kw = {}
     if case == "rkl2":
         opt.update(adv_flux=H.ADV_OFF, diff_time=H.DIFF_RKL2); kw.update(adv_flux=orc.ADV_OFF, diff_time=orc.DIFF_RKL2)
