@@ -138,8 +138,11 @@ int hft_set_grid_diffusivity(hft_ctx* ctx, int32_t r, double alpha_nu);
  * Owned by the caller, consumed before the call returns (synchronises the stream).  Each theta-flux takes the mean of the two
  * nu values on its face, each phi-flux likewise, the polar-cap fluxes of App. A (:624-648) the face means of row f = 0 / n_theta:
  * exactly the coefficients a_{j+-1,k}, a_{j,k+-1} of Eq. 28, applied in difference form.  Once any realization has a map,
- * every realization is advanced by the one-launch-per-stage kernel k_sts_stage_map (the others with their nu(theta) profile
- * or scalar value): with phi-dependent coefficients the temporally blocked kernel does not apply.
+ * every realization is advanced through the nu(theta, phi) kernels (the others with their nu(theta) profile or scalar value):
+ * k_sts_mpipe, 4 stages per launch, with the polar-cap values of a block from the polar-band kernel k_sts_mcapseq (n_phi a
+ * multiple of 16 bytes / sizeof(value), more than 8 stages per step), else one launch per stage (k_sts_stage_mapv /
+ * k_sts_stage_map; also with sts_block = 1).  The zonal-mean cap recurrence of k_sts_pipe does not apply: the coefficients
+ * depend on phi.
  * hft_stable_dt and the STS stage count use the Gershgorin bound max |a_{j,k}| over every cell of the map.  A later
  * hft_set_diffusivity_profile / hft_set_grid_diffusivity for realization r replaces its map.  Needs
  * hft_options.diffusivity_map = 1 at hft_create, else HFT_ERR_ARG. */
