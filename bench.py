@@ -39,7 +39,7 @@ def kernel_source_hash():
     import hashlib
     h = hashlib.sha1()
     d = os.path.join(ROOT, "paper_2501_06377_b200", "csrc")
-    for f in ("hft_sts_blocked.cuh", "hft_sts_pipe.cuh", "hft_sts_upipe.cuh"):
+    for f in ("hft_sts_blocked.cuh", "hft_sts_pipe.cuh", "hft_sts_upipe.cuh", "hft_sts_mpipe.cuh"):
         with open(os.path.join(d, f), "rb") as fh:
             h.update(fh.read())
     return h.hexdigest()[:12]
@@ -57,7 +57,7 @@ def record_traffic(csv_path, profile, config):
     scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
     acc = {}
     for r in data:
-        m = re.search(r"(k_sts_u?pipe)<(double|float), (?:(double|float), )?(?:\(int\))?(\d+)", r[ix["Kernel Name"]])
+        m = re.search(r"(k_sts_[um]?pipe)<(double|float), (?:(double|float), )?(?:\(int\))?(\d+)", r[ix["Kernel Name"]])
         if not m:
             continue
         name = "%s<%s,%s>" % (m.group(1), ",".join(x for x in (m.group(2), m.group(3)) if x), m.group(4))
@@ -379,6 +379,14 @@ def main():
     def b_alg(r, w):
         return (9 + stage_passes * r["s"]) * w
 
+    def traffic_keys(kern):
+        """Per-launch DRAM bytes of the last committed ncu --set full capture of `kern` (profiles/traffic.json), or traffic = None."""
+        t = ncu_traffic(kern, args.config)
+        if not t:
+            return {"traffic": None}
+        return {"traffic": t["dram_bytes_per_launch"], "traffic_source": t["profile"], "traffic_head": t["git_head"],
+                "traffic_stale": t["source_sha1"] != kernel_source_hash()}   # true: the kernel sources changed since that capture
+
     def roofline_of(r):
         """The dominant kernel's distance from its roofs, from the CUDA-event samples of this run."""
         if not r["kernel_ms"]:
@@ -405,9 +413,9 @@ def main():
             useful = 14 * spl * cells_launch / sec
             alu_peak = ALU_PEAK_FMA_PER_S[dtype]
             return {"bound": "alu", "achieved": 2 * useful / 1e12, "peak": 2 * alu_peak / 1e12, "unit": "TFLOP/s", "frac": useful / alu_peak,
-                    "traffic": None, "kernel": "k_sts_mpipe<%s,4>" % ("double" if dtype == "f64" else "float"), "stages_per_launch": spl,
+                    "kernel": "k_sts_mpipe<%s,4>" % ("double" if dtype == "f64" else "float"), "stages_per_launch": spl,
                     "avg_launch_ms": r["kernel_ms"], "sampled_launches": r["kernel_samples"],
-                    "frac_with_halo": useful * cols / (cols - 8) / alu_peak,
+                    "frac_with_halo": useful * cols / (cols - 8) / alu_peak, **traffic_keys("k_sts_mpipe<%s,4>" % ("double" if dtype == "f64" else "float")),
                     "hbm_algorithmic": {"achieved": alg_gbs, "peak": peak, "unit": "GB/s", "frac": alg_gbs / peak, "peak_source": peak_src,
                                         "meaning": "speed-up over the HBM roofline of one launch per stage (5 passes per stage with nu(theta, phi))"},
                     "dram": {"achieved": 6 * field_bytes / sec / 1e9, "peak": peak, "unit": "GB/s", "frac": 6 * field_bytes / sec / 1e9 / peak,
@@ -432,12 +440,8 @@ def main():
                                    "meaning": "speed-up over the HBM roofline of one launch per stage (4 passes per stage); > 1 because 8 stages stay on chip"},
                "dram": {"achieved": 5 * field_bytes / sec / 1e9, "peak": peak, "unit": "GB/s", "frac": 5 * field_bytes / sec / 1e9 / peak,
                         "meaning": "the 5 array passes per launch this kernel actually moves (3 in, 2 out) / time"}}
-        t = ncu_traffic(kern, args.config) if spl > 7 else None
-        if t:
-            out["traffic"] = t["dram_bytes_per_launch"]
-            out["traffic_source"] = t["profile"]
-            out["traffic_head"] = t["git_head"]
-            out["traffic_stale"] = t["source_sha1"] != kernel_source_hash()   # true: the kernel sources changed since that capture
+        if spl > 7:
+            out.update(traffic_keys(kern))
         return out
 
     frac_step = res["value"] / world * b_alg(res, wbytes) / (peak * 1e9)
