@@ -198,6 +198,21 @@ int hft_assimilate_diagnostics(hft_ctx* ctx, const void* d_obs, const void* d_we
  * Synchronises the stream. */
 int hft_diagnostics(hft_ctx* ctx, double* h_out);
 
+/* hft_diagnostics for callers that may not allocate or synchronise (code under CUDA graph capture, tight serving loops):
+ * the same flux integrals (:225-230) of a field the CALLER holds, written to device memory the caller holds.
+ *   d_field  device, [n_real][n_theta+2][n_phi] dense in the context dtype, rows 0 and n_theta+1 the polar caps (the layout of
+ *            hft_get_full, realizations back to back); read only.
+ *   d_out    device, [n_real][4] doubles = {signed, unsigned, Phi+, Phi-} in G*radius_cm^2, as hft_diagnostics.
+ * Enqueues two kernels on the context's stream and returns: no cudaMalloc / cudaFree, no copy to the host, no synchronisation.
+ * The per-CTA partial sums live in ONE static device array of the library (HFT_NOALLOC_MAX_REAL x 64 x 2 doubles = 1 MiB,
+ * held by every GPU that loads the library until the process exits); the first call on a device resolves its address
+ * (cudaGetSymbolAddress, no allocation).  n_real > HFT_NOALLOC_MAX_REAL: HFT_ERR_ARG, text in hft_last_cuda_error.
+ * Every call -- of every context on that device -- uses the same array: it keeps the previous call's contents (each call
+ * overwrites all it reads, nothing needs clearing), and two calls that overlap on the GPU (different streams / contexts
+ * without an ordering between them) RACE on it.  Results are bit-identical to hft_diagnostics of the same field. */
+#define HFT_NOALLOC_MAX_REAL 1024
+int hft_diagnostics_noalloc(hft_ctx* ctx, const void* d_field, double* d_out);
+
 /* Remaining run-history diagnostics.  h_out[n_real][13]:
  *   0..3  Phi+ and Phi- over the north polar region, then over the south polar region: the cells whose centre has
  *         |latitude| >= polar_lat_deg (0..90), polar caps included, in G*radius_cm^2;

@@ -12,6 +12,7 @@
 
 #include <atomic>
 #include <cmath>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1259,3 +1260,61 @@ int hft_kernel_time(hft_ctx* c, double* h_ms, int64_t* h_launches, int64_t* h_st
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------ hft_diagnostics_noalloc
+// The flux diagnostics for callers that may not allocate: the CTA partials of k_flux_partials, which
+// hft_diagnostics keeps in a cudaMalloc'ed buffer of the context, go to a file-scope device array instead.  Every GPU that
+// loads the library holds the array (HFT_NOALLOC_MAX_REAL x RED_CTAS x 2 doubles = 1 MiB) until the process exits.
+static __device__ __align__(256) double g_noalloc_fluxpart[(size_t)HFT_NOALLOC_MAX_REAL * RED_CTAS * 2];
+
+namespace {
+
+// In host code g_noalloc_fluxpart names a host-side stand-in, not device memory: the kernels get the device address,
+// resolved once per device with that device current.
+std::mutex g_noalloc_mutex;
+double* g_noalloc_ptr[64] = {nullptr};
+
+int noalloc_scratch(hft_ctx* c, double** out) {
+    if (c->dev < 0 || c->dev >= 64) return HFT_ERR_DEVICE;
+    std::lock_guard<std::mutex> lk(g_noalloc_mutex);
+    if (!g_noalloc_ptr[c->dev]) {
+        double* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_noalloc_fluxpart);   // the calling entry point made c->dev current
+        if (e != cudaSuccess || !p) return cuda_fail(c, e, "cudaGetSymbolAddress(g_noalloc_fluxpart)");
+        g_noalloc_ptr[c->dev] = p;
+    }
+    *out = g_noalloc_ptr[c->dev];
+    return HFT_OK;
+}
+
+template <typename real>
+int diagnostics_noalloc_impl(hft_ctx* c, const real* d_field, double* d_out, double* part) {
+    Geom G = c->G;                      // the caller's array is dense: [n_real][n_theta + 2][n_phi]
+    G.pitch = G.np;
+    G.rstride = (size_t)(G.nt + 2) * G.np;
+    dim3 gp(RED_CTAS, c->nr);
+    const double scale = c->grid.radius_cm * c->grid.radius_cm;
+    // every element of part[r][0..RED_CTAS-1][0..1] is written by k_flux_partials before k_flux_finalize reads it: what an
+    // earlier call left in the array is never read, nothing has to be cleared
+    k_flux_partials<real, 0><<<gp, 256, 0, c->stream>>>(d_field, nullptr, nullptr, 0, tables_of<real>(c), G, part);
+    k_flux_finalize<real, 0><<<(c->nr + 63) / 64, 64, 0, c->stream>>>(d_field, part, RED_CTAS, nullptr, 0, tables_of<real>(c), G, scale, d_out);
+    c->launches += 2;
+    return check_launch(c);
+}
+
+}  // namespace
+
+extern "C" int hft_diagnostics_noalloc(hft_ctx* c, const void* d_field, double* d_out) {
+    DevGuard dg_(c);
+    if (!c || !d_field || !d_out) return HFT_ERR_ARG;
+    if (c->nr > HFT_NOALLOC_MAX_REAL) {
+        c->cuda_err = "hft_diagnostics_noalloc: n_real = " + std::to_string(c->nr) + " exceeds HFT_NOALLOC_MAX_REAL = " +
+                      std::to_string(HFT_NOALLOC_MAX_REAL) + " (the size of the static scratch array)";
+        return HFT_ERR_ARG;
+    }
+    double* part = nullptr;
+    const int rc = noalloc_scratch(c, &part);
+    if (rc != HFT_OK) return rc;
+    return c->fp64() ? diagnostics_noalloc_impl<double>(c, (const double*)d_field, d_out, part)
+                     : diagnostics_noalloc_impl<float>(c, (const float*)d_field, d_out, part);
+}

@@ -19,7 +19,7 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 
 EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_theta_nodes", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_diffusivity_map", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
-           "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_assimilate_diagnostics", "hft_diagnostics", "hft_diagnostics_ext", "hft_stable_dt",
+           "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_assimilate_diagnostics", "hft_diagnostics", "hft_diagnostics_noalloc", "hft_diagnostics_ext", "hft_stable_dt",
            "hft_sts_stage_count", "hft_synchronize", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
            "hft_last_cuda_error"]
 
@@ -66,6 +66,7 @@ _lib.hft_step.argtypes = [C.c_void_p, C.c_int32, C.c_double]
 _lib.hft_assimilate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32]
 _lib.hft_assimilate_diagnostics.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.c_int32, C.POINTER(C.c_double)]
 _lib.hft_diagnostics.argtypes = [C.c_void_p, C.POINTER(C.c_double)]
+_lib.hft_diagnostics_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.hft_diagnostics_ext.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_double)]
 _lib.hft_stable_dt.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
 _lib.hft_sts_stage_count.argtypes = [C.c_void_p, C.c_double, C.POINTER(C.c_int32)]
@@ -234,6 +235,14 @@ class Context:
         out = np.zeros((self.n_real, 4))
         self._ck(_lib.hft_diagnostics(self._h, out.ctypes.data_as(C.POINTER(C.c_double))), "hft_diagnostics")
         return out
+
+    def diagnostics_noalloc(self, field: torch.Tensor, out: torch.Tensor) -> None:
+        """hft_diagnostics of a caller-held field [n_real][n_theta+2][n_phi] into a caller-held device tensor out[n_real][4]
+        (float64); allocates nothing, asynchronous (hft.h: hft_diagnostics_noalloc)."""
+        assert field.is_cuda and field.dtype == self.tdtype and field.is_contiguous()
+        assert tuple(field.shape) == (self.n_real, self.n_theta + 2, self.n_phi)
+        assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and tuple(out.shape) == (self.n_real, 4)
+        self._ck(_lib.hft_diagnostics_noalloc(self._h, C.c_void_p(field.data_ptr()), C.c_void_p(out.data_ptr())), "hft_diagnostics_noalloc")
 
     def diagnostics_ext(self, polar_lat_deg=60.0):
         out = np.zeros((self.n_real, 13))
