@@ -127,6 +127,13 @@ struct MPipeCfg {
     // copies and later reads only its own 16 bytes); one row ahead in registers left the kernel waiting on DRAM latency
     static constexpr int DP = 6, D = DP + 1;
     static constexpr int WARP_BYTES = 4 * D * 32 * 16;     // cur, prev, F, NU
+    // The row metric the operator needs -- 1/(sin(theta_j) dtheta_j), 1/(sin(theta_j) dphi)^2 per cell row, sin(theta) / dtheta per
+    // theta-face -- for the rows of this CTA's theta segment sits in shared memory behind the rings, filled once per CTA.
+    // (Fetched from the global tables where it is used -- 10 warp-uniform LDGs per row-step -- a quarter of all warp samples
+    // were multiplies waiting for one of them: profiles/r02_blocked_kernels.md.)
+    static constexpr int MTAB_ROWS = 1024;                 // >= rows per segment + 2 K + U + 1: the host picks the segments so
+    static constexpr int MTAB_BYTES = MTAB_ROWS * 3 * (int)sizeof(real);
+    static constexpr int SMEM_BYTES = MPIPE_WARPS * WARP_BYTES + MTAB_BYTES;
 };
 
 // Per-warp state.  Every register window ROTATES instead of moving (as in k_sts_pipe): the row loop is unrolled U = 6 times,
@@ -150,6 +157,7 @@ struct MPipeWarp {
     const real *gcur, *gprev, *gF, *gNU;    // this lane's columns of row 0
     real *gocur, *goprev, *gY0;
     real* ring;
+    const real *mt2, *mtf;   // shared: {rdt_j, rdp_j^2} and sth rdf of row / face (index - first table row); mt2, mtf: row t
     const double *capN, *capS;
     int nt, pitch, ja, jb, slot;
     bool wr;
@@ -189,8 +197,7 @@ struct MPipeWarp {
         // conductances of row t: face t+1/2 (rows 0..nt) and the phi-faces of cell row t (rows 1..nt)
         const real nuSw = __shfl_up_sync(full, nuS[C - 1], 1);
         {
-            const int tf = min(t, nt);
-            const real fs = T.sth[tf] * T.rdf[tf];
+            const real fs = mtf[0];
 #pragma unroll
             for (int q = 0; q < C; q++) {
                 const real w = q == 0 ? nuSw : nuS[q > 0 ? q - 1 : 0];
@@ -215,7 +222,9 @@ struct MPipeWarp {
             const int wS = pmod(PH - l, U), wN = pmod(PH - l - 1, U);                               // size-6 windows: rows j, j-1
             real res[C];
             if (!GEN || (j >= 1 && j <= nt)) {
-                const real rt = T.rdt[j], rp = T.rdp[j] * T.rdp[j];
+                real m2[2];
+                vload<real, 2>(m2, mt2 - 2 * l);
+                const real rt = m2[0], rp = m2[1];
                 const real cmu = A.mu[l - 1], cnu = A.nu[l - 1], ca = A.a[l - 1], cg = A.g[l - 1];
                 const real west = __shfl_up_sync(full, u[l - 1][sC][C - 1], 1);
                 const real east = __shfl_down_sync(full, u[l - 1][sC][0], 1);
@@ -262,6 +271,7 @@ struct MPipeWarp {
                 vstore<real, C>(goprev + off, u[K - 1][pmod(PH - K, 3)]);
             }
         }
+        mt2 += 2; mtf += 1;
     }
 
     template <int PH, bool GEN>
@@ -276,14 +286,28 @@ __global__ void __launch_bounds__(MPIPE_WARPS * 32, sizeof(real) == 8 ? 2 : 3)
 k_sts_mpipe(const __grid_constant__ MPipeArgs<real> A, const __grid_constant__ Tables<real> T, Geom G) {
     using P = MPipeCfg<real, K>;
     constexpr int C = P::C, D = P::D, DP = P::DP;
+    extern __shared__ __align__(128) unsigned char mpipe_smem[];
     const int lane = threadIdx.x & 31;
-    const int strip = blockIdx.x * MPIPE_WARPS + (threadIdx.x >> 5);
-    if (strip >= A.nstrips) return;                           // warp-uniform; no block-level barrier in this kernel
     const int r = blockIdx.z, nt = G.nt, np = G.np;
     MPipeWarp<real, K> W(A, T);
     W.nt = nt; W.pitch = G.pitch;
     W.ja = blockIdx.y * A.rows_per_seg; W.jb = min(W.ja + A.rows_per_seg, nt + 2);   // output rows [ja, jb)
     const int t0 = max(W.ja - K, 0), tend = W.jb - 1 + K;
+    {   // metric table of rows t0 - K .. tend + 5 (the last row-step of the 6-fold unrolled loop), by the whole CTA
+        real* mt = reinterpret_cast<real*>(mpipe_smem + MPIPE_WARPS * P::WARP_BYTES);
+        const int jlo = t0 - K, n = tend + 6 - jlo;
+        for (int i = threadIdx.x; i < n; i += blockDim.x) {
+            const int j = jlo + i, tf = min(max(j, 0), nt);
+            const bool in = j >= 1 && j <= nt;
+            mt[2 * i] = in ? T.rdt[j] : (real)0;
+            mt[2 * i + 1] = in ? T.rdp[j] * T.rdp[j] : (real)0;
+            mt[2 * P::MTAB_ROWS + i] = T.sth[tf] * T.rdf[tf];
+        }
+        W.mt2 = mt + 2 * K; W.mtf = mt + 2 * P::MTAB_ROWS + K;   // row t0
+    }
+    __syncthreads();                                          // the only block-level barrier, before any warp leaves
+    const int strip = blockIdx.x * MPIPE_WARPS + (threadIdx.x >> 5);
+    if (strip >= A.nstrips) return;                           // warp-uniform
     const int uc = strip * P::WOUT - P::HALO + lane * C;      // unwrapped first column of this lane
     int col = uc % np;
     if (col < 0) col += np;                                   // n_phi % C == 0: the C columns never straddle the seam
@@ -309,7 +333,6 @@ k_sts_mpipe(const __grid_constant__ MPipeArgs<real> A, const __grid_constant__ T
         vload<real, C>(W.nuN, W.gNU + (size_t)(t0 - 1) * G.pitch);
         W.nuNw = __shfl_up_sync(0xffffffffu, W.nuN[C - 1], 1);
     }
-    extern __shared__ __align__(128) unsigned char mpipe_smem[];
     W.ring = reinterpret_cast<real*>(mpipe_smem + (size_t)(threadIdx.x >> 5) * P::WARP_BYTES) + lane * C;   // this lane's 16 bytes
     for (int i = 0; i < 4 * D; i++) vstore<real, C>(W.ring + i * 32 * C, W.nuN);   // a defined ring (the NU slot of row nt+1 is read)
     __syncwarp();
@@ -335,7 +358,7 @@ int sts_mpipe_launch(const StsBlockedPlan<real>& P, MapArgs<real>& M, Tables<rea
                      const real* cur, const real* prev, real* ocur, real* oprev, bool last, int64_t* launches) {
     constexpr int K = MPIPE_K;
     using PC = MPipeCfg<real, K>;
-    const int smem = MPIPE_WARPS * PC::WARP_BYTES;
+    const int smem = PC::SMEM_BYTES;
     const int slots = resident_ctas(k_sts_mpipe<real, K>, MPIPE_WARPS * 32, smem);
     if (slots < 1) return -1;
     MPipeArgs<real> a;
@@ -349,11 +372,13 @@ int sts_mpipe_launch(const StsBlockedPlan<real>& P, MapArgs<real>& M, Tables<rea
     const int ctas_x = (a.nstrips + MPIPE_WARPS - 1) / MPIPE_WARPS;
     int nseg = 1;
     long best = -1;
-    for (int n = 1; n <= 64 && (G.nt + 2) / n >= K; n++) {   // theta segments: minimise waves x row-steps per segment
+    for (int n = 1; n <= 128 && (G.nt + 2) / n >= K; n++) {   // theta segments: minimise waves x row-steps per segment
         const long rows = (G.nt + 2 + n - 1) / n + 2 * K;
+        if (rows + K + 8 > PC::MTAB_ROWS) continue;             // the segment's metric table has to fit its shared-memory slot
         const long waves = ((long)ctas_x * n * G.nr + slots - 1) / slots;
         if (best < 0 || waves * rows < best) { best = waves * rows; nseg = n; }
     }
+    if (best < 0) return -1;
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
     nseg = (G.nt + 2 + a.rows_per_seg - 1) / a.rows_per_seg;
     dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
