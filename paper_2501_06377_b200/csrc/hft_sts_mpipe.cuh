@@ -288,7 +288,7 @@ k_sts_mpipe(const __grid_constant__ MPipeArgs<real> A, const __grid_constant__ T
     constexpr int C = P::C, D = P::D, DP = P::DP;
     extern __shared__ __align__(128) unsigned char mpipe_smem[];
     const int lane = threadIdx.x & 31;
-    const int r = blockIdx.z, nt = G.nt, np = G.np;
+    const int nt = G.nt, np = G.np;
     MPipeWarp<real, K> W(A, T);
     W.nt = nt; W.pitch = G.pitch;
     W.ja = blockIdx.y * A.rows_per_seg; W.jb = min(W.ja + A.rows_per_seg, nt + 2);   // output rows [ja, jb)
@@ -306,8 +306,12 @@ k_sts_mpipe(const __grid_constant__ MPipeArgs<real> A, const __grid_constant__ T
         W.mt2 = mt + 2 * K; W.mtf = mt + 2 * P::MTAB_ROWS + K;   // row t0
     }
     __syncthreads();                                          // the only block-level barrier, before any warp leaves
-    const int strip = blockIdx.x * MPIPE_WARPS + (threadIdx.x >> 5);
-    if (strip >= A.nstrips) return;                           // warp-uniform
+    // a warp's work item: (realization, strip) of this CTA's theta segment, strips fastest -- the items of all realizations are
+    // dealt to the CTAs as one list, so that only the last CTA of a segment can have idle warps (with one CTA row per
+    // realization 2 of 20 (fp32) / 3 of 40 (fp64) warp slots of cfg 3 stayed empty)
+    const int item = blockIdx.x * MPIPE_WARPS + (threadIdx.x >> 5);
+    if (item >= A.nstrips * G.nr) return;                     // warp-uniform
+    const int r = item / A.nstrips, strip = item - r * A.nstrips;
     const int uc = strip * P::WOUT - P::HALO + lane * C;      // unwrapped first column of this lane
     int col = uc % np;
     if (col < 0) col += np;                                   // n_phi % C == 0: the C columns never straddle the seam
@@ -369,19 +373,19 @@ int sts_mpipe_launch(const StsBlockedPlan<real>& P, MapArgs<real>& M, Tables<rea
     }
     a.last = last;
     a.nstrips = (G.np + PC::WOUT - 1) / PC::WOUT;
-    const int ctas_x = (a.nstrips + MPIPE_WARPS - 1) / MPIPE_WARPS;
+    const long ctas_x = ((long)a.nstrips * G.nr + MPIPE_WARPS - 1) / MPIPE_WARPS;   // per theta segment
     int nseg = 1;
     long best = -1;
     for (int n = 1; n <= 128 && (G.nt + 2) / n >= K; n++) {   // theta segments: minimise waves x row-steps per segment
         const long rows = (G.nt + 2 + n - 1) / n + 2 * K;
         if (rows + K + 8 > PC::MTAB_ROWS) continue;             // the segment's metric table has to fit its shared-memory slot
-        const long waves = ((long)ctas_x * n * G.nr + slots - 1) / slots;
+        const long waves = (ctas_x * n + slots - 1) / slots;
         if (best < 0 || waves * rows < best) { best = waves * rows; nseg = n; }
     }
-    if (best < 0) return -1;
+    if (best < 0 || ctas_x > 0x7fffffffL) return -1;
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
     nseg = (G.nt + 2 + a.rows_per_seg - 1) / a.rows_per_seg;
-    dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
+    dim3 gc(2, G.nr), g((unsigned)ctas_x, nseg);
     k_sts_mcapseq<real, K><<<gc, 256, 0, P.stream>>>(a, M, T, G, scratch, P.capseq);
     bool armed = false;
     P.prof_begin(P.user, &armed);

@@ -301,9 +301,12 @@ __global__ void __launch_bounds__(PipeShape<real>::WARPS * 32, PipeShape<real>::
     extern __shared__ __align__(128) unsigned char pipe_smem[];
     const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
     constexpr int PIPE_WARPS = PipeShape<real>::WARPS;
-    const int strip = blockIdx.x * PIPE_WARPS + wrp;
-    if (strip >= A.nstrips) return;   // warp-uniform; the kernel has no block-level barrier
-    const int r = blockIdx.z, nt = G.nt, np = G.np;
+    // a warp's work item: (realization, strip) of theta segment blockIdx.y, strips fastest; the items of all realizations
+    // are dealt to the CTAs as one list, so only the last CTA of a segment can have idle warps
+    const int item = blockIdx.x * PIPE_WARPS + wrp;
+    if (item >= A.nstrips * G.nr) return;   // warp-uniform; the kernel has no block-level barrier
+    const int r = item / A.nstrips, strip = item - r * A.nstrips;
+    const int nt = G.nt, np = G.np;
     PipeWarp<real, K, SPLIT> W(A);
     W.nt = nt; W.pitch = G.pitch; W.lane = lane;
     W.ja = blockIdx.y * A.rows_per_seg;
@@ -383,7 +386,7 @@ int sts_pipe_launch_impl(const StsBlockedPlan<real>& P, Tables<real>& T, const G
     }
     a.has_prev = 1; a.last = last;
     a.nstrips = (G.np + PC::WOUT - 1) / PC::WOUT;
-    const int ctas_x = (a.nstrips + PIPE_WARPS - 1) / PIPE_WARPS;
+    const long ctas_x = ((long)a.nstrips * G.nr + PIPE_WARPS - 1) / PIPE_WARPS;   // per theta segment
     // theta segments: every segment re-streams K rows above and below its own (the cone of K stages), and the grid
     // runs in waves of `slots` CTAs; take the count that minimises waves x row-steps per segment
     int nseg = 1;
@@ -392,12 +395,13 @@ int sts_pipe_launch_impl(const StsBlockedPlan<real>& P, Tables<real>& T, const G
     // they re-stream more rows than they own -- cfg 1, one 512x1024 realization, runs 22 strips x 32 segments)
     for (int n = 1; n <= 64 && (G.nt + 2) / n >= K; n++) {
         const long rows = (G.nt + 2 + n - 1) / n + 2 * K;
-        const long waves = ((long)ctas_x * n * G.nr + slots - 1) / slots;
+        const long waves = (ctas_x * n + slots - 1) / slots;
         if (best < 0 || waves * rows < best) { best = waves * rows; nseg = n; }
     }
+    if (ctas_x > 0x7fffffffL) return -1;
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
     nseg = (G.nt + 2 + a.rows_per_seg - 1) / a.rows_per_seg;   // no empty segment
-    dim3 gc(2, G.nr), g(ctas_x, nseg, G.nr);
+    dim3 gc(2, G.nr), g((unsigned)ctas_x, nseg);
     k_sts_capseq<real, K><<<gc, 32 * STS_KMAX, 0, P.stream>>>(a, T, G, P.capseq);
     bool armed = false;
     P.prof_begin(P.user, &armed);

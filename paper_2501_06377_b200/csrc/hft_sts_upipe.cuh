@@ -284,9 +284,10 @@ k_sts_upipe(const __grid_constant__ UArgs<real, creal, K> A, const __grid_consta
     constexpr int C = P::C, U = P::U, D = P::D, DP = P::DP, ROW = P::ROW;
     extern __shared__ __align__(128) unsigned char upipe_smem[];
     const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-    const int strip = blockIdx.x * P::WARPS + wrp;
-    if (strip >= A.nstrips) return;   // warp-uniform; the kernel has no block-level barrier
-    const int r = blockIdx.z, nt = G.nt, np = G.np;
+    const int item = blockIdx.x * P::WARPS + wrp;   // (realization, strip) of theta segment blockIdx.y, as in k_sts_pipe
+    if (item >= A.nstrips * G.nr) return;           // warp-uniform; the kernel has no block-level barrier
+    const int r = item / A.nstrips, strip = item - r * A.nstrips;
+    const int nt = G.nt, np = G.np;
     UPipeWarp<real, creal, K, SPLIT> Wp(A);
     Wp.nt = nt; Wp.pitch = G.pitch;
     Wp.kap = UV::dup((creal)A.kappa[r]);
@@ -412,20 +413,21 @@ int sts_upipe_launch_impl(const StsBlockedPlan<real>& P, const UPipePlan& UP, Ta
     a.PiK = (creal)Pi; a.PiKm1 = (creal)Pim1;
     a.last = last;
     a.nstrips = (G.np + PC::WOUT - 1) / PC::WOUT;
-    const int ctas_x = (a.nstrips + PC::WARPS - 1) / PC::WARPS;
+    const long ctas_x = ((long)a.nstrips * G.nr + PC::WARPS - 1) / PC::WARPS;   // per theta segment
     // theta segments: minimise waves x row-steps per segment (see sts_pipe_launch_impl)
     int nseg = 1;
     long best = -1;
     for (int n = 1; n <= 64 && (G.nt + 2) / n >= K; n++) {
         const long rows = (G.nt + 2 + n - 1) / n + 2 * K;
-        const long waves = ((long)ctas_x * n * G.nr + slots - 1) / slots;
+        const long waves = (ctas_x * n + slots - 1) / slots;
         if (best < 0 || waves * rows < best) { best = waves * rows; nseg = n; }
     }
+    if (ctas_x > 0x7fffffffL) return -1;
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
     nseg = (G.nt + 2 + a.rows_per_seg - 1) / a.rows_per_seg;
     a.rows_per_seg_u = a.rows_per_seg;
     a.niter = (a.rows_per_seg + 2 * K + PC::U - 1) / PC::U;   // row-steps t0 .. t0 + rows_per_seg + 2K - 1 of every segment
-    dim3 g(ctas_x, nseg, G.nr);
+    dim3 g((unsigned)ctas_x, nseg);
     bool armed = false;
     P.prof_begin(P.user, &armed);
     k_sts_upipe<real, creal, K, SPLIT><<<g, PC::WARPS * 32, smem, P.stream>>>(a, G);
