@@ -34,6 +34,7 @@ namespace hft {
 
 constexpr int MPIPE_K = 4;
 constexpr int MPIPE_WARPS = 4;
+constexpr int MCAP_THREADS = 1024;
 
 template <typename real>
 struct MPipeArgs {
@@ -45,12 +46,13 @@ struct MPipeArgs {
 };
 
 // ------------------------------------------------------------------ the polar band
-// grid (2 poles, R), block 256.  Band row d = distance from the pole in rows (d = 0: the cap).  Three level buffers of
+// grid (2 poles, R), block MCAP_THREADS (the band is short and every stage ends in a CTA-wide barrier: the kernel is bound by
+// the latency of its L2 round trips, so it takes the largest CTA).  Band row d = distance from the pole in rows (d = 0: the cap).  Three level buffers of
 // (K+1) x n_phi doubles per (pole, realization) in global scratch (L2-resident: 120 KB at n_phi = 2048) rotate as
 // level l-2 / l-1 / l; a CTA-wide barrier separates the stages (global writes of a CTA are visible to it after the barrier).
 // All arithmetic in fp64 whatever the state type: the K values are boundary data for the main kernel.
 template <typename real, int K>
-__global__ void __launch_bounds__(256) k_sts_mcapseq(MPipeArgs<real> A, MapArgs<real> M, Tables<real> T, Geom G, double* scratch,
+__global__ void __launch_bounds__(MCAP_THREADS) k_sts_mcapseq(MPipeArgs<real> A, MapArgs<real> M, Tables<real> T, Geom G, double* scratch,
                                                      double* capseq) {
     __shared__ double red[32];
     __shared__ double s_cap[3];
@@ -386,7 +388,7 @@ int sts_mpipe_launch(const StsBlockedPlan<real>& P, MapArgs<real>& M, Tables<rea
     a.rows_per_seg = (G.nt + 2 + nseg - 1) / nseg;
     nseg = (G.nt + 2 + a.rows_per_seg - 1) / a.rows_per_seg;
     dim3 gc(2, G.nr), g((unsigned)ctas_x, nseg);
-    k_sts_mcapseq<real, K><<<gc, 256, 0, P.stream>>>(a, M, T, G, scratch, P.capseq);
+    k_sts_mcapseq<real, K><<<gc, MCAP_THREADS, 0, P.stream>>>(a, M, T, G, scratch, P.capseq);
     bool armed = false;
     P.prof_begin(P.user, &armed);
     k_sts_mpipe<real, K><<<g, MPIPE_WARPS * 32, smem, P.stream>>>(a, T, G);
