@@ -533,7 +533,7 @@ int advect(hft_ctx* c, double dt) {
         sts.push_back({B, S, A, 2.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0});
         sts.push_back({A, nullptr, B, 0.0, 1.0, 0.5});
     }
-    dim3 g(G.nbxa, (G.nt + RPT - 1) / RPT, c->nr), gc(G.nbx, 2, c->nr);
+    dim3 g(G.nbxa, (G.nt + RPT - 1) / RPT, c->nr), gu(G.nbxa, (G.nt + ADV_RPT - 1) / ADV_RPT, c->nr), gc(G.nbx, 2, c->nr);
     real* att[kNumAttArrays] = {nullptr};
     if (c->att_any) {
         for (int i = 0; i < kNumAttArrays; i++) att[i] = (real*)c->att[i];
@@ -554,6 +554,7 @@ int advect(hft_ctx* c, double dt) {
         bool armed;
         prof_begin(c, 2, armed);
         if (c->att_any) k_adv_stage_att<real><<<g, TX, 0, c->stream>>>(a, T, G);
+        else if (!T.nonuniform && !a.upwind_only) k_adv_stage_u<real><<<gu, TX, 0, c->stream>>>(a, T, G);   // uniform theta grid, WENO3
         else k_adv_stage<real><<<g, TX, 0, c->stream>>>(a, T, G);
         prof_end(c, armed, 1);
         k_adv_caps<real><<<gc, TX, 0, c->stream>>>(a, T, G);

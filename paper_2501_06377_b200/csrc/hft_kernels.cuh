@@ -314,6 +314,103 @@ __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> 
     }
 }
 
+// k_adv_stage on a uniform theta grid with WENO3 fluxes, every shared quantity of the theta sweep evaluated once per row: the
+// LLF products A_j = B_j lm_j, P_j = B_j lp_j, their row differences and the smoothness terms (eps + d^2)^2 are each used
+// by two neighbouring faces, so they move through register windows (k_adv_stage forms three products, two differences and
+// two smoothness terms per face and side).  Row pointers advance by the pitch; the per-row tables are read one new entry
+// per row.  ADV_RPT rows per thread: the first face of a thread's strip is the one face it evaluates without writing a row.
+// Face f (between rows f and f+1), App. B with D = 1/2, 1/3, 2/3 (weno3_side):
+//   right-moving part from (A_{f-1}, A_f, A_{f+1}), left-moving part from (P_{f+2}, P_{f+1}, P_f); upwind at f <= 1, f >= nt-1.
+constexpr int ADV_RPT = 32;
+
+template <typename real>
+__device__ __forceinline__ real weno3_shared(real near, real p0, real other, real s_q0, real s_q1) {
+    // weno3_side with q0^2, q1^2 already turned into s = (eps + q^2)^2 and p0 = 1.5 near - 0.5 far given
+    const real p1 = (real)0.5 * (near + other);
+    const real a0 = s_q1, a1 = (real)2 * s_q0;
+    return pos_div(a0 * p0 + a1 * p1, a0 + a1);
+}
+
+template <typename real>
+__global__ void __launch_bounds__(TX) k_adv_stage_u(AdvArgs<real> A, Tables<real> T, Geom G) {
+    __shared__ double red[32];
+    const int r = blockIdx.z;
+    const int lane = threadIdx.x & 31;
+    const int k = (blockIdx.x * (TX / 32) + (threadIdx.x >> 5)) * 31 + lane;   // lane 31: the first column of the next warp
+    const int np = G.np, nt = G.nt;
+    const bool live = lane < 31 && k < np;          // this lane writes column k
+    const int k0 = k % np;
+    const int km1 = (k0 + np - 1) % np, km2 = (k0 + np - 2) % np, kp1 = (k0 + 1) % np;
+    const int j0 = 1 + blockIdx.y * ADV_RPT;        // rows 1..nt only; caps are done by k_adv_caps
+    const int j1 = min(j0 + ADV_RPT, nt + 1);
+    const size_t base = (size_t)r * G.rstride;
+    const real* in = A.in + base;
+    const real* lm = T.lm + (size_t)r * (nt + 2);
+    const real* lp = T.lp + (size_t)r * (nt + 2);
+    const real* vtf = T.vtf + (size_t)r * (nt + 1);
+    const real* pm = T.pm + (size_t)r * (nt + 2);
+    const real* pp = T.pp + (size_t)r * (nt + 2);
+    const real eps = T.eps_t;
+    auto cl = [&](int j) -> int { return min(max(j, 0), nt + 1); };
+    auto ld = [&](int j) -> real { return in[(size_t)cl(j) * G.pitch + k0]; };
+    auto sm = [&](real q) -> real { const real e = eps + q * q; return e * e; };
+
+    // rows f-1 .. f+2 around the first face f = j0 - 1
+    real w0 = ld(j0 - 2), w1 = ld(j0 - 1), w2 = ld(j0), w3 = ld(j0 + 1);
+    // windows at face f: A_{f-1}, A_f, A_{f+1};  P_f, P_{f+1}, P_{f+2}   (table rows outside 0..nt+1 feed upwind faces only)
+    real Am = w0 * lm[cl(j0 - 2)], Ac = w1 * lm[cl(j0 - 1)], Ap = w2 * lm[j0];
+    real Pc = w1 * lp[cl(j0 - 1)], Pp = w2 * lp[j0], Pq = w3 * lp[cl(j0 + 1)];
+    real qa0 = Ac - Am, qa1 = Ap - Ac;              // right-moving: q0 = near - far, q1 = other - near
+    real qp0 = Pp - Pq, qp1 = Pc - Pp;              // left-moving:  near = P_{f+1}, far = P_{f+2}, other = P_f
+    real sa0 = sm(qa0), sa1 = sm(qa1), sp0 = sm(qp0), sp1 = sm(qp1);
+    auto face = [&](int f, real b0, real bp1) -> real {
+        if (f <= 1 || f >= nt - 1) return upwind(vtf[f], b0, bp1);
+        const real um = weno3_shared(Ac, (real)1.5 * Ac - (real)0.5 * Am, Ap, sa0, sa1);
+        const real up = weno3_shared(Pp, (real)1.5 * Pp - (real)0.5 * Pq, Pc, sp0, sp1);
+        return up + um;
+    };
+    real Fn = face(j0 - 1, w1, w2);
+    double sumN = 0.0, sumS = 0.0;
+    if (j0 == 1) sumN = live ? (double)Fn : 0.0;
+    const real* row = in + (size_t)j0 * G.pitch;                     // row j
+    const real* nxt = in + (size_t)cl(j0 + 2) * G.pitch + k0;        // row j + 2, this column
+    const real* fnp = A.fn + base + (size_t)j0 * G.pitch + k0;
+    real* outp = A.out + base + (size_t)j0 * G.pitch + k0;
+    real sthn = T.sth[j0 - 1];
+    const bool blend = A.ca != (real)0;
+    for (int j = j0; j < j1; j++) {
+        const real w4 = *nxt;
+        const real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1];
+        const real fnv = blend ? *fnp : (real)0;
+        // slide the windows to face j: one new product, difference and smoothness term per side
+        Am = Ac; Ac = Ap; Ap = w3 * lm[j + 1];
+        Pc = Pp; Pp = Pq; Pq = w4 * lp[cl(j + 2)];
+        qa0 = qa1; sa0 = sa1; qa1 = Ap - Ac; sa1 = sm(qa1);
+        qp1 = qp0; sp1 = sp0; qp0 = Pp - Pq; sp0 = sm(qp0);
+        const real Fs = face(j, w2, w3);
+        const real Fw = phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, 0);
+        const real Fe = __shfl_down_sync(0xffffffffu, Fw, 1);   // face k+1/2 = the west face of column k+1 (same operands, same bits)
+        const real sths = T.sth[j];
+        const real tend = (sths * Fs - sthn * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
+        real o = A.cb * w2 - A.cdt * tend;
+        if (blend) o = A.ca * fnv + o;
+        if (live) *outp = o;
+        if (j == nt) sumS = live ? (double)Fs : 0.0;
+        Fn = Fs; sthn = sths;
+        w0 = w1; w1 = w2; w2 = w3; w3 = w4;
+        row += G.pitch; fnp += G.pitch; outp += G.pitch;
+        if (j + 3 <= nt + 1) nxt += G.pitch;                    // row j + 3 of the next iteration, clamped to the south cap
+    }
+    if (j0 == 1) {
+        double t = block_sum(sumN, red);
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbxa + blockIdx.x] = t;
+    }
+    if (j0 <= nt && nt < j1) {
+        double t = block_sum(sumS, red);
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbxa + blockIdx.x] = t;
+    }
+}
+
 // The same stage with flow attenuation (Eq. 5): per-cell LLF half-speeds (k_att_halfspeeds) instead of per-row tables,
 // both LLF parts live in phi.  A thread streams RPT rows of its column; B and the theta half-speeds move through
 // register windows (one new row of each per row-step), and ALL operands of a row are requested before its arithmetic
