@@ -344,7 +344,7 @@ __global__ void __launch_bounds__(TX) k_adv_stage_u(AdvArgs<real> A, Tables<real
     const int j0 = 1 + blockIdx.y * ADV_RPT;        // rows 1..nt only; caps are done by k_adv_caps
     const int j1 = min(j0 + ADV_RPT, nt + 1);
     const size_t base = (size_t)r * G.rstride;
-    const real* in = A.in + base;
+    const real* __restrict__ in = A.in + base;   // (in, fn and out never alias: the SSPRK stages ping-pong between arrays)
     const real* lm = T.lm + (size_t)r * (nt + 2);
     const real* lp = T.lp + (size_t)r * (nt + 2);
     const real* vtf = T.vtf + (size_t)r * (nt + 1);
@@ -372,12 +372,14 @@ __global__ void __launch_bounds__(TX) k_adv_stage_u(AdvArgs<real> A, Tables<real
     real Fn = face(j0 - 1, w1, w2);
     double sumN = 0.0, sumS = 0.0;
     if (j0 == 1) sumN = live ? (double)Fn : 0.0;
-    const real* row = in + (size_t)j0 * G.pitch;                     // row j
-    const real* nxt = in + (size_t)cl(j0 + 2) * G.pitch + k0;        // row j + 2, this column
-    const real* fnp = A.fn + base + (size_t)j0 * G.pitch + k0;
-    real* outp = A.out + base + (size_t)j0 * G.pitch + k0;
+    const real* __restrict__ row = in + (size_t)j0 * G.pitch;                     // row j
+    const real* __restrict__ nxt = in + (size_t)cl(j0 + 2) * G.pitch + k0;        // row j + 2, this column
+    const real* __restrict__ fnp = A.fn + base + (size_t)j0 * G.pitch + k0;
+    real* __restrict__ outp = A.out + base + (size_t)j0 * G.pitch + k0;
     real sthn = T.sth[j0 - 1];
     const bool blend = A.ca != (real)0;
+    // unrolled: the window shifts become register renaming, and the loads of the next rows move above this row's arithmetic
+#pragma unroll 4
     for (int j = j0; j < j1; j++) {
         const real w4 = *nxt;
         const real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1];
