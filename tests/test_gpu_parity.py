@@ -752,6 +752,30 @@ def test_latitude_dependent_diffusivity(dtype, block):
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_diffusivity_map_tall_grid_segments(dtype):
+    """k_sts_mpipe keeps the row metric of a CTA's theta segment in a shared-memory table of 1024 rows: a grid of 1500 rows
+    cannot be one segment, whatever the occupancy says (the host skips segment counts whose table would not fit), and its
+    segments meet at rows that are not multiples of anything.  nu(theta, phi) rough in both directions; diffusion only."""
+    H = hft()
+    nphi = 64 if dtype == "f64" else 128                         # one strip of 32 lanes x C columns, halo wrapping onto itself
+    w = wl.scaled(wl.config(3), 1500, nphi, n_real=2)
+    ctx, o = make_pair(w, dtype, diffusivity_map=1, adv_flux=H.ADV_OFF)
+    rng = np.random.default_rng(77)
+    for r in range(2):
+        m = 200.0 + 400.0 * rng.random((w.n_theta + 1, w.n_phi))
+        ctx.set_diffusivity_map(r, m); o.set_diffusivity_map(r, m)
+    _, gd = ctx.stable_dt()
+    dt = 40.0 * gd
+    s = ctx.sts_stage_count(dt)
+    assert s > 8 and s == o.sts_stage_count(dt, orc.DIFF_RKG2)
+    n0 = ctx.launch_count()
+    ctx.step(2, dt); o.step(2, dt, adv_flux=orc.ADV_OFF)
+    assert ctx.launch_count() - n0 < 2 * s                       # blocked: about s / 2 launches per step, not s
+    compare(ctx, o, TOL[dtype], "nu(theta,phi) tall grid")
+    ctx.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("case", ["rkg2_adv", "rkl2", "euler"])
 @pytest.mark.parametrize("nphi", [264, 263])
 @pytest.mark.parametrize("block", [0, 1])
