@@ -432,7 +432,7 @@ def main():
                     "dram": {"achieved": 6 * field_bytes / sec / 1e9, "peak": peak, "unit": "GB/s", "frac": 6 * field_bytes / sec / 1e9 / peak,
                              "meaning": "the 6 array passes per launch this kernel moves (3 fields + nu in, 2 out) / time"}}
         mixed = dtype == "f32" and r["f32_arith"] == 0
-        upipe = mixed or args.sts_kernel == 2
+        upipe = mixed or args.sts_kernel == 2 or (dtype == "f64" and args.sts_kernel == 0)   # the library's choice (hft.h: sts_kernel)
         arith = "f64" if (dtype == "f64" or mixed) else "f32"
         kern = ("k_sts_upipe<%s,%s,8>" % ("float" if dtype == "f32" else "double", "double" if arith == "f64" else "float")) if upipe \
             else "k_sts_pipe<%s,8>" % ("double" if dtype == "f64" else "float")

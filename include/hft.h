@@ -86,7 +86,9 @@ typedef struct {
                                  fp64 kernel and half its memory.  1 = fp32 arithmetic throughout: 2.1 x the rate, but every stage
                                  rounds to 24 bits and the same run ends 1.4e-5 .. 2.2e-5 from the fp64 oracle.  The fp64-register
                                  path needs k_sts_upipe (see sts_kernel); batches it cannot take run in fp32 arithmetic */
-    int32_t sts_kernel;       /* which temporally blocked kernel: 0 (default) = the library's choice; 1 = k_sts_pipe (per-realization
+    int32_t sts_kernel;       /* which temporally blocked kernel: 0 (default) = the library's choice (k_sts_upipe, where the batch
+                                 allows it, for fp64 states and for fp32 states with f32_arith = 0; k_sts_pipe for fp32
+                                 arithmetic); 1 = k_sts_pipe (per-realization
                                  coefficient tables through shared memory; any batch); 2 = k_sts_upipe (one coefficient table
                                  through the uniform datapath) whenever the batch shares one table up to the factor nu_r and it
                                  fits the constant bank (n_theta <= 2048), else k_sts_pipe */

@@ -453,9 +453,10 @@ int prepare_upipe(hft_ctx* c, int scheme, int s, double dt) {
     c->up_version = c->tab_version; c->up_scheme = scheme; c->up_s = s; c->up_dt = dt;
     up.ok = false;
     const int nt = c->G.nt;
-    // default (0): k_sts_upipe only where it is the only kernel: fp32 storage with fp64 block arithmetic (f32_arith = 0)
+    // default (0): k_sts_upipe wherever the block arithmetic is fp64 -- fp64 states, and fp32 storage with fp64 block
+    // arithmetic (f32_arith = 0), where it is the only kernel; fp32 arithmetic stays with k_sts_pipe (FFMA2), measured equal
     const bool want_mixed = !c->fp64() && c->opt.f32_arith == 0;
-    const bool want = c->opt.sts_kernel == 2 || (c->opt.sts_kernel == 0 && want_mixed);
+    const bool want = c->opt.sts_kernel == 2 || (c->opt.sts_kernel == 0 && (want_mixed || c->fp64()));
     if (!want || !c->shape_common || nt > UTAB_MAX_ROWS) return HFT_OK;
     for (int r = 0; r < c->nr; r++)
         if (!(c->nu_scale[r] >= 0.0) || !std::isfinite(c->nu_scale[r])) return HFT_OK;

@@ -72,7 +72,7 @@ struct UCfg {
     static constexpr int NF = K + 1;
     // loop body as in PipeCfg: fp64 arithmetic rotates the F slots by unrolling lcm(3, K+1) row-steps; fp32 runs a
     // 3-row-step body with a sliding F window
-    static constexpr bool SHIFTF = sizeof(creal) == 4;
+    static constexpr bool SHIFTF = true;
     static constexpr int U = SHIFTF ? 3 : ((NF % 3 == 0) ? NF : 3 * NF);
     static constexpr int NFW = SHIFTF ? K + 3 : NF;
     static constexpr int D = NF, DP = D - 2;
