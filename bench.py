@@ -242,6 +242,7 @@ def main():
     ap.add_argument("--paper-case", choices=["diffusion", "advdiff"], default=None,
                     help="time one of the two validation runs the paper prints wall times for (context, not the bench metric)")
     ap.add_argument("--paper-grid-even", action="store_true", help="--paper-case on 510 x 1024 instead of the paper's 510 x 1023")
+    ap.add_argument("--alu-probe", action="store_true", help="print the FMA issue rates hft_probe_fma_rate measures on this GPU and exit")
     ap.add_argument("--record-traffic", default=None, metavar="RAW_CSV", help="no GPU: store the per-launch DRAM bytes of an ncu raw-page export in profiles/traffic.json")
     ap.add_argument("--traffic-profile", default="", help="with --record-traffic: the profiles/*.md summary the capture belongs to")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -251,6 +252,15 @@ def main():
     args = ap.parse_args()
     if args.record_traffic:
         record_traffic(args.record_traffic, args.traffic_profile, args.config)
+        return
+    if args.alu_probe:
+        # the denominators of the "alu" roofline, re-measured: FMA lane-operations per second per operand pattern (hft.h)
+        from paper_2501_06377_b200 import hft
+        torch.cuda.set_device(0)
+        names = {0: "two_shared_operands", 1: "three_register_operands", 2: "constant_bank_operand"}
+        out = {"alu_probe_fma_per_s": {dt: {names[p]: hft.probe_fma_rate(dt, p) for p in (0, 1, 2)} for dt in ("f64", "f32")},
+               "used_as_peak": ALU_PEAK_FMA_PER_S}
+        print(json.dumps(out))
         return
     if args.paper_case:
         run_paper_case(args)
@@ -443,7 +453,8 @@ def main():
         out = {"bound": "alu", "achieved": 2 * useful / 1e12, "peak": 2 * alu_peak / 1e12, "unit": "TFLOP/s", "frac": useful / alu_peak,
                "traffic": None, "kernel": kern, "stages_per_launch": spl, "avg_launch_ms": r["kernel_ms"],
                "sampled_launches": r["kernel_samples"],
-               "peak_source": "FP%s FMA issue rate measured on this pool with a register-only loop (profiles/r01_pipe_cfg3_gen2.md), x 2 flops" % arith[1:],
+               "peak_source": "FP%s FMA issue rate: 64 (fp64) / 128 (fp32) lanes per clock and SM x 148 SMs x the clock under the power "
+                              "cap, as measured with the library's register-only loop (hft_probe_fma_rate; bench.py --alu-probe), x 2 flops" % arith[1:],
                "frac_with_halo_and_extra_ops": executed / alu_peak,
                # context, not distances to a roof of this kernel: the rate expressed in the bytes a stage-by-stage code would
                # move (SURVEY 8(d) B_alg) over the measured copy bandwidth -- how much faster than ANY such code could be

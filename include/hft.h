@@ -251,6 +251,14 @@ int hft_launch_count(hft_ctx* ctx, int64_t* h_count);
 int hft_profile_kernels(hft_ctx* ctx, int32_t which);
 int hft_kernel_time(hft_ctx* ctx, double* h_ms, int64_t* h_launches, int64_t* h_stages);
 
+/* Not part of the time-stepping path: the FMA issue rate of the current device, measured with a register-only loop (16
+ * independent chains per thread, 4 CTAs of 128 threads per SM, ~1 ms) -- the denominator of bench.py's "alu" roofline
+ * (DESIGN.md section 6), so that it can be re-measured on any box.  dtype 0 = fp32, 1 = fp64.  pattern 0: x = fma(x, a, b)
+ * with a, b shared by all FMAs of a thread; 1: three distinct register operands per FMA; 2: one operand from the constant
+ * bank.  *h_lane_fma_per_s = FMA lane-operations per second (x 2 = flop/s).  Allocates and frees two small device buffers,
+ * runs on the default stream, synchronises. */
+int hft_probe_fma_rate(int32_t dtype, int32_t pattern, double* h_lane_fma_per_s);
+
 const char* hft_error_string(int code);
 const char* hft_last_cuda_error(hft_ctx* ctx);
 

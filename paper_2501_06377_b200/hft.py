@@ -20,7 +20,7 @@ _lib = C.CDLL(LIB_PATH)
 
 EXPORTS = ["hft_workspace_bytes", "hft_create", "hft_destroy", "hft_set_theta_nodes", "hft_set_flow_tables", "hft_set_diffusivity_profile", "hft_set_grid_diffusivity", "hft_set_diffusivity_map", "hft_set_attenuation", "hft_set_rfe", "hft_get_rfe_map", "hft_set_map", "hft_get_map",
            "hft_get_full", "hft_set_full", "hft_step", "hft_assimilate", "hft_assimilate_diagnostics", "hft_diagnostics", "hft_diagnostics_noalloc", "hft_diagnostics_ext", "hft_stable_dt",
-           "hft_sts_stage_count", "hft_synchronize", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_error_string",
+           "hft_sts_stage_count", "hft_synchronize", "hft_launch_count", "hft_profile_kernels", "hft_kernel_time", "hft_probe_fma_rate", "hft_error_string",
            "hft_last_cuda_error"]
 
 ADV_OFF, ADV_UPWIND, ADV_WENO3 = 0, 1, 2
@@ -74,6 +74,7 @@ _lib.hft_launch_count.argtypes = [C.c_void_p, C.POINTER(C.c_int64)]
 _lib.hft_synchronize.argtypes = [C.c_void_p]
 _lib.hft_profile_kernels.argtypes = [C.c_void_p, C.c_int32]
 _lib.hft_kernel_time.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+_lib.hft_probe_fma_rate.argtypes = [C.c_int32, C.c_int32, C.POINTER(C.c_double)]
 _lib.hft_error_string.argtypes = [C.c_int]
 _lib.hft_error_string.restype = C.c_char_p
 _lib.hft_last_cuda_error.argtypes = [C.c_void_p]
@@ -86,6 +87,15 @@ class HftError(RuntimeError):
 
 def error_string(code: int) -> str:
     return _lib.hft_error_string(int(code)).decode()
+
+
+def probe_fma_rate(dtype="f64", pattern=0) -> float:
+    """FMA lane-operations per second of the current device (hft.h: hft_probe_fma_rate)."""
+    out = C.c_double()
+    rc = _lib.hft_probe_fma_rate(1 if dtype == "f64" else 0, int(pattern), C.byref(out))
+    if rc != 0:
+        raise HftError(f"hft_probe_fma_rate: {error_string(rc)}")
+    return out.value
 
 
 def workspace_bytes(n_theta, n_phi, n_real, dtype="f64", opt=None) -> int:

@@ -955,3 +955,18 @@ def test_no_write_outside_caller_buffers(dtype, nt, nphi, opt):
     assert bool((big[:G] == 0xA5).all()) and bool((big[G + need:] == 0xA5).all()), "write outside the workspace"
     assert bool((outbig[:G] == 0x5A).all()) and bool((outbig[-G:] == 0x5A).all()), "write outside the get_map buffer"
     ctx.close()
+
+
+def test_fma_rate_probe():
+    """hft_probe_fma_rate (the denominator of bench.py's "alu" roofline): sane on a B200 -- fp64 near 64 lanes per clock and SM,
+    fp32 near 128, and three register operands per DFMA slower than a shared or constant operand."""
+    H = hft()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    r64 = [H.probe_fma_rate("f64", p) for p in (0, 1, 2)]
+    r32 = [H.probe_fma_rate("f32", p) for p in (0, 1, 2)]
+    per_clk = lambda r: r / sms / 1.965e9                        # lanes per clock and SM at the maximum SM clock
+    assert 40 < per_clk(r64[0]) < 70 and 40 < per_clk(r64[2]) < 70, r64
+    assert 80 < per_clk(r32[0]) < 140, r32
+    assert r64[1] < 0.9 * r64[2], r64
+    with pytest.raises(Exception):
+        H.probe_fma_rate("f64", 3)
