@@ -970,3 +970,27 @@ def test_fma_rate_probe():
     assert r64[1] < 0.9 * r64[2], r64
     with pytest.raises(Exception):
         H.probe_fma_rate("f64", 3)
+
+
+def test_interleaved_contexts_share_the_constant_table():
+    """k_sts_upipe (the default for fp64 states and for fp32 states with fp64 block arithmetic) reads its coefficient table
+    from the constant bank, which is process-wide state per device: contexts take turns, the library tracks the owner and
+    re-uploads on a change.  Three contexts -- two fp64 grids of different size and one fp32 -- stepped in turn, one step
+    at a time, must each end where their oracle does."""
+    H = hft()
+    cases = [("f64", wl.scaled(wl.config(3), 90, 200, n_real=2)), ("f64", wl.scaled(wl.config(2), 61, 136, n_real=3)),
+             ("f32", wl.scaled(wl.config(3), 75, 264, n_real=2))]
+    pairs, dts = [], []
+    for dtype, w in cases:
+        ctx, o = make_pair(w, dtype, adv_flux=H.ADV_OFF)
+        _, dif = o.stable_dt()
+        dt = 120.0 * dif
+        assert ctx.sts_stage_count(dt) > 10                      # blocked path
+        pairs.append((dtype, ctx, o)); dts.append(dt)
+    for step in range(3):
+        for (dtype, ctx, o), dt in zip(pairs, dts):
+            ctx.step(1, dt)
+    for (dtype, ctx, o), dt in zip(pairs, dts):
+        o.step(3, dt, adv_flux=orc.ADV_OFF)
+        compare(ctx, o, TOL[dtype], "interleaved contexts")
+        ctx.close()
