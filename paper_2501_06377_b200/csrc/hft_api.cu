@@ -535,6 +535,8 @@ int advect(hft_ctx* c, double dt) {
         sts.push_back({A, nullptr, B, 0.0, 1.0, 0.5});
     }
     dim3 g(G.nbxa, (G.nt + RPT - 1) / RPT, c->nr), gu(G.nbxa, (G.nt + ADV_RPT - 1) / ADV_RPT, c->nr), gc(G.nbx, 2, c->nr);
+    const int nbxt = (G.np + ATT_COLS - 1) / ATT_COLS;   // k_adv_stage_att_u: 28 columns per warp
+    dim3 gt(nbxt, (G.nt + ADV_RPT - 1) / ADV_RPT, c->nr);
     real* att[kNumAttArrays] = {nullptr};
     if (c->att_any) {
         for (int i = 0; i < kNumAttArrays; i++) att[i] = (real*)c->att[i];
@@ -554,7 +556,10 @@ int advect(hft_ctx* c, double dt) {
         a.VT = att[0]; a.VP = att[1]; a.LMt = att[2]; a.LPt = att[3]; a.LMp = att[4]; a.LPp = att[5];
         bool armed;
         prof_begin(c, 2, armed);
-        if (c->att_any) k_adv_stage_att<real><<<g, TX, 0, c->stream>>>(a, T, G);
+        const bool fast = !T.nonuniform && !a.upwind_only;   // uniform theta grid, WENO3: the kernels with shared theta-sweep terms
+        a.nparts = (c->att_any && fast) ? nbxt : G.nbxa;
+        if (c->att_any && fast) k_adv_stage_att_u<real><<<gt, TX, 0, c->stream>>>(a, T, G);
+        else if (c->att_any) k_adv_stage_att<real><<<g, TX, 0, c->stream>>>(a, T, G);
         else if (!T.nonuniform && !a.upwind_only) k_adv_stage_u<real><<<gu, TX, 0, c->stream>>>(a, T, G);   // uniform theta grid, WENO3
         else k_adv_stage<real><<<g, TX, 0, c->stream>>>(a, T, G);
         prof_end(c, armed, 1);
@@ -867,7 +872,7 @@ int hft_create(const hft_grid* grid, int32_t n_real, const hft_params* h_params,
     int rc = HFT_OK;
     auto fail = [&](int code) { hft_destroy(c); return code; };
     cudaError_t e;
-    const size_t partb = (size_t)n_real * 2 * c->G.nbxa * sizeof(double);   // nbxa >= nbx
+    const size_t partb = (size_t)n_real * 2 * ((grid->n_phi + ATT_COLS - 1) / ATT_COLS) * sizeof(double);   // the most CTAs along phi any stage kernel uses
     if ((e = cudaMalloc((void**)&c->d_part[0], partb)) != cudaSuccess || (e = cudaMalloc((void**)&c->d_part[1], partb)) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_fluxpart, (size_t)n_real * RED_CTAS * 2 * sizeof(double))) != cudaSuccess ||
         (e = cudaMalloc((void**)&c->d_capinfo, (size_t)n_real * 4 * sizeof(double))) != cudaSuccess ||

@@ -233,6 +233,7 @@ struct AdvArgs {
     const real* VP;   // attenuated v_phi at face k-1/2 (rows 1..nt)
     const real *LMt, *LPt;   // theta LLF half-speeds of cell (j,k): (v_{j-1/2} + alpha)/2, (v_{j+1/2} - alpha)/2
     const real *LMp, *LPp;   // phi   LLF half-speeds of cell (j,k): (v_{k-1/2} + alpha)/2, (v_{k+1/2} - alpha)/2
+    int nparts;              // CTAs along phi of the stage kernel = partial sums per (realization, pole) in `part`
 };
 
 // theta-face flux at face f (between rows f and f+1) from rows f-1, f, f+1, f+2 of one column.
@@ -306,11 +307,11 @@ __global__ void __launch_bounds__(TX) k_adv_stage(AdvArgs<real> A, Tables<real> 
     }
     if (j0 == 1) {
         double t = block_sum(sumN, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbxa + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * A.nparts + blockIdx.x] = t;
     }
     if (j0 <= nt && nt < j1) {
         double t = block_sum(sumS, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbxa + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * A.nparts + blockIdx.x] = t;
     }
 }
 
@@ -405,11 +406,11 @@ __global__ void __launch_bounds__(TX) k_adv_stage_u(AdvArgs<real> A, Tables<real
     }
     if (j0 == 1) {
         double t = block_sum(sumN, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbxa + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * A.nparts + blockIdx.x] = t;
     }
     if (j0 <= nt && nt < j1) {
         double t = block_sum(sumS, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbxa + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * A.nparts + blockIdx.x] = t;
     }
 }
 
@@ -490,11 +491,100 @@ __global__ void __launch_bounds__(TX) k_adv_stage_att(AdvArgs<real> A, Tables<re
     }
     if (j0 == 1) {
         double t = block_sum(sumN, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * G.nbxa + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * A.nparts + blockIdx.x] = t;
     }
     if (j0 <= nt && nt < j1) {
         double t = block_sum(sumS, red);
-        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * G.nbxa + blockIdx.x] = t;
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * A.nparts + blockIdx.x] = t;
+    }
+}
+
+// k_adv_stage_att on a uniform theta grid with WENO3 fluxes, own-column loads only.  A warp covers 32 consecutive columns and
+// writes the 28 in the middle (lanes 2..29): the phi stencil of a face reaches two columns west and one east, and every
+// neighbour value -- the LLF products B LMp, B LPp of the cells next door -- comes from the neighbouring lanes by shuffle
+// instead of nine more loads per row (k_adv_stage_att: 13 loads per row and thread, 7 of them re-reads of other columns'
+// operands).  The theta sweep shares its products, differences and smoothness terms between faces as k_adv_stage_u does.
+constexpr int ATT_COLS = (TX / 32) * 28;
+
+template <typename real>
+__global__ void __launch_bounds__(TX) k_adv_stage_att_u(AdvArgs<real> A, Tables<real> T, Geom G) {
+    __shared__ double red[32];
+    const int r = blockIdx.z;
+    const int lane = threadIdx.x & 31;
+    const int np = G.np, nt = G.nt;
+    const int k = (blockIdx.x * (TX / 32) + (threadIdx.x >> 5)) * 28 + lane - 2;   // lanes 0, 1, 30, 31: neighbours only
+    const bool live = lane >= 2 && lane < 30 && k < np;
+    int k0 = k % np;
+    if (k0 < 0) k0 += np;
+    const int j0 = 1 + blockIdx.y * ADV_RPT;
+    const int j1 = min(j0 + ADV_RPT, nt + 1);
+    const size_t base = (size_t)r * G.rstride + k0;
+    const real eps = T.eps_t;
+    auto cl = [&](int j) -> int { return min(max(j, 0), nt + 1); };
+    auto at = [&](const real* p, int j) -> real { return p[base + (size_t)cl(j) * G.pitch]; };
+    auto sm = [&](real q) -> real { const real e = eps + q * q; return e * e; };
+
+    real w1 = at(A.in, j0 - 1), w2 = at(A.in, j0), w3 = at(A.in, j0 + 1);
+    // windows at face f = j0 - 1: A_{f-1}, A_f, A_{f+1} (B LMt) and P_f, P_{f+1}, P_{f+2} (B LPt)
+    real Am = at(A.in, j0 - 2) * at(A.LMt, j0 - 2), Ac = w1 * at(A.LMt, j0 - 1), Ap = w2 * at(A.LMt, j0);
+    real Pc = w1 * at(A.LPt, j0 - 1), Pp = w2 * at(A.LPt, j0), Pq = w3 * at(A.LPt, j0 + 1);
+    real qa1 = Ap - Ac, qp0 = Pp - Pq;
+    real sa0 = sm(Ac - Am), sa1 = sm(qa1), sp0 = sm(qp0), sp1 = sm(Pc - Pp);
+    auto face = [&](int f, real b0, real bp1) -> real {
+        if (f <= 1 || f >= nt - 1) return upwind(A.VT[base + (size_t)f * G.pitch], b0, bp1);
+        const real um = weno3_shared(Ac, (real)1.5 * Ac - (real)0.5 * Am, Ap, sa0, sa1);
+        const real up = weno3_shared(Pp, (real)1.5 * Pp - (real)0.5 * Pq, Pc, sp0, sp1);
+        return up + um;
+    };
+    real Fn = face(j0 - 1, w1, w2);
+    double sumN = 0.0, sumS = 0.0;
+    if (j0 == 1) sumN = live ? (double)Fn : 0.0;
+    const size_t p = G.pitch;
+    const real* __restrict__ inn = A.in + base + (size_t)cl(j0 + 2) * p;     // B row j + 2
+    const real* __restrict__ lmt = A.LMt + base + (size_t)(j0 + 1) * p;      // LMt row j + 1
+    const real* __restrict__ lpt = A.LPt + base + (size_t)cl(j0 + 2) * p;    // LPt row j + 2
+    const real* __restrict__ lmp = A.LMp + base + (size_t)j0 * p;            // row j
+    const real* __restrict__ lpp = A.LPp + base + (size_t)j0 * p;
+    const real* __restrict__ fnp = A.fn + base + (size_t)j0 * p;
+    real* __restrict__ outp = A.out + base + (size_t)j0 * p;
+    real sthn = T.sth[j0 - 1];
+    const bool blend = A.ca != (real)0;
+    const unsigned full = 0xffffffffu;
+    for (int j = j0; j < j1; j++) {
+        // ---- every load of this row first: six streams, this lane's column only
+        const real w4 = *inn, m3 = *lmt, p3 = *lpt, am = *lmp, ap = *lpp;
+        const real fnv = blend ? *fnp : (real)0;
+        // ---- theta: slide the windows to face j
+        Am = Ac; Ac = Ap; Ap = w3 * m3;
+        Pc = Pp; Pp = Pq; Pq = w4 * p3;
+        sa0 = sa1; qa1 = Ap - Ac; sa1 = sm(qa1);
+        sp1 = sp0; qp0 = Pp - Pq; sp0 = sm(qp0);
+        const real Fs = face(j, w2, w3);
+        // ---- phi: this cell's LLF products, the neighbours' by shuffle.  Face k-1/2: LM of cells k-2, k-1, k; LP of k+1, k, k-1
+        const real a0 = w2 * am, b0 = w2 * ap;
+        const real a1 = __shfl_up_sync(full, a0, 1), a2 = __shfl_up_sync(full, a0, 2);
+        const real b1 = __shfl_up_sync(full, b0, 1), bp = __shfl_down_sync(full, b0, 1);
+        const real Fw = weno3_side(bp, b0, b1, T.eps_p) + weno3_side(a2, a1, a0, T.eps_p);   // valid on lanes 2..30
+        const real Fe = __shfl_down_sync(full, Fw, 1);
+        const real sths = T.sth[j];
+        const real tend = (sths * Fs - sthn * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
+        real o = A.cb * w2 - A.cdt * tend;
+        if (blend) o = A.ca * fnv + o;
+        if (live) *outp = o;
+        if (j == nt) sumS = live ? (double)Fs : 0.0;
+        Fn = Fs; sthn = sths;
+        w1 = w2; w2 = w3; w3 = w4;
+        lmp += p; lpp += p; fnp += p; outp += p;
+        if (j + 2 <= nt + 1) lmt += p;                       // LMt row j + 2 next (unused beyond the south cap)
+        if (j + 3 <= nt + 1) { inn += p; lpt += p; }
+    }
+    if (j0 == 1) {
+        double t = block_sum(sumN, red);
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 0) * A.nparts + blockIdx.x] = t;
+    }
+    if (j0 <= nt && nt < j1) {
+        double t = block_sum(sumS, red);
+        if (threadIdx.x == 0) A.part[((size_t)r * 2 + 1) * A.nparts + blockIdx.x] = t;
     }
 }
 
@@ -507,7 +597,7 @@ __global__ void __launch_bounds__(TX) k_adv_caps(AdvArgs<real> A, Tables<real> T
     if (k >= G.np) return;
     const int j = pole == 0 ? 0 : G.nt + 1;
     const size_t off = (size_t)r * G.rstride + (size_t)j * G.pitch;
-    double S = sum_partials(A.part + ((size_t)r * 2 + pole) * G.nbxa, G.nbxa);
+    double S = sum_partials(A.part + ((size_t)r * 2 + pole) * A.nparts, A.nparts);
     real tend = (real)((pole == 0 ? 1.0 : -1.0) * (T.adv_capc[pole] * S));
     real o = A.cb * A.in[off] - A.cdt * tend;
     if (A.ca != (real)0) o = A.ca * A.fn[off] + o;
