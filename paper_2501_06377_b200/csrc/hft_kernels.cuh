@@ -550,6 +550,7 @@ __global__ void __launch_bounds__(TX) k_adv_stage_att_u(AdvArgs<real> A, Tables<
     real sthn = T.sth[j0 - 1];
     const bool blend = A.ca != (real)0;
     const unsigned full = 0xffffffffu;
+#pragma unroll 2
     for (int j = j0; j < j1; j++) {
         // ---- every load of this row first: six streams, this lane's column only
         const real w4 = *inn, m3 = *lmt, p3 = *lpt, am = *lmp, ap = *lpp;
