@@ -634,11 +634,14 @@ def cell_sum(w):
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("case", ["weno", "upwind", "strang"])
-def test_flow_attenuation(dtype, case):
+@pytest.mark.parametrize("nphi", [200, 345, 40])
+def test_flow_attenuation(dtype, case, nphi):
     """flow attenuation Eq. 5 (:100), per-realization B0 (one realization off), strong active regions
-    (|Br| up to ~3 B0) on a ragged grid; WENO3 + SSPRK(4,3) + STS, upwind + Euler, and inside a Strang step."""
+    (|Br| up to ~3 B0) on a ragged grid; WENO3 + SSPRK(4,3) + STS, upwind + Euler, and inside a Strang step.  n_phi = 345:
+    k_adv_stage_att_u (28 columns per warp) and the other stage kernels (31) use different numbers of CTAs along phi, hence
+    of polar partial sums; n_phi = 40: a warp's 32 columns wrap around the seam onto themselves."""
     H = hft()
-    w = wl.scaled(wl.config(3), 52, 200, n_real=3)
+    w = wl.scaled(wl.config(3), 52, nphi, n_real=3)
     maps = torch.stack([wl.bipolar_map(w.n_theta, w.n_phi, 8, 50 + r, amp=(100.0, 1500.0), sigma_deg=8.0) for r in range(3)])
     maps_t = maps.to(torch.float64 if dtype == "f64" else torch.float32)
     opt = dict(adv_flux=H.ADV_UPWIND, adv_time=H.TIME_EULER) if case == "upwind" else {}
