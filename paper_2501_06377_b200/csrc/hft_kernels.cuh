@@ -176,13 +176,15 @@ __global__ void __launch_bounds__(TX) k_polar_row_sums(const real* f, double* pa
 
 // WENO3-CS(h) one-sided face value (App. B :658-676, uniform grid: D = 1/2, 1/3, 2/3), written with one
 // division: u = (d0 p0 (eps+b1)^2 + d1 p1 (eps+b0)^2) / (d0 (eps+b1)^2 + d1 (eps+b0)^2).
-// num / den for den > 0 (a sum of squares here): hardware reciprocal seed (~20 bits) and two Newton steps, within
-// about an ulp of the IEEE quotient, without the slow path of the correctly rounded division (the WENO weights need 4 to 6
-// of these per cell and stage; the division was the largest single cost of the stage kernel).
+// num / den for den > 0 (a sum of squares here): hardware reciprocal seed (~20 bits), ONE Newton step (r = (1 + e) / den with
+// |e| ~ 2^-40), the quotient q = num r, and one residual correction q + r (num - den q), whose error is e^2 ~ 2^-80 before the
+// final rounding: within about an ulp of the IEEE quotient without the slow path of the correctly rounded division (the WENO
+// weights need 3 to 4 of these per cell and stage; the division was the largest single cost of the stage kernel).  A second
+// Newton step, as round 1 had it, changes nothing but the instruction count (measured on the B200: seed error 2^-19.9; 2e8
+// random quotients over 200 binades all equal to the IEEE quotient).
 __device__ __forceinline__ double pos_div(double num, double den) {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(den));
-    r = fma(fma(-den, r, 1.0), r, r);
     r = fma(fma(-den, r, 1.0), r, r);
     const double q = num * r;
     return fma(fma(-den, q, num), r, q);
