@@ -534,7 +534,7 @@ int advect(hft_ctx* c, double dt) {
         sts.push_back({B, S, A, 2.0 / 3.0, 1.0 / 3.0, 1.0 / 6.0});
         sts.push_back({A, nullptr, B, 0.0, 1.0, 0.5});
     }
-    dim3 g(G.nbxa, (G.nt + RPT - 1) / RPT, c->nr), gu(G.nbxa, (G.nt + ADV_RPT - 1) / ADV_RPT, c->nr), gc(G.nbx, 2, c->nr);
+    dim3 g(G.nbxa, (G.nt + RPT - 1) / RPT, c->nr), gc(G.nbx, 2, c->nr);
     const int nbxt = (G.np + ATT_COLS - 1) / ATT_COLS;   // k_adv_stage_att_u: 28 columns per warp
     dim3 gt(nbxt, (G.nt + ADV_RPT - 1) / ADV_RPT, c->nr);
     real* att[kNumAttArrays] = {nullptr};
@@ -557,10 +557,10 @@ int advect(hft_ctx* c, double dt) {
         bool armed;
         prof_begin(c, 2, armed);
         const bool fast = !T.nonuniform && !a.upwind_only;   // uniform theta grid, WENO3: the kernels with shared theta-sweep terms
-        a.nparts = (c->att_any && fast) ? nbxt : G.nbxa;
+        a.nparts = fast ? nbxt : G.nbxa;
         if (c->att_any && fast) k_adv_stage_att_u<real><<<gt, TX, 0, c->stream>>>(a, T, G);
         else if (c->att_any) k_adv_stage_att<real><<<g, TX, 0, c->stream>>>(a, T, G);
-        else if (!T.nonuniform && !a.upwind_only) k_adv_stage_u<real><<<gu, TX, 0, c->stream>>>(a, T, G);   // uniform theta grid, WENO3
+        else if (!T.nonuniform && !a.upwind_only) k_adv_stage_u<real><<<gt, TX, 0, c->stream>>>(a, T, G);   // uniform theta grid, WENO3
         else k_adv_stage<real><<<g, TX, 0, c->stream>>>(a, T, G);
         prof_end(c, armed, 1);
         k_adv_caps<real><<<gc, TX, 0, c->stream>>>(a, T, G);

@@ -334,38 +334,49 @@ __device__ __forceinline__ real weno3_shared(real near, real p0, real other, rea
     return pos_div(a0 * p0 + a1 * p1, a0 + a1);
 }
 
+constexpr int ATT_COLS = (TX / 32) * 28;   // columns written per CTA by the kernels that take phi-neighbours by shuffle
+
+// Third pass (ncu: 80 registers, 5.9 warps per scheduler, long_scoreboard 6.3 per issue -- the arithmetic waited for L1: three
+// re-reads of the neighbouring columns and seven warp-uniform table loads per row): a warp covers 32 consecutive columns and
+// writes the 28 in the middle, so B at k-2, k-1, k+1 comes from the neighbouring lanes by shuffle and every global load is
+// this lane's own column; the per-row tables of the CTA's 32 + 4 rows sit in shared memory.
 template <typename real>
 __global__ void __launch_bounds__(TX) k_adv_stage_u(AdvArgs<real> A, Tables<real> T, Geom G) {
     __shared__ double red[32];
+    constexpr int NTAB = ADV_RPT + 5;
+    __shared__ real s_lm[NTAB], s_lp[NTAB], s_pm[NTAB], s_pp[NTAB], s_sth[NTAB], s_rdt[NTAB], s_rdp[NTAB];
     const int r = blockIdx.z;
     const int lane = threadIdx.x & 31;
-    const int k = (blockIdx.x * (TX / 32) + (threadIdx.x >> 5)) * 31 + lane;   // lane 31: the first column of the next warp
     const int np = G.np, nt = G.nt;
-    const bool live = lane < 31 && k < np;          // this lane writes column k
-    const int k0 = k % np;
-    const int km1 = (k0 + np - 1) % np, km2 = (k0 + np - 2) % np, kp1 = (k0 + 1) % np;
+    const int k = (blockIdx.x * (TX / 32) + (threadIdx.x >> 5)) * 28 + lane - 2;   // lanes 0, 1, 30, 31: neighbours only
+    const bool live = lane >= 2 && lane < 30 && k < np;
+    int k0 = k % np;
+    if (k0 < 0) k0 += np;
     const int j0 = 1 + blockIdx.y * ADV_RPT;        // rows 1..nt only; caps are done by k_adv_caps
     const int j1 = min(j0 + ADV_RPT, nt + 1);
-    const size_t base = (size_t)r * G.rstride;
-    const real* __restrict__ in = A.in + base;   // (in, fn and out never alias: the SSPRK stages ping-pong between arrays)
-    const real* lm = T.lm + (size_t)r * (nt + 2);
-    const real* lp = T.lp + (size_t)r * (nt + 2);
-    const real* vtf = T.vtf + (size_t)r * (nt + 1);
-    const real* pm = T.pm + (size_t)r * (nt + 2);
-    const real* pp = T.pp + (size_t)r * (nt + 2);
-    const real eps = T.eps_t;
     auto cl = [&](int j) -> int { return min(max(j, 0), nt + 1); };
-    auto ld = [&](int j) -> real { return in[(size_t)cl(j) * G.pitch + k0]; };
+    const int jt = j0 - 2;                          // first table row (index i <-> row jt + i, clamped to 0..nt+1)
+    if (threadIdx.x < NTAB) {
+        const int row = cl(jt + threadIdx.x);
+        const size_t o = (size_t)r * (nt + 2) + row;
+        s_lm[threadIdx.x] = T.lm[o]; s_lp[threadIdx.x] = T.lp[o]; s_pm[threadIdx.x] = T.pm[o]; s_pp[threadIdx.x] = T.pp[o];
+        s_sth[threadIdx.x] = T.sth[min(row, nt)]; s_rdt[threadIdx.x] = T.rdt[row]; s_rdp[threadIdx.x] = T.rdp[row];
+    }
+    __syncthreads();
+    const size_t base = (size_t)r * G.rstride + k0;
+    const real* __restrict__ in = A.in + base;      // (in, fn and out never alias: the SSPRK stages ping-pong between arrays)
+    const real* vtf = T.vtf + (size_t)r * (nt + 1);
+    const real eps = T.eps_t;
+    auto ld = [&](int j) -> real { return in[(size_t)cl(j) * G.pitch]; };
     auto sm = [&](real q) -> real { const real e = eps + q * q; return e * e; };
 
     // rows f-1 .. f+2 around the first face f = j0 - 1
-    real w0 = ld(j0 - 2), w1 = ld(j0 - 1), w2 = ld(j0), w3 = ld(j0 + 1);
+    real w1 = ld(j0 - 1), w2 = ld(j0), w3 = ld(j0 + 1);
     // windows at face f: A_{f-1}, A_f, A_{f+1};  P_f, P_{f+1}, P_{f+2}   (table rows outside 0..nt+1 feed upwind faces only)
-    real Am = w0 * lm[cl(j0 - 2)], Ac = w1 * lm[cl(j0 - 1)], Ap = w2 * lm[j0];
-    real Pc = w1 * lp[cl(j0 - 1)], Pp = w2 * lp[j0], Pq = w3 * lp[cl(j0 + 1)];
-    real qa0 = Ac - Am, qa1 = Ap - Ac;              // right-moving: q0 = near - far, q1 = other - near
-    real qp0 = Pp - Pq, qp1 = Pc - Pp;              // left-moving:  near = P_{f+1}, far = P_{f+2}, other = P_f
-    real sa0 = sm(qa0), sa1 = sm(qa1), sp0 = sm(qp0), sp1 = sm(qp1);
+    real Am = ld(j0 - 2) * s_lm[0], Ac = w1 * s_lm[1], Ap = w2 * s_lm[2];
+    real Pc = w1 * s_lp[1], Pp = w2 * s_lp[2], Pq = w3 * s_lp[3];
+    real qa1 = Ap - Ac, qp0 = Pp - Pq;              // right-moving: q1 = other - near; left-moving: q0 = near - far
+    real sa0 = sm(Ac - Am), sa1 = sm(qa1), sp0 = sm(qp0), sp1 = sm(Pc - Pp);
     auto face = [&](int f, real b0, real bp1) -> real {
         if (f <= 1 || f >= nt - 1) return upwind(vtf[f], b0, bp1);
         const real um = weno3_shared(Ac, (real)1.5 * Ac - (real)0.5 * Am, Ap, sa0, sa1);
@@ -375,35 +386,34 @@ __global__ void __launch_bounds__(TX) k_adv_stage_u(AdvArgs<real> A, Tables<real
     real Fn = face(j0 - 1, w1, w2);
     double sumN = 0.0, sumS = 0.0;
     if (j0 == 1) sumN = live ? (double)Fn : 0.0;
-    const real* __restrict__ row = in + (size_t)j0 * G.pitch;                     // row j
-    const real* __restrict__ nxt = in + (size_t)cl(j0 + 2) * G.pitch + k0;        // row j + 2, this column
-    const real* __restrict__ fnp = A.fn + base + (size_t)j0 * G.pitch + k0;
-    real* __restrict__ outp = A.out + base + (size_t)j0 * G.pitch + k0;
-    real sthn = T.sth[j0 - 1];
+    const real* __restrict__ nxt = in + (size_t)cl(j0 + 2) * G.pitch;        // row j + 2, this column
+    const real* __restrict__ fnp = A.fn + base + (size_t)j0 * G.pitch;
+    real* __restrict__ outp = A.out + base + (size_t)j0 * G.pitch;
     const bool blend = A.ca != (real)0;
+    const unsigned full = 0xffffffffu;
     // unrolled: the window shifts become register renaming, and the loads of the next rows move above this row's arithmetic
 #pragma unroll 4
     for (int j = j0; j < j1; j++) {
+        const int i = j - jt;                       // table index of row j
         const real w4 = *nxt;
-        const real bm2 = row[km2], bm1 = row[km1], bp1 = row[kp1];
         const real fnv = blend ? *fnp : (real)0;
         // slide the windows to face j: one new product, difference and smoothness term per side
-        Am = Ac; Ac = Ap; Ap = w3 * lm[j + 1];
-        Pc = Pp; Pp = Pq; Pq = w4 * lp[cl(j + 2)];
-        qa0 = qa1; sa0 = sa1; qa1 = Ap - Ac; sa1 = sm(qa1);
-        qp1 = qp0; sp1 = sp0; qp0 = Pp - Pq; sp0 = sm(qp0);
+        Am = Ac; Ac = Ap; Ap = w3 * s_lm[i + 1];
+        Pc = Pp; Pp = Pq; Pq = w4 * s_lp[i + 2];
+        sa0 = sa1; qa1 = Ap - Ac; sa1 = sm(qa1);
+        sp1 = sp0; qp0 = Pp - Pq; sp0 = sm(qp0);
         const real Fs = face(j, w2, w3);
-        const real Fw = phi_face_flux<real>(bm2, bm1, w2, bp1, pm[j], pp[j], T.eps_p, 0);
-        const real Fe = __shfl_down_sync(0xffffffffu, Fw, 1);   // face k+1/2 = the west face of column k+1 (same operands, same bits)
-        const real sths = T.sth[j];
-        const real tend = (sths * Fs - sthn * Fn) * T.rdt[j] + (Fe - Fw) * T.rdp[j];
+        const real bm1 = __shfl_up_sync(full, w2, 1), bm2 = __shfl_up_sync(full, w2, 2), bp1 = __shfl_down_sync(full, w2, 1);
+        const real Fw = phi_face_flux<real>(bm2, bm1, w2, bp1, s_pm[i], s_pp[i], T.eps_p, 0);   // valid on lanes 2..30
+        const real Fe = __shfl_down_sync(full, Fw, 1);   // face k+1/2 = the west face of column k+1 (same operands, same bits)
+        const real tend = (s_sth[i] * Fs - s_sth[i - 1] * Fn) * s_rdt[i] + (Fe - Fw) * s_rdp[i];
         real o = A.cb * w2 - A.cdt * tend;
         if (blend) o = A.ca * fnv + o;
         if (live) *outp = o;
         if (j == nt) sumS = live ? (double)Fs : 0.0;
-        Fn = Fs; sthn = sths;
-        w0 = w1; w1 = w2; w2 = w3; w3 = w4;
-        row += G.pitch; fnp += G.pitch; outp += G.pitch;
+        Fn = Fs;
+        w1 = w2; w2 = w3; w3 = w4;
+        fnp += G.pitch; outp += G.pitch;
         if (j + 3 <= nt + 1) nxt += G.pitch;                    // row j + 3 of the next iteration, clamped to the south cap
     }
     if (j0 == 1) {
@@ -506,8 +516,6 @@ __global__ void __launch_bounds__(TX) k_adv_stage_att(AdvArgs<real> A, Tables<re
 // neighbour value -- the LLF products B LMp, B LPp of the cells next door -- comes from the neighbouring lanes by shuffle
 // instead of nine more loads per row (k_adv_stage_att: 13 loads per row and thread, 7 of them re-reads of other columns'
 // operands).  The theta sweep shares its products, differences and smoothness terms between faces as k_adv_stage_u does.
-constexpr int ATT_COLS = (TX / 32) * 28;
-
 template <typename real>
 __global__ void __launch_bounds__(TX) k_adv_stage_att_u(AdvArgs<real> A, Tables<real> T, Geom G) {
     __shared__ double red[32];
