@@ -196,7 +196,7 @@ def run_paper_case(args):
     u = wl.soccer_ball_full(nt, nphi)
     rot = 1.80766e3 if args.paper_case == "advdiff" else 0.0
     ctx = hft.Context(nt, nphi, [[500.0, rot, 0, 0, 0, 0, 0]], dtype=args.dtype,
-                      adv_flux=hft.ADV_WENO3 if rot else hft.ADV_OFF, sts_block=args.sts_block)
+                      adv_flux=hft.ADV_WENO3 if rot else hft.ADV_OFF, sts_block=args.sts_block, sts_kernel=args.sts_kernel)
     ut = torch.from_numpy(u).to(ctx.tdtype).cuda().contiguous()
     n = round(672.0 / 0.62) if rot else 1
     dt = 672.0 / n

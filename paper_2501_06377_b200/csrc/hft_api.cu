@@ -535,8 +535,12 @@ int advect(hft_ctx* c, double dt) {
         sts.push_back({A, nullptr, B, 0.0, 1.0, 0.5});
     }
     dim3 g(G.nbxa, (G.nt + RPT - 1) / RPT, c->nr), gc(G.nbx, 2, c->nr);
-    const int nbxt = (G.np + ATT_COLS - 1) / ATT_COLS;   // k_adv_stage_att_u: 28 columns per warp
-    dim3 gt(nbxt, (G.nt + ADV_RPT - 1) / ADV_RPT, c->nr);
+    const int nbxt = (G.np + ATT_COLS - 1) / ATT_COLS;   // k_adv_stage_u / k_adv_stage_att_u: 28 columns per warp
+    // rows per thread: 32 on a full batch (the first face of a strip is evaluated without writing a row); on a small batch
+    // shorter strips, so that every SM still gets several CTAs (one 510 x 1023 realization: 160 CTAs at 32 rows, 640 at 8)
+    int rpt = ADV_RPT;
+    while (rpt > 8 && (long)nbxt * ((G.nt + rpt - 1) / rpt) * c->nr < 148L * 8) rpt /= 2;
+    dim3 gt(nbxt, (G.nt + rpt - 1) / rpt, c->nr);
     real* att[kNumAttArrays] = {nullptr};
     if (c->att_any) {
         for (int i = 0; i < kNumAttArrays; i++) att[i] = (real*)c->att[i];
@@ -558,6 +562,7 @@ int advect(hft_ctx* c, double dt) {
         prof_begin(c, 2, armed);
         const bool fast = !T.nonuniform && !a.upwind_only;   // uniform theta grid, WENO3: the kernels with shared theta-sweep terms
         a.nparts = fast ? nbxt : G.nbxa;
+        a.rpt = rpt;
         if (c->att_any && fast) k_adv_stage_att_u<real><<<gt, TX, 0, c->stream>>>(a, T, G);
         else if (c->att_any) k_adv_stage_att<real><<<g, TX, 0, c->stream>>>(a, T, G);
         else if (!T.nonuniform && !a.upwind_only) k_adv_stage_u<real><<<gt, TX, 0, c->stream>>>(a, T, G);   // uniform theta grid, WENO3

@@ -236,6 +236,7 @@ struct AdvArgs {
     const real *LMt, *LPt;   // theta LLF half-speeds of cell (j,k): (v_{j-1/2} + alpha)/2, (v_{j+1/2} - alpha)/2
     const real *LMp, *LPp;   // phi   LLF half-speeds of cell (j,k): (v_{k-1/2} + alpha)/2, (v_{k+1/2} - alpha)/2
     int nparts;              // CTAs along phi of the stage kernel = partial sums per (realization, pole) in `part`
+    int rpt;                 // k_adv_stage_u / k_adv_stage_att_u: rows per thread, <= ADV_RPT (fewer on small batches: more CTAs)
 };
 
 // theta-face flux at face f (between rows f and f+1) from rows f-1, f, f+1, f+2 of one column.
@@ -352,8 +353,8 @@ __global__ void __launch_bounds__(TX) k_adv_stage_u(AdvArgs<real> A, Tables<real
     const bool live = lane >= 2 && lane < 30 && k < np;
     int k0 = k % np;
     if (k0 < 0) k0 += np;
-    const int j0 = 1 + blockIdx.y * ADV_RPT;        // rows 1..nt only; caps are done by k_adv_caps
-    const int j1 = min(j0 + ADV_RPT, nt + 1);
+    const int j0 = 1 + blockIdx.y * A.rpt;          // rows 1..nt only; caps are done by k_adv_caps
+    const int j1 = min(j0 + A.rpt, nt + 1);
     auto cl = [&](int j) -> int { return min(max(j, 0), nt + 1); };
     const int jt = j0 - 2;                          // first table row (index i <-> row jt + i, clamped to 0..nt+1)
     if (threadIdx.x < NTAB) {
@@ -526,8 +527,8 @@ __global__ void __launch_bounds__(TX) k_adv_stage_att_u(AdvArgs<real> A, Tables<
     const bool live = lane >= 2 && lane < 30 && k < np;
     int k0 = k % np;
     if (k0 < 0) k0 += np;
-    const int j0 = 1 + blockIdx.y * ADV_RPT;
-    const int j1 = min(j0 + ADV_RPT, nt + 1);
+    const int j0 = 1 + blockIdx.y * A.rpt;
+    const int j1 = min(j0 + A.rpt, nt + 1);
     const size_t base = (size_t)r * G.rstride + k0;
     const real eps = T.eps_t;
     auto cl = [&](int j) -> int { return min(max(j, 0), nt + 1); };
